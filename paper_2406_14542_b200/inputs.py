@@ -1,0 +1,117 @@
+"""Seeded synthetic inputs shared by the CUDA path's tests/bench and the oracle.
+
+This module holds NO arithmetic of the method (no Legendre functions, no FFT, no kernels): only
+random draws and the geometry of the workloads.  Recipes follow BASELINE.json `configs` and
+SURVEY.md 8(d); see DESIGN.md "Input recipe".
+
+* points uniform on the sphere: theta = arccos(U[-1,1]), phi ~ U[0, 2 pi)
+* CMB-lensing-like points (config 2): an equi-angular ring grid displaced per pixel by
+  arXiv 2406.14542 Eq. C1 with iid Gaussian deflection components
+  (sigma = 2.5 arcmin => |alpha| ~ Rayleigh(sigma)); the paper's real deflection fields
+   are not available offline, this stands in for them.
+* a_lm: complex, m >= 0, real-field convention, m-major triangular layout
+  idx(l, m) = m (2 lmax + 1 - m)/2 + l; white (C_l = 1) or C_l = 1/(l+1)^2.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+ARCMIN = np.pi / 180.0 / 60.0
+
+
+def nlm(lmax: int, mmax: int) -> int:
+    return (mmax + 1) * (lmax + 1) - mmax * (mmax + 1) // 2
+
+
+def lm_index(lmax: int, l, m):
+    return m * (2 * lmax + 1 - m) // 2 + l
+
+
+def uniform_sphere_points(npts: int, seed: int):
+    rng = np.random.default_rng(seed)
+    theta = np.arccos(rng.uniform(-1.0, 1.0, size=npts))
+    phi = rng.uniform(0.0, 2.0 * np.pi, size=npts)
+    return theta, phi
+
+
+def random_alm(lmax: int, mmax: int, seed: int, spectrum: str = "white"):
+    """Complex alm with E|a_lm|^2 = C_l.  'white': Re, Im ~ N(0,1) for m > 0 and a_l0 ~ N(0,1) real
+    (BASELINE.json configs 1 and 3).  'inv_l2': C_l = 1/(l+1)^2, Re, Im variance C_l/2, a_l0 real
+    with variance C_l (configs 2 and 4)."""
+    rng = np.random.default_rng(seed + 1000003)
+    n = nlm(lmax, mmax)
+    re = rng.standard_normal(n)
+    im = rng.standard_normal(n)
+    alm = np.empty(n, dtype=np.complex128)
+    if spectrum == "white":
+        alm.real, alm.imag = re, im
+        alm[: lmax + 1] = re[: lmax + 1]
+    elif spectrum == "inv_l2":
+        for m in range(mmax + 1):
+            lo = lm_index(lmax, m, m)
+            l = np.arange(m, lmax + 1)
+            amp = 1.0 / (l + 1.0)
+            sl = slice(lo, lo + lmax - m + 1)
+            if m == 0:
+                alm[sl] = re[sl] * amp
+            else:
+                alm[sl] = (re[sl] + 1j * im[sl]) * (amp / np.sqrt(2.0))
+    else:
+        raise ValueError(spectrum)
+    return alm
+
+
+def random_map(npts: int, seed: int):
+    rng = np.random.default_rng(seed + 2000003)
+    return rng.standard_normal(npts)
+
+
+def lensing_like_points(nrings: int, npix: int, seed: int, sigma: float = 2.5 * ARCMIN):
+    """nrings x npix equi-angular grid theta_i = pi (i + 1/2)/nrings, phi_j = 2 pi j/npix (ring-major
+    order), each pixel displaced along a random direction by Eq. C1:
+        n' = cos(a) n + sin(a)/a (a_theta e_theta + a_phi e_phi),  a = |(a_theta, a_phi)|.
+    Returns theta', phi' in [0, pi] x [0, 2 pi)."""
+    rng = np.random.default_rng(seed)
+    th = np.pi * (np.arange(nrings) + 0.5) / nrings
+    ph = 2.0 * np.pi * np.arange(npix) / npix
+    theta = np.repeat(th, npix)
+    phi = np.tile(ph, nrings)
+    a_t = rng.normal(0.0, sigma, size=theta.shape[0])
+    a_p = rng.normal(0.0, sigma, size=theta.shape[0])
+    a = np.hypot(a_t, a_p)
+    st, ct, sp, cp = np.sin(theta), np.cos(theta), np.sin(phi), np.cos(phi)
+    n = np.stack([st * cp, st * sp, ct])
+    e_t = np.stack([ct * cp, ct * sp, -st])
+    e_p = np.stack([-sp, cp, np.zeros_like(sp)])
+    with np.errstate(invalid="ignore", divide="ignore"):
+        sinc = np.where(a > 0, np.sin(a) / a, 1.0)
+    npr = np.cos(a) * n + sinc * (a_t * e_t + a_p * e_p)
+    theta2 = np.arccos(np.clip(npr[2], -1.0, 1.0))
+    phi2 = np.mod(np.arctan2(npr[1], npr[0]), 2.0 * np.pi)
+    phi2[phi2 >= 2.0 * np.pi] = 0.0
+    return theta2, phi2
+
+
+# BASELINE.json `configs`, in order.  npts / spectrum / eps / dtype per config.
+CONFIGS = {
+    1: dict(lmax=63, mmax=63, eps=1e-10, dtype="f64", npts=16384, points="uniform", spectrum="white", seed=0),
+    2: dict(lmax=1023, mmax=1023, eps=1e-10, dtype="f64", npts=2048 * 2048, points="lensing", spectrum="inv_l2", seed=2),
+    3: dict(lmax=4095, mmax=4095, eps=1e-10, dtype="f64", npts=4 * 4096 * 4096, points="uniform", spectrum="white", seed=3),
+    4: dict(lmax=8191, mmax=8191, eps=1e-8, dtype="f64", npts=2 * 8192 * 8192, points="uniform", spectrum="inv_l2", seed=4),
+}
+
+
+def make_config(i: int, npts: int | None = None):
+    """(cfg, theta, phi, alm, x) for BASELINE config i; `npts` overrides the point count (tests)."""
+    cfg = dict(CONFIGS[i])
+    if npts is not None:
+        cfg["npts"] = int(npts)
+    if cfg["points"] == "uniform":
+        theta, phi = uniform_sphere_points(cfg["npts"], cfg["seed"])
+    else:
+        side = int(round(np.sqrt(cfg["npts"])))
+        theta, phi = lensing_like_points(side, side, cfg["seed"])
+        cfg["npts"] = side * side
+    alm = random_alm(cfg["lmax"], cfg["mmax"], cfg["seed"], cfg["spectrum"])
+    x = random_map(cfg["npts"], cfg["seed"])
+    return cfg, theta, phi, alm, x

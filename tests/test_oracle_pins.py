@@ -1,0 +1,260 @@
+"""Pins for the CPU oracle (oracle/): everything here is CPU-only and checks the oracle against
+things OTHER than itself -- closed forms, library routines (mpmath, scipy), invariants.
+
+Citations: arXiv 2406.14542 Eq. 1-3, fn. 4; readings G1-G3, G12
+and pins P1-P8 in DESIGN.md / SURVEY.md 8(c).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2406_14542_b200 import inputs
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "plm_mpmath.txt")
+
+
+def single_alm(lmax, mmax, l, m, val):
+    a = np.zeros(inputs.nlm(lmax, mmax), dtype=np.complex128)
+    a[inputs.lm_index(lmax, l, m)] = val
+    return a
+
+
+def closed_form(l, m, th, ph):
+    """Orthonormal, Condon-Shortley Y_lm for l <= 2 (textbook table)."""
+    s, c = np.sin(th), np.cos(th)
+    e = np.exp(1j * m * ph)
+    tab = {
+        (0, 0): np.sqrt(1 / (4 * np.pi)) * np.ones_like(th),
+        (1, 0): np.sqrt(3 / (4 * np.pi)) * c,
+        (1, 1): -np.sqrt(3 / (8 * np.pi)) * s,
+        (2, 0): np.sqrt(5 / (16 * np.pi)) * (3 * c * c - 1),
+        (2, 1): -np.sqrt(15 / (8 * np.pi)) * s * c,
+        (2, 2): np.sqrt(15 / (32 * np.pi)) * s * s,
+    }
+    return tab[(l, m)] * e
+
+
+# ---- P1: closed forms, through the full synthesis entry point (layout, w_m, phase) ------------
+@pytest.mark.parametrize("l,m", [(0, 0), (1, 0), (1, 1), (2, 0), (2, 1), (2, 2)])
+@pytest.mark.parametrize("prec", ["d", "ld"])
+def test_closed_forms_synthesis(oracle, l, m, prec):
+    rng = np.random.default_rng(l * 10 + m)
+    th = np.arccos(rng.uniform(-1, 1, 200))
+    ph = rng.uniform(0, 2 * np.pi, 200)
+    lmax, mmax = 5, 4
+    a = 0.7 - 1.3j if m > 0 else 0.7 + 0j
+    f = oracle.synthesis(lmax, mmax, th, ph, single_alm(lmax, mmax, l, m, a), prec)
+    wm = 1.0 if m == 0 else 2.0
+    ref = wm * np.real(a * closed_form(l, m, th, ph))
+    assert np.max(np.abs(f - ref)) < 2e-15
+
+
+def test_im_al0_ignored(oracle):
+    th, ph = inputs.uniform_sphere_points(50, 1)
+    a = inputs.random_alm(6, 6, 1)
+    b = a.copy()
+    b[:7] += 1j * np.arange(1, 8)
+    assert np.array_equal(oracle.synthesis(6, 6, th, ph, a), oracle.synthesis(6, 6, th, ph, b))
+
+
+# ---- P5: mpmath library values (stored; generator beside the file) ---------------------------
+def _golden():
+    rows = []
+    for line in open(GOLDEN):
+        if line.startswith("#") or not line.strip():
+            continue
+        l, m, thx, frac, ex = line.split()
+        rows.append((int(l), int(m), float.fromhex(thx), float(frac), int(ex)))
+    return rows
+
+
+@pytest.mark.parametrize("prec,eps", [("ld", 2.0 ** -64), ("d", 2.0 ** -53)])
+def test_plm_vs_mpmath_golden(oracle, prec, eps):
+    for l, m, th, frac, ex in _golden():
+        mant, e2 = oracle.plm(l, m, th, prec)
+        # same binary exponent, or off by one when the fraction sits at the 0.5/1 boundary
+        assert abs(e2 - ex) <= 1, (l, m, th)
+        got = mant * 2.0 ** (e2 - ex)
+        # near a zero of Pbar (equator, odd l+m) the value is set by cos(theta) rounding: skip rel check
+        if abs(np.cos(th)) < 1e-15:
+            continue
+        # rounding of cos(theta) moves theta by eps/sin(theta); dPbar/dtheta ~ l Pbar; plus O(l) steps
+        tol = eps * (2000.0 + 8.0 * l / max(np.sin(th), 1e-3))
+        assert abs(got / frac - 1.0) < tol, (l, m, th, got / frac - 1.0, tol)
+
+
+def test_plm_vs_mpmath_live(oracle):
+    mp = pytest.importorskip("mpmath")
+    mp.mp.dps = 40
+    rng = np.random.default_rng(7)
+    for _ in range(60):
+        l = int(rng.integers(0, 300))
+        m = int(rng.integers(0, l + 1))
+        th = float(np.arccos(rng.uniform(-1, 1)))
+        ref = mp.re(mp.spherharm(l, m, mp.mpf(th), 0, maxprec=100000))
+        got = oracle.plm_value(l, m, th, "ld")
+        scale = np.sqrt((2 * l + 1) / (4 * np.pi))
+        assert abs(got - float(ref)) < 1e-14 * scale, (l, m, th)
+
+
+# ---- P6: scipy library cross-check through synthesis and adjoint -----------------------------
+def test_vs_scipy_sph_harm(oracle):
+    sp = pytest.importorskip("scipy.special")
+    if not hasattr(sp, "sph_harm_y"):
+        pytest.skip("scipy without sph_harm_y")
+    lmax = mmax = 40
+    th, ph = inputs.uniform_sphere_points(300, 11)
+    a = inputs.random_alm(lmax, mmax, 11)
+    ref = np.zeros(300)
+    for m in range(mmax + 1):
+        for l in range(m, lmax + 1):
+            y = sp.sph_harm_y(l, m, th, ph)
+            c = a[inputs.lm_index(lmax, l, m)]
+            ref += (c.real * y.real) if m == 0 else 2 * np.real(c * y)
+    f = oracle.synthesis(lmax, mmax, th, ph, a)
+    assert np.linalg.norm(f - ref) / np.linalg.norm(ref) < 5e-14
+    # adjoint: c_lm = sum_j x_j conj(Y_lm)
+    x = inputs.random_map(300, 11)
+    c = oracle.adjoint(lmax, mmax, th, ph, x)
+    for (l, m) in [(0, 0), (7, 0), (7, 3), (40, 40), (39, 1), (40, 0)]:
+        r = np.sum(x * np.conj(sp.sph_harm_y(l, m, th, ph)))
+        if m == 0:
+            r = r.real
+        assert abs(c[inputs.lm_index(lmax, l, m)] - r) < 1e-12
+
+
+# ---- P2: addition theorem sum_m |Y_lm|^2 = (2l+1)/4pi, incl. near-pole and large l -----------
+@pytest.mark.parametrize("l", [0, 1, 15, 200, 1023, 4095])
+@pytest.mark.parametrize("theta", [1e-3, 0.05, 0.9, np.pi / 2, 3.0])
+def test_addition_theorem(oracle, l, theta):
+    tot = oracle.plm_value(l, 0, theta) ** 2
+    for m in range(1, l + 1):
+        tot += 2 * oracle.plm_value(l, m, theta) ** 2
+    tol = 2e-10 if l > 1000 else 1e-11
+    assert abs(tot / ((2 * l + 1) / (4 * np.pi)) - 1) < tol
+
+
+# ---- parity Pbar_lm(pi - theta) = (-1)^(l+m) Pbar_lm(theta) ------------------------------------
+def test_parity(oracle):
+    for (l, m, th) in [(5, 2, 0.4), (6, 2, 0.4), (101, 50, 1.1), (100, 50, 1.1)]:
+        a = oracle.plm_value(l, m, th, "ld")
+        b = oracle.plm_value(l, m, np.pi - th, "ld")
+        assert abs(b - (-1) ** (l + m) * a) < 1e-13 * (1 + abs(a))
+
+
+# ---- P3: orthonormality under Gauss-Legendre quadrature ---------------------------------------
+@pytest.mark.parametrize("lmax,mmax", [(0, 0), (7, 7), (24, 24), (32, 20)])
+def test_gauss_legendre_orthonormality(oracle, lmax, mmax):
+    xg, wg = np.polynomial.legendre.leggauss(lmax + 1)
+    nph = 2 * lmax + 2
+    th = np.repeat(np.arccos(xg), nph)
+    ph = np.tile(2 * np.pi * np.arange(nph) / nph, lmax + 1)
+    w = np.repeat(wg, nph) * (2 * np.pi / nph)
+    a = inputs.random_alm(lmax, mmax, 5)
+    f = oracle.synthesis(lmax, mmax, th, ph, a)
+    back = oracle.adjoint(lmax, mmax, th, ph, w * f)
+    assert np.max(np.abs(back - a)) < 1e-13 * max(1.0, np.max(np.abs(a))) * (lmax + 1)
+
+
+# ---- P4: adjoint identity with the G3 inner product -------------------------------------------
+@pytest.mark.parametrize("lmax,mmax,npts", [(12, 12, 500), (63, 63, 2000), (63, 17, 1000)])
+def test_adjoint_identity(oracle, lmax, mmax, npts):
+    th, ph = inputs.uniform_sphere_points(npts, 3)
+    a = inputs.random_alm(lmax, mmax, 3)
+    x = inputs.random_map(npts, 3)
+    f = oracle.synthesis(lmax, mmax, th, ph, a)
+    c = oracle.adjoint(lmax, mmax, th, ph, x)
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+    rhs = oracle.inner_alm(lmax, mmax, a, c)
+    assert abs(lhs - rhs) < 1e-13 * np.linalg.norm(f) * np.linalg.norm(x)
+
+
+def test_adjoint_m0_imag_zero(oracle):
+    th, ph = inputs.uniform_sphere_points(100, 4)
+    c = oracle.adjoint(8, 8, th, ph, inputs.random_map(100, 4))
+    assert np.all(c[:9].imag == 0.0)
+
+
+# ---- P8: special cases ------------------------------------------------------------------------
+def test_lmax_zero(oracle):
+    th, ph = inputs.uniform_sphere_points(20, 5)
+    f = oracle.synthesis(0, 0, th, ph, np.array([2.5 + 0j]))
+    assert np.allclose(f, 2.5 / np.sqrt(4 * np.pi), rtol=0, atol=3e-16)
+
+
+def test_poles_exact(oracle):
+    # theta = 0 or pi: only m = 0 contributes; Pbar_l0(0) = sqrt((2l+1)/4pi), (-1)^l at pi
+    lmax = 20
+    a = inputs.random_alm(lmax, lmax, 6)
+    th = np.array([0.0, np.pi])
+    ph = np.array([0.3, 1.7])
+    f = oracle.synthesis(lmax, lmax, th, ph, a)
+    l = np.arange(lmax + 1)
+    n = np.sqrt((2 * l + 1) / (4 * np.pi))
+    assert abs(f[0] - np.sum(a[: lmax + 1].real * n)) < 1e-13
+    # theta = pi is the binary64 nearest pi: sin = 1.2e-16, so m >= 1 terms are ~1e-16
+    assert abs(f[1] - np.sum(a[: lmax + 1].real * n * (-1.0) ** l)) < 1e-13
+
+
+def test_single_point_adjoint(oracle):
+    sp = pytest.importorskip("scipy.special")
+    th, ph = np.array([1.234]), np.array([4.321])
+    c = oracle.adjoint(9, 9, th, ph, np.array([1.7]))
+    for (l, m) in [(0, 0), (3, 2), (9, 9), (9, 0)]:
+        r = 1.7 * np.conj(sp.sph_harm_y(l, m, th[0], ph[0]))
+        r = r.real if m == 0 else r
+        assert abs(c[inputs.lm_index(9, l, m)] - r) < 1e-14
+
+
+def test_ring_sum_matches_synthesis(oracle):
+    lmax = mmax = 30
+    m = 7
+    a = inputs.random_alm(lmax, mmax, 8)
+    lo = inputs.lm_index(lmax, m, m)
+    am = a[lo: lo + lmax - m + 1]
+    th = np.linspace(0.0, np.pi, 17)
+    F = oracle.ring_sum(lmax, m, th, am)
+    only = np.zeros_like(a)
+    only[lo: lo + lmax - m + 1] = am
+    ph = np.full_like(th, 0.37)
+    f = oracle.synthesis(lmax, mmax, th, ph, only)
+    assert np.max(np.abs(f - 2 * np.real(F * np.exp(1j * m * ph)))) < 1e-14
+
+
+def test_columns_match_full_adjoint(oracle):
+    lmax = 25
+    th, ph = inputs.uniform_sphere_points(300, 9)
+    x = inputs.random_map(300, 9)
+    c = oracle.adjoint(lmax, lmax, th, ph, x)
+    cols = oracle.adjoint_columns(lmax, [0, 3, 25], th, ph, x)
+    for q, m in enumerate([0, 3, 25]):
+        lo = inputs.lm_index(lmax, m, m)
+        assert np.array_equal(cols[q, m:], c[lo: lo + lmax - m + 1])
+        assert np.all(cols[q, :m] == 0)
+
+
+def test_double_vs_long_double(oracle):
+    lmax = 200
+    th, ph = inputs.uniform_sphere_points(200, 10)
+    a = inputs.random_alm(lmax, lmax, 10)
+    fd = oracle.synthesis(lmax, lmax, th, ph, a, "d")
+    fl = oracle.synthesis(lmax, lmax, th, ph, a, "ld")
+    assert np.linalg.norm(fd - fl) / np.linalg.norm(fl) < 1e-13
+
+
+def test_large_lmax_rescaling_synthesis_vs_mpmath(oracle):
+    """One high-l coefficient whose Pbar underflows binary64 at the seed: the synthesis entry point
+    must reproduce w_m Re(a Y_lm) with Y_lm from mpmath (exercises O2 inside the real code path)."""
+    mp = pytest.importorskip("mpmath")
+    mp.mp.dps = 40
+    lmax = mmax = 2100
+    l, m = 2100, 2000            # Pbar_mm(0.4) ~ sin(0.4)^2000 ~ 1e-820
+    th = np.array([0.4, 1.2, 2.9])
+    ph = np.array([0.1, 2.2, 5.0])
+    a = single_alm(lmax, mmax, l, m, 1.0 + 0.5j)
+    f = oracle.synthesis(lmax, mmax, th, ph, a)
+    for j in range(3):
+        y = mp.spherharm(l, m, mp.mpf(float(th[j])), mp.mpf(float(ph[j])), maxprec=400000)
+        ref = 2 * float(mp.re(mp.mpc(1.0, 0.5) * y))
+        assert abs(f[j] - ref) < 5e-12 * max(abs(ref), 1e-30) + 1e-300
