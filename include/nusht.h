@@ -1,0 +1,153 @@
+/*
+ * nusht.h -- C ABI of the B200-native nonuniform spin-0 spherical harmonic transform (nuSHT)
+ * defined in arXiv 2406.14542 ("cunuSHT").  Citations are PAPER.md:<line> of the paper text.
+ *
+ * The library computes, to a requested accuracy eps (Eq. 9-10),
+ *   synthesis / type 2 (Eq. 3):  f_j  = sum_{l<=lmax} sum_m c_lm Y_lm(theta_j, phi_j)
+ *   adjoint   / type 1 (Eq. 2):  c_lm = sum_j f_j conj(Y_lm(theta_j, phi_j))
+ * by the double-Fourier-sphere factorisation Y = N F D S (Eq. 5-6): ring Legendre
+ * transform onto an equi-angular theta grid (S), doubling theta to [0, 2 pi) (D), uniform FFT (F),
+ * nonuniform FFT to the points (N); the adjoint runs the transposed chain.  "Plan once, execute
+ * repeatedly"; nothing touches host memory between stages.
+ *
+ * Conventions (readings G1-G3, G11, G12):
+ *   Y_lm = Pbar_lm(theta) e^{i m phi}, orthonormal on the sphere, Condon-Shortley phase (Eq. 1,
+ *   PAPER.md:47-49; fn. 4).  Real field, only m >= 0 stored:
+ *     f_j = sum_l Re(a_l0) Pbar_l0 + 2 sum_{m=1}^{mmax} Re[ e^{i m phi_j} sum_l a_lm Pbar_lm(theta_j) ].
+ *   Im(a_l0) is ignored by synthesis and returned as exactly 0 by the adjoint.
+ *   The adjoint is the transpose (no quadrature weights), with respect to
+ *     <a, c> = sum_l a_l0 c_l0 + 2 sum_{m>=1} Re(a_lm conj(c_lm))   and   <f, x> = sum_j f_j x_j.
+ *
+ * Layouts:
+ *   alm : nlm = (mmax+1)(lmax+1) - mmax(mmax+1)/2 complex numbers of the plan's dtype, interleaved
+ *         (re, im), m-major triangular: idx(l, m) = m (2 lmax + 1 - m)/2 + l, 0 <= m <= mmax, m <= l <= lmax.
+ *   map : npts reals of the plan's dtype, in the caller's point order.
+ *   theta, phi : npts binary64 each, for both dtypes.  theta in [0, pi] (poles allowed), phi any
+ *         finite value (wrapped mod 2 pi).  Duplicate points are allowed.
+ *
+ * Ownership: every data pointer is caller-owned.  Unless a function says HOST, pointers are DEVICE
+ * pointers on the current CUDA device.  nusht_plan copies what it needs from theta/phi (they may
+ * be freed afterwards) and owns all workspace.  nusht_synthesis / nusht_adjoint allocate nothing,
+ * touch no host memory, enqueue on `stream` (a cudaStream_t passed as void*; NULL = default
+ * stream) and return without synchronising.  nusht_adjoint OVERWRITES alm.  A plan must not be
+ * used from two streams at once (shared workspace).
+ *
+ * Errors: every call returns a status; nothing throws or exits.  There is no CPU fallback: without
+ * a CUDA device nusht_plan returns NUSHT_ERR_CUDA.
+ */
+#ifndef NUSHT_H
+#define NUSHT_H
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define NUSHT_API __attribute__((visibility("default")))
+#else
+#define NUSHT_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nusht_plan_s nusht_plan_t; /* opaque, library-owned */
+
+enum { NUSHT_F64 = 0, NUSHT_F32 = 1 };
+
+enum {
+    NUSHT_OK = 0,
+    NUSHT_ERR_INVALID_ARG = -1, /* bad lmax/mmax/npts/eps/dtype or NULL pointer */
+    NUSHT_ERR_ALLOC = -2,       /* device or host allocation failed */
+    NUSHT_ERR_CUDA = -3,        /* CUDA runtime / launch error (also: no device) */
+    NUSHT_ERR_CUFFT = -4,       /* cuFFT plan or exec error */
+    NUSHT_ERR_UNSUPPORTED = -5, /* valid request this build does not implement */
+    NUSHT_ERR_BAD_POINTS = -6   /* NaN/Inf coordinates or theta outside [0, pi] */
+};
+
+/* Stage slots reported by nusht_stage_times. */
+enum {
+    NUSHT_SYN_ALM_PREP = 0,  /* a1 prologue: coefficient scaling + odd-class fold (O(lmax^2)) */
+    NUSHT_SYN_LEGENDRE = 1,  /* a1 + a2: Legendre synthesis with fused DFS doubling */
+    NUSHT_SYN_FFT_THETA = 2, /* a3: theta FFT of the doubled rings (cuFFT) */
+    NUSHT_SYN_DECONV_PAD = 3,/* a4: kernel deconvolution + zero-pad to the fine grid */
+    NUSHT_SYN_FFT_FINE_THETA = 4, /* a5, theta pass (cuFFT) */
+    NUSHT_SYN_FFT_FINE_PHI = 5,   /* a5, phi C2R pass (cuFFT) */
+    NUSHT_SYN_INTERP = 6,    /* a7: type-2 interpolation */
+    NUSHT_ADJ_SPREAD = 0,    /* a8: type-1 spreading (includes zeroing the fine grid) */
+    NUSHT_ADJ_FFT_FINE_PHI = 1,   /* a9: phi R2C (cuFFT) */
+    NUSHT_ADJ_FFT_FINE_THETA = 2, /* a9: theta forward FFT on the fine grid (cuFFT) */
+    NUSHT_ADJ_DECONV_TRUNC = 3,   /* a9: truncate to |k| <= lmax + deconvolve */
+    NUSHT_ADJ_FFT_THETA = 4, /* a9: theta inverse FFT back to the doubled rings (cuFFT) */
+    NUSHT_ADJ_LEGENDRE = 5,  /* a10 + a11: fold + adjoint Legendre */
+    NUSHT_ADJ_ALM_POST = 6,  /* a11 epilogue: odd-class unfold + scaling */
+    NUSHT_NUM_STAGES = 7
+};
+
+typedef struct {
+    int lmax, mmax, dtype;
+    int64_t npts, nlm;
+    double eps;
+    int n_rings;        /* N_r: Clenshaw-Curtis rings theta_k = pi k/(N_r-1), k = 0..N_r-1 */
+    int n_theta;        /* doubled length 2 (N_r - 1) (App. B; reading G4) */
+    int n_theta_fine;   /* up-sampled grid, theta direction (covers [0, 2 pi)) */
+    int n_phi_fine;     /* up-sampled grid, phi direction */
+    int kernel_width;   /* w: taps per dimension of the exponential-of-semicircle kernel */
+    int kernel_degree;  /* degree of the piecewise polynomial that evaluates it */
+    double kernel_beta; /* phi_ES(z) = exp(beta (sqrt(1 - z^2) - 1)) */
+    double sigma;       /* up-sampling factor */
+    int64_t workspace_bytes; /* device memory owned by the plan */
+    double plan_ms;     /* wall time of nusht_plan (sort + tables + cuFFT plans) */
+} nusht_info_t;
+
+/* Build a plan: choose grid sizes / kernel width from (lmax, mmax, eps), build recurrence and
+ * deconvolution tables, counting-sort the points into strips (planning is done
+ * before, and excluded from, the transforms).  Synchronous; may synchronise the device.
+ *   lmax >= 0, 0 <= mmax <= lmax, 0 <= npts < 2^31, dtype NUSHT_F64 | NUSHT_F32,
+ *   eps in [1e-13, 1e-1] (F64) or [1e-6, 1e-1] (F32); theta/phi DEVICE pointers (may be NULL iff npts == 0). */
+NUSHT_API int nusht_plan(nusht_plan_t** out, int lmax, int mmax, int64_t npts, const double* theta,
+               const double* phi, double eps, int dtype);
+
+/* Synthesis, Eq. 3 / Eq. 5: alm (DEVICE, nlm complex) -> map (DEVICE, npts real).  npts == 0: no-op. */
+NUSHT_API int nusht_synthesis(nusht_plan_t* plan, const void* alm, void* map, void* stream);
+
+/* Adjoint, Eq. 2 / Eq. 6: map (DEVICE, npts real) -> alm (DEVICE, nlm complex, overwritten).
+ * npts == 0: alm is set to zero. */
+NUSHT_API int nusht_adjoint(nusht_plan_t* plan, const void* map, void* alm, void* stream);
+
+/* Free the plan and everything it owns.  NULL is accepted. */
+NUSHT_API int nusht_destroy(nusht_plan_t* plan);
+
+/* Same transforms with HOST buffers (pinned or pageable): the call copies the input to a
+ * plan-owned device buffer, runs the transform, copies the result back, all on `stream`, and
+ * returns without synchronising (the caller synchronises the stream before reading the output). */
+NUSHT_API int nusht_synthesis_host(nusht_plan_t* plan, const void* alm_host, void* map_host, void* stream);
+NUSHT_API int nusht_adjoint_host(nusht_plan_t* plan, const void* map_host, void* alm_host, void* stream);
+
+/* Stage entry points (tests and per-stage measurement).
+ * Legendre synthesis + DFS doubling alone: alm -> Ftilde, DEVICE complex128
+ * [(mmax+1)][n_theta], theta-contiguous:
+ *   Ftilde[m][r] = F_m(theta_r) for r < N_r,  (-1)^m F_m(theta_{n_theta - r}) for r >= N_r  (Fig. 1).
+ * Its transpose (a10-a11): Gtilde (same layout) -> alm. */
+NUSHT_API int nusht_stage_legendre_synthesis(nusht_plan_t* plan, const void* alm, void* ftilde, void* stream);
+NUSHT_API int nusht_stage_legendre_adjoint(nusht_plan_t* plan, const void* gtilde, void* alm, void* stream);
+/* nuFFT stages alone (a7 / a8) on the plan's half fine grid: DEVICE real [n_theta_fine/2 + 1][n_phi_fine]
+ * of the plan's dtype; rows outside [0, pi] are reached through the DFS mirror symmetry.
+ * interp reads `grid`, writes `map`; spread zeroes `grid` then accumulates `map` into it. */
+NUSHT_API int nusht_stage_interp(nusht_plan_t* plan, const void* grid, void* map, void* stream);
+NUSHT_API int nusht_stage_spread(nusht_plan_t* plan, const void* map, void* grid, void* stream);
+
+/* Per-stage CUDA-event timing.  enable != 0 makes every following synthesis/adjoint record events
+ * around each stage (no extra synchronisation).  nusht_stage_times synchronises the events of the
+ * last call of kind `which` (0 synthesis, 1 adjoint) and writes up to n (<= NUSHT_NUM_STAGES) times in ms. */
+NUSHT_API int nusht_set_stage_timing(nusht_plan_t* plan, int enable);
+NUSHT_API int nusht_stage_times(nusht_plan_t* plan, int which, float* ms, int n);
+
+NUSHT_API int nusht_plan_info(const nusht_plan_t* plan, nusht_info_t* info);
+NUSHT_API const char* nusht_strerror(int code);
+/* Library version string, e.g. "nusht-b200 0.1 (sm_100a)". */
+NUSHT_API const char* nusht_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NUSHT_H */

@@ -1,0 +1,271 @@
+// api.cu -- the C ABI of libnusht.so (include/nusht.h): plan construction, the two transforms,
+// stage entry points, timing.  Orchestration only; the arithmetic lives in legendre.cu,
+// fourier.cu and nufft.cu.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <chrono>
+#include <new>
+
+#include "nusht_internal.cuh"
+
+static thread_local char g_last_error[512] = "";
+
+void nusht_note_cuda_error(cudaError_t e, const char* what, const char* file, int line) {
+    snprintf(g_last_error, sizeof(g_last_error), "CUDA error %d (%s) at %s:%d: %s", (int)e, cudaGetErrorString(e),
+             file, line, what);
+    if (getenv("NUSHT_VERBOSE")) fprintf(stderr, "[nusht] %s\n", g_last_error);
+    cudaGetLastError();   // clear the sticky-free error state
+}
+void nusht_note_cufft_error(int r, const char* what, const char* file, int line) {
+    snprintf(g_last_error, sizeof(g_last_error), "cuFFT error %d at %s:%d: %s", r, file, line, what);
+    if (getenv("NUSHT_VERBOSE")) fprintf(stderr, "[nusht] %s\n", g_last_error);
+}
+
+// smallest even n >= nmin whose only prime factors are 2, 3, 5, 7 (App. B "good numbers")
+static int good_even_size(int nmin) {
+    int n = nmin + (nmin & 1);
+    for (;; n += 2) {
+        int k = n;
+        for (int pr : {2, 3, 5, 7})
+            while (k % pr == 0) k /= pr;
+        if (k == 1) return n;
+    }
+}
+
+extern "C" const char* nusht_version(void) { return "nusht-b200 0.1 (sm_100a)"; }
+
+extern "C" const char* nusht_strerror(int code) {
+    switch (code) {
+        case NUSHT_OK: return "ok";
+        case NUSHT_ERR_INVALID_ARG: return "invalid argument";
+        case NUSHT_ERR_ALLOC: return "allocation failed";
+        case NUSHT_ERR_CUDA: return g_last_error[0] ? g_last_error : "CUDA error";
+        case NUSHT_ERR_CUFFT: return g_last_error[0] ? g_last_error : "cuFFT error";
+        case NUSHT_ERR_UNSUPPORTED: return "unsupported request";
+        case NUSHT_ERR_BAD_POINTS: return "bad point coordinates (NaN/Inf or theta outside [0, pi])";
+    }
+    return "unknown status";
+}
+
+static void plan_release(nusht_plan_s* p) {
+    if (!p) return;
+    legendre_free(p);
+    fourier_free(p);
+    nufft_free(p);
+    cudaFree(p->d_stage_alm);
+    cudaFree(p->d_stage_map);
+    for (int k = 0; k < 2; ++k)
+        for (int i = 0; i <= NUSHT_NUM_STAGES; ++i)
+            if (p->ev[k][i]) cudaEventDestroy(p->ev[k][i]);
+    delete p;
+}
+
+extern "C" int nusht_destroy(nusht_plan_t* plan) {
+    plan_release(plan);
+    return NUSHT_OK;
+}
+
+extern "C" int nusht_plan(nusht_plan_t** out, int lmax, int mmax, int64_t npts, const double* theta,
+                          const double* phi, double eps, int dtype) {
+    if (!out) return NUSHT_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (lmax < 0 || mmax < 0 || mmax > lmax || npts < 0 || npts >= ((int64_t)1 << 31)) return NUSHT_ERR_INVALID_ARG;
+    if (dtype != NUSHT_F64 && dtype != NUSHT_F32) return NUSHT_ERR_INVALID_ARG;
+    if (!(eps <= 1e-1)) return NUSHT_ERR_INVALID_ARG;
+    if (dtype == NUSHT_F64 && !(eps >= 1e-13)) return NUSHT_ERR_INVALID_ARG;
+    if (dtype == NUSHT_F32 && !(eps >= 1e-6)) return NUSHT_ERR_INVALID_ARG;
+    if (npts > 0 && (!theta || !phi)) return NUSHT_ERR_INVALID_ARG;
+    if (lmax > 32000) return NUSHT_ERR_UNSUPPORTED;
+
+    const auto t0 = std::chrono::steady_clock::now();
+    int dev = 0;
+    NUSHT_CUDA_TRY(cudaGetDevice(&dev));
+
+    nusht_plan_s* p = new (std::nothrow) nusht_plan_s();
+    if (!p) return NUSHT_ERR_ALLOC;
+    p->lmax = lmax;
+    p->mmax = mmax;
+    p->npts = npts;
+    p->eps = eps;
+    p->dtype = dtype;
+    p->device = dev;
+    p->nlm = (int64_t)(mmax + 1) * (lmax + 1) - (int64_t)mmax * (mmax + 1) / 2;
+
+    int st = nufft_choose_kernel(p);
+    if (st == NUSHT_OK) {
+        // Clenshaw-Curtis rings: N_r >= lmax + 2 with the doubled length 2 (N_r - 1) a good FFT size (reading G4/G5)
+        const int nth2 = good_even_size(2 * (lmax + 1));
+        p->lg.lmax = lmax;
+        p->lg.mmax = mmax;
+        p->lg.nth2 = nth2;
+        p->lg.nr = nth2 / 2 + 1;
+        p->lg.npairs = (p->lg.nr + 1) / 2;
+        p->lg.has_equator = p->lg.nr & 1;
+        // fine grid: up-sampling sigma = 2 of the 2 lmax + 2 (2 mmax + 2) Fourier modes (reading G7)
+        const int w = p->ng.w;
+        int nth = 2 * (2 * lmax + 2), nph = 2 * (2 * mmax + 2);
+        if (nth < 2 * w + 2) nth = 2 * w + 2;
+        if (nph < 2 * w + 2) nph = 2 * w + 2;
+        p->ng.nth = good_even_size(nth);
+        p->ng.nph = good_even_size(nph);
+        p->ng.nrow_half = p->ng.nth / 2 + 1;
+        st = legendre_build_tables(p);
+    }
+    if (st == NUSHT_OK) st = fourier_build(p);
+    if (st == NUSHT_OK) st = nufft_sort_points(p, theta, phi);
+    if (st == NUSHT_OK) {
+        for (int k = 0; k < 2 && st == NUSHT_OK; ++k)
+            for (int i = 0; i <= NUSHT_NUM_STAGES; ++i)
+                if (cudaEventCreate(&p->ev[k][i]) != cudaSuccess) {
+                    st = NUSHT_ERR_CUDA;
+                    break;
+                }
+    }
+    if (st == NUSHT_OK && cudaDeviceSynchronize() != cudaSuccess) st = NUSHT_ERR_CUDA;
+    if (st != NUSHT_OK) {
+        plan_release(p);
+        return st;
+    }
+    p->plan_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    *out = p;
+    return NUSHT_OK;
+}
+
+extern "C" int nusht_plan_info(const nusht_plan_t* p, nusht_info_t* info) {
+    if (!p || !info) return NUSHT_ERR_INVALID_ARG;
+    memset(info, 0, sizeof(*info));
+    info->lmax = p->lmax;
+    info->mmax = p->mmax;
+    info->dtype = p->dtype;
+    info->npts = p->npts;
+    info->nlm = p->nlm;
+    info->eps = p->eps;
+    info->n_rings = p->lg.nr;
+    info->n_theta = p->lg.nth2;
+    info->n_theta_fine = p->ng.nth;
+    info->n_phi_fine = p->ng.nph;
+    info->kernel_width = p->ng.w;
+    info->kernel_degree = p->ng.deg;
+    info->kernel_beta = p->beta;
+    info->sigma = p->sigma;
+    info->workspace_bytes = p->workspace_bytes;
+    info->plan_ms = p->plan_ms;
+    return NUSHT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// transforms
+// ---------------------------------------------------------------------------------------------
+#define STAGE_MARK(kind, i)                                                    \
+    do {                                                                       \
+        if (p->timing) NUSHT_CUDA_TRY(cudaEventRecord(p->ev[(kind)][(i)], s)); \
+    } while (0)
+
+static size_t real_size(const nusht_plan_s* p) { return p->dtype == NUSHT_F64 ? 8 : 4; }
+
+extern "C" int nusht_synthesis(nusht_plan_t* p, const void* alm, void* map, void* stream) {
+    if (!p || !alm || (!map && p->npts > 0)) return NUSHT_ERR_INVALID_ARG;
+    if (p->npts == 0) return NUSHT_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaEvent_t fev[5];
+    STAGE_MARK(0, 0);
+    NUSHT_TRY(legendre_alm_prep(p, alm, s));
+    STAGE_MARK(0, 1);
+    NUSHT_TRY(legendre_synthesis(p, p->d_ft, s));
+    // stages 2..5 are bracketed inside fourier_synthesis: ev[2] .. ev[6]
+    for (int i = 0; i < 5; ++i) fev[i] = p->ev[0][2 + i];
+    NUSHT_TRY(fourier_synthesis(p, s, p->timing ? fev : nullptr));
+    NUSHT_TRY(nufft_interp(p, p->d_grid, map, s));
+    STAGE_MARK(0, 7);
+    if (p->timing) p->ev_valid[0] = true;
+    return NUSHT_OK;
+}
+
+extern "C" int nusht_adjoint(nusht_plan_t* p, const void* map, void* alm, void* stream) {
+    if (!p || !alm || (!map && p->npts > 0)) return NUSHT_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (p->npts == 0) {
+        NUSHT_CUDA_TRY(cudaMemsetAsync(alm, 0, (size_t)p->nlm * 2 * real_size(p), s));
+        return NUSHT_OK;
+    }
+    cudaEvent_t fev[5];
+    STAGE_MARK(1, 0);
+    NUSHT_TRY(nufft_spread(p, map, p->d_grid, s));
+    // stages 1..4 are bracketed inside fourier_adjoint: ev[1] .. ev[5]
+    for (int i = 0; i < 5; ++i) fev[i] = p->ev[1][1 + i];
+    NUSHT_TRY(fourier_adjoint(p, s, p->timing ? fev : nullptr));
+    NUSHT_TRY(legendre_adjoint(p, p->d_ft, s));
+    STAGE_MARK(1, 6);
+    NUSHT_TRY(legendre_alm_post(p, alm, s));
+    STAGE_MARK(1, 7);
+    if (p->timing) p->ev_valid[1] = true;
+    return NUSHT_OK;
+}
+
+extern "C" int nusht_synthesis_host(nusht_plan_t* p, const void* alm_host, void* map_host, void* stream) {
+    if (!p || !alm_host || (!map_host && p->npts > 0)) return NUSHT_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t abytes = (size_t)p->nlm * 2 * real_size(p), mbytes = (size_t)p->npts * real_size(p);
+    if (!p->d_stage_alm) NUSHT_CUDA_TRY(cudaMalloc(&p->d_stage_alm, abytes ? abytes : 16));
+    if (!p->d_stage_map) NUSHT_CUDA_TRY(cudaMalloc(&p->d_stage_map, mbytes ? mbytes : 16));
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_stage_alm, alm_host, abytes, cudaMemcpyHostToDevice, s));
+    NUSHT_TRY(nusht_synthesis(p, p->d_stage_alm, p->d_stage_map, stream));
+    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(map_host, p->d_stage_map, mbytes, cudaMemcpyDeviceToHost, s));
+    return NUSHT_OK;
+}
+
+extern "C" int nusht_adjoint_host(nusht_plan_t* p, const void* map_host, void* alm_host, void* stream) {
+    if (!p || !alm_host || (!map_host && p->npts > 0)) return NUSHT_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t abytes = (size_t)p->nlm * 2 * real_size(p), mbytes = (size_t)p->npts * real_size(p);
+    if (!p->d_stage_alm) NUSHT_CUDA_TRY(cudaMalloc(&p->d_stage_alm, abytes ? abytes : 16));
+    if (!p->d_stage_map) NUSHT_CUDA_TRY(cudaMalloc(&p->d_stage_map, mbytes ? mbytes : 16));
+    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_stage_map, map_host, mbytes, cudaMemcpyHostToDevice, s));
+    NUSHT_TRY(nusht_adjoint(p, p->d_stage_map, p->d_stage_alm, stream));
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(alm_host, p->d_stage_alm, abytes, cudaMemcpyDeviceToHost, s));
+    return NUSHT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// stage entry points
+// ---------------------------------------------------------------------------------------------
+extern "C" int nusht_stage_legendre_synthesis(nusht_plan_t* p, const void* alm, void* ftilde, void* stream) {
+    if (!p || !alm || !ftilde) return NUSHT_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    NUSHT_TRY(legendre_alm_prep(p, alm, s));
+    return legendre_synthesis(p, (double2*)ftilde, s);
+}
+
+extern "C" int nusht_stage_legendre_adjoint(nusht_plan_t* p, const void* gtilde, void* alm, void* stream) {
+    if (!p || !alm || !gtilde) return NUSHT_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    NUSHT_TRY(legendre_adjoint(p, (const double2*)gtilde, s));
+    return legendre_alm_post(p, alm, s);
+}
+
+extern "C" int nusht_stage_interp(nusht_plan_t* p, const void* grid, void* map, void* stream) {
+    if (!p || !grid || (!map && p->npts > 0)) return NUSHT_ERR_INVALID_ARG;
+    return nufft_interp(p, grid, map, (cudaStream_t)stream);
+}
+
+extern "C" int nusht_stage_spread(nusht_plan_t* p, const void* map, void* grid, void* stream) {
+    if (!p || !grid || (!map && p->npts > 0)) return NUSHT_ERR_INVALID_ARG;
+    return nufft_spread(p, map, grid, (cudaStream_t)stream);
+}
+
+extern "C" int nusht_set_stage_timing(nusht_plan_t* p, int enable) {
+    if (!p) return NUSHT_ERR_INVALID_ARG;
+    p->timing = enable ? 1 : 0;
+    if (!enable) p->ev_valid[0] = p->ev_valid[1] = false;
+    return NUSHT_OK;
+}
+
+extern "C" int nusht_stage_times(nusht_plan_t* p, int which, float* ms, int n) {
+    if (!p || !ms || which < 0 || which > 1 || n < 0 || n > NUSHT_NUM_STAGES) return NUSHT_ERR_INVALID_ARG;
+    if (!p->ev_valid[which]) return NUSHT_ERR_INVALID_ARG;
+    NUSHT_CUDA_TRY(cudaEventSynchronize(p->ev[which][NUSHT_NUM_STAGES]));
+    for (int i = 0; i < n; ++i) NUSHT_CUDA_TRY(cudaEventElapsedTime(&ms[i], p->ev[which][i], p->ev[which][i + 1]));
+    return NUSHT_OK;
+}

@@ -1,0 +1,246 @@
+// fourier.cu -- uniform-FFT part of the nuSHT (operator F and the grid side of N; arXiv
+// 2406.14542 Eq. 5-6).
+//
+// Only the theta FFT of F survives: the phi FFTs of S and F cancel, so the Legendre
+// stage hands over Ftilde[m][r] in m-space and
+//   a3  c[m,k]  = (1/Ntheta) sum_r Ftilde[m][r] e^{-2 pi i k r/Ntheta},  |k| <= lmax       (cuFFT)
+//   a4  B[m][k mod n_theta] = c[m,k] p_theta(k) p_phi(m), zero elsewhere   (deconvolve + zero-pad)
+//   a5  H[m][a] = sum_k B[m][k] e^{+2 pi i k a/n_theta}                                  (cuFFT)
+//       g[a][b] = sum_m w_m Re(H[m][a] e^{+2 pi i m b/n_phi}),  rows a = 0..n_theta/2   (cuFFT C2R)
+// and the adjoint (a9) runs the transposed chain: R2C, zero-extend in theta, forward FFT, truncate
+// and deconvolve with the SAME factors, inverse FFT of length Ntheta.
+// p(k) = 1/psihat(k): psihat is the Fourier transform of the piecewise-polynomial kernel that the
+// interpolation actually evaluates (nufft.cu), so p is exact for that kernel.
+// cuFFT is used for the FFTs only; everything else here is our own kernels.
+#include <math.h>
+#include <stdio.h>
+
+#include <vector>
+
+#include "nusht_internal.cuh"
+
+namespace {
+
+template <typename T> struct Cplx;
+template <> struct Cplx<double> { using type = double2; };
+template <> struct Cplx<float> { using type = float2; };
+
+// a4: one thread per fine-grid theta frequency slot k' of column m
+template <typename T>
+__global__ void k_deconv_pad(int L, int M, int nth2, int nth, const double2* __restrict__ ft,
+                             const double* __restrict__ pth, const double* __restrict__ pph,
+                             typename Cplx<T>::type* __restrict__ h) {
+    const int kp = blockIdx.x * blockDim.x + threadIdx.x;
+    const int m = blockIdx.y;
+    if (kp >= nth) return;
+    int k;
+    bool in = true;
+    if (kp <= L) k = kp;
+    else if (kp >= nth - L) k = kp - nth;
+    else { k = 0; in = false; }
+    typename Cplx<T>::type out;
+    out.x = 0;
+    out.y = 0;
+    if (in) {
+        const double2 c = ft[(int64_t)m * nth2 + (k >= 0 ? k : k + nth2)];
+        const double f = pth[k + L] * pph[m];
+        out.x = (T)(c.x * f);
+        out.y = (T)(c.y * f);
+    }
+    h[(int64_t)m * nth + kp] = out;
+}
+
+// a9: truncate to |k| <= lmax and deconvolve; one thread per slot r of the doubled-ring spectrum
+template <typename T>
+__global__ void k_deconv_trunc(int L, int M, int nth2, int nth, const typename Cplx<T>::type* __restrict__ h,
+                               const double* __restrict__ pth, const double* __restrict__ pph,
+                               double2* __restrict__ ft) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const int m = blockIdx.y;
+    if (r >= nth2) return;
+    int k;
+    bool in = true;
+    if (r <= L) k = r;
+    else if (r >= nth2 - L) k = r - nth2;
+    else { k = 0; in = false; }
+    double2 out = make_double2(0.0, 0.0);
+    if (in) {
+        const typename Cplx<T>::type c = h[(int64_t)m * nth + (k >= 0 ? k : k + nth)];
+        const double f = pth[k + L] * pph[m];
+        out.x = (double)c.x * f;
+        out.y = (double)c.y * f;
+    }
+    ft[(int64_t)m * nth2 + r] = out;
+}
+
+}  // namespace
+
+template <typename T>
+static int f_alloc(T** ptr, size_t bytes, nusht_plan_s* p) {
+    if (bytes == 0) bytes = 16;
+    NUSHT_CUDA_TRY(cudaMalloc((void**)ptr, bytes));
+    p->workspace_bytes += (int64_t)bytes;
+    return NUSHT_OK;
+}
+
+int fourier_build(nusht_plan_s* p) {
+    const int L = p->lmax, M = p->mmax;
+    const NufftGeom& g = p->ng;
+    const int nth2 = p->lg.nth2;
+    const bool f64 = p->dtype == NUSHT_F64;
+    const size_t csz = f64 ? 16 : 8, rsz = f64 ? 8 : 4;
+
+    // deconvolution tables (host, extended precision inside nufft_kernel_ft); 1/Ntheta folded into p_theta
+    std::vector<double> pth(2 * L + 1), pph(M + 1);
+    for (int k = 0; k <= L; ++k) {
+        const double v = 1.0 / (nufft_kernel_ft(p, (double)k, g.nth) * (double)nth2);
+        pth[L + k] = v;
+        pth[L - k] = v;
+    }
+    for (int m = 0; m <= M; ++m) pph[m] = 1.0 / nufft_kernel_ft(p, (double)m, g.nph);
+    NUSHT_TRY(f_alloc(&p->d_pth, sizeof(double) * (2 * L + 1), p));
+    NUSHT_TRY(f_alloc(&p->d_pph, sizeof(double) * (M + 1), p));
+    NUSHT_CUDA_TRY(cudaMemcpy(p->d_pth, pth.data(), sizeof(double) * (2 * L + 1), cudaMemcpyHostToDevice));
+    NUSHT_CUDA_TRY(cudaMemcpy(p->d_pph, pph.data(), sizeof(double) * (M + 1), cudaMemcpyHostToDevice));
+
+    const size_t hbytes = (size_t)(g.nph / 2 + 1) * (size_t)g.nth * csz;
+    const size_t gbytes = (size_t)g.nrow_half * (size_t)g.nph * rsz;
+    NUSHT_TRY(f_alloc(&p->d_h, hbytes, p));
+    NUSHT_TRY(f_alloc(&p->d_grid, gbytes, p));
+    NUSHT_CUDA_TRY(cudaMemset(p->d_h, 0, hbytes));
+    NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
+
+    // cuFFT plans
+    size_t ws = 0, wtot = 0;
+    {
+        int n[1] = {nth2};
+        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_theta_coarse));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_coarse, 1, n, nullptr, 1, nth2, nullptr, 1, nth2, CUFFT_Z2Z,
+                                          M + 1, &ws));
+        wtot += ws;
+    }
+    {
+        int n[1] = {g.nth};
+        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_theta_fine));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_fine, 1, n, nullptr, 1, g.nth, nullptr, 1, g.nth,
+                                          f64 ? CUFFT_Z2Z : CUFFT_C2C, M + 1, &ws));
+        wtot += ws;
+    }
+    {
+        int n[1] = {g.nph};
+        int inembed[1] = {g.nph / 2 + 1}, onembed[1] = {g.nph};
+        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi_c2r));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_c2r, 1, n, inembed, g.nth, 1, onembed, 1, g.nph,
+                                          f64 ? CUFFT_Z2D : CUFFT_C2R, g.nrow_half, &ws));
+        wtot += ws;
+        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi_r2c));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_r2c, 1, n, onembed, 1, g.nph, inembed, g.nth, 1,
+                                          f64 ? CUFFT_D2Z : CUFFT_R2C, g.nrow_half, &ws));
+        wtot += ws;
+    }
+    p->workspace_bytes += (int64_t)wtot;
+    p->have_fft = true;
+    return NUSHT_OK;
+}
+
+#define REC(i)                                                   \
+    do {                                                         \
+        if (ev) NUSHT_CUDA_TRY(cudaEventRecord(ev[(i)], s));     \
+    } while (0)
+
+// synthesis: d_ft (Ftilde) -> d_grid.  ev (optional) = events at the boundaries of stages 2..5:
+// ev[0] before a3, ev[1] after a3, ev[2] after a4, ev[3] after a5-theta, ev[4] after a5-phi.
+int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
+    const int L = p->lmax, M = p->mmax;
+    const NufftGeom& g = p->ng;
+    const int nth2 = p->lg.nth2;
+    const bool f64 = p->dtype == NUSHT_F64;
+    const size_t csz = f64 ? 16 : 8;
+    REC(0);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_coarse, s));
+    NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_coarse, (cufftDoubleComplex*)p->d_ft, (cufftDoubleComplex*)p->d_ft,
+                                 CUFFT_FORWARD));
+    REC(1);
+    {
+        dim3 grid((g.nth + 255) / 256, M + 1);
+        if (f64)
+            k_deconv_pad<double><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, p->d_ft, p->d_pth, p->d_pph, (double2*)p->d_h);
+        else
+            k_deconv_pad<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, p->d_ft, p->d_pth, p->d_pph, (float2*)p->d_h);
+        NUSHT_CUDA_TRY(cudaGetLastError());
+        // rows m > mmax of H must be zero for the C2R; cuFFT may clobber its input, so re-zero them
+        const size_t tail = (size_t)(g.nph / 2 - M) * (size_t)g.nth * csz;
+        NUSHT_CUDA_TRY(cudaMemsetAsync((char*)p->d_h + (size_t)(M + 1) * g.nth * csz, 0, tail, s));
+    }
+    REC(2);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_fine, s));
+    if (f64)
+        NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_fine, (cufftDoubleComplex*)p->d_h, (cufftDoubleComplex*)p->d_h,
+                                     CUFFT_INVERSE));
+    else
+        NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_theta_fine, (cufftComplex*)p->d_h, (cufftComplex*)p->d_h, CUFFT_INVERSE));
+    REC(3);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi_c2r, s));
+    if (f64)
+        NUSHT_CUFFT_TRY(cufftExecZ2D(p->fft_phi_c2r, (cufftDoubleComplex*)p->d_h, (cufftDoubleReal*)p->d_grid));
+    else
+        NUSHT_CUFFT_TRY(cufftExecC2R(p->fft_phi_c2r, (cufftComplex*)p->d_h, (cufftReal*)p->d_grid));
+    REC(4);
+    return NUSHT_OK;
+}
+
+// adjoint: d_grid -> d_ft (Gtilde).  ev[0] before R2C, ev[1] after R2C, ev[2] after fine theta FFT,
+// ev[3] after truncate/deconvolve, ev[4] after the coarse inverse FFT.
+int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
+    const int L = p->lmax, M = p->mmax;
+    const NufftGeom& g = p->ng;
+    const int nth2 = p->lg.nth2;
+    const bool f64 = p->dtype == NUSHT_F64;
+    const size_t csz = f64 ? 16 : 8;
+    REC(0);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi_r2c, s));
+    if (f64)
+        NUSHT_CUFFT_TRY(cufftExecD2Z(p->fft_phi_r2c, (cufftDoubleReal*)p->d_grid, (cufftDoubleComplex*)p->d_h));
+    else
+        NUSHT_CUFFT_TRY(cufftExecR2C(p->fft_phi_r2c, (cufftReal*)p->d_grid, (cufftComplex*)p->d_h));
+    // transpose of "keep rows 0..n_theta/2 of the theta FFT output": zero-extend to the full period
+    if (g.nth - g.nrow_half > 0)
+        NUSHT_CUDA_TRY(cudaMemset2DAsync((char*)p->d_h + (size_t)g.nrow_half * csz, (size_t)g.nth * csz, 0,
+                                         (size_t)(g.nth - g.nrow_half) * csz, (size_t)(M + 1), s));
+    REC(1);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_fine, s));
+    if (f64)
+        NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_fine, (cufftDoubleComplex*)p->d_h, (cufftDoubleComplex*)p->d_h,
+                                     CUFFT_FORWARD));
+    else
+        NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_theta_fine, (cufftComplex*)p->d_h, (cufftComplex*)p->d_h, CUFFT_FORWARD));
+    REC(2);
+    {
+        dim3 grid((nth2 + 255) / 256, M + 1);
+        if (f64)
+            k_deconv_trunc<double><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, (const double2*)p->d_h, p->d_pth, p->d_pph,
+                                                        p->d_ft);
+        else
+            k_deconv_trunc<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, (const float2*)p->d_h, p->d_pth, p->d_pph,
+                                                       p->d_ft);
+        NUSHT_CUDA_TRY(cudaGetLastError());
+    }
+    REC(3);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_coarse, s));
+    NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_coarse, (cufftDoubleComplex*)p->d_ft, (cufftDoubleComplex*)p->d_ft,
+                                 CUFFT_INVERSE));
+    REC(4);
+    return NUSHT_OK;
+}
+#undef REC
+
+void fourier_free(nusht_plan_s* p) {
+    if (p->fft_theta_coarse) cufftDestroy(p->fft_theta_coarse);
+    if (p->fft_theta_fine) cufftDestroy(p->fft_theta_fine);
+    if (p->fft_phi_c2r) cufftDestroy(p->fft_phi_c2r);
+    if (p->fft_phi_r2c) cufftDestroy(p->fft_phi_r2c);
+    p->fft_theta_coarse = p->fft_theta_fine = p->fft_phi_c2r = p->fft_phi_r2c = 0;
+    cudaFree(p->d_pth); cudaFree(p->d_pph); cudaFree(p->d_h); cudaFree(p->d_grid);
+    p->d_pth = p->d_pph = nullptr;
+    p->d_h = p->d_grid = nullptr;
+}

@@ -1,0 +1,730 @@
+// legendre.cu -- ring Legendre stage of the nuSHT (operators S, D and their transposes; arXiv
+// 2406.14542 Eq. 5-6).
+//
+//   synthesis:  F_m(theta_k) = sum_{l=m}^{lmax} a_lm Pbar_lm(theta_k) on the Clenshaw-Curtis rings
+//               theta_k = pi k/(N_r-1), written directly in doubled (DFS) form
+//               Ftilde[m][r] = F_m(theta_r) (r < N_r),  (-1)^m F_m(theta_{Ntheta-r}) (r >= N_r).
+//   adjoint:    c_lm = sum_k Pbar_lm(theta_k) G_m[k],  G = fold(Gtilde)  (no quadrature weights).
+//
+// Pbar_lm is generated on the fly with the x^2-stepping recurrence of the paper's
+// ref. [42] (Ishioka 2018), derived here from  x Pbar_l = c_{l+1} Pbar_{l+1} + c_l Pbar_{l-1},
+// c_l^2 = (l^2-m^2)/(4 l^2-1):
+//   even class  q_n = Pbar_{m+2n}:   q_{n+1} = A_n (x^2 - D_n) q_n - C_n q_{n-1}
+//   scaled      q_n = sigma_n qh_n:  qh_{n+1} = (alpha_n x^2 + beta_n) qh_n + qh_{n-1}      (2 FMA)
+//   odd class   Pbar_{m+2n+1} = (x q_n - c_{m+2n} Pbar_{m+2n-1})/c_{m+2n+1}  is folded into the
+//               coefficients once per transform (O(lmax^2)):  sum_n b_n Pbar_{m+2n+1} =
+//               x sum_j (r_j/c_{m+2j+1}) q_j,  r_j = b_j - rho_j r_{j+1},  rho_j = c_{m+2j+2}/c_{m+2j+3}.
+// One thread owns R north/south ring pairs (Pbar_lm(pi-theta) = (-1)^{l+m} Pbar_lm(theta)): per pair
+// and per two l it issues 2 FMA of recurrence and 4 FMA of accumulation.  Underflow of
+// Pbar_mm ~ sin^m(theta) is handled with a per-pair power-of-two exponent counter: while it is
+// positive the pair is "dead" (true value < 2^-232) and contributes nothing.
+//
+// The CPU oracle (oracle/) uses the plain three-term recurrence in l and shares nothing with this file.
+#include <math.h>
+#include <stdio.h>
+
+#include <vector>
+
+#include "nusht_internal.cuh"
+
+namespace {
+
+constexpr int LEG_THREADS = 128;   // 4 warps
+constexpr int LEG_WARPS = LEG_THREADS / 32;
+constexpr int LEG_TN = 128;        // n-steps (pairs of l) per shared-memory tile
+constexpr int LEG_CHUNK = 8;       // n-steps between exponent checks
+constexpr int LEG_R = 4;           // ring pairs per thread
+constexpr double SCALE_UP_LIMIT = 1.157920892373162e+77;   // 2^256
+constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
+
+struct LegParams {
+    int lmax, mmax, nr, nth2, npairs, has_equator;
+    const int64_t* eoff;
+    const double2* ab;
+    const double* x2;
+    const double* x;
+    const double2* logsin;
+    const double2* logkap;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra.uni WAIT_DONE;\n"
+        "bra.uni WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// TMA 1-D bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
+// plan-time tables, one thread per m (sequential in n: sigma is a two-step product)
+// ---------------------------------------------------------------------------------------------
+__global__ void k_legendre_tables(int L, int M, const int64_t* __restrict__ eoff, double2* __restrict__ ab,
+                                  double* __restrict__ sig, double* __restrict__ sodd, double* __restrict__ rho) {
+    int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m > M) return;
+    const int ne = (L - m) / 2 + 1;
+    const int64_t o = eoff[m];
+    auto c2 = [m](int l) -> double {   // c_l^2, exact integer numerator/denominator
+        double num = (double)((long long)(l - m) * (long long)(l + m));
+        double den = 4.0 * (double)l * (double)l - 1.0;
+        return num / den;
+    };
+    double sg_prev = 0.0, sg = 1.0;
+    for (int n = 0; n < ne; ++n) {
+        const int l = m + 2 * n;
+        const double c2l = (n == 0) ? 0.0 : c2(l);
+        const double c2lm1 = (n == 0) ? 0.0 : c2(l - 1);
+        const double c2l1 = c2(l + 1), c2l2 = c2(l + 2), c2l3 = c2(l + 3);
+        const double A = 1.0 / sqrt(c2l1 * c2l2);
+        const double D = c2l1 + c2l;
+        const double C = sqrt(c2l * c2lm1) * A;
+        const double sg_next = (n == 0) ? 1.0 : -C * sg_prev;
+        const double alpha = A * sg / sg_next;
+        ab[o + n] = make_double2(alpha, -alpha * D);
+        sig[o + n] = sg;
+        sodd[o + n] = sg / sqrt(c2l1);
+        rho[o + n] = sqrt(c2l2 / c2l3);
+        sg_prev = sg;
+        sg = sg_next;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1 prologue: alm -> (ae, ao): even-class scaling and odd-class fold, one thread per m.
+//   ae_j = a_{m+2j} sigma_j;   r_j = a_{m+2j+1} - rho_j r_{j+1};   ao_j = r_j sodd_j
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void k_alm_prep(int L, int M, const int64_t* __restrict__ eoff, const T* __restrict__ alm,
+                           const double* __restrict__ sig, const double* __restrict__ sodd,
+                           const double* __restrict__ rho, double4* __restrict__ aeo) {
+    int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m > M) return;
+    const int ne = (L - m) / 2 + 1;
+    const int no = (L - m + 1) / 2;
+    const int64_t o = eoff[m];
+    const T* col = alm + 2 * ((int64_t)m * (2 * L + 1 - m) / 2);   // col[2*l], col[2*l+1] for l >= m
+    double rre = 0.0, rim = 0.0;
+    for (int j = ne - 1; j >= 0; --j) {
+        const int le = m + 2 * j;
+        double bre = 0.0, bim = 0.0;
+        if (j < no) {
+            bre = (double)col[2 * (le + 1)];
+            bim = (double)col[2 * (le + 1) + 1];
+        }
+        const double rh = rho[o + j];
+        rre = fma(-rh, rre, bre);
+        rim = fma(-rh, rim, bim);
+        const double sg = sig[o + j], so = sodd[o + j];
+        double4 v;
+        v.x = (double)col[2 * le] * sg;
+        v.y = (double)col[2 * le + 1] * sg;
+        v.z = rre * so;
+        v.w = rim * so;
+        if (m == 0) { v.y = 0.0; v.w = 0.0; }   // Im(a_l0) is ignored (G3)
+        aeo[o + j] = v;
+    }
+}
+
+// a11 epilogue: (e~, o~) -> alm.  c_{m+2n} = sigma_n e~_n;  u_n = sodd_n o~_n;
+//   v_n = u_n - rho_{n-1} v_{n-1};  c_{m+2n+1} = v_n   (transpose of the fold above).
+template <typename T>
+__global__ void k_alm_post(int L, int M, const int64_t* __restrict__ eoff, const double4* __restrict__ eo,
+                           const double* __restrict__ sig, const double* __restrict__ sodd,
+                           const double* __restrict__ rho, T* __restrict__ alm) {
+    int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m > M) return;
+    const int ne = (L - m) / 2 + 1;
+    const int no = (L - m + 1) / 2;
+    const int64_t o = eoff[m];
+    T* col = alm + 2 * ((int64_t)m * (2 * L + 1 - m) / 2);
+    double vre = 0.0, vim = 0.0, rprev = 0.0;
+    for (int n = 0; n < ne; ++n) {
+        const double4 v = eo[o + n];
+        const double sg = sig[o + n], so = sodd[o + n];
+        const int le = m + 2 * n;
+        col[2 * le] = (T)(v.x * sg);
+        col[2 * le + 1] = (m == 0) ? (T)0 : (T)(v.y * sg);
+        vre = fma(-rprev, vre, v.z * so);
+        vim = fma(-rprev, vim, v.w * so);
+        if (n < no) {
+            col[2 * (le + 1)] = (T)vre;
+            col[2 * (le + 1) + 1] = (m == 0) ? (T)0 : (T)vim;
+        }
+        rprev = rho[o + n];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// per-pair seed: qh_0 = Pbar_mm(theta_j) = (-1)^m 2^(lk_m + m log2 sin theta_j), as p * 2^(-512 e)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void seed_pair(const LegParams& P, int m, int j, bool valid, double& p, int& e) {
+    p = 0.0;
+    e = 0;
+    if (!valid) return;
+    const double2 lk = P.logkap[m];
+    if (m == 0) {
+        p = exp2(lk.x + lk.y);
+        return;
+    }
+    if (j == 0) return;   // poles: sin(theta) = 0, Pbar_lm = 0 for m > 0
+    const double2 ls = P.logsin[j];
+    const double dm = (double)m;
+    // (mh + err) = m * ls.x exactly;  s = mh + lk.x with two-sum error err2
+    const double mh = dm * ls.x;
+    const double err = fma(dm, ls.x, -mh);
+    const double s = mh + lk.x;
+    const double bb = s - mh;
+    const double err2 = (mh - (s - bb)) + (lk.x - bb);
+    const double low = err + err2 + fma(dm, ls.y, lk.y);
+    int ee = 0;
+    if (s < -800.0) ee = (int)floor((-s + 256.0) * (1.0 / 512.0));
+    const double expo = s + 512.0 * (double)ee;      // exact: s has < 2^16 magnitude
+    const double ip = rint(expo);
+    const double fr = (expo - ip) + low;
+    p = scalbn(exp2(fr), (int)ip);
+    if (m & 1) p = -p;
+    e = ee;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1 + a2: Legendre synthesis with fused DFS doubling.  grid = (pair blocks, m).
+// ---------------------------------------------------------------------------------------------
+template <int R>
+__global__ void __launch_bounds__(LEG_THREADS)
+k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restrict__ ft) {
+    __shared__ __align__(16) double2 s_ab[2][LEG_TN];
+    __shared__ __align__(32) double4 s_aeo[2][LEG_TN];
+    __shared__ __align__(8) uint64_t s_bar[2];
+
+    const int m = blockIdx.y;
+    const int L = P.lmax;
+    const int ne = (L - m) / 2 + 1;
+    const int64_t o = P.eoff[m];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int jb = (blockIdx.x * LEG_WARPS + warp) * (32 * R);
+    const int ntiles = (ne + LEG_TN - 1) / LEG_TN;
+
+    if (tid == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int tile) {
+        const int st = tile & 1;
+        const int cnt = min(LEG_TN, ne - tile * LEG_TN);
+        mbar_expect_tx(&s_bar[st], (uint32_t)cnt * 48u);
+        bulk_g2s(&s_ab[st][0], P.ab + o + (int64_t)tile * LEG_TN, (uint32_t)cnt * 16u, &s_bar[st]);
+        bulk_g2s(&s_aeo[st][0], aeo + o + (int64_t)tile * LEG_TN, (uint32_t)cnt * 32u, &s_bar[st]);
+    };
+    if (tid == 0) {
+        issue(0);
+        if (ntiles > 1) issue(1);
+    }
+
+    double x2[R], p0[R], p1[R], ere[R], eim[R], ore_[R], oim[R];
+    int ex[R];
+    bool valid[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jb + r * 32 + lane;
+        valid[r] = j < P.npairs;
+        x2[r] = valid[r] ? P.x2[j] : 0.0;
+        seed_pair(P, m, j, valid[r], p1[r], ex[r]);
+        p0[r] = 0.0;
+        ere[r] = eim[r] = ore_[r] = oim[r] = 0.0;
+    }
+    const bool warp_has_work = jb < P.npairs;
+
+    for (int tile = 0; tile < ntiles; ++tile) {
+        const int st = tile & 1;
+        const int cnt = min(LEG_TN, ne - tile * LEG_TN);
+        mbar_wait(&s_bar[st], (uint32_t)((tile >> 1) & 1));
+        if (warp_has_work) {
+            for (int i0 = 0; i0 < cnt; i0 += LEG_CHUNK) {
+                const int ns = min(LEG_CHUNK, cnt - i0);
+                bool any_dead = false, any_live = false;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    any_dead |= (ex[r] > 0);
+                    any_live |= (valid[r] && ex[r] == 0);
+                }
+                const bool w_dead = __any_sync(0xffffffffu, any_dead);
+                const bool w_live = __any_sync(0xffffffffu, any_live);
+                if (!w_dead) {
+                    // all pairs live: 6 FMA per pair per step, no checks
+                    if (ns == LEG_CHUNK) {
+#pragma unroll
+                        for (int i = 0; i < LEG_CHUNK; ++i) {
+                            const double2 ab = s_ab[st][i0 + i];
+                            const double4 c = s_aeo[st][i0 + i];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double t = fma(ab.x, x2[r], ab.y);
+                                ere[r] = fma(c.x, p1[r], ere[r]);
+                                eim[r] = fma(c.y, p1[r], eim[r]);
+                                ore_[r] = fma(c.z, p1[r], ore_[r]);
+                                oim[r] = fma(c.w, p1[r], oim[r]);
+                                const double pn = fma(t, p1[r], p0[r]);
+                                p0[r] = p1[r];
+                                p1[r] = pn;
+                            }
+                        }
+                    } else {
+                        for (int i = 0; i < ns; ++i) {
+                            const double2 ab = s_ab[st][i0 + i];
+                            const double4 c = s_aeo[st][i0 + i];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double t = fma(ab.x, x2[r], ab.y);
+                                ere[r] = fma(c.x, p1[r], ere[r]);
+                                eim[r] = fma(c.y, p1[r], eim[r]);
+                                ore_[r] = fma(c.z, p1[r], ore_[r]);
+                                oim[r] = fma(c.w, p1[r], oim[r]);
+                                const double pn = fma(t, p1[r], p0[r]);
+                                p0[r] = p1[r];
+                                p1[r] = pn;
+                            }
+                        }
+                    }
+                } else {
+                    if (w_live) {
+                        // mixed: pairs that were live at the start of the chunk accumulate
+                        for (int i = 0; i < ns; ++i) {
+                            const double2 ab = s_ab[st][i0 + i];
+                            const double4 c = s_aeo[st][i0 + i];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double t = fma(ab.x, x2[r], ab.y);
+                                const double pm = (ex[r] == 0) ? p1[r] : 0.0;
+                                ere[r] = fma(c.x, pm, ere[r]);
+                                eim[r] = fma(c.y, pm, eim[r]);
+                                ore_[r] = fma(c.z, pm, ore_[r]);
+                                oim[r] = fma(c.w, pm, oim[r]);
+                                const double pn = fma(t, p1[r], p0[r]);
+                                p0[r] = p1[r];
+                                p1[r] = pn;
+                            }
+                        }
+                    } else {
+                        // every pair of the warp still below range: recurrence only (2 FMA)
+                        for (int i = 0; i < ns; ++i) {
+                            const double2 ab = s_ab[st][i0 + i];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double t = fma(ab.x, x2[r], ab.y);
+                                const double pn = fma(t, p1[r], p0[r]);
+                                p0[r] = p1[r];
+                                p1[r] = pn;
+                            }
+                        }
+                    }
+                    // exponent bookkeeping once per chunk: growth over 8 steps is < 2^32
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        if (ex[r] > 0 && fabs(p1[r]) > SCALE_UP_LIMIT) {
+                            p1[r] *= SCALE_DOWN;
+                            p0[r] *= SCALE_DOWN;
+                            ex[r] -= 1;
+                        }
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        if (tid == 0 && tile + 2 < ntiles) issue(tile + 2);
+    }
+
+    if (!warp_has_work) return;
+    // a2: fused DFS doubling (Fig. 1): north = E + x O, south = E - x O;
+    // mirror rows carry (-1)^m (phi -> phi + pi).
+    const double sgn = (m & 1) ? -1.0 : 1.0;
+    double2* row = ft + (int64_t)m * P.nth2;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jb + r * 32 + lane;
+        if (!valid[r]) continue;
+        const double x = P.x[j];
+        const double2 nv = make_double2(fma(x, ore_[r], ere[r]), fma(x, oim[r], eim[r]));
+        const double2 sv = make_double2(fma(-x, ore_[r], ere[r]), fma(-x, oim[r], eim[r]));
+        const int ks = P.nr - 1 - j;   // south ring index
+        row[j] = nv;
+        if (j != 0) row[P.nth2 - j] = make_double2(sgn * nv.x, sgn * nv.y);
+        if (ks != j) {
+            row[ks] = sv;
+            if (j != 0) row[P.nth2 - ks] = make_double2(sgn * sv.x, sgn * sv.y);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a10 + a11: fold + adjoint Legendre.  One CTA per m, looping over blocks of ring pairs; per
+// n-step every thread forms 4 partial sums over its R pairs, 8 steps x 4 sums are reduced across
+// the warp with a 31-shuffle transposing butterfly, across warps through shared memory, and
+// accumulated into eo[m][n] by the CTA itself (deterministic, no atomics).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double shfl_xor_d(double v, int mask) {
+    return __shfl_xor_sync(0xffffffffu, v, mask);
+}
+
+// v[0..31] per lane -> lane l returns sum over lanes of v[l]
+__device__ __forceinline__ double warp_transpose_reduce32(double (&v)[32], int lane) {
+#pragma unroll
+    for (int half = 16; half >= 1; half >>= 1) {
+        const bool up = (lane & half) != 0;
+#pragma unroll
+        for (int i = 0; i < half; ++i) {
+            const double keep = up ? v[i + half] : v[i];
+            const double send = up ? v[i] : v[i + half];
+            v[i] = keep + shfl_xor_d(send, half);
+        }
+    }
+    return v[0];
+}
+
+template <int R>
+__global__ void __launch_bounds__(LEG_THREADS)
+k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restrict__ eo) {
+    __shared__ __align__(16) double2 s_ab[2][LEG_TN];
+    __shared__ __align__(16) double s_red[LEG_WARPS][LEG_TN * 4];
+    __shared__ __align__(8) uint64_t s_bar[2];
+
+    const int m = blockIdx.x;
+    const int L = P.lmax;
+    const int ne = (L - m) / 2 + 1;
+    const int64_t o = P.eoff[m];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ntiles = (ne + LEG_TN - 1) / LEG_TN;
+    const int pairs_per_pass = LEG_THREADS * R;
+    const int npass = (P.npairs + pairs_per_pass - 1) / pairs_per_pass;
+    const double sgn = (m & 1) ? -1.0 : 1.0;
+    const double2* row = gt + (int64_t)m * P.nth2;
+
+    if (tid == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int tile) {
+        const int st = tile & 1;
+        const int cnt = min(LEG_TN, ne - tile * LEG_TN);
+        mbar_expect_tx(&s_bar[st], (uint32_t)cnt * 16u);
+        bulk_g2s(&s_ab[st][0], P.ab + o + (int64_t)tile * LEG_TN, (uint32_t)cnt * 16u, &s_bar[st]);
+    };
+    uint32_t uses[2] = {0u, 0u};   // completed phases of each stage's mbarrier (same in every thread)
+
+    for (int pass = 0; pass < npass; ++pass) {
+        const int jb = pass * pairs_per_pass + warp * (32 * R);
+        const bool warp_has_work = jb < P.npairs;
+        double x2[R], p0[R], p1[R], gere[R], geim[R], gore[R], goim[R];
+        int ex[R];
+        bool valid[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int j = jb + r * 32 + lane;
+            valid[r] = j < P.npairs;
+            x2[r] = valid[r] ? P.x2[j] : 0.0;
+            seed_pair(P, m, j, valid[r], p1[r], ex[r]);
+            p0[r] = 0.0;
+            gere[r] = geim[r] = gore[r] = goim[r] = 0.0;
+            if (valid[r]) {
+                // a10 fold (D^T): G[k] = Gt[k] + (-1)^m Gt[Ntheta-k] away from the poles
+                const int kn = j, ks = P.nr - 1 - j;
+                double2 gn = row[kn];
+                if (kn != 0) {
+                    const double2 t = row[P.nth2 - kn];
+                    gn.x = fma(sgn, t.x, gn.x);
+                    gn.y = fma(sgn, t.y, gn.y);
+                }
+                double2 gs = make_double2(0.0, 0.0);
+                if (ks != kn) {
+                    gs = row[ks];
+                    if (kn != 0) {
+                        const double2 t = row[P.nth2 - ks];
+                        gs.x = fma(sgn, t.x, gs.x);
+                        gs.y = fma(sgn, t.y, gs.y);
+                    }
+                }
+                const double x = P.x[j];
+                gere[r] = gn.x + gs.x;
+                geim[r] = gn.y + gs.y;
+                gore[r] = x * (gn.x - gs.x);
+                goim[r] = x * (gn.y - gs.y);
+            }
+        }
+        if (tid == 0) {
+            // the two stages are free here: every tile of the previous pass was consumed
+            issue(0);
+            if (ntiles > 1) issue(1);
+        }
+        for (int tile = 0; tile < ntiles; ++tile) {
+            const int st = tile & 1;
+            const int cnt = min(LEG_TN, ne - tile * LEG_TN);
+            mbar_wait(&s_bar[st], uses[st] & 1u);
+            uses[st] += 1u;
+            if (warp_has_work) {
+                for (int i0 = 0; i0 < cnt; i0 += LEG_CHUNK) {
+                    const int ns = min(LEG_CHUNK, cnt - i0);
+                    bool any_dead = false, any_live = false;
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        any_dead |= (ex[r] > 0);
+                        any_live |= (valid[r] && ex[r] == 0);
+                    }
+                    const bool w_dead = __any_sync(0xffffffffu, any_dead);
+                    const bool w_live = __any_sync(0xffffffffu, any_live);
+                    if (w_live) {
+                        double v[32];
+#pragma unroll
+                        for (int q = 0; q < 32; ++q) v[q] = 0.0;
+                        if (!w_dead && ns == LEG_CHUNK) {
+#pragma unroll
+                            for (int i = 0; i < LEG_CHUNK; ++i) {
+                                const double2 ab = s_ab[st][i0 + i];
+#pragma unroll
+                                for (int r = 0; r < R; ++r) {
+                                    const double t = fma(ab.x, x2[r], ab.y);
+                                    v[4 * i + 0] = fma(p1[r], gere[r], v[4 * i + 0]);
+                                    v[4 * i + 1] = fma(p1[r], geim[r], v[4 * i + 1]);
+                                    v[4 * i + 2] = fma(p1[r], gore[r], v[4 * i + 2]);
+                                    v[4 * i + 3] = fma(p1[r], goim[r], v[4 * i + 3]);
+                                    const double pn = fma(t, p1[r], p0[r]);
+                                    p0[r] = p1[r];
+                                    p1[r] = pn;
+                                }
+                            }
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < LEG_CHUNK; ++i) {
+                                const bool on = i < ns;
+                                const double2 ab = s_ab[st][min(i0 + i, LEG_TN - 1)];
+#pragma unroll
+                                for (int r = 0; r < R; ++r) {
+                                    const double t = fma(ab.x, x2[r], ab.y);
+                                    const double pm = (on && ex[r] == 0) ? p1[r] : 0.0;
+                                    v[4 * i + 0] = fma(pm, gere[r], v[4 * i + 0]);
+                                    v[4 * i + 1] = fma(pm, geim[r], v[4 * i + 1]);
+                                    v[4 * i + 2] = fma(pm, gore[r], v[4 * i + 2]);
+                                    v[4 * i + 3] = fma(pm, goim[r], v[4 * i + 3]);
+                                    if (on) {
+                                        const double pn = fma(t, p1[r], p0[r]);
+                                        p0[r] = p1[r];
+                                        p1[r] = pn;
+                                    }
+                                }
+                            }
+                        }
+                        const double tot = warp_transpose_reduce32(v, lane);
+                        s_red[warp][4 * i0 + lane] = tot;
+                    } else {
+                        for (int i = 0; i < ns; ++i) {
+                            const double2 ab = s_ab[st][i0 + i];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double t = fma(ab.x, x2[r], ab.y);
+                                const double pn = fma(t, p1[r], p0[r]);
+                                p0[r] = p1[r];
+                                p1[r] = pn;
+                            }
+                        }
+                        s_red[warp][4 * i0 + lane] = 0.0;
+                    }
+                    if (w_dead) {
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            if (ex[r] > 0 && fabs(p1[r]) > SCALE_UP_LIMIT) {
+                                p1[r] *= SCALE_DOWN;
+                                p0[r] *= SCALE_DOWN;
+                                ex[r] -= 1;
+                            }
+                        }
+                    }
+                }
+            } else if (tile == 0) {
+                // idle warp in this pass: its slice must read as zero for every tile of the pass
+                for (int q = lane; q < 4 * LEG_TN; q += 32) s_red[warp][q] = 0.0;
+            }
+            __syncthreads();
+            // cross-warp sum of this tile and accumulation into eo (same thread -> same address every pass)
+            {
+                double* out = reinterpret_cast<double*>(eo + o + (int64_t)tile * LEG_TN);
+                for (int q = tid; q < 4 * cnt; q += LEG_THREADS) {
+                    double sum = 0.0;
+#pragma unroll
+                    for (int wq = 0; wq < LEG_WARPS; ++wq) sum += s_red[wq][q];
+                    if (pass == 0) out[q] = sum;
+                    else out[q] += sum;
+                }
+            }
+            __syncthreads();
+            if (tid == 0 && tile + 2 < ntiles) issue(tile + 2);
+        }
+    }
+}
+
+}  // namespace
+
+// =============================================================================================
+// host side
+// =============================================================================================
+static LegParams make_params(const nusht_plan_s* p) {
+    LegParams P;
+    P.lmax = p->lmax;
+    P.mmax = p->mmax;
+    P.nr = p->lg.nr;
+    P.nth2 = p->lg.nth2;
+    P.npairs = p->lg.npairs;
+    P.has_equator = p->lg.has_equator;
+    P.eoff = p->d_eoff;
+    P.ab = p->d_ab;
+    P.x2 = p->d_x2;
+    P.x = p->d_x;
+    P.logsin = p->d_logsin;
+    P.logkap = p->d_logkap;
+    return P;
+}
+
+template <typename T>
+static int dev_alloc(T** ptr, size_t count, nusht_plan_s* p) {
+    size_t bytes = count * sizeof(T);
+    if (bytes == 0) bytes = sizeof(T);
+    NUSHT_CUDA_TRY(cudaMalloc((void**)ptr, bytes));
+    p->workspace_bytes += (int64_t)bytes;
+    return NUSHT_OK;
+}
+
+int legendre_build_tables(nusht_plan_s* p) {
+    const int L = p->lmax, M = p->mmax;
+    const LegendreGeom& g = p->lg;
+    // column offsets
+    std::vector<int64_t> eoff(M + 2);
+    int64_t acc = 0;
+    for (int m = 0; m <= M; ++m) {
+        eoff[m] = acc;
+        acc += (L - m) / 2 + 1;
+    }
+    eoff[M + 1] = acc;
+    p->n_e_total = acc;
+    NUSHT_TRY(dev_alloc(&p->d_eoff, (size_t)M + 2, p));
+    NUSHT_CUDA_TRY(cudaMemcpy(p->d_eoff, eoff.data(), sizeof(int64_t) * (M + 2), cudaMemcpyHostToDevice));
+    NUSHT_TRY(dev_alloc(&p->d_ab, (size_t)acc, p));
+    NUSHT_TRY(dev_alloc(&p->d_sig, (size_t)acc, p));
+    NUSHT_TRY(dev_alloc(&p->d_sodd, (size_t)acc, p));
+    NUSHT_TRY(dev_alloc(&p->d_rho, (size_t)acc, p));
+    NUSHT_TRY(dev_alloc(&p->d_aeo, (size_t)acc, p));
+    NUSHT_TRY(dev_alloc(&p->d_ft, (size_t)(M + 1) * (size_t)g.nth2, p));
+    {
+        const int threads = 32;
+        k_legendre_tables<<<(M + 1 + threads - 1) / threads, threads>>>(L, M, p->d_eoff, p->d_ab, p->d_sig,
+                                                                         p->d_sodd, p->d_rho);
+        NUSHT_CUDA_TRY(cudaGetLastError());
+    }
+    // ring tables in extended precision on the host: theta_j = pi j/(nr-1)
+    const long double PI_L = 3.14159265358979323846264338327950288L;
+    std::vector<double> x2(g.npairs), x(g.npairs);
+    std::vector<double2> ls(g.npairs);
+    for (int j = 0; j < g.npairs; ++j) {
+        long double th = PI_L * (long double)j / (long double)(g.nr - 1);
+        long double c = cosl(th), s = sinl(th);
+        if (g.has_equator && j == g.npairs - 1) c = 0.0L;
+        x[j] = (double)c;
+        x2[j] = (double)(c * c);
+        if (j == 0) {
+            ls[j] = make_double2(0.0, 0.0);   // unused: poles are special-cased
+        } else {
+            long double v = log2l(s);
+            double hi = (double)v;
+            ls[j] = make_double2(hi, (double)(v - (long double)hi));
+        }
+    }
+    std::vector<double2> lk(M + 1);
+    {
+        long double v = -0.5L * log2l(4.0L * PI_L);
+        for (int m = 0; m <= M; ++m) {
+            if (m > 0) v += 0.5L * log2l((long double)(2 * m + 1) / (long double)(2 * m));
+            double hi = (double)v;
+            lk[m] = make_double2(hi, (double)(v - (long double)hi));
+        }
+    }
+    NUSHT_TRY(dev_alloc(&p->d_x2, (size_t)g.npairs, p));
+    NUSHT_TRY(dev_alloc(&p->d_x, (size_t)g.npairs, p));
+    NUSHT_TRY(dev_alloc(&p->d_logsin, (size_t)g.npairs, p));
+    NUSHT_TRY(dev_alloc(&p->d_logkap, (size_t)M + 1, p));
+    NUSHT_CUDA_TRY(cudaMemcpy(p->d_x2, x2.data(), sizeof(double) * g.npairs, cudaMemcpyHostToDevice));
+    NUSHT_CUDA_TRY(cudaMemcpy(p->d_x, x.data(), sizeof(double) * g.npairs, cudaMemcpyHostToDevice));
+    NUSHT_CUDA_TRY(cudaMemcpy(p->d_logsin, ls.data(), sizeof(double2) * g.npairs, cudaMemcpyHostToDevice));
+    NUSHT_CUDA_TRY(cudaMemcpy(p->d_logkap, lk.data(), sizeof(double2) * (M + 1), cudaMemcpyHostToDevice));
+    NUSHT_CUDA_TRY(cudaDeviceSynchronize());
+    return NUSHT_OK;
+}
+
+int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s) {
+    const int threads = 32, blocks = (p->mmax + 1 + threads - 1) / threads;
+    if (p->dtype == NUSHT_F64)
+        k_alm_prep<double><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, (const double*)alm, p->d_sig,
+                                                      p->d_sodd, p->d_rho, p->d_aeo);
+    else
+        k_alm_prep<float><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, (const float*)alm, p->d_sig,
+                                                     p->d_sodd, p->d_rho, p->d_aeo);
+    NUSHT_CUDA_TRY(cudaGetLastError());
+    return NUSHT_OK;
+}
+
+int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s) {
+    const int pairs_per_cta = LEG_THREADS * LEG_R;
+    dim3 grid((p->lg.npairs + pairs_per_cta - 1) / pairs_per_cta, p->mmax + 1);
+    k_legendre_synth<LEG_R><<<grid, LEG_THREADS, 0, s>>>(make_params(p), p->d_aeo, ft);
+    NUSHT_CUDA_TRY(cudaGetLastError());
+    return NUSHT_OK;
+}
+
+int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
+    k_legendre_adjoint<LEG_R><<<p->mmax + 1, LEG_THREADS, 0, s>>>(make_params(p), gt, p->d_aeo);
+    NUSHT_CUDA_TRY(cudaGetLastError());
+    return NUSHT_OK;
+}
+
+int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s) {
+    const int threads = 32, blocks = (p->mmax + 1 + threads - 1) / threads;
+    if (p->dtype == NUSHT_F64)
+        k_alm_post<double><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, p->d_aeo, p->d_sig, p->d_sodd,
+                                                      p->d_rho, (double*)alm);
+    else
+        k_alm_post<float><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, p->d_aeo, p->d_sig, p->d_sodd,
+                                                     p->d_rho, (float*)alm);
+    NUSHT_CUDA_TRY(cudaGetLastError());
+    return NUSHT_OK;
+}
+
+void legendre_free(nusht_plan_s* p) {
+    cudaFree(p->d_eoff); cudaFree(p->d_ab); cudaFree(p->d_sig); cudaFree(p->d_sodd); cudaFree(p->d_rho);
+    cudaFree(p->d_aeo); cudaFree(p->d_ft); cudaFree(p->d_x2); cudaFree(p->d_x); cudaFree(p->d_logsin);
+    cudaFree(p->d_logkap);
+    p->d_eoff = nullptr; p->d_ab = nullptr; p->d_sig = p->d_sodd = p->d_rho = nullptr; p->d_aeo = nullptr;
+    p->d_ft = nullptr; p->d_x2 = p->d_x = nullptr; p->d_logsin = p->d_logkap = nullptr;
+}

@@ -1,0 +1,135 @@
+// nusht_internal.cuh -- plan object and stage launchers shared by the translation units of
+// libnusht.so.  Nothing here is visible across the C ABI (include/nusht.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+
+#include "../../include/nusht.h"
+
+#define NUSHT_CUDA_TRY(expr)                                   \
+    do {                                                       \
+        cudaError_t _e = (expr);                               \
+        if (_e != cudaSuccess) {                               \
+            nusht_note_cuda_error(_e, #expr, __FILE__, __LINE__); \
+            return (_e == cudaErrorMemoryAllocation) ? NUSHT_ERR_ALLOC : NUSHT_ERR_CUDA; \
+        }                                                      \
+    } while (0)
+
+#define NUSHT_CUFFT_TRY(expr)                                  \
+    do {                                                       \
+        cufftResult _r = (expr);                               \
+        if (_r != CUFFT_SUCCESS) {                             \
+            nusht_note_cufft_error((int)_r, #expr, __FILE__, __LINE__); \
+            return (_r == CUFFT_ALLOC_FAILED) ? NUSHT_ERR_ALLOC : NUSHT_ERR_CUFFT; \
+        }                                                      \
+    } while (0)
+
+#define NUSHT_TRY(expr)              \
+    do {                             \
+        int _s = (expr);             \
+        if (_s != NUSHT_OK) return _s; \
+    } while (0)
+
+void nusht_note_cuda_error(cudaError_t e, const char* what, const char* file, int line);
+void nusht_note_cufft_error(int r, const char* what, const char* file, int line);
+
+// ---- nuFFT geometry ------------------------------------------------------------------------
+constexpr int NUSHT_MAX_W = 16;          // kernel width limit (eps = 1e-13 -> w = 14)
+constexpr int NUSHT_MAX_DEG = 17;        // polynomial degree limit (degree = w)
+constexpr int NUSHT_SEG_ROWS = 128;      // theta rows of patch origins per work item (strip segment)
+
+struct NufftGeom {
+    int nth, nph;        // fine grid (theta covers [0, 2 pi), phi covers [0, 2 pi))
+    int nrow_half;       // nth/2 + 1 stored rows (theta in [0, pi])
+    int w, fl;           // kernel width, floor(w/2)
+    int deg;             // polynomial degree
+    int mb;              // strip width in patch-origin columns = 33 - w
+    int nstrip;          // ceil(nph / mb)
+    int nseg;            // ceil((nth/2 + 2) / NUSHT_SEG_ROWS)
+    double inv_hth, inv_hph;  // nth/(2 pi), nph/(2 pi)
+};
+
+// ---- Legendre geometry ---------------------------------------------------------------------
+struct LegendreGeom {
+    int lmax, mmax;
+    int nr;              // rings on [0, pi]
+    int nth2;            // doubled length 2 (nr - 1)
+    int npairs;          // ring pairs (north j, south nr-1-j): ceil(nr/2)
+    int has_equator;     // nr odd: last pair is the equator ring alone
+};
+
+struct nusht_plan_s {
+    int lmax = 0, mmax = 0, dtype = 0;
+    int64_t npts = 0, nlm = 0;
+    double eps = 0, sigma = 2.0, beta = 0;
+    int device = 0;
+    LegendreGeom lg{};
+    NufftGeom ng{};
+    int64_t workspace_bytes = 0;
+    double plan_ms = 0;
+
+    // --- Legendre tables (device) ---
+    int64_t* d_eoff = nullptr;      // [mmax+2] offsets of column m in the per-(m,n) tables
+    int64_t n_e_total = 0;          // sum_m ne(m)
+    double2* d_ab = nullptr;        // (alpha_n, beta_n) of the x^2-stepping recurrence
+    double* d_sig = nullptr;        // sigma_n: even-class scaling
+    double* d_sodd = nullptr;       // sigma_n / c_{m+2n+1}: odd-class scaling
+    double* d_rho = nullptr;        // c_{m+2n+2}/c_{m+2n+3}: odd-class fold ratio
+    double* d_x2 = nullptr;         // cos^2(theta_j) per ring pair
+    double* d_x = nullptr;          // cos(theta_j)
+    double2* d_logsin = nullptr;    // log2 sin(theta_j) as (hi, lo)
+    double2* d_logkap = nullptr;    // log2 |Pbar_mm| prefactor per m as (hi, lo)
+    // --- Legendre work buffers ---
+    double4* d_aeo = nullptr;       // scaled coefficients per (m,n): (ae.re, ae.im, ao.re, ao.im)
+    double2* d_ft = nullptr;        // Ftilde / Gtilde: [mmax+1][nth2] complex128
+    // --- Fourier stage ---
+    double* d_pth = nullptr;        // deconvolution factors p_theta(k), k = -lmax..lmax
+    double* d_pph = nullptr;        // p_phi(m), m = 0..mmax
+    void* d_h = nullptr;            // fine half-spectrum [nph/2+1][nth] complex (dtype)
+    void* d_grid = nullptr;         // fine real grid [nth/2+1][nph] (dtype)
+    cufftHandle fft_theta_coarse = 0;  // Z2Z, length nth2, batch mmax+1
+    cufftHandle fft_theta_fine = 0;    // C2C (dtype), length nth, batch mmax+1
+    cufftHandle fft_phi_c2r = 0;       // C2R (dtype), length nph, batch nth/2+1, strided input
+    cufftHandle fft_phi_r2c = 0;       // R2C (dtype), strided output
+    bool have_fft = false;
+    // --- points ---
+    double* d_px = nullptr;         // sorted theta in fine-grid units
+    double* d_py = nullptr;         // sorted phi in fine-grid units
+    int* d_perm = nullptr;          // sorted position -> caller index
+    int* d_item_off = nullptr;      // [nseg*nstrip + 1] start of each (segment, strip) work item
+    int* d_item_order = nullptr;    // work items sorted by decreasing point count
+    int n_items = 0;
+    void* kernel_host = nullptr;    // nufft.cu: host model of the kernel polynomial
+    // --- host-buffer staging (allocated on first use of *_host) ---
+    void* d_stage_alm = nullptr;
+    void* d_stage_map = nullptr;
+    // --- stage timing ---
+    int timing = 0;
+    cudaEvent_t ev[2][NUSHT_NUM_STAGES + 1] = {};
+    bool ev_valid[2] = {false, false};
+};
+
+// ---- legendre.cu ----
+int legendre_build_tables(nusht_plan_s* p);
+int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s);
+int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s);
+int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s);
+int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s);
+void legendre_free(nusht_plan_s* p);
+
+// ---- fourier.cu ----
+int fourier_build(nusht_plan_s* p);
+int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev);   // ft -> grid
+int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev);     // grid -> ft
+void fourier_free(nusht_plan_s* p);
+
+// ---- nufft.cu ----
+int nufft_choose_kernel(nusht_plan_s* p);   // w, beta, degree, polynomial + deconvolution tables
+int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi);
+int nufft_interp(nusht_plan_s* p, const void* grid, void* map, cudaStream_t s);
+int nufft_spread(nusht_plan_s* p, const void* map, void* grid, cudaStream_t s);
+void nufft_free(nusht_plan_s* p);
+// host-side kernel model used by fourier_build: Fourier transform of the piecewise-polynomial kernel
+double nufft_kernel_ft(const nusht_plan_s* p, double k, int n);

@@ -1,0 +1,213 @@
+"""Thin ctypes binding of libnusht.so (include/nusht.h): same names, argument marshalling only.
+
+Every step of the transform runs in the CUDA library; torch is used for device memory and streams.
+There is no CPU fallback: if the library has not been built, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libnusht.so")
+
+NUSHT_F64, NUSHT_F32 = 0, 1
+NUSHT_OK = 0
+NUM_STAGES = 7
+SYN_STAGES = ["alm_prep", "legendre", "fft_theta", "deconv_pad", "fft_fine_theta", "fft_fine_phi", "interp"]
+ADJ_STAGES = ["spread", "fft_fine_phi", "fft_fine_theta", "deconv_trunc", "fft_theta", "legendre", "alm_post"]
+EXPORTS = [
+    "nusht_plan", "nusht_synthesis", "nusht_adjoint", "nusht_destroy", "nusht_synthesis_host",
+    "nusht_adjoint_host", "nusht_stage_legendre_synthesis", "nusht_stage_legendre_adjoint",
+    "nusht_stage_interp", "nusht_stage_spread", "nusht_set_stage_timing", "nusht_stage_times",
+    "nusht_plan_info", "nusht_strerror", "nusht_version",
+]
+
+
+class NushtInfo(ctypes.Structure):
+    _fields_ = [
+        ("lmax", ctypes.c_int), ("mmax", ctypes.c_int), ("dtype", ctypes.c_int),
+        ("npts", ctypes.c_int64), ("nlm", ctypes.c_int64), ("eps", ctypes.c_double),
+        ("n_rings", ctypes.c_int), ("n_theta", ctypes.c_int), ("n_theta_fine", ctypes.c_int),
+        ("n_phi_fine", ctypes.c_int), ("kernel_width", ctypes.c_int), ("kernel_degree", ctypes.c_int),
+        ("kernel_beta", ctypes.c_double), ("sigma", ctypes.c_double),
+        ("workspace_bytes", ctypes.c_int64), ("plan_ms", ctypes.c_double),
+    ]
+
+
+class NushtError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("nusht error %d: %s" % (code, msg))
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(_LIBPATH):
+        raise ImportError(
+            "libnusht.so is not built (run `python -m paper_2406_14542_b200.build`); there is no CPU fallback")
+    lib = ctypes.CDLL(_LIBPATH)
+    vp, ip = ctypes.c_void_p, ctypes.c_int
+    lib.nusht_plan.argtypes = [ctypes.POINTER(vp), ip, ip, ctypes.c_int64, vp, vp, ctypes.c_double, ip]
+    for name in ("nusht_synthesis", "nusht_adjoint", "nusht_synthesis_host", "nusht_adjoint_host",
+                 "nusht_stage_legendre_synthesis", "nusht_stage_legendre_adjoint", "nusht_stage_interp",
+                 "nusht_stage_spread"):
+        getattr(lib, name).argtypes = [vp, vp, vp, vp]
+        getattr(lib, name).restype = ip
+    lib.nusht_plan.restype = ip
+    lib.nusht_destroy.argtypes = [vp]
+    lib.nusht_destroy.restype = ip
+    lib.nusht_set_stage_timing.argtypes = [vp, ip]
+    lib.nusht_set_stage_timing.restype = ip
+    lib.nusht_stage_times.argtypes = [vp, ip, ctypes.POINTER(ctypes.c_float), ip]
+    lib.nusht_stage_times.restype = ip
+    lib.nusht_plan_info.argtypes = [vp, ctypes.POINTER(NushtInfo)]
+    lib.nusht_plan_info.restype = ip
+    lib.nusht_strerror.argtypes = [ip]
+    lib.nusht_strerror.restype = ctypes.c_char_p
+    lib.nusht_version.restype = ctypes.c_char_p
+    return lib
+
+
+lib = _load()
+
+
+def _check(code):
+    if code != NUSHT_OK:
+        raise NushtError(code, lib.nusht_strerror(code).decode())
+
+
+def version() -> str:
+    return lib.nusht_version().decode()
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+class Plan:
+    """nusht_plan(lmax, mmax, npts, theta, phi, eps, dtype): theta/phi are CUDA float64 tensors."""
+
+    def __init__(self, lmax, mmax, theta, phi, eps, dtype="f64"):
+        self._h = ctypes.c_void_p()
+        self.dtype = NUSHT_F64 if dtype in ("f64", NUSHT_F64) else NUSHT_F32
+        npts = 0 if theta is None else int(theta.numel())
+        if npts:
+            if not (theta.is_cuda and phi.is_cuda and theta.dtype == torch.float64 and phi.dtype == torch.float64):
+                raise TypeError("theta/phi must be CUDA float64 tensors")
+            theta, phi = theta.contiguous(), phi.contiguous()
+            tp, pp = theta.data_ptr(), phi.data_ptr()
+        else:
+            tp = pp = None
+        _check(lib.nusht_plan(ctypes.byref(self._h), int(lmax), int(mmax), npts, tp, pp, float(eps), self.dtype))
+        self.info = NushtInfo()
+        _check(lib.nusht_plan_info(self._h, ctypes.byref(self.info)))
+        self.lmax, self.mmax, self.npts, self.nlm = int(lmax), int(mmax), npts, int(self.info.nlm)
+        self.rdtype = torch.float64 if self.dtype == NUSHT_F64 else torch.float32
+        self.cdtype = torch.complex128 if self.dtype == NUSHT_F64 else torch.complex64
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib.nusht_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # ---- marshalling helpers ----
+    def _alm_arg(self, alm, device=True):
+        if alm.dtype != self.cdtype or alm.numel() != self.nlm or alm.is_cuda != device or not alm.is_contiguous():
+            raise TypeError("alm must be a contiguous %s tensor of %d entries on %s"
+                            % (self.cdtype, self.nlm, "cuda" if device else "cpu"))
+        return alm.data_ptr()
+
+    def _map_arg(self, m, device=True):
+        if m.dtype != self.rdtype or m.numel() != self.npts or m.is_cuda != device or not m.is_contiguous():
+            raise TypeError("map must be a contiguous %s tensor of %d entries on %s"
+                            % (self.rdtype, self.npts, "cuda" if device else "cpu"))
+        return m.data_ptr() if self.npts else None
+
+    # ---- transforms ----
+    def synthesis(self, alm, out=None, stream=None):
+        if out is None:
+            out = torch.empty(self.npts, dtype=self.rdtype, device=alm.device)
+        _check(lib.nusht_synthesis(self._h, self._alm_arg(alm), self._map_arg(out), _stream_ptr(stream)))
+        return out
+
+    def adjoint(self, x, out=None, stream=None):
+        if out is None:
+            out = torch.empty(self.nlm, dtype=self.cdtype, device="cuda")
+        _check(lib.nusht_adjoint(self._h, self._map_arg(x), self._alm_arg(out), _stream_ptr(stream)))
+        return out
+
+    def synthesis_host(self, alm_host, out_host, stream=None):
+        _check(lib.nusht_synthesis_host(self._h, self._alm_arg(alm_host, False), self._map_arg(out_host, False),
+                                        _stream_ptr(stream)))
+        return out_host
+
+    def adjoint_host(self, x_host, out_host, stream=None):
+        _check(lib.nusht_adjoint_host(self._h, self._map_arg(x_host, False), self._alm_arg(out_host, False),
+                                      _stream_ptr(stream)))
+        return out_host
+
+    # ---- stages ----
+    def stage_legendre_synthesis(self, alm, stream=None):
+        out = torch.empty((self.mmax + 1, self.info.n_theta), dtype=torch.complex128, device="cuda")
+        _check(lib.nusht_stage_legendre_synthesis(self._h, self._alm_arg(alm), out.data_ptr(), _stream_ptr(stream)))
+        return out
+
+    def stage_legendre_adjoint(self, gt, stream=None):
+        if gt.dtype != torch.complex128 or tuple(gt.shape) != (self.mmax + 1, self.info.n_theta) or not gt.is_cuda:
+            raise TypeError("gtilde must be CUDA complex128 [(mmax+1), n_theta]")
+        out = torch.empty(self.nlm, dtype=self.cdtype, device="cuda")
+        _check(lib.nusht_stage_legendre_adjoint(self._h, gt.contiguous().data_ptr(), out.data_ptr(),
+                                                _stream_ptr(stream)))
+        return out
+
+    def grid_shape(self):
+        return (self.info.n_theta_fine // 2 + 1, self.info.n_phi_fine)
+
+    def stage_interp(self, grid, stream=None):
+        if grid.dtype != self.rdtype or tuple(grid.shape) != self.grid_shape() or not grid.is_cuda:
+            raise TypeError("grid must be CUDA %s %s" % (self.rdtype, self.grid_shape()))
+        out = torch.empty(self.npts, dtype=self.rdtype, device="cuda")
+        _check(lib.nusht_stage_interp(self._h, grid.contiguous().data_ptr(), self._map_arg(out), _stream_ptr(stream)))
+        return out
+
+    def stage_spread(self, x, stream=None):
+        out = torch.empty(self.grid_shape(), dtype=self.rdtype, device="cuda")
+        _check(lib.nusht_stage_spread(self._h, self._map_arg(x), out.data_ptr(), _stream_ptr(stream)))
+        return out
+
+    # ---- timing ----
+    def set_stage_timing(self, enable=True):
+        _check(lib.nusht_set_stage_timing(self._h, 1 if enable else 0))
+
+    def stage_times(self, which):
+        buf = (ctypes.c_float * NUM_STAGES)()
+        _check(lib.nusht_stage_times(self._h, 0 if which in (0, "synthesis") else 1, buf, NUM_STAGES))
+        names = SYN_STAGES if which in (0, "synthesis") else ADJ_STAGES
+        return {n: float(buf[i]) for i, n in enumerate(names)}
+
+
+def nusht_plan(lmax, mmax, npts, theta, phi, eps, dtype="f64"):
+    assert npts == (0 if theta is None else theta.numel())
+    return Plan(lmax, mmax, theta, phi, eps, dtype)
+
+
+def nusht_synthesis(plan, alm, map_out=None, stream=None):
+    return plan.synthesis(alm, map_out, stream)
+
+
+def nusht_adjoint(plan, x, alm_out=None, stream=None):
+    return plan.adjoint(x, alm_out, stream)
+
+
+def nusht_destroy(plan):
+    plan.destroy()

@@ -1,0 +1,200 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the ctypes binding) against the CPU
+oracle on the same seeded inputs.  Bars (BASELINE.json north_star): relative l2 error <= 10 eps in
+FP64 (Eq. 9-10), GPU adjointness <= 1e-12 relative."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from paper_2406_14542_b200 import inputs  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def nusht():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2406_14542_b200 import nusht as n
+    return n
+
+
+def rel(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def cu(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def ring_reference(oracle, L, M, alm, nr, nth2, prec="ld"):
+    """Doubled ring map from the oracle's ring_sum (a1 + a2 by their definition)."""
+    th = np.pi * np.arange(nr) / (nr - 1)
+    out = np.zeros((M + 1, nth2), dtype=np.complex128)
+    for m in range(M + 1):
+        lo = inputs.lm_index(L, m, m)
+        am = alm[lo: lo + L - m + 1].copy()
+        if m == 0:
+            am = am.real + 0j
+        F = oracle.ring_sum(L, m, th, am, prec)
+        out[m, :nr] = F
+        r = np.arange(nr, nth2)
+        out[m, nr:] = (-1) ** m * F[nth2 - r]
+    return out
+
+
+# ---- stage a1 + a2 -----------------------------------------------------------------------------
+@pytest.mark.parametrize("L,M", [(0, 0), (1, 1), (5, 3), (63, 63), (64, 64), (255, 200), (700, 700)])
+def test_legendre_synthesis_stage(nusht, oracle, L, M):
+    alm = inputs.random_alm(L, M, 21)
+    plan = nusht.Plan(L, M, None, None, 1e-10)
+    ft = plan.stage_legendre_synthesis(cu(alm)).cpu().numpy()
+    ref = ring_reference(oracle, L, M, alm, plan.info.n_rings, plan.info.n_theta)
+    assert rel(ft, ref) < 2e-12 * max(1.0, L / 100.0)
+    # per-m check so that a single bad column cannot hide in the norm
+    for m in range(M + 1):
+        assert np.linalg.norm(ft[m] - ref[m]) <= 1e-11 * max(1.0, L / 100.0) * (np.linalg.norm(ref[m]) + 1e-300) + 1e-13, m
+    plan.destroy()
+
+
+def test_legendre_synthesis_large_l_rescaling(nusht, oracle):
+    """lmax = 4095: Pbar_mm underflows binary64 for most (m, ring); sampled columns against the oracle."""
+    L = M = 4095
+    alm = inputs.random_alm(L, M, 22)
+    plan = nusht.Plan(L, M, None, None, 1e-10)
+    ft = plan.stage_legendre_synthesis(cu(alm)).cpu().numpy()
+    nr, nth2 = plan.info.n_rings, plan.info.n_theta
+    th = np.pi * np.arange(nr) / (nr - 1)
+    for m in [0, 1, 2, 37, 1000, 2047, 2048, 3000, 4000, 4094, 4095]:
+        lo = inputs.lm_index(L, m, m)
+        am = alm[lo: lo + L - m + 1].copy()
+        if m == 0:
+            am = am.real + 0j
+        F = oracle.ring_sum(L, m, th, am, "ld")
+        tol = 2e-10 if m < 3 else 5e-12     # low m: cos(theta)^2 rounding next to the poles
+        assert np.linalg.norm(ft[m, :nr] - F) <= tol * np.linalg.norm(F), m
+        r = np.arange(nr, nth2)
+        assert np.array_equal(ft[m, nr:], (-1) ** m * ft[m, nth2 - r]), m
+    plan.destroy()
+
+
+# ---- stage a10 + a11: transpose of a1 + a2 -----------------------------------------------------
+@pytest.mark.parametrize("L,M", [(0, 0), (5, 3), (63, 63), (255, 200), (700, 700)])
+def test_legendre_adjoint_is_transpose(nusht, L, M):
+    rng = np.random.default_rng(5)
+    plan = nusht.Plan(L, M, None, None, 1e-10)
+    nth2 = plan.info.n_theta
+    alm = inputs.random_alm(L, M, 23)
+    gt = rng.standard_normal((M + 1, nth2)) + 1j * rng.standard_normal((M + 1, nth2))
+    ft = plan.stage_legendre_synthesis(cu(alm)).cpu().numpy()
+    c = plan.stage_legendre_adjoint(cu(gt)).cpu().numpy()
+    # <D S a, g> with weights w_m on the m axis  ==  <a, S^T D^T g> in the G3 inner product
+    wm = np.full(M + 1, 2.0)
+    wm[0] = 1.0
+    ft0 = ft.copy()
+    g0 = gt.copy()
+    lhs = np.sum(wm[:, None] * (ft0.real * g0.real + ft0.imag * g0.imag))
+    # m = 0 row: synthesis output is real, so only Re(g) pairs with it
+    lhs -= np.sum(ft0[0].imag * g0[0].imag)
+    a = alm.copy()
+    n0 = L + 1
+    rhs = np.sum(a[:n0].real * c[:n0].real) + 2 * np.sum(a[n0:].real * c[n0:].real + a[n0:].imag * c[n0:].imag)
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(ft) * np.linalg.norm(gt)
+    assert np.all(c[:n0].imag == 0)
+    plan.destroy()
+
+
+# ---- nuFFT stage pair --------------------------------------------------------------------------
+@pytest.mark.parametrize("eps", [1e-3, 1e-6, 1e-10, 1e-13])
+def test_spread_is_transpose_of_interp(nusht, eps):
+    L = 40
+    theta, phi = inputs.uniform_sphere_points(5000, 31)
+    theta[:4] = [0.0, np.pi, 1e-9, np.pi - 1e-9]
+    phi[:4] = [0.0, 2 * np.pi - 1e-12, 6.0, 1e-15]
+    plan = nusht.Plan(L, L, cu(theta), cu(phi), eps)
+    rng = np.random.default_rng(32)
+    g = rng.standard_normal(plan.grid_shape())
+    x = rng.standard_normal(5000)
+    f = plan.stage_interp(cu(g)).cpu().numpy()
+    gs = plan.stage_spread(cu(x)).cpu().numpy()
+    lhs, rhs = np.dot(f, x), np.sum(g * gs)
+    assert abs(lhs - rhs) <= 1e-13 * np.linalg.norm(f) * np.linalg.norm(x) * 10
+    plan.destroy()
+
+
+# ---- full transforms, config 1 (BASELINE.json configs[0]) in full ------------------------------
+def test_config1_full(nusht, oracle):
+    cfg, theta, phi, alm, x = inputs.make_config(1)
+    L, M, eps = cfg["lmax"], cfg["mmax"], cfg["eps"]
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps)
+    f = plan.synthesis(cu(alm)).cpu().numpy()
+    c = plan.adjoint(cu(x)).cpu().numpy()
+    f_ref = oracle.synthesis(L, M, theta, phi, alm, "ld")
+    c_ref = oracle.adjoint(L, M, theta, phi, x, "ld")
+    assert rel(f, f_ref) <= 10 * eps
+    assert rel(c, c_ref) <= 10 * eps
+    # GPU adjointness <S a, x> = <a, S^T x> to 1e-12
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+    rhs = oracle.inner_alm(L, M, alm, c)
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("eps", [1e-2, 1e-4, 1e-6, 1e-8, 1e-12])
+@pytest.mark.parametrize("L,M,npts", [(63, 63, 3000), (47, 20, 2000)])
+def test_eps_sweep_small(nusht, oracle, eps, L, M, npts):
+    theta, phi = inputs.uniform_sphere_points(npts, 41)
+    theta[:3] = [0.0, np.pi, 1e-9]          # poles are legal points (reading G11)
+    phi[3] = -7.5                            # phi is wrapped mod 2 pi
+    alm = inputs.random_alm(L, M, 41)
+    x = inputs.random_map(npts, 41)
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps)
+    f = plan.synthesis(cu(alm)).cpu().numpy()
+    c = plan.adjoint(cu(x)).cpu().numpy()
+    assert rel(f, oracle.synthesis(L, M, theta, phi, alm, "ld")) <= 10 * eps
+    assert rel(c, oracle.adjoint(L, M, theta, phi, x, "ld")) <= 10 * eps
+    plan.destroy()
+
+
+def test_edge_cases(nusht, oracle):
+    # npts = 0: synthesis no-op, adjoint writes zeros
+    plan = nusht.Plan(8, 8, None, None, 1e-6)
+    out = torch.full((plan.nlm,), 3.0 + 1j, dtype=torch.complex128, device="cuda")
+    plan.adjoint(torch.empty(0, dtype=torch.float64, device="cuda"), out)
+    assert torch.all(out == 0)
+    plan.destroy()
+    # lmax = 0
+    theta, phi = inputs.uniform_sphere_points(100, 51)
+    plan = nusht.Plan(0, 0, cu(theta), cu(phi), 1e-8)
+    f = plan.synthesis(cu(np.array([2.5 + 7j]))).cpu().numpy()
+    assert np.max(np.abs(f - 2.5 / np.sqrt(4 * np.pi))) < 1e-7
+    plan.destroy()
+    # a single point, duplicated points
+    th = np.array([1.234, 1.234, 0.3]); ph = np.array([4.321, 4.321, 0.0])
+    plan = nusht.Plan(9, 9, cu(th), cu(ph), 1e-10)
+    c = plan.adjoint(cu(np.array([1.0, 0.7, 0.0]))).cpu().numpy()
+    assert rel(c, oracle.adjoint(9, 9, th[:1], ph[:1], np.array([1.7]), "ld")) < 1e-9
+    plan.destroy()
+    # bad points are rejected
+    bad = theta.copy(); bad[5] = 3.2
+    with pytest.raises(nusht.NushtError) as e:
+        nusht.Plan(8, 8, cu(bad), cu(phi), 1e-6)
+    assert e.value.code == -6
+    bad = phi.copy(); bad[7] = np.nan
+    with pytest.raises(nusht.NushtError):
+        nusht.Plan(8, 8, cu(theta), cu(bad), 1e-6)
+
+
+def test_host_buffer_calls_match_device_calls(nusht):
+    cfg, theta, phi, alm, x = inputs.make_config(1, npts=2000)
+    plan = nusht.Plan(cfg["lmax"], cfg["mmax"], cu(theta), cu(phi), cfg["eps"])
+    f = plan.synthesis(cu(alm)).cpu()
+    c = plan.adjoint(cu(x)).cpu()
+    fh = torch.empty(2000, dtype=torch.float64).pin_memory()
+    ch = torch.empty(plan.nlm, dtype=torch.complex128).pin_memory()
+    plan.synthesis_host(torch.from_numpy(alm).pin_memory(), fh)
+    torch.cuda.synchronize()
+    plan.adjoint_host(torch.from_numpy(x).pin_memory(), ch)
+    torch.cuda.synchronize()
+    assert torch.equal(fh, f)
+    assert torch.allclose(ch, c, rtol=0, atol=1e-12 * float(c.abs().max()))
+    plan.destroy()
