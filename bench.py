@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- the nuSHT hot path on synthetic BASELINE.json workloads.
+
+A step = one synthesis (Eq. 3) + one adjoint (Eq. 2) of arXiv 2406.14542 on the same plan, back
+to back, inputs resident in HBM.  Default workload: BASELINE.json configs[2] (the configuration
+the metric "nuSHT synth+adjoint ms at lmax=4095" is quoted on): lmax = mmax = 4095, FP64,
+eps = 1e-10, 67,108,864 uniform random points, white a_lm.  Planning (point sort, tables, cuFFT
+plans) is excluded from the timed region, as in the paper.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4] [--impl reference]
+
+Prints ONE JSON line (rank 0).  Multi-GPU: the method is single-GPU: N ranks run N
+independent replicas ("replicas only"), no collective on the data path.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2406_14542_b200 import inputs  # noqa: E402
+
+METRIC = "nusht_synth_plus_adjoint_ms"
+FP64_FMA_PER_CLK_PER_SM = 64          # B200: 148 SMs x 64 FP64 FMA/clk
+N_SM = 148
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--npts", type=int, default=None, help="override the point count (debugging)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        busy = sorted(sm)[len(sm) // 2:] if sm else []      # upper half = samples under load
+        return {"sm_mhz": float(np.median(busy)) if busy else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg, theta, phi, alm, x, seconds):
+    """Time the oracle as it stands on a bounded sample of the same workload; extrapolate to the
+    full point count.  Returns (ms per full step extrapolated, description dict)."""
+    from oracle import oracle as o
+    L, M = cfg["lmax"], cfg["mmax"]
+    nlm = inputs.nlm(L, M)
+    steps_per_s = 3.0e8 * max(1, o.num_threads()) / 8.0      # rough prior, refined by a probe
+    probe = max(8, min(len(theta), int(0.5 * steps_per_s / nlm)))
+    t0 = time.perf_counter()
+    o.synthesis(L, M, theta[:probe], phi[:probe], alm)
+    dt = max(time.perf_counter() - t0, 1e-4)
+    n = int(max(8, min(len(theta), probe * (seconds / 2.0) / dt)))
+    t0 = time.perf_counter()
+    o.synthesis(L, M, theta[:n], phi[:n], alm)
+    t_syn = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    o.adjoint(L, M, theta[:n], phi[:n], x[:n])
+    t_adj = time.perf_counter() - t0
+    scale = len(theta) / n
+    ms_full = (t_syn + t_adj) * scale * 1e3
+    return ms_full, {"value": ms_full, "unit": "ms", "cores": o.num_threads(), "kind": "oracle",
+                     "sample": "direct sums (oracle/nusht_oracle.c, binary64, OpenMP) on the first %d of %d points "
+                               "at lmax=%d: synthesis %.2f s + adjoint %.2f s, extrapolated x%.0f to the full point count"
+                               % (n, len(theta), L, t_syn, t_adj, scale),
+                     "steps_per_s": 2 * nlm * n / (t_syn + t_adj)}
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    cfg = dict(inputs.CONFIGS[args.config])
+    npts_full = args.npts or cfg["npts"]
+    # the oracle only ever sees a sample: generate just a prefix-sized workload with the config's recipe
+    nsample = min(npts_full, 1 << 16)
+    cfg2, theta, phi, alm, x = inputs.make_config(args.config, npts=nsample)
+    vals, last = [], None
+    per_step = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
+    for i in range(args.warmup + args.steps):
+        ms, desc = oracle_sample(cfg2, theta, phi, alm, x, per_step)
+        ms *= npts_full / len(theta)
+        desc["value"] = ms
+        desc["sample"] += "; then x%.0f from the %d-point generated prefix to %d points" % (
+            npts_full / len(theta), len(theta), npts_full)
+        if i >= args.warmup:
+            vals.append(ms)
+            last = desc
+    v = float(np.mean(vals))
+    last["value"] = v
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": workload_config(cfg, npts_full), "cpu_baseline": last,
+           "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def workload_config(cfg, npts):
+    return {"workload": "BASELINE.json config lmax=%d eps=%g: %d %s points, %s a_lm; step = synthesis + adjoint"
+                        % (cfg["lmax"], cfg["eps"], npts, cfg["points"], cfg["spectrum"]),
+            "lmax": cfg["lmax"], "mmax": cfg["mmax"], "npts": int(npts), "eps": cfg["eps"],
+            "l2": "inputs larger than L2 (alm %.0f MB, map %.0f MB, fine grid > 126 MB at lmax >= 1023)"
+                  % (inputs.nlm(cfg["lmax"], cfg["mmax"]) * 16 / 1e6, npts * 8 / 1e6),
+            "parallelism": "replicas"}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
+
+
+def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz):
+    """Algorithmic work per stage over its CUDA-event time."""
+    hbm, hbm_src, sm_max = measured_peaks()
+    L, M = cfg["lmax"], cfg["mmax"]
+    nlm = inputs.nlm(L, M)
+    npairs = (info.n_rings + 1) // 2
+    fp64_peak = N_SM * FP64_FMA_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12        # TFLOP/s at max clock
+    leg_flop = 2.0 * 3.0 * nlm * npairs                                           # 3 FMA per (l, m, ring pair)
+    nth2, nth, nph = info.n_theta, info.n_theta_fine, info.n_phi_fine
+    grid_bytes = (nth // 2 + 1) * nph * 8
+    nu_bytes = npts * (16 + 8) + grid_bytes
+    out = {}
+
+    def alu(name, ms):
+        a = leg_flop / (ms * 1e-3) / 1e12
+        out[name] = {"bound": "alu", "achieved": a, "peak": fp64_peak, "unit": "TFLOP/s", "frac": a / fp64_peak,
+                     "traffic": None, "ms": ms,
+                     "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x %.0f MHz (max SM clock)" % sm_max,
+                     "frac_at_sampled_clock": (a / (fp64_peak * sm_mhz / sm_max)) if sm_mhz else None}
+
+    def mem(name, ms, nbytes):
+        a = nbytes / (ms * 1e-3) / 1e9
+        out[name] = {"bound": "hbm", "achieved": a, "peak": hbm, "unit": "GB/s", "frac": a / hbm, "traffic": None,
+                     "ms": ms, "peak_source": hbm_src, "algorithmic_bytes": nbytes}
+
+    alu("legendre_synthesis", syn_ms["legendre"])
+    alu("legendre_adjoint", adj_ms["legendre"])
+    mem("interp", syn_ms["interp"], nu_bytes)
+    mem("spread", adj_ms["spread"], nu_bytes + grid_bytes)      # + zeroing the grid
+    fft_ms = syn_ms["fft_theta"] + syn_ms["deconv_pad"] + syn_ms["fft_fine_theta"] + syn_ms["fft_fine_phi"]
+    fft_bytes = (2 * (M + 1) * nth2 * 16 + (M + 1) * (2 * L + 1) * 16 + (M + 1) * nth * 16
+                 + 2 * (M + 1) * nth * 16 + (nth // 2 + 1) * ((M + 1) * 16 + nph * 8))
+    mem("fourier_synthesis", fft_ms, fft_bytes)
+    fft_ms_a = adj_ms["fft_theta"] + adj_ms["deconv_trunc"] + adj_ms["fft_fine_theta"] + adj_ms["fft_fine_phi"]
+    mem("fourier_adjoint", fft_ms_a, fft_bytes)
+    return out
+
+
+def run_b200(args, rank, world):
+    import torch
+    import torch.distributed as dist
+    from paper_2406_14542_b200 import nusht
+
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    cfg, theta, phi, alm, x = inputs.make_config(args.config, npts=args.npts)
+    npts = len(theta)
+    L, M, eps = cfg["lmax"], cfg["mmax"], cfg["eps"]
+    d_theta, d_phi = torch.from_numpy(theta).cuda(), torch.from_numpy(phi).cuda()
+    plan = nusht.Plan(L, M, d_theta, d_phi, eps, cfg["dtype"])
+    del d_theta, d_phi
+    d_alm, d_x = torch.from_numpy(alm).cuda(), torch.from_numpy(x).cuda()
+    d_map = torch.empty(npts, dtype=torch.float64, device="cuda")
+    d_out = torch.empty(plan.nlm, dtype=torch.complex128, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        plan.synthesis(d_alm, d_map, stream)
+        plan.adjoint(d_x, d_out, stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    plan.set_stage_timing(True)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    syn_acc, adj_acc = {}, {}
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+        # reading the plan's per-stage events needs the step to have finished: a sync between steps
+        # (a few microseconds of idle against a multi-millisecond step), no extra work in the region
+        for acc, t in ((syn_acc, plan.stage_times("synthesis")), (adj_acc, plan.stage_times("adjoint"))):
+            for k, v in t.items():
+                acc[k] = acc.get(k, 0.0) + v / args.steps
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / args.steps
+    if world > 1:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # end to end through the host-buffer C-ABI calls: pinned host inputs, H2D + D2H inside the region
+    e2e = None
+    if not args.no_e2e:
+        h_alm, h_x = torch.from_numpy(alm).pin_memory(), torch.from_numpy(x).pin_memory()
+        h_map = torch.empty(npts, dtype=torch.float64).pin_memory()
+        h_out = torch.empty(plan.nlm, dtype=torch.complex128).pin_memory()
+        plan.set_stage_timing(False)
+        for _ in range(2):
+            plan.synthesis_host(h_alm, h_map, stream)
+            plan.adjoint_host(h_x, h_out, stream)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            plan.synthesis_host(h_alm, h_map, stream)
+            plan.adjoint_host(h_x, h_out, stream)
+            stream.synchronize()
+        barrier()
+        e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
+        if world > 1:
+            t = torch.tensor([e2e_ms], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_ms = float(t.item())
+        nb = plan.nlm * 16 + npts * 8
+        e2e = {"value": e2e_ms / world, "unit": "ms", "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb,
+               "checksum": float(h_map[:1024].double().sum().item())}
+    if rank != 0:
+        return
+    roofs = stage_rooflines(cfg, plan.info, npts, syn_acc, adj_acc, clocks.get("sm_mhz"))
+    own = ["legendre_synthesis", "legendre_adjoint", "interp", "spread"]
+    dominant = max(own, key=lambda k: roofs[k]["ms"])
+    roof = dict(roofs[dominant])
+    roof["kernel"] = dominant
+    out = {
+        "metric": METRIC, "value": ms / world, "unit": "ms", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, npts),
+        "transforms_per_s": 2e3 * world / ms, "points_per_s": 2.0 * npts * world / (ms * 1e-3),
+        "synthesis_ms": sum(syn_acc.values()), "adjoint_ms": sum(adj_acc.values()),
+        "stage_ms": {"synthesis": syn_acc, "adjoint": adj_acc},
+        "roofline": roof, "stage_rooflines": roofs, "clocks": clocks, "e2e": e2e,
+        "gpu_launches": 8 * args.steps,      # our kernels per step: 4 per transform (cuFFT/memset not counted)
+        "plan": {"ms": plan.info.plan_ms, "workspace_gb": plan.info.workspace_bytes / 1e9,
+                 "n_rings": plan.info.n_rings, "n_theta": plan.info.n_theta, "n_theta_fine": plan.info.n_theta_fine,
+                 "n_phi_fine": plan.info.n_phi_fine, "kernel_width": plan.info.kernel_width},
+    }
+    if not args.no_cpu_baseline and world == 1:
+        ns = min(npts, 1 << 16)
+        _, desc = oracle_sample(cfg, theta[:ns], phi[:ns], alm, x[:ns], args.cpu_seconds)
+        desc["value"] *= npts / ns
+        desc["sample"] += "; then x%.0f from the %d-point prefix to %d points" % (npts / ns, ns, npts)
+        out["cpu_baseline"] = desc
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    run_b200(args, rank, world)
+
+
+if __name__ == "__main__":
+    main()
