@@ -114,67 +114,122 @@ __global__ void k_legendre_tables(int L, int M, const int64_t* __restrict__ eoff
 }
 
 // ---------------------------------------------------------------------------------------------
-// a1 prologue: alm -> (ae, ao): even-class scaling and odd-class fold, one thread per m.
+// a1 prologue: alm -> (ae, ao): even-class scaling and odd-class fold, one WARP per m.
 //   ae_j = a_{m+2j} sigma_j;   r_j = a_{m+2j+1} - rho_j r_{j+1};   ao_j = r_j sodd_j
+// The first-order recurrence in j is evaluated 32 entries at a time as a warp suffix scan of the
+// affine maps r -> b_j - rho_j r (|rho_j| < 1, so the composition is as stable as the sequential
+// form), carrying r across tiles from high j to low j.  All loads and stores are coalesced.
 // ---------------------------------------------------------------------------------------------
+constexpr int PREP_THREADS = 128;
+
 template <typename T>
-__global__ void k_alm_prep(int L, int M, const int64_t* __restrict__ eoff, const T* __restrict__ alm,
-                           const double* __restrict__ sig, const double* __restrict__ sodd,
-                           const double* __restrict__ rho, double4* __restrict__ aeo) {
-    int m = blockIdx.x * blockDim.x + threadIdx.x;
+__global__ void __launch_bounds__(PREP_THREADS)
+k_alm_prep(int L, int M, const int64_t* __restrict__ eoff, const T* __restrict__ alm,
+           const double* __restrict__ sig, const double* __restrict__ sodd,
+           const double* __restrict__ rho, double4* __restrict__ aeo) {
+    const int m = blockIdx.x * (PREP_THREADS / 32) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
     if (m > M) return;
     const int ne = (L - m) / 2 + 1;
     const int no = (L - m + 1) / 2;
     const int64_t o = eoff[m];
     const T* col = alm + 2 * ((int64_t)m * (2 * L + 1 - m) / 2);   // col[2*l], col[2*l+1] for l >= m
-    double rre = 0.0, rim = 0.0;
-    for (int j = ne - 1; j >= 0; --j) {
-        const int le = m + 2 * j;
-        double bre = 0.0, bim = 0.0;
-        if (j < no) {
-            bre = (double)col[2 * (le + 1)];
-            bim = (double)col[2 * (le + 1) + 1];
+    double cre = 0.0, cim = 0.0;   // r_{j+1} entering the tile from above
+    for (int base = ((ne - 1) / 32) * 32; base >= 0; base -= 32) {
+        const int j = base + lane;
+        const bool in = j < ne;
+        double are = 0.0, aim = 0.0, bre = 0.0, bim = 0.0, S = 0.0, sg = 0.0, so = 0.0;
+        if (in) {
+            const int le = m + 2 * j;
+            are = (double)col[2 * le];
+            aim = (double)col[2 * le + 1];
+            if (j < no) {
+                bre = (double)col[2 * le + 2];
+                bim = (double)col[2 * le + 3];
+            }
+            S = -rho[o + j];
+            sg = sig[o + j];
+            so = sodd[o + j];
         }
-        const double rh = rho[o + j];
-        rre = fma(-rh, rre, bre);
-        rim = fma(-rh, rim, bim);
-        const double sg = sig[o + j], so = sodd[o + j];
-        double4 v;
-        v.x = (double)col[2 * le] * sg;
-        v.y = (double)col[2 * le + 1] * sg;
-        v.z = rre * so;
-        v.w = rim * so;
-        if (m == 0) { v.y = 0.0; v.w = 0.0; }   // Im(a_l0) is ignored (G3)
-        aeo[o + j] = v;
+        // suffix scan: after it, r_j = B + S * (r entering the tile)
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const double S2 = __shfl_down_sync(0xffffffffu, S, d);
+            const double B2re = __shfl_down_sync(0xffffffffu, bre, d);
+            const double B2im = __shfl_down_sync(0xffffffffu, bim, d);
+            if (lane + d < 32) {
+                bre = fma(S, B2re, bre);
+                bim = fma(S, B2im, bim);
+                S *= S2;
+            }
+        }
+        const double rre = fma(S, cre, bre), rim = fma(S, cim, bim);
+        if (in) {
+            double4 v;
+            v.x = are * sg;
+            v.y = aim * sg;
+            v.z = rre * so;
+            v.w = rim * so;
+            if (m == 0) { v.y = 0.0; v.w = 0.0; }   // Im(a_l0) is ignored (G3)
+            aeo[o + j] = v;
+        }
+        cre = __shfl_sync(0xffffffffu, rre, 0);
+        cim = __shfl_sync(0xffffffffu, rim, 0);
     }
 }
 
 // a11 epilogue: (e~, o~) -> alm.  c_{m+2n} = sigma_n e~_n;  u_n = sodd_n o~_n;
-//   v_n = u_n - rho_{n-1} v_{n-1};  c_{m+2n+1} = v_n   (transpose of the fold above).
+//   v_n = u_n - rho_{n-1} v_{n-1};  c_{m+2n+1} = v_n   (transpose of the fold above), one warp
+// per m, prefix scan of the affine maps v -> u_n - rho_{n-1} v.
 template <typename T>
-__global__ void k_alm_post(int L, int M, const int64_t* __restrict__ eoff, const double4* __restrict__ eo,
-                           const double* __restrict__ sig, const double* __restrict__ sodd,
-                           const double* __restrict__ rho, T* __restrict__ alm) {
-    int m = blockIdx.x * blockDim.x + threadIdx.x;
+__global__ void __launch_bounds__(PREP_THREADS)
+k_alm_post(int L, int M, const int64_t* __restrict__ eoff, const double4* __restrict__ eo,
+           const double* __restrict__ sig, const double* __restrict__ sodd,
+           const double* __restrict__ rho, T* __restrict__ alm) {
+    const int m = blockIdx.x * (PREP_THREADS / 32) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
     if (m > M) return;
     const int ne = (L - m) / 2 + 1;
     const int no = (L - m + 1) / 2;
     const int64_t o = eoff[m];
     T* col = alm + 2 * ((int64_t)m * (2 * L + 1 - m) / 2);
-    double vre = 0.0, vim = 0.0, rprev = 0.0;
-    for (int n = 0; n < ne; ++n) {
-        const double4 v = eo[o + n];
-        const double sg = sig[o + n], so = sodd[o + n];
-        const int le = m + 2 * n;
-        col[2 * le] = (T)(v.x * sg);
-        col[2 * le + 1] = (m == 0) ? (T)0 : (T)(v.y * sg);
-        vre = fma(-rprev, vre, v.z * so);
-        vim = fma(-rprev, vim, v.w * so);
-        if (n < no) {
-            col[2 * (le + 1)] = (T)vre;
-            col[2 * (le + 1) + 1] = (m == 0) ? (T)0 : (T)vim;
+    double cre = 0.0, cim = 0.0;   // v_{n-1} entering the tile from below
+    for (int base = 0; base < ne; base += 32) {
+        const int n = base + lane;
+        const bool in = n < ne;
+        double ere = 0.0, eim = 0.0, ure = 0.0, uim = 0.0, S = 0.0;
+        if (in) {
+            const double4 v = eo[o + n];
+            const double sg = sig[o + n], so = sodd[o + n];
+            ere = v.x * sg;
+            eim = v.y * sg;
+            ure = v.z * so;
+            uim = v.w * so;
+            S = (n > 0) ? -rho[o + n - 1] : 0.0;
         }
-        rprev = rho[o + n];
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const double S2 = __shfl_up_sync(0xffffffffu, S, d);
+            const double U2re = __shfl_up_sync(0xffffffffu, ure, d);
+            const double U2im = __shfl_up_sync(0xffffffffu, uim, d);
+            if (lane >= d) {
+                ure = fma(S, U2re, ure);
+                uim = fma(S, U2im, uim);
+                S *= S2;
+            }
+        }
+        const double vre = fma(S, cre, ure), vim = fma(S, cim, uim);
+        if (in) {
+            const int le = m + 2 * n;
+            col[2 * le] = (T)ere;
+            col[2 * le + 1] = (m == 0) ? (T)0 : (T)eim;
+            if (n < no) {
+                col[2 * le + 2] = (T)vre;
+                col[2 * le + 3] = (m == 0) ? (T)0 : (T)vim;
+            }
+        }
+        cre = __shfl_sync(0xffffffffu, vre, 31);
+        cim = __shfl_sync(0xffffffffu, vim, 31);
     }
 }
 
@@ -684,7 +739,7 @@ int legendre_build_tables(nusht_plan_s* p) {
 }
 
 int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s) {
-    const int threads = 32, blocks = (p->mmax + 1 + threads - 1) / threads;
+    const int threads = PREP_THREADS, blocks = (p->mmax + 1 + threads / 32 - 1) / (threads / 32);
     if (p->dtype == NUSHT_F64)
         k_alm_prep<double><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, (const double*)alm, p->d_sig,
                                                       p->d_sodd, p->d_rho, p->d_aeo);
@@ -710,7 +765,7 @@ int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
 }
 
 int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s) {
-    const int threads = 32, blocks = (p->mmax + 1 + threads - 1) / threads;
+    const int threads = PREP_THREADS, blocks = (p->mmax + 1 + threads / 32 - 1) / (threads / 32);
     if (p->dtype == NUSHT_F64)
         k_alm_post<double><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, p->d_aeo, p->d_sig, p->d_sodd,
                                                       p->d_rho, (double*)alm);

@@ -196,15 +196,29 @@ __global__ void k_point_scatter(SortGeom g, int64_t npts, const double* __restri
 // kernel evaluation: w polynomials of degree DEG in u, coefficients read from the kernel-parameter
 // constant bank (uniform operands, no loads)
 // ---------------------------------------------------------------------------------------------
+// The kernel is even, so tap W-1-i is tap i evaluated at -u: c[W-1-i][d] = (-1)^d c[i][d] (enforced
+// exactly at plan time).  Taps i and W-1-i share the even and odd parts E_i(u^2) +- u O_i(u^2).
 template <int W, typename T>
 __device__ __forceinline__ void eval_taps(const KernelPoly<T>& kp, T u, T (&k)[W]) {
     constexpr int DEG = poly_degree(W);
+    constexpr int DE = DEG & ~1;            // highest even power
+    constexpr int DO = (DEG - 1) | 1;       // highest odd power
+    const T u2 = u * u;
 #pragma unroll
-    for (int i = 0; i < W; ++i) {
-        T acc = kp.c[i][DEG];
+    for (int i = 0; i < W / 2; ++i) {
+        T e = kp.c[i][DE], o = kp.c[i][DO];
 #pragma unroll
-        for (int d = DEG - 1; d >= 0; --d) acc = fma(acc, u, kp.c[i][d]);
-        k[i] = acc;
+        for (int d = DE - 2; d >= 0; d -= 2) e = fma(e, u2, kp.c[i][d]);
+#pragma unroll
+        for (int d = DO - 2; d >= 1; d -= 2) o = fma(o, u2, kp.c[i][d]);
+        k[i] = fma(u, o, e);
+        k[W - 1 - i] = fma(-u, o, e);
+    }
+    if (W & 1) {
+        T e = kp.c[W / 2][DE];
+#pragma unroll
+        for (int d = DE - 2; d >= 0; d -= 2) e = fma(e, u2, kp.c[W / 2][d]);
+        k[W / 2] = e;
     }
 }
 
@@ -297,8 +311,9 @@ k_interp(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
         }
         __syncwarp();
         const int npt = min(32, end - batch);
-        for (int j = 0; j < npt; ++j) {
-            const int2 org = ws.org[j];
+        int j = 0;
+        int2 org = ws.org[0];
+        while (j < npt) {
             // ---- slide the register window down to row org.x (warp-uniform) ----
             if (org.x != a_base) {
                 int d = (a_base == INT_MIN) ? W : org.x - a_base;
@@ -308,6 +323,7 @@ k_interp(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
                     for (int i = 0; i < W; ++i) win[i] = grid[grid_index(g, a_base + i, col_n, col_m)];
                     nxt = grid[grid_index(g, a_base + W, col_n, col_m)];
                 } else {
+#pragma unroll 1
                     for (; d > 0; --d) {
 #pragma unroll
                         for (int i = 0; i + 1 < W; ++i) win[i] = win[i + 1];
@@ -317,22 +333,34 @@ k_interp(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
                     }
                 }
             }
-            // ---- theta contraction in registers, phi weight per lane ----
-            T acc = 0;
-            if constexpr (sizeof(T) == 8) {
+            // ---- all points of the batch whose footprint starts on this row: the window is
+            //      loop-invariant here, so it stays in place in registers ----
+#pragma unroll 1
+            do {
+                // theta contraction in registers (two independent chains), phi weight per lane
+                T acc0 = 0, acc1 = 0;
+                if constexpr (sizeof(T) == 8) {
 #pragma unroll
-                for (int i = 0; i + 1 < W; i += 2) {
-                    const double2 kk = *reinterpret_cast<const double2*>(&ws.th[j][i]);
-                    acc = fma(kk.x, win[i], acc);
-                    acc = fma(kk.y, win[i + 1], acc);
+                    for (int i = 0; i + 1 < W; i += 2) {
+                        const double2 kk = *reinterpret_cast<const double2*>(&ws.th[j][i]);
+                        acc0 = fma(kk.x, win[i], acc0);
+                        acc1 = fma(kk.y, win[i + 1], acc1);
+                    }
+                    if (W & 1) acc0 = fma(ws.th[j][W - 1], win[W - 1], acc0);
+                } else {
+#pragma unroll
+                    for (int i = 0; i + 1 < W; i += 2) {
+                        acc0 = fma(ws.th[j][i], win[i], acc0);
+                        acc1 = fma(ws.th[j][i + 1], win[i + 1], acc1);
+                    }
+                    if (W & 1) acc0 = fma(ws.th[j][W - 1], win[W - 1], acc0);
                 }
-                if (W & 1) acc = fma(ws.th[j][W - 1], win[W - 1], acc);
-            } else {
-#pragma unroll
-                for (int i = 0; i < W; ++i) acc = fma(ws.th[j][i], win[i], acc);
-            }
-            const int t = lane - org.y;
-            if (t >= 0 && t < W) ws.part[j][t] = acc * ws.ph[j][t];
+                const unsigned t = (unsigned)(lane - org.y);
+                if (t < (unsigned)W) ws.part[j][t] = (acc0 + acc1) * ws.ph[j][t];
+                ++j;
+                if (j >= npt) break;
+                org = ws.org[j];
+            } while (org.x == a_base);
         }
         __syncwarp();
         if (has) {
@@ -402,8 +430,9 @@ k_spread(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
         }
         __syncwarp();
         const int npt = min(32, end - batch);
-        for (int j = 0; j < npt; ++j) {
-            const int2 org = ws.org[j];
+        int j = 0;
+        int2 org = ws.org[0];
+        while (j < npt) {
             if (org.x != a_base) {
                 if (a_base == INT_MIN) {
                     a_base = org.x;
@@ -418,6 +447,7 @@ k_spread(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
                         }
                         a_base = org.x;
                     } else {
+#pragma unroll 1
                         for (; d > 0; --d) {
                             if (acc[0] != (T)0) atomicAdd(&grid[grid_index(g, a_base, col_n, col_m)], acc[0]);
 #pragma unroll
@@ -428,20 +458,27 @@ k_spread(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
                     }
                 }
             }
-            const int t = lane - org.y;
-            const T kph = (t >= 0 && t < W) ? ws.ph[j][t] : (T)0;
-            if constexpr (sizeof(T) == 8) {
+            // all points of the batch whose footprint starts on this row
+#pragma unroll 1
+            do {
+                const unsigned t = (unsigned)(lane - org.y);
+                const T kph = (t < (unsigned)W) ? ws.ph[j][t] : (T)0;
+                if constexpr (sizeof(T) == 8) {
 #pragma unroll
-                for (int i = 0; i + 1 < W; i += 2) {
-                    const double2 kk = *reinterpret_cast<const double2*>(&ws.th[j][i]);
-                    acc[i] = fma(kk.x, kph, acc[i]);
-                    acc[i + 1] = fma(kk.y, kph, acc[i + 1]);
+                    for (int i = 0; i + 1 < W; i += 2) {
+                        const double2 kk = *reinterpret_cast<const double2*>(&ws.th[j][i]);
+                        acc[i] = fma(kk.x, kph, acc[i]);
+                        acc[i + 1] = fma(kk.y, kph, acc[i + 1]);
+                    }
+                    if (W & 1) acc[W - 1] = fma(ws.th[j][W - 1], kph, acc[W - 1]);
+                } else {
+#pragma unroll
+                    for (int i = 0; i < W; ++i) acc[i] = fma(ws.th[j][i], kph, acc[i]);
                 }
-                if (W & 1) acc[W - 1] = fma(ws.th[j][W - 1], kph, acc[W - 1]);
-            } else {
-#pragma unroll
-                for (int i = 0; i < W; ++i) acc[i] = fma(ws.th[j][i], kph, acc[i]);
-            }
+                ++j;
+                if (j >= npt) break;
+                org = ws.org[j];
+            } while (org.x == a_base);
         }
         __syncwarp();
     }
@@ -583,6 +620,17 @@ int nufft_choose_kernel(nusht_plan_s* p) {
         }
         for (int q = 0; q <= NUSHT_MAX_DEG; ++q) h->c[i][q] = (q < nn) ? mono[q] : 0.0L;
     }
+    // the kernel is even: make tap w-1-i exactly tap i mirrored (the fit gives this up to rounding),
+    // which is what eval_taps relies on; the deconvolution factors use these same coefficients
+    for (int i = 0; i < w / 2; ++i)
+        for (int q = 0; q <= NUSHT_MAX_DEG; ++q) {
+            const long double sgn = (q & 1) ? -1.0L : 1.0L;
+            const long double v = 0.5L * (h->c[i][q] + sgn * h->c[w - 1 - i][q]);
+            h->c[i][q] = v;
+            h->c[w - 1 - i][q] = sgn * v;
+        }
+    if (w & 1)
+        for (int q = 1; q <= NUSHT_MAX_DEG; q += 2) h->c[w / 2][q] = 0.0L;
     p->kernel_host = h;
     return NUSHT_OK;
 }
