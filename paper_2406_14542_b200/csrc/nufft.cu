@@ -243,7 +243,7 @@ struct WarpScratch {
     T th[32][SK];       // per point: theta-direction weights (broadcast reads, 128-bit where possible)
     T ph[32][SP];       // per point: phi-direction weights (lane-indexed reads)
     T part[32][SP];     // interp: per point, per active lane partial sums
-    int2 org[32];       // per point: (a0, lane of first footprint column)
+    int oy[32];         // per point: lane of the first footprint column
 };
 
 // fine-grid row/column of logical row a (may lie beyond a pole) for a lane
@@ -254,6 +254,61 @@ __device__ __forceinline__ int64_t grid_index(const NufftGeom& g, int a, int col
     const bool mirror = am > g.nth / 2;
     const int row = mirror ? g.nth - am : am;
     return (int64_t)row * g.nph + (mirror ? col_m : col_n);
+}
+
+// ---------------------------------------------------------------------------------------------
+// per-batch prologue shared by a7 and a8: lane `lane` evaluates the 2W weights of point batch+lane
+// and publishes them; returns the bit mask of points that start a new row run (points are sorted
+// by the row a0 of their footprint origin inside a work item).
+// ---------------------------------------------------------------------------------------------
+template <typename T> struct Vec2;
+template <> struct Vec2<double> { using type = double2; };
+template <> struct Vec2<float> { using type = float2; };
+
+template <int W, typename T>
+__device__ __forceinline__ unsigned publish_weights(WarpScratch<W, T>& ws, const KernelPoly<T>& kp, int lane,
+                                                    bool has, double X, double Y, T val, int c0, int& a0) {
+    using V2 = typename Vec2<T>::type;
+    const double a0d = ceil(X - 0.5 * W), b0d = ceil(Y - 0.5 * W);
+    const T ut = (T)(2.0 * ((a0d + 0.5 * W) - X) - 1.0);
+    const T up = (T)(2.0 * ((b0d + 0.5 * W) - Y) - 1.0);
+    T k[W];
+    eval_taps<W, T>(kp, ut, k);
+#pragma unroll
+    for (int i = 0; i + 1 < W; i += 2) {
+        V2 v;
+        v.x = val * k[i];
+        v.y = val * k[i + 1];
+        *reinterpret_cast<V2*>(&ws.th[lane][i]) = v;
+    }
+    if (W & 1) {
+        V2 v;
+        v.x = val * k[W - 1];
+        v.y = 0;
+        *reinterpret_cast<V2*>(&ws.th[lane][W - 1]) = v;
+    }
+    eval_taps<W, T>(kp, up, k);
+#pragma unroll
+    for (int i = 0; i < W; ++i) ws.ph[lane][i] = k[i];
+    ws.oy[lane] = (int)b0d - c0;
+    a0 = (int)a0d;
+    const int a0_prev = __shfl_up_sync(0xffffffffu, a0, 1);
+    return __ballot_sync(0xffffffffu, has && (lane == 0 || a0 != a0_prev));
+}
+
+// theta contraction of one point against the register window: two independent FMA chains
+template <int W, typename T>
+__device__ __forceinline__ T contract(const T* th, const T (&win)[W]) {
+    using V2 = typename Vec2<T>::type;
+    T acc0 = 0, acc1 = 0;
+#pragma unroll
+    for (int i = 0; i + 1 < W; i += 2) {
+        const V2 kk = *reinterpret_cast<const V2*>(th + i);
+        acc0 = fma(kk.x, win[i], acc0);
+        acc1 = fma(kk.y, win[i + 1], acc1);
+    }
+    if (W & 1) acc0 = fma(th[W - 1], win[W - 1], acc0);
+    return acc0 + acc1;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -284,41 +339,32 @@ k_interp(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
     T nxt = 0;    // prefetched row a_base + W
     int a_base = INT_MIN;
 
+    // coordinates of the next batch are loaded one batch ahead
+    double Xn = 0.0, Yn = 0.0;
+    if (start + lane < end) {
+        Xn = P.px[start + lane];
+        Yn = P.py[start + lane];
+    }
     for (int batch = start; batch < end; batch += 32) {
         const int idx = batch + lane;
         const bool has = idx < end;
-        // ---- each lane evaluates the 2W weights of its own point ----
-        {
-            const double X = has ? P.px[idx] : 0.0, Y = has ? P.py[idx] : 0.0;
-            const double a0d = ceil(X - 0.5 * W), b0d = ceil(Y - 0.5 * W);
-            const T ut = (T)(2.0 * ((a0d + 0.5 * W) - X) - 1.0);
-            const T up = (T)(2.0 * ((b0d + 0.5 * W) - Y) - 1.0);
-            T k[W];
-            eval_taps<W, T>(kp, ut, k);
-            if constexpr (sizeof(T) == 8) {
-#pragma unroll
-                for (int i = 0; i + 1 < W; i += 2)
-                    *reinterpret_cast<double2*>(&ws.th[lane][i]) = make_double2(k[i], k[i + 1]);
-                if (W & 1) *reinterpret_cast<double2*>(&ws.th[lane][W - 1]) = make_double2(k[W - 1], 0.0);
-            } else {
-#pragma unroll
-                for (int i = 0; i < W; ++i) ws.th[lane][i] = k[i];
-            }
-            eval_taps<W, T>(kp, up, k);
-#pragma unroll
-            for (int i = 0; i < W; ++i) ws.ph[lane][i] = k[i];
-            ws.org[lane] = make_int2((int)a0d, (int)b0d - c0);
+        const double X = Xn, Y = Yn;
+        if (idx + 32 < end) {
+            Xn = P.px[idx + 32];
+            Yn = P.py[idx + 32];
         }
+        int a0;
+        const unsigned starts = publish_weights<W, T>(ws, kp, lane, has, X, Y, (T)1, c0, a0);
         __syncwarp();
         const int npt = min(32, end - batch);
         int j = 0;
-        int2 org = ws.org[0];
         while (j < npt) {
-            // ---- slide the register window down to row org.x (warp-uniform) ----
-            if (org.x != a_base) {
-                int d = (a_base == INT_MIN) ? W : org.x - a_base;
+            // ---- slide the register window down to the row of point j (warp-uniform) ----
+            const int row = __shfl_sync(0xffffffffu, a0, j);
+            if (row != a_base) {
+                int d = (a_base == INT_MIN) ? W : row - a_base;
                 if (d >= W) {
-                    a_base = org.x;
+                    a_base = row;
 #pragma unroll
                     for (int i = 0; i < W; ++i) win[i] = grid[grid_index(g, a_base + i, col_n, col_m)];
                     nxt = grid[grid_index(g, a_base + W, col_n, col_m)];
@@ -333,34 +379,26 @@ k_interp(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
                     }
                 }
             }
-            // ---- all points of the batch whose footprint starts on this row: the window is
-            //      loop-invariant here, so it stays in place in registers ----
+            // ---- the run of points whose footprint starts on this row: the window is loop-invariant,
+            //      two points per iteration for instruction-level parallelism ----
+            const unsigned rest = (j < 31) ? (starts >> (j + 1)) : 0u;
+            const int run_end = rest ? j + __ffs(rest) : npt;
 #pragma unroll 1
-            do {
-                // theta contraction in registers (two independent chains), phi weight per lane
-                T acc0 = 0, acc1 = 0;
-                if constexpr (sizeof(T) == 8) {
-#pragma unroll
-                    for (int i = 0; i + 1 < W; i += 2) {
-                        const double2 kk = *reinterpret_cast<const double2*>(&ws.th[j][i]);
-                        acc0 = fma(kk.x, win[i], acc0);
-                        acc1 = fma(kk.y, win[i + 1], acc1);
-                    }
-                    if (W & 1) acc0 = fma(ws.th[j][W - 1], win[W - 1], acc0);
-                } else {
-#pragma unroll
-                    for (int i = 0; i + 1 < W; i += 2) {
-                        acc0 = fma(ws.th[j][i], win[i], acc0);
-                        acc1 = fma(ws.th[j][i + 1], win[i + 1], acc1);
-                    }
-                    if (W & 1) acc0 = fma(ws.th[j][W - 1], win[W - 1], acc0);
-                }
-                const unsigned t = (unsigned)(lane - org.y);
-                if (t < (unsigned)W) ws.part[j][t] = (acc0 + acc1) * ws.ph[j][t];
+            for (; j + 1 < run_end; j += 2) {
+                const T s0 = contract<W, T>(&ws.th[j][0], win);
+                const T s1 = contract<W, T>(&ws.th[j + 1][0], win);
+                const unsigned t0 = (unsigned)(lane - ws.oy[j]), t1 = (unsigned)(lane - ws.oy[j + 1]);
+                const T p0 = (t0 < (unsigned)W) ? ws.ph[j][t0] : (T)0;
+                const T p1 = (t1 < (unsigned)W) ? ws.ph[j + 1][t1] : (T)0;
+                if (t0 < (unsigned)W) ws.part[j][t0] = s0 * p0;
+                if (t1 < (unsigned)W) ws.part[j + 1][t1] = s1 * p1;
+            }
+            if (j < run_end) {
+                const T s0 = contract<W, T>(&ws.th[j][0], win);
+                const unsigned t0 = (unsigned)(lane - ws.oy[j]);
+                if (t0 < (unsigned)W) ws.part[j][t0] = s0 * ws.ph[j][t0];
                 ++j;
-                if (j >= npt) break;
-                org = ws.org[j];
-            } while (org.x == a_base);
+            }
         }
         __syncwarp();
         if (has) {
@@ -376,6 +414,18 @@ k_interp(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
 // ---------------------------------------------------------------------------------------------
 // a8: type-1 spreading (grid must be zero on entry)
 // ---------------------------------------------------------------------------------------------
+template <int W, typename T>
+__device__ __forceinline__ void spread_point(const T* th, T kph, T (&acc)[W]) {
+    using V2 = typename Vec2<T>::type;
+#pragma unroll
+    for (int i = 0; i + 1 < W; i += 2) {
+        const V2 kk = *reinterpret_cast<const V2*>(th + i);
+        acc[i] = fma(kk.x, kph, acc[i]);
+        acc[i + 1] = fma(kk.y, kph, acc[i + 1]);
+    }
+    if (W & 1) acc[W - 1] = fma(th[W - 1], kph, acc[W - 1]);
+}
+
 template <int W, typename T>
 __global__ void __launch_bounds__(nu_warps<W, T>() * 32)
 k_spread(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<T> kp,
@@ -402,42 +452,36 @@ k_spread(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
     for (int i = 0; i < W; ++i) acc[i] = 0;
     int a_base = INT_MIN;
 
+    double Xn = 0.0, Yn = 0.0;
+    T vn = 0;
+    if (start + lane < end) {
+        Xn = P.px[start + lane];
+        Yn = P.py[start + lane];
+        vn = map[P.perm[start + lane]];
+    }
     for (int batch = start; batch < end; batch += 32) {
         const int idx = batch + lane;
         const bool has = idx < end;
-        {
-            const double X = has ? P.px[idx] : 0.0, Y = has ? P.py[idx] : 0.0;
-            const T val = has ? map[P.perm[idx]] : (T)0;
-            const double a0d = ceil(X - 0.5 * W), b0d = ceil(Y - 0.5 * W);
-            const T ut = (T)(2.0 * ((a0d + 0.5 * W) - X) - 1.0);
-            const T up = (T)(2.0 * ((b0d + 0.5 * W) - Y) - 1.0);
-            T k[W];
-            eval_taps<W, T>(kp, ut, k);
-            // the point's value rides on the theta weights
-            if constexpr (sizeof(T) == 8) {
-#pragma unroll
-                for (int i = 0; i + 1 < W; i += 2)
-                    *reinterpret_cast<double2*>(&ws.th[lane][i]) = make_double2(val * k[i], val * k[i + 1]);
-                if (W & 1) *reinterpret_cast<double2*>(&ws.th[lane][W - 1]) = make_double2(val * k[W - 1], 0.0);
-            } else {
-#pragma unroll
-                for (int i = 0; i < W; ++i) ws.th[lane][i] = val * k[i];
-            }
-            eval_taps<W, T>(kp, up, k);
-#pragma unroll
-            for (int i = 0; i < W; ++i) ws.ph[lane][i] = k[i];
-            ws.org[lane] = make_int2((int)a0d, (int)b0d - c0);
+        const double X = Xn, Y = Yn;
+        const T val = has ? vn : (T)0;
+        if (idx + 32 < end) {
+            Xn = P.px[idx + 32];
+            Yn = P.py[idx + 32];
+            vn = map[P.perm[idx + 32]];
         }
+        int a0;
+        // the point's value rides on the theta weights
+        const unsigned starts = publish_weights<W, T>(ws, kp, lane, has, X, Y, val, c0, a0);
         __syncwarp();
         const int npt = min(32, end - batch);
         int j = 0;
-        int2 org = ws.org[0];
         while (j < npt) {
-            if (org.x != a_base) {
+            const int row = __shfl_sync(0xffffffffu, a0, j);
+            if (row != a_base) {
                 if (a_base == INT_MIN) {
-                    a_base = org.x;
+                    a_base = row;
                 } else {
-                    int d = org.x - a_base;
+                    int d = row - a_base;
                     if (d >= W) {
                         // flush the whole window
 #pragma unroll
@@ -445,7 +489,7 @@ k_spread(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
                             if (acc[i] != (T)0) atomicAdd(&grid[grid_index(g, a_base + i, col_n, col_m)], acc[i]);
                             acc[i] = 0;
                         }
-                        a_base = org.x;
+                        a_base = row;
                     } else {
 #pragma unroll 1
                         for (; d > 0; --d) {
@@ -458,27 +502,22 @@ k_spread(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
                     }
                 }
             }
-            // all points of the batch whose footprint starts on this row
+            const unsigned rest = (j < 31) ? (starts >> (j + 1)) : 0u;
+            const int run_end = rest ? j + __ffs(rest) : npt;
 #pragma unroll 1
-            do {
-                const unsigned t = (unsigned)(lane - org.y);
-                const T kph = (t < (unsigned)W) ? ws.ph[j][t] : (T)0;
-                if constexpr (sizeof(T) == 8) {
-#pragma unroll
-                    for (int i = 0; i + 1 < W; i += 2) {
-                        const double2 kk = *reinterpret_cast<const double2*>(&ws.th[j][i]);
-                        acc[i] = fma(kk.x, kph, acc[i]);
-                        acc[i + 1] = fma(kk.y, kph, acc[i + 1]);
-                    }
-                    if (W & 1) acc[W - 1] = fma(ws.th[j][W - 1], kph, acc[W - 1]);
-                } else {
-#pragma unroll
-                    for (int i = 0; i < W; ++i) acc[i] = fma(ws.th[j][i], kph, acc[i]);
-                }
+            for (; j + 1 < run_end; j += 2) {
+                const unsigned t0 = (unsigned)(lane - ws.oy[j]), t1 = (unsigned)(lane - ws.oy[j + 1]);
+                const T p0 = (t0 < (unsigned)W) ? ws.ph[j][t0] : (T)0;
+                const T p1 = (t1 < (unsigned)W) ? ws.ph[j + 1][t1] : (T)0;
+                spread_point<W, T>(&ws.th[j][0], p0, acc);
+                spread_point<W, T>(&ws.th[j + 1][0], p1, acc);
+            }
+            if (j < run_end) {
+                const unsigned t0 = (unsigned)(lane - ws.oy[j]);
+                const T p0 = (t0 < (unsigned)W) ? ws.ph[j][t0] : (T)0;
+                spread_point<W, T>(&ws.th[j][0], p0, acc);
                 ++j;
-                if (j >= npt) break;
-                org = ws.org[j];
-            } while (org.x == a_base);
+            }
         }
         __syncwarp();
     }
@@ -539,6 +578,398 @@ int dispatch_spread(int w, const NufftParams& P, const KernelHost& h, const void
     return NUSHT_ERR_UNSUPPORTED;
 }
 
+// =============================================================================================
+// FP64 path: a7 / a8 on the FP64 tensor-core instruction (mma.sync m8n8k4 f64, SASS DMMA).
+//
+// Why: with the register-window scheme above every lane needs all W theta weights of every point,
+// i.e. W*8 bytes x 32 lanes of shared-memory -> register traffic per point.  At W = 11 that is 11
+// shared-memory wavefronts per point and the LSU data pipe (one wavefront per clock per SM)
+// saturates (ncu: 73-90 % of peak, profiles/) long before the FP64 pipe does.  DMMA performs the
+// broadcast inside the tensor core: each lane holds ONE element of the weight fragment, and one
+// instruction does 256 FMA at the full FP64 rate of the SM (measured 37.1 TFLOP/s, same pipe as DFMA).
+//
+// Geometry.  A strip is 8*NT grid columns (NT n-tiles of 8), of which mb = 8*NT - W + 1 are
+// footprint origins.  Lane = (g = lane/4, t = lane%4).  The row window has S = 4*KS slots
+// (interp; KS k-steps) or S = 8*MT slots (spread; MT m-tiles), used circularly: grid row r lives
+// in slot r mod S, so sliding the window never moves registers.  A tile is up to 8 (interp) or 4
+// (spread) consecutive points of the row-sorted list whose origins a0 lie within S - W rows of the
+// first one, so that every footprint of the tile is inside the S resident rows.
+//   interp:  D[p][c] = sum_k A[p][k] B[k][c],  A[p][k] = th_p[(k - a0_p) mod S] (0 beyond W taps),
+//            B[k][c] = window row in slot k at strip column c;  f_p = sum_c D[p][c] ph_p[c - b0_p].
+//   spread:  C[k][c] += sum_p A[k][p] B[p][c], A[k][p] = x_p th_p[(k - a0_p) mod S],
+//            B[p][c] = ph_p[c - b0_p];  finished rows are flushed with global atomics.
+// Fragment layouts (PTX ISA, mma.m8n8k4.f64): A row = g, col = t; B row = t, col = g;
+// C/D row = g, cols = 2t, 2t+1.  N-tile nt, column n  <->  strip column NT*n + nt, so that a lane's
+// elements are contiguous columns: B lanes hold columns NT*g .. NT*g+NT-1, C/D lanes hold columns
+// 2*NT*t .. 2*NT*t+2*NT-1.
+// =============================================================================================
+__device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+__host__ __device__ constexpr int mma_nt(int w) { return w <= 8 ? 2 : 3; }                 // n-tiles per strip
+__host__ __device__ constexpr int mma_ks(int w) { return w <= 6 ? 2 : (w <= 10 ? 3 : (w <= 14 ? 4 : 5)); }
+__host__ __device__ constexpr int mma_mt(int w) { return w <= 6 ? 1 : (w <= 14 ? 2 : 3); }
+__host__ __device__ constexpr int mma_th_stride(int s) { return s <= 8 ? 12 : (s <= 16 ? 20 : 36); }  // = 4 or 12 mod 16
+
+template <int W, int S>
+struct MmaScratch {
+    static constexpr int STH = mma_th_stride(S);
+    static constexpr int SP = W | 1;
+    double th[32][STH];   // per point: theta weights, zero-padded to S slots
+    double ph[32][SP];    // per point: phi weights
+    double res[32];       // interp: per point result
+    int oy[32];           // per point: strip column of the first footprint column
+};
+
+// lane `lane` evaluates the weights of its own point and publishes them; returns a0 of the point
+template <int W, int S>
+__device__ __forceinline__ int mma_publish(MmaScratch<W, S>& ws, const KernelPoly<double>& kp, int lane, double X,
+                                           double Y, double val, int c0) {
+    const double a0d = ceil(X - 0.5 * W), b0d = ceil(Y - 0.5 * W);
+    const double ut = 2.0 * ((a0d + 0.5 * W) - X) - 1.0;
+    const double up = 2.0 * ((b0d + 0.5 * W) - Y) - 1.0;
+    double k[W];
+    eval_taps<W, double>(kp, ut, k);
+#pragma unroll
+    for (int i = 0; i < S; i += 2) {
+        double2 v;
+        v.x = (i < W) ? val * k[i < W ? i : 0] : 0.0;
+        v.y = (i + 1 < W) ? val * k[i + 1 < W ? i + 1 : 0] : 0.0;
+        *reinterpret_cast<double2*>(&ws.th[lane][i]) = v;
+    }
+    eval_taps<W, double>(kp, up, k);
+#pragma unroll
+    for (int i = 0; i < W; ++i) ws.ph[lane][i] = k[i];
+    ws.oy[lane] = (int)b0d - c0;
+    return (int)a0d;
+}
+
+// fine-grid row offset and mirror flag of logical row a (may lie beyond a pole)
+__device__ __forceinline__ int64_t grid_row(const NufftGeom& g, int a, bool& mirror) {
+    int am = a;
+    if (am < 0) am += g.nth;
+    if (am >= g.nth) am -= g.nth;
+    mirror = am > g.nth / 2;
+    return (int64_t)(mirror ? g.nth - am : am) * g.nph;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a7: type-2 interpolation, FP64 / DMMA
+// ---------------------------------------------------------------------------------------------
+template <int W>
+__global__ void __launch_bounds__(128)
+k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<double> kp,
+             const double* __restrict__ grid, double* __restrict__ map) {
+    constexpr int NT = mma_nt(W), KS = mma_ks(W), S = 4 * KS, SPAN = S - W, OFF = 2 * S;
+    using WS = MmaScratch<W, S>;
+    __shared__ __align__(16) WS s_ws[4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int item = blockIdx.x * 4 + warp;
+    if (item >= P.n_items) return;
+    const int start = P.item_off[item], end = P.item_off[item + 1];
+    if (start >= end) return;
+    WS& ws = s_ws[warp];
+    const NufftGeom& g = P.g;
+    const int strip = item % g.nstrip;
+    const int c0 = strip * g.mb - g.fl;   // global column of strip column 0
+    const int gq = lane >> 2, t = lane & 3;
+    int colb_n[NT], colb_m[NT];           // global columns (plain / mirrored) of this lane's B elements
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        int c = (c0 + NT * gq + nt) % g.nph;
+        if (c < 0) c += g.nph;
+        colb_n[nt] = c;
+        c += g.nph / 2;
+        colb_m[nt] = (c >= g.nph) ? c - g.nph : c;
+    }
+    double win[KS][NT];                   // win[ks][nt]: row in slot 4 ks + t, strip column NT g + nt
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) win[ks][nt] = 0.0;
+    int loaded_hi = INT_MIN;              // rows [loaded_hi - S, loaded_hi) are resident
+
+    // group q = rows 4q .. 4q+3 (offset by OFF); lane t loads row 4q + t if it lies in [rb, re)
+    auto load_group = [&](int q, int rb, int re, double (&v)[NT]) -> bool {
+        const int rr = 4 * q + t;
+        const bool in = rr >= rb && rr < re;
+        if (in) {
+            bool mirror;
+            const int64_t ro = grid_row(g, rr - OFF, mirror);
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) v[nt] = grid[ro + (mirror ? colb_m[nt] : colb_n[nt])];
+        }
+        return in;
+    };
+    // static register indices + predicates only (a run-time index would put the window in local memory)
+    auto commit_group = [&](int q, bool in, const double (&v)[NT]) {
+        const int ks = q % KS;
+#pragma unroll
+        for (int ksi = 0; ksi < KS; ++ksi)
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) win[ksi][nt] = (in && ks == ksi) ? v[nt] : win[ksi][nt];
+    };
+
+    double Xn = 0.0, Yn = 0.0;
+    if (start + lane < end) {
+        Xn = P.px[start + lane];
+        Yn = P.py[start + lane];
+    }
+    for (int batch = start; batch < end; batch += 32) {
+        const int idx = batch + lane;
+        const bool has = idx < end;
+        const double X = Xn, Y = Yn;
+        if (idx + 32 < end) {
+            Xn = P.px[idx + 32];
+            Yn = P.py[idx + 32];
+        }
+        const int a0 = mma_publish<W, S>(ws, kp, lane, X, Y, has ? 1.0 : 0.0, c0);
+        __syncwarp();
+        const int npt = min(32, end - batch);
+        int j0 = 0;
+        while (j0 < npt) {
+            // ---- tile: up to 8 consecutive points within SPAN rows of the first ----
+            const int row0 = __shfl_sync(0xffffffffu, a0, j0);
+            const unsigned fit = __ballot_sync(0xffffffffu, has && lane >= j0 && a0 - row0 <= SPAN);
+            const int cnt = min(8, __popc(fit));
+            // ---- rows [row0, row0 + S) must be resident.  Normally the previous tile prefetched them;
+            //      this synchronous fill runs for the first tile of an item and after large row jumps ----
+            if (loaded_hi < row0 + S) {
+                const int rb = max(loaded_hi, row0) + OFF, re = row0 + S + OFF;
+                for (int q = rb >> 2; q <= (re - 1) >> 2; ++q) {
+                    double v[NT];
+                    const bool in = load_group(q, rb, re, v);
+                    commit_group(q, in, v);
+                }
+                loaded_hi = row0 + S;
+            }
+            // ---- prefetch the rows the NEXT tile adds (at most two groups of 4 rows); they are committed
+            //      into the circular window after this tile's DMMAs, whose slots they recycle ----
+            int nrow0 = INT_MIN;
+            if (j0 + cnt < npt) nrow0 = __shfl_sync(0xffffffffu, a0, j0 + cnt);
+            else if (batch + 32 < end) nrow0 = __shfl_sync(0xffffffffu, (int)ceil(Xn - 0.5 * W), 0);
+            double pv0[NT], pv1[NT];
+            bool pin0 = false, pin1 = false, have1 = false;
+            int pq = 0, new_hi = loaded_hi;
+            const bool have0 = nrow0 != INT_MIN && nrow0 + S > loaded_hi;
+            if (have0) {
+                const int rb = loaded_hi + OFF, re = nrow0 + S + OFF;
+                pq = rb >> 2;
+                pin0 = load_group(pq, rb, re, pv0);
+                have1 = ((re - 1) >> 2) > pq;
+                if (have1) pin1 = load_group(pq + 1, rb, re, pv1);
+                new_hi = min(re, 4 * (pq + 2)) - OFF;
+            }
+            // ---- A fragments: theta weights of point j0 + g in circular slot order ----
+            const int jp = min(j0 + gq, 31);
+            const int a0p = __shfl_sync(0xffffffffu, a0, jp);
+            const int sp = (a0p + OFF) % S;
+            const bool live = gq < cnt;
+            double d[NT][2];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) d[nt][0] = d[nt][1] = 0.0;
+#pragma unroll
+            for (int ks = 0; ks < KS; ++ks) {
+                int i = 4 * ks + t - sp;
+                if (i < 0) i += S;
+                const double a = live ? ws.th[jp][i] : 0.0;
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) dmma_m8n8k4(d[nt][0], d[nt][1], a, win[ks][nt]);
+            }
+            if (have0) commit_group(pq, pin0, pv0);
+            if (have1) commit_group(pq + 1, pin1, pv1);
+            loaded_hi = new_hi;
+            // ---- phi contraction: this lane holds strip columns 2 NT t .. 2 NT t + 2 NT - 1 of point g ----
+            const int oy = ws.oy[jp];
+            double sum = 0.0;
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const unsigned ip = (unsigned)(NT * (2 * t + e) + nt - oy);
+                    const double wgt = (ip < (unsigned)W) ? ws.ph[jp][ip] : 0.0;
+                    sum = fma(d[nt][e], wgt, sum);
+                }
+            sum += __shfl_xor_sync(0xffffffffu, sum, 1);
+            sum += __shfl_xor_sync(0xffffffffu, sum, 2);
+            if (t == 0 && live) ws.res[jp] = sum;
+            j0 += cnt;
+        }
+        __syncwarp();
+        if (has) map[P.perm[idx]] = ws.res[lane];
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a8: type-1 spreading, FP64 / DMMA (grid must be zero on entry)
+// ---------------------------------------------------------------------------------------------
+template <int W>
+__global__ void __launch_bounds__(128)
+k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<double> kp,
+             const double* __restrict__ map, double* __restrict__ grid) {
+    constexpr int NT = mma_nt(W), MT = mma_mt(W), S = 8 * MT, SPAN = S - W, OFF = 2 * S;
+    using WS = MmaScratch<W, S>;
+    __shared__ __align__(16) WS s_ws[4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int item = blockIdx.x * 4 + warp;
+    if (item >= P.n_items) return;
+    const int start = P.item_off[item], end = P.item_off[item + 1];
+    if (start >= end) return;
+    WS& ws = s_ws[warp];
+    const NufftGeom& g = P.g;
+    const int strip = item % g.nstrip;
+    const int c0 = strip * g.mb - g.fl;
+    const int gq = lane >> 2, t = lane & 3;
+    int colc_n[2 * NT], colc_m[2 * NT];   // global columns of this lane's accumulator elements
+#pragma unroll
+    for (int q = 0; q < 2 * NT; ++q) {
+        // accumulator element (nt, e) sits at strip column NT (2t + e) + nt; q = NT e + nt
+        int c = (c0 + 2 * NT * t + q) % g.nph;
+        if (c < 0) c += g.nph;
+        colc_n[q] = c;
+        c += g.nph / 2;
+        colc_m[q] = (c >= g.nph) ? c - g.nph : c;
+    }
+    double acc[MT][NT][2];                // acc[mt][nt][e]: slot 8 mt + g, strip column NT (2t+e) + nt
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) acc[mt][nt][0] = acc[mt][nt][1] = 0.0;
+    int a_lo = INT_MIN;                   // slots hold rows [a_lo, a_lo + S)
+
+    // flush rows r0 .. r0 + n - 1 (n <= 8: one row per value of g) to the grid and clear their slots
+    auto flush_group = [&](int r0, int n) {
+        const int s0 = (r0 + OFF) % S;
+        const int i = (gq - s0) & 7;      // slot s0 + i is the one of this group with (slot & 7) == g
+        const bool rowhit = i < n;
+        int s = s0 + i;
+        if (s >= S) s -= S;
+        bool mirror;
+        const int64_t ro = grid_row(g, r0 + i, mirror);
+        // static indices + predicates only: a run-time index into acc would put it in local memory
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            const bool hit = rowhit && (mt == (s >> 3));
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const double v = acc[mt][nt][e];
+                    const int q = NT * e + nt;
+                    if (hit && v != 0.0) atomicAdd(&grid[ro + (mirror ? colc_m[q] : colc_n[q])], v);
+                    acc[mt][nt][e] = hit ? 0.0 : v;
+                }
+        }
+    };
+    constexpr int FG = SPAN >= 4 ? 4 : (SPAN >= 2 ? 2 : 1);   // rows flushed together
+
+    double Xn = 0.0, Yn = 0.0, vn = 0.0;
+    if (start + lane < end) {
+        Xn = P.px[start + lane];
+        Yn = P.py[start + lane];
+        vn = map[P.perm[start + lane]];
+    }
+    for (int batch = start; batch < end; batch += 32) {
+        const int idx = batch + lane;
+        const bool has = idx < end;
+        const double X = Xn, Y = Yn, val = has ? vn : 0.0;
+        if (idx + 32 < end) {
+            Xn = P.px[idx + 32];
+            Yn = P.py[idx + 32];
+            vn = map[P.perm[idx + 32]];
+        }
+        // the point's value rides on the theta weights
+        const int a0 = mma_publish<W, S>(ws, kp, lane, X, Y, val, c0);
+        __syncwarp();
+        const int npt = min(32, end - batch);
+        int j0 = 0;
+        while (j0 < npt) {
+            // ---- tile: up to 4 consecutive points within SPAN rows of the first ----
+            const int row0 = __shfl_sync(0xffffffffu, a0, j0);
+            // ---- rows below row0 are complete: flush them FG at a time (slots hold [a_lo, a_lo + S)) ----
+            if (a_lo == INT_MIN) a_lo = row0;
+            if (row0 - a_lo >= S) {
+#pragma unroll 1
+                for (int k = 0; k < S; k += 8) flush_group(a_lo + k, 8);
+                a_lo = row0;
+            }
+#pragma unroll 1
+            while (row0 - a_lo >= FG) {
+                flush_group(a_lo, FG);
+                a_lo += FG;
+            }
+            const unsigned fit = __ballot_sync(0xffffffffu, has && lane >= j0 && a0 - a_lo <= SPAN);
+            const int cnt = min(4, __popc(fit));
+            // ---- fragments: A[slot][point t] and B[point t][column], point = j0 + t ----
+            const int jp = min(j0 + t, 31);
+            const int a0p = __shfl_sync(0xffffffffu, a0, jp);
+            const int sp = (a0p + OFF) % S;
+            const int oy = ws.oy[jp];
+            const bool live = t < cnt;
+            double a[MT], b[NT];
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                int i = 8 * mt + gq - sp;
+                if (i < 0) i += S;
+                a[mt] = live ? ws.th[jp][i] : 0.0;
+            }
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                const unsigned ip = (unsigned)(NT * gq + nt - oy);
+                b[nt] = (ip < (unsigned)W) ? ws.ph[jp][ip] : 0.0;
+            }
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) dmma_m8n8k4(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
+            j0 += cnt;
+        }
+        __syncwarp();
+    }
+    if (a_lo != INT_MIN) {
+#pragma unroll 1
+        for (int k = 0; k < S; k += 8) flush_group(a_lo + k, 8);
+    }
+}
+
+template <int W>
+int launch_interp_mma(const NufftParams& P, const KernelHost& h, const void* grid, void* map, cudaStream_t s) {
+    const KernelPoly<double> kp = make_device_poly<double>(h);
+    k_interp_mma<W><<<(P.n_items + 3) / 4, 128, 0, s>>>(P, kp, (const double*)grid, (double*)map);
+    NUSHT_CUDA_TRY(cudaGetLastError());
+    return NUSHT_OK;
+}
+template <int W>
+int launch_spread_mma(const NufftParams& P, const KernelHost& h, const void* map, void* grid, cudaStream_t s) {
+    const KernelPoly<double> kp = make_device_poly<double>(h);
+    k_spread_mma<W><<<(P.n_items + 3) / 4, 128, 0, s>>>(P, kp, (const double*)map, (double*)grid);
+    NUSHT_CUDA_TRY(cudaGetLastError());
+    return NUSHT_OK;
+}
+
+int dispatch_interp_mma(int w, const NufftParams& P, const KernelHost& h, const void* grid, void* map, cudaStream_t s) {
+    switch (w) {
+#define NUSHT_CASE(WW) case WW: return launch_interp_mma<WW>(P, h, grid, map, s);
+        NUSHT_CASE(2) NUSHT_CASE(3) NUSHT_CASE(4) NUSHT_CASE(5) NUSHT_CASE(6) NUSHT_CASE(7) NUSHT_CASE(8)
+        NUSHT_CASE(9) NUSHT_CASE(10) NUSHT_CASE(11) NUSHT_CASE(12) NUSHT_CASE(13) NUSHT_CASE(14)   // eps >= 1e-13 -> w <= 14
+#undef NUSHT_CASE
+    }
+    return NUSHT_ERR_UNSUPPORTED;
+}
+int dispatch_spread_mma(int w, const NufftParams& P, const KernelHost& h, const void* map, void* grid, cudaStream_t s) {
+    switch (w) {
+#define NUSHT_CASE(WW) case WW: return launch_spread_mma<WW>(P, h, map, grid, s);
+        NUSHT_CASE(2) NUSHT_CASE(3) NUSHT_CASE(4) NUSHT_CASE(5) NUSHT_CASE(6) NUSHT_CASE(7) NUSHT_CASE(8)
+        NUSHT_CASE(9) NUSHT_CASE(10) NUSHT_CASE(11) NUSHT_CASE(12) NUSHT_CASE(13) NUSHT_CASE(14)   // eps >= 1e-13 -> w <= 14
+#undef NUSHT_CASE
+    }
+    return NUSHT_ERR_UNSUPPORTED;
+}
+
 // ---- host: Gauss-Legendre nodes (Newton on P_n), extended precision ----
 void gauss_legendre(int n, std::vector<long double>& x, std::vector<long double>& wt) {
     const long double PI_L = 3.14159265358979323846264338327950288L;
@@ -586,7 +1017,9 @@ int nufft_choose_kernel(nusht_plan_s* p) {
     p->ng.w = w;
     p->ng.fl = w / 2;
     p->ng.deg = h->deg;
-    p->ng.mb = 33 - w;
+    // strip width in footprint-origin columns: FP64 runs on the DMMA kernels (8 NT columns per strip),
+    // FP32 on the register-window kernels (32 columns per strip)
+    p->ng.mb = (p->dtype == NUSHT_F64) ? 8 * mma_nt(w) - w + 1 : 33 - w;
     // Chebyshev interpolation of tap i on u in [-1,1]:  z = (u + 1 - w + 2 i)/w
     const long double PI_L = 3.14159265358979323846264338327950288L;
     const int d = h->deg, nn = d + 1;
@@ -753,7 +1186,7 @@ int nufft_interp(nusht_plan_s* p, const void* grid, void* map, cudaStream_t s) {
     if (p->npts == 0) return NUSHT_OK;
     const KernelHost* h = g_kernel_of(p);
     const NufftParams P = make_nufft_params(p);
-    if (p->dtype == NUSHT_F64) return dispatch_interp<double>(p->ng.w, P, *h, grid, map, s);
+    if (p->dtype == NUSHT_F64) return dispatch_interp_mma(p->ng.w, P, *h, grid, map, s);
     return dispatch_interp<float>(p->ng.w, P, *h, grid, map, s);
 }
 
@@ -763,7 +1196,7 @@ int nufft_spread(nusht_plan_s* p, const void* map, void* grid, cudaStream_t s) {
     if (p->npts == 0) return NUSHT_OK;
     const KernelHost* h = g_kernel_of(p);
     const NufftParams P = make_nufft_params(p);
-    if (p->dtype == NUSHT_F64) return dispatch_spread<double>(p->ng.w, P, *h, map, grid, s);
+    if (p->dtype == NUSHT_F64) return dispatch_spread_mma(p->ng.w, P, *h, map, grid, s);
     return dispatch_spread<float>(p->ng.w, P, *h, map, grid, s);
 }
 

@@ -45,7 +45,7 @@ struct NufftGeom {
     int nrow_half;       // nth/2 + 1 stored rows (theta in [0, pi])
     int w, fl;           // kernel width, floor(w/2)
     int deg;             // polynomial degree
-    int mb;              // strip width in patch-origin columns = 33 - w
+    int mb;              // strip width in footprint-origin columns (strip columns - w + 1)
     int nstrip;          // ceil(nph / mb)
     int nseg;            // ceil((nth/2 + 2) / NUSHT_SEG_ROWS)
     double inv_hth, inv_hph;  // nth/(2 pi), nph/(2 pi)
