@@ -34,6 +34,10 @@ constexpr int LEG_WARPS = LEG_THREADS / 32;
 constexpr int LEG_TN = 128;        // n-steps (pairs of l) per shared-memory tile
 constexpr int LEG_CHUNK = 8;       // n-steps between exponent checks
 constexpr int LEG_R = 4;           // ring pairs per thread
+// synthesis: one warp per CTA, so that warps with different live/dead histories never wait for each other
+constexpr int SYN_THREADS = 32;
+constexpr int SYN_WARPS = SYN_THREADS / 32;
+constexpr int SYN_TN = 64;
 constexpr double SCALE_UP_LIMIT = 1.157920892373162e+77;   // 2^256
 constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
 
@@ -269,10 +273,10 @@ __device__ __forceinline__ void seed_pair(const LegParams& P, int m, int j, bool
 // a1 + a2: Legendre synthesis with fused DFS doubling.  grid = (pair blocks, m).
 // ---------------------------------------------------------------------------------------------
 template <int R>
-__global__ void __launch_bounds__(LEG_THREADS)
+__global__ void __launch_bounds__(SYN_THREADS)
 k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restrict__ ft) {
-    __shared__ __align__(16) double2 s_ab[2][LEG_TN];
-    __shared__ __align__(32) double4 s_aeo[2][LEG_TN];
+    __shared__ __align__(16) double2 s_ab[2][SYN_TN];
+    __shared__ __align__(32) double4 s_aeo[2][SYN_TN];
     __shared__ __align__(8) uint64_t s_bar[2];
 
     const int m = blockIdx.y;
@@ -280,8 +284,8 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
     const int ne = (L - m) / 2 + 1;
     const int64_t o = P.eoff[m];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int jb = (blockIdx.x * LEG_WARPS + warp) * (32 * R);
-    const int ntiles = (ne + LEG_TN - 1) / LEG_TN;
+    const int jb = (blockIdx.x * SYN_WARPS + warp) * (32 * R);
+    const int ntiles = (ne + SYN_TN - 1) / SYN_TN;
 
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
@@ -291,10 +295,10 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
     __syncthreads();
     auto issue = [&](int tile) {
         const int st = tile & 1;
-        const int cnt = min(LEG_TN, ne - tile * LEG_TN);
+        const int cnt = min(SYN_TN, ne - tile * SYN_TN);
         mbar_expect_tx(&s_bar[st], (uint32_t)cnt * 48u);
-        bulk_g2s(&s_ab[st][0], P.ab + o + (int64_t)tile * LEG_TN, (uint32_t)cnt * 16u, &s_bar[st]);
-        bulk_g2s(&s_aeo[st][0], aeo + o + (int64_t)tile * LEG_TN, (uint32_t)cnt * 32u, &s_bar[st]);
+        bulk_g2s(&s_ab[st][0], P.ab + o + (int64_t)tile * SYN_TN, (uint32_t)cnt * 16u, &s_bar[st]);
+        bulk_g2s(&s_aeo[st][0], aeo + o + (int64_t)tile * SYN_TN, (uint32_t)cnt * 32u, &s_bar[st]);
     };
     if (tid == 0) {
         issue(0);
@@ -317,7 +321,7 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
 
     for (int tile = 0; tile < ntiles; ++tile) {
         const int st = tile & 1;
-        const int cnt = min(LEG_TN, ne - tile * LEG_TN);
+        const int cnt = min(SYN_TN, ne - tile * SYN_TN);
         mbar_wait(&s_bar[st], (uint32_t)((tile >> 1) & 1));
         if (warp_has_work) {
             for (int i0 = 0; i0 < cnt; i0 += LEG_CHUNK) {
@@ -751,9 +755,9 @@ int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s) {
 }
 
 int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s) {
-    const int pairs_per_cta = LEG_THREADS * LEG_R;
+    const int pairs_per_cta = SYN_THREADS * LEG_R;
     dim3 grid((p->lg.npairs + pairs_per_cta - 1) / pairs_per_cta, p->mmax + 1);
-    k_legendre_synth<LEG_R><<<grid, LEG_THREADS, 0, s>>>(make_params(p), p->d_aeo, ft);
+    k_legendre_synth<LEG_R><<<grid, SYN_THREADS, 0, s>>>(make_params(p), p->d_aeo, ft);
     NUSHT_CUDA_TRY(cudaGetLastError());
     return NUSHT_OK;
 }

@@ -691,6 +691,16 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) win[ks][nt] = 0.0;
     int loaded_hi = INT_MIN;              // rows [loaded_hi - S, loaded_hi) are resident
+    int pf_hi = INT_MIN;                  // rows below pf_hi have been prefetched into L1
+    constexpr int PF_AHEAD = 8;
+    int colp_n, colp_m;                   // prefetch: lane covers strip columns 3 (lane & 7) ..
+    {
+        int c = (c0 + min(3 * (lane & 7), 8 * NT - 1)) % g.nph;
+        if (c < 0) c += g.nph;
+        colp_n = c;
+        c += g.nph / 2;
+        colp_m = (c >= g.nph) ? c - g.nph : c;
+    }
 
     // group q = rows 4q .. 4q+3 (offset by OFF); lane t loads row 4q + t if it lies in [rb, re)
     auto load_group = [&](int q, int rb, int re, double (&v)[NT]) -> bool {
@@ -726,6 +736,7 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             Xn = P.px[idx + 32];
             Yn = P.py[idx + 32];
         }
+        const int dst = has ? P.perm[idx] : 0;
         const int a0 = mma_publish<W, S>(ws, kp, lane, X, Y, has ? 1.0 : 0.0, c0);
         __syncwarp();
         const int npt = min(32, end - batch);
@@ -735,8 +746,16 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             const int row0 = __shfl_sync(0xffffffffu, a0, j0);
             const unsigned fit = __ballot_sync(0xffffffffu, has && lane >= j0 && a0 - row0 <= SPAN);
             const int cnt = min(8, __popc(fit));
-            // ---- rows [row0, row0 + S) must be resident.  Normally the previous tile prefetched them;
-            //      this synchronous fill runs for the first tile of an item and after large row jumps ----
+            // ---- L1 prefetch of the rows coming up: one instruction covers 4 rows (lane = row r4, 24-byte
+            //      chunk c8: every 32-byte sector of a <= 256-byte strip row is touched) ----
+            if (pf_hi < row0 + S + PF_AHEAD) {
+                if (pf_hi < row0 + S) pf_hi = row0 + S;
+                bool mirror;
+                const int64_t ro = grid_row(g, min(pf_hi + (lane >> 3), g.nth / 2), mirror);   // clamped: stays inside the grid
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(grid + ro + (mirror ? colp_m : colp_n)));
+                pf_hi += 4;
+            }
+            // ---- make rows [row0, row0 + S) resident (circular slots) ----
             if (loaded_hi < row0 + S) {
                 const int rb = max(loaded_hi, row0) + OFF, re = row0 + S + OFF;
                 for (int q = rb >> 2; q <= (re - 1) >> 2; ++q) {
@@ -745,23 +764,6 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
                     commit_group(q, in, v);
                 }
                 loaded_hi = row0 + S;
-            }
-            // ---- prefetch the rows the NEXT tile adds (at most two groups of 4 rows); they are committed
-            //      into the circular window after this tile's DMMAs, whose slots they recycle ----
-            int nrow0 = INT_MIN;
-            if (j0 + cnt < npt) nrow0 = __shfl_sync(0xffffffffu, a0, j0 + cnt);
-            else if (batch + 32 < end) nrow0 = __shfl_sync(0xffffffffu, (int)ceil(Xn - 0.5 * W), 0);
-            double pv0[NT], pv1[NT];
-            bool pin0 = false, pin1 = false, have1 = false;
-            int pq = 0, new_hi = loaded_hi;
-            const bool have0 = nrow0 != INT_MIN && nrow0 + S > loaded_hi;
-            if (have0) {
-                const int rb = loaded_hi + OFF, re = nrow0 + S + OFF;
-                pq = rb >> 2;
-                pin0 = load_group(pq, rb, re, pv0);
-                have1 = ((re - 1) >> 2) > pq;
-                if (have1) pin1 = load_group(pq + 1, rb, re, pv1);
-                new_hi = min(re, 4 * (pq + 2)) - OFF;
             }
             // ---- A fragments: theta weights of point j0 + g in circular slot order ----
             const int jp = min(j0 + gq, 31);
@@ -779,9 +781,6 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) dmma_m8n8k4(d[nt][0], d[nt][1], a, win[ks][nt]);
             }
-            if (have0) commit_group(pq, pin0, pv0);
-            if (have1) commit_group(pq + 1, pin1, pv1);
-            loaded_hi = new_hi;
             // ---- phi contraction: this lane holds strip columns 2 NT t .. 2 NT t + 2 NT - 1 of point g ----
             const int oy = ws.oy[jp];
             double sum = 0.0;
@@ -799,7 +798,7 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             j0 += cnt;
         }
         __syncwarp();
-        if (has) map[P.perm[idx]] = ws.res[lane];
+        if (has) map[dst] = ws.res[lane];
         __syncwarp();
     }
 }
