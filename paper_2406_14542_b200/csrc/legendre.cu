@@ -38,6 +38,10 @@ constexpr int LEG_R = 4;           // ring pairs per thread
 constexpr int SYN_THREADS = 32;
 constexpr int SYN_WARPS = SYN_THREADS / 32;
 constexpr int SYN_TN = 64;
+// adjoint: one warp per CTA as well; more ring pairs per thread halve the cost of the cross-lane reduction
+constexpr int ADJ_R = 8;
+constexpr int ADJ_TN = 64;
+constexpr int ADJ_CHUNK = 4;       // n-steps per transposing reduction / exponent check
 constexpr double SCALE_UP_LIMIT = 1.157920892373162e+77;   // 2^256
 constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
 
@@ -465,184 +469,180 @@ __device__ __forceinline__ double warp_transpose_reduce32(double (&v)[32], int l
     return v[0];
 }
 
+// v[0..15] per lane -> returns, in lanes 2q and 2q+1, the sum over all lanes of v[q]
+__device__ __forceinline__ double warp_transpose_reduce16(double (&v)[16], int lane) {
+#pragma unroll
+    for (int half = 8; half >= 1; half >>= 1) {
+        const int mask = 2 * half;
+        const bool up = (lane & mask) != 0;
+#pragma unroll
+        for (int i = 0; i < half; ++i) {
+            const double keep = up ? v[i + half] : v[i];
+            const double send = up ? v[i] : v[i + half];
+            v[i] = keep + shfl_xor_d(send, mask);
+        }
+    }
+    return v[0] + shfl_xor_d(v[0], 1);
+}
+
+// One warp per CTA: the warp owns 32 R ring pairs of one m for all n, forms the 4 partial sums of
+// every n-step over its rings (transposing butterfly, 4 steps x 4 sums at a time) and adds them to
+// eo[m][n] with native FP64 global reductions (RED.ADD.F64); eo must be zero on entry.  No warp
+// ever waits for another one, whatever its mix of live and dead ring pairs.
 template <int R>
-__global__ void __launch_bounds__(LEG_THREADS)
+__global__ void __launch_bounds__(32)
 k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restrict__ eo) {
-    __shared__ __align__(16) double2 s_ab[2][LEG_TN];
-    __shared__ __align__(16) double s_red[LEG_WARPS][LEG_TN * 4];
+    __shared__ __align__(16) double2 s_ab[2][ADJ_TN];
     __shared__ __align__(8) uint64_t s_bar[2];
 
-    const int m = blockIdx.x;
+    const int m = blockIdx.y;
     const int L = P.lmax;
     const int ne = (L - m) / 2 + 1;
     const int64_t o = P.eoff[m];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int ntiles = (ne + LEG_TN - 1) / LEG_TN;
-    const int pairs_per_pass = LEG_THREADS * R;
-    const int npass = (P.npairs + pairs_per_pass - 1) / pairs_per_pass;
+    const int lane = threadIdx.x;
+    const int jb = blockIdx.x * (32 * R);
+    const int ntiles = (ne + ADJ_TN - 1) / ADJ_TN;
     const double sgn = (m & 1) ? -1.0 : 1.0;
     const double2* row = gt + (int64_t)m * P.nth2;
 
-    if (tid == 0) {
+    if (lane == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
         mbar_fence_init();
     }
-    __syncthreads();
+    __syncwarp();
     auto issue = [&](int tile) {
         const int st = tile & 1;
-        const int cnt = min(LEG_TN, ne - tile * LEG_TN);
+        const int cnt = min(ADJ_TN, ne - tile * ADJ_TN);
         mbar_expect_tx(&s_bar[st], (uint32_t)cnt * 16u);
-        bulk_g2s(&s_ab[st][0], P.ab + o + (int64_t)tile * LEG_TN, (uint32_t)cnt * 16u, &s_bar[st]);
+        bulk_g2s(&s_ab[st][0], P.ab + o + (int64_t)tile * ADJ_TN, (uint32_t)cnt * 16u, &s_bar[st]);
     };
-    uint32_t uses[2] = {0u, 0u};   // completed phases of each stage's mbarrier (same in every thread)
+    if (lane == 0) {
+        issue(0);
+        if (ntiles > 1) issue(1);
+    }
 
-    for (int pass = 0; pass < npass; ++pass) {
-        const int jb = pass * pairs_per_pass + warp * (32 * R);
-        const bool warp_has_work = jb < P.npairs;
-        double x2[R], p0[R], p1[R], gere[R], geim[R], gore[R], goim[R];
-        int ex[R];
-        bool valid[R];
+    double x2[R], p0[R], p1[R], gere[R], geim[R], gore[R], goim[R];
+    int ex[R];
+    bool valid[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int j = jb + r * 32 + lane;
-            valid[r] = j < P.npairs;
-            x2[r] = valid[r] ? P.x2[j] : 0.0;
-            seed_pair(P, m, j, valid[r], p1[r], ex[r]);
-            p0[r] = 0.0;
-            gere[r] = geim[r] = gore[r] = goim[r] = 0.0;
-            if (valid[r]) {
-                // a10 fold (D^T): G[k] = Gt[k] + (-1)^m Gt[Ntheta-k] away from the poles
-                const int kn = j, ks = P.nr - 1 - j;
-                double2 gn = row[kn];
-                if (kn != 0) {
-                    const double2 t = row[P.nth2 - kn];
-                    gn.x = fma(sgn, t.x, gn.x);
-                    gn.y = fma(sgn, t.y, gn.y);
-                }
-                double2 gs = make_double2(0.0, 0.0);
-                if (ks != kn) {
-                    gs = row[ks];
-                    if (kn != 0) {
-                        const double2 t = row[P.nth2 - ks];
-                        gs.x = fma(sgn, t.x, gs.x);
-                        gs.y = fma(sgn, t.y, gs.y);
-                    }
-                }
-                const double x = P.x[j];
-                gere[r] = gn.x + gs.x;
-                geim[r] = gn.y + gs.y;
-                gore[r] = x * (gn.x - gs.x);
-                goim[r] = x * (gn.y - gs.y);
+    for (int r = 0; r < R; ++r) {
+        const int j = jb + r * 32 + lane;
+        valid[r] = j < P.npairs;
+        x2[r] = valid[r] ? P.x2[j] : 0.0;
+        seed_pair(P, m, j, valid[r], p1[r], ex[r]);
+        p0[r] = 0.0;
+        gere[r] = geim[r] = gore[r] = goim[r] = 0.0;
+        if (valid[r]) {
+            // a10 fold (D^T): G[k] = Gt[k] + (-1)^m Gt[Ntheta-k] away from the poles
+            const int kn = j, ks = P.nr - 1 - j;
+            double2 gn = row[kn];
+            if (kn != 0) {
+                const double2 t = row[P.nth2 - kn];
+                gn.x = fma(sgn, t.x, gn.x);
+                gn.y = fma(sgn, t.y, gn.y);
             }
+            double2 gs = make_double2(0.0, 0.0);
+            if (ks != kn) {
+                gs = row[ks];
+                if (kn != 0) {
+                    const double2 t = row[P.nth2 - ks];
+                    gs.x = fma(sgn, t.x, gs.x);
+                    gs.y = fma(sgn, t.y, gs.y);
+                }
+            }
+            const double x = P.x[j];
+            gere[r] = gn.x + gs.x;
+            geim[r] = gn.y + gs.y;
+            gore[r] = x * (gn.x - gs.x);
+            goim[r] = x * (gn.y - gs.y);
         }
-        if (tid == 0) {
-            // the two stages are free here: every tile of the previous pass was consumed
-            issue(0);
-            if (ntiles > 1) issue(1);
-        }
-        for (int tile = 0; tile < ntiles; ++tile) {
-            const int st = tile & 1;
-            const int cnt = min(LEG_TN, ne - tile * LEG_TN);
-            mbar_wait(&s_bar[st], uses[st] & 1u);
-            uses[st] += 1u;
-            if (warp_has_work) {
-                for (int i0 = 0; i0 < cnt; i0 += LEG_CHUNK) {
-                    const int ns = min(LEG_CHUNK, cnt - i0);
-                    bool any_dead = false, any_live = false;
+    }
+
+    for (int tile = 0; tile < ntiles; ++tile) {
+        const int st = tile & 1;
+        const int cnt = min(ADJ_TN, ne - tile * ADJ_TN);
+        mbar_wait(&s_bar[st], (uint32_t)((tile >> 1) & 1));
+        for (int i0 = 0; i0 < cnt; i0 += ADJ_CHUNK) {
+            const int ns = min(ADJ_CHUNK, cnt - i0);
+            bool any_dead = false, any_live = false;
 #pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        any_dead |= (ex[r] > 0);
-                        any_live |= (valid[r] && ex[r] == 0);
-                    }
-                    const bool w_dead = __any_sync(0xffffffffu, any_dead);
-                    const bool w_live = __any_sync(0xffffffffu, any_live);
-                    if (w_live) {
-                        double v[32];
+            for (int r = 0; r < R; ++r) {
+                any_dead |= (ex[r] > 0);
+                any_live |= (valid[r] && ex[r] == 0);
+            }
+            const bool w_dead = __any_sync(0xffffffffu, any_dead);
+            const bool w_live = __any_sync(0xffffffffu, any_live);
+            if (w_live) {
+                double v[4 * ADJ_CHUNK];
 #pragma unroll
-                        for (int q = 0; q < 32; ++q) v[q] = 0.0;
-                        if (!w_dead && ns == LEG_CHUNK) {
+                for (int q = 0; q < 4 * ADJ_CHUNK; ++q) v[q] = 0.0;
+                if (!w_dead && ns == ADJ_CHUNK) {
 #pragma unroll
-                            for (int i = 0; i < LEG_CHUNK; ++i) {
-                                const double2 ab = s_ab[st][i0 + i];
+                    for (int i = 0; i < ADJ_CHUNK; ++i) {
+                        const double2 ab = s_ab[st][i0 + i];
 #pragma unroll
-                                for (int r = 0; r < R; ++r) {
-                                    const double t = fma(ab.x, x2[r], ab.y);
-                                    v[4 * i + 0] = fma(p1[r], gere[r], v[4 * i + 0]);
-                                    v[4 * i + 1] = fma(p1[r], geim[r], v[4 * i + 1]);
-                                    v[4 * i + 2] = fma(p1[r], gore[r], v[4 * i + 2]);
-                                    v[4 * i + 3] = fma(p1[r], goim[r], v[4 * i + 3]);
-                                    const double pn = fma(t, p1[r], p0[r]);
-                                    p0[r] = p1[r];
-                                    p1[r] = pn;
-                                }
-                            }
-                        } else {
-#pragma unroll
-                            for (int i = 0; i < LEG_CHUNK; ++i) {
-                                const bool on = i < ns;
-                                const double2 ab = s_ab[st][min(i0 + i, LEG_TN - 1)];
-#pragma unroll
-                                for (int r = 0; r < R; ++r) {
-                                    const double t = fma(ab.x, x2[r], ab.y);
-                                    const double pm = (on && ex[r] == 0) ? p1[r] : 0.0;
-                                    v[4 * i + 0] = fma(pm, gere[r], v[4 * i + 0]);
-                                    v[4 * i + 1] = fma(pm, geim[r], v[4 * i + 1]);
-                                    v[4 * i + 2] = fma(pm, gore[r], v[4 * i + 2]);
-                                    v[4 * i + 3] = fma(pm, goim[r], v[4 * i + 3]);
-                                    if (on) {
-                                        const double pn = fma(t, p1[r], p0[r]);
-                                        p0[r] = p1[r];
-                                        p1[r] = pn;
-                                    }
-                                }
-                            }
+                        for (int r = 0; r < R; ++r) {
+                            const double t = fma(ab.x, x2[r], ab.y);
+                            v[4 * i + 0] = fma(p1[r], gere[r], v[4 * i + 0]);
+                            v[4 * i + 1] = fma(p1[r], geim[r], v[4 * i + 1]);
+                            v[4 * i + 2] = fma(p1[r], gore[r], v[4 * i + 2]);
+                            v[4 * i + 3] = fma(p1[r], goim[r], v[4 * i + 3]);
+                            const double pn = fma(t, p1[r], p0[r]);
+                            p0[r] = p1[r];
+                            p1[r] = pn;
                         }
-                        const double tot = warp_transpose_reduce32(v, lane);
-                        s_red[warp][4 * i0 + lane] = tot;
-                    } else {
-                        for (int i = 0; i < ns; ++i) {
-                            const double2 ab = s_ab[st][i0 + i];
+                    }
+                } else {
 #pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                const double t = fma(ab.x, x2[r], ab.y);
+                    for (int i = 0; i < ADJ_CHUNK; ++i) {
+                        const bool on = i < ns;
+                        const double2 ab = s_ab[st][min(i0 + i, ADJ_TN - 1)];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const double t = fma(ab.x, x2[r], ab.y);
+                            const double pm = (on && ex[r] == 0) ? p1[r] : 0.0;
+                            v[4 * i + 0] = fma(pm, gere[r], v[4 * i + 0]);
+                            v[4 * i + 1] = fma(pm, geim[r], v[4 * i + 1]);
+                            v[4 * i + 2] = fma(pm, gore[r], v[4 * i + 2]);
+                            v[4 * i + 3] = fma(pm, goim[r], v[4 * i + 3]);
+                            if (on) {
                                 const double pn = fma(t, p1[r], p0[r]);
                                 p0[r] = p1[r];
                                 p1[r] = pn;
                             }
                         }
-                        s_red[warp][4 * i0 + lane] = 0.0;
-                    }
-                    if (w_dead) {
-#pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            if (ex[r] > 0 && fabs(p1[r]) > SCALE_UP_LIMIT) {
-                                p1[r] *= SCALE_DOWN;
-                                p0[r] *= SCALE_DOWN;
-                                ex[r] -= 1;
-                            }
-                        }
                     }
                 }
-            } else if (tile == 0) {
-                // idle warp in this pass: its slice must read as zero for every tile of the pass
-                for (int q = lane; q < 4 * LEG_TN; q += 32) s_red[warp][q] = 0.0;
-            }
-            __syncthreads();
-            // cross-warp sum of this tile and accumulation into eo (same thread -> same address every pass)
-            {
-                double* out = reinterpret_cast<double*>(eo + o + (int64_t)tile * LEG_TN);
-                for (int q = tid; q < 4 * cnt; q += LEG_THREADS) {
-                    double sum = 0.0;
+                const double tot = warp_transpose_reduce16(v, lane);
+                const int q = lane >> 1;          // value index 4 * step + component
+                if (!(lane & 1) && (q >> 2) < ns)
+                    atomicAdd(reinterpret_cast<double*>(eo + o + (int64_t)tile * ADJ_TN + i0) + q, tot);
+            } else {
+                for (int i = 0; i < ns; ++i) {
+                    const double2 ab = s_ab[st][i0 + i];
 #pragma unroll
-                    for (int wq = 0; wq < LEG_WARPS; ++wq) sum += s_red[wq][q];
-                    if (pass == 0) out[q] = sum;
-                    else out[q] += sum;
+                    for (int r = 0; r < R; ++r) {
+                        const double t = fma(ab.x, x2[r], ab.y);
+                        const double pn = fma(t, p1[r], p0[r]);
+                        p0[r] = p1[r];
+                        p1[r] = pn;
+                    }
                 }
             }
-            __syncthreads();
-            if (tid == 0 && tile + 2 < ntiles) issue(tile + 2);
+            if (w_dead) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if (ex[r] > 0 && fabs(p1[r]) > SCALE_UP_LIMIT) {
+                        p1[r] *= SCALE_DOWN;
+                        p0[r] *= SCALE_DOWN;
+                        ex[r] -= 1;
+                    }
+                }
+            }
         }
+        __syncwarp();
+        if (lane == 0 && tile + 2 < ntiles) issue(tile + 2);
     }
 }
 
@@ -763,7 +763,11 @@ int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s) {
 }
 
 int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
-    k_legendre_adjoint<LEG_R><<<p->mmax + 1, LEG_THREADS, 0, s>>>(make_params(p), gt, p->d_aeo);
+    // the kernel accumulates with global reductions
+    NUSHT_CUDA_TRY(cudaMemsetAsync(p->d_aeo, 0, sizeof(double4) * (size_t)p->n_e_total, s));
+    const int pairs_per_cta = 32 * ADJ_R;
+    dim3 grid((p->lg.npairs + pairs_per_cta - 1) / pairs_per_cta, p->mmax + 1);
+    k_legendre_adjoint<ADJ_R><<<grid, 32, 0, s>>>(make_params(p), gt, p->d_aeo);
     NUSHT_CUDA_TRY(cudaGetLastError());
     return NUSHT_OK;
 }
