@@ -39,7 +39,7 @@ constexpr int SYN_THREADS = 32;
 constexpr int SYN_WARPS = SYN_THREADS / 32;
 constexpr int SYN_TN = 64;
 // adjoint: one warp per CTA as well; more ring pairs per thread halve the cost of the cross-lane reduction
-constexpr int ADJ_R = 8;
+constexpr int ADJ_R = 4;
 constexpr int ADJ_TN = 64;
 constexpr int ADJ_CHUNK = 4;       // n-steps per transposing reduction / exponent check
 constexpr double SCALE_UP_LIMIT = 1.157920892373162e+77;   // 2^256
@@ -486,13 +486,16 @@ __device__ __forceinline__ double warp_transpose_reduce16(double (&v)[16], int l
 }
 
 // One warp per CTA: the warp owns 32 R ring pairs of one m for all n, forms the 4 partial sums of
-// every n-step over its rings (transposing butterfly, 4 steps x 4 sums at a time) and adds them to
-// eo[m][n] with native FP64 global reductions (RED.ADD.F64); eo must be zero on entry.  No warp
-// ever waits for another one, whatever its mix of live and dead ring pairs.
+// every n-step over its rings (4 steps x 4 sums at a time, transposed through shared memory) and
+// adds them to eo[m][n] with native FP64 global reductions (RED.ADD.F64); eo must be zero on entry.
+// No warp ever waits for another one, whatever its mix of live and dead ring pairs.  A dead pair
+// (scaled value below range) keeps G = 0 in registers, so the inner loop needs no masks; its folded
+// G values are loaded when the pair comes into range.
 template <int R>
 __global__ void __launch_bounds__(32)
 k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restrict__ eo) {
     __shared__ __align__(16) double2 s_ab[2][ADJ_TN];
+    __shared__ __align__(16) double s_tr[4 * ADJ_CHUNK][33];
     __shared__ __align__(8) uint64_t s_bar[2];
 
     const int m = blockIdx.y;
@@ -525,6 +528,31 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
     double x2[R], p0[R], p1[R], gere[R], geim[R], gore[R], goim[R];
     int ex[R];
     bool valid[R];
+    // a10 fold (D^T) of ring pair j: G[k] = Gt[k] + (-1)^m Gt[Ntheta-k] away from the poles, then the
+    // even / odd (in l - m) combinations of the north and south ring
+    auto load_g = [&](int j, double& ere, double& eim, double& ore_, double& oim) {
+        const int kn = j, ks = P.nr - 1 - j;
+        double2 gn = row[kn];
+        if (kn != 0) {
+            const double2 t = row[P.nth2 - kn];
+            gn.x = fma(sgn, t.x, gn.x);
+            gn.y = fma(sgn, t.y, gn.y);
+        }
+        double2 gs = make_double2(0.0, 0.0);
+        if (ks != kn) {
+            gs = row[ks];
+            if (kn != 0) {
+                const double2 t = row[P.nth2 - ks];
+                gs.x = fma(sgn, t.x, gs.x);
+                gs.y = fma(sgn, t.y, gs.y);
+            }
+        }
+        const double x = P.x[j];
+        ere = gn.x + gs.x;
+        eim = gn.y + gs.y;
+        ore_ = x * (gn.x - gs.x);
+        oim = x * (gn.y - gs.y);
+    };
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int j = jb + r * 32 + lane;
@@ -533,30 +561,7 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
         seed_pair(P, m, j, valid[r], p1[r], ex[r]);
         p0[r] = 0.0;
         gere[r] = geim[r] = gore[r] = goim[r] = 0.0;
-        if (valid[r]) {
-            // a10 fold (D^T): G[k] = Gt[k] + (-1)^m Gt[Ntheta-k] away from the poles
-            const int kn = j, ks = P.nr - 1 - j;
-            double2 gn = row[kn];
-            if (kn != 0) {
-                const double2 t = row[P.nth2 - kn];
-                gn.x = fma(sgn, t.x, gn.x);
-                gn.y = fma(sgn, t.y, gn.y);
-            }
-            double2 gs = make_double2(0.0, 0.0);
-            if (ks != kn) {
-                gs = row[ks];
-                if (kn != 0) {
-                    const double2 t = row[P.nth2 - ks];
-                    gs.x = fma(sgn, t.x, gs.x);
-                    gs.y = fma(sgn, t.y, gs.y);
-                }
-            }
-            const double x = P.x[j];
-            gere[r] = gn.x + gs.x;
-            geim[r] = gn.y + gs.y;
-            gore[r] = x * (gn.x - gs.x);
-            goim[r] = x * (gn.y - gs.y);
-        }
+        if (valid[r] && ex[r] == 0) load_g(j, gere[r], geim[r], gore[r], goim[r]);
     }
 
     for (int tile = 0; tile < ntiles; ++tile) {
@@ -574,50 +579,43 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
             const bool w_dead = __any_sync(0xffffffffu, any_dead);
             const bool w_live = __any_sync(0xffffffffu, any_live);
             if (w_live) {
+                // always ADJ_CHUNK steps: beyond the end of the column the sums are dropped below and
+                // the recurrence state is never used again
                 double v[4 * ADJ_CHUNK];
 #pragma unroll
                 for (int q = 0; q < 4 * ADJ_CHUNK; ++q) v[q] = 0.0;
-                if (!w_dead && ns == ADJ_CHUNK) {
 #pragma unroll
-                    for (int i = 0; i < ADJ_CHUNK; ++i) {
-                        const double2 ab = s_ab[st][i0 + i];
+                for (int i = 0; i < ADJ_CHUNK; ++i) {
+                    const double2 ab = s_ab[st][min(i0 + i, cnt - 1)];
 #pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            const double t = fma(ab.x, x2[r], ab.y);
-                            v[4 * i + 0] = fma(p1[r], gere[r], v[4 * i + 0]);
-                            v[4 * i + 1] = fma(p1[r], geim[r], v[4 * i + 1]);
-                            v[4 * i + 2] = fma(p1[r], gore[r], v[4 * i + 2]);
-                            v[4 * i + 3] = fma(p1[r], goim[r], v[4 * i + 3]);
-                            const double pn = fma(t, p1[r], p0[r]);
-                            p0[r] = p1[r];
-                            p1[r] = pn;
-                        }
-                    }
-                } else {
-#pragma unroll
-                    for (int i = 0; i < ADJ_CHUNK; ++i) {
-                        const bool on = i < ns;
-                        const double2 ab = s_ab[st][min(i0 + i, ADJ_TN - 1)];
-#pragma unroll
-                        for (int r = 0; r < R; ++r) {
-                            const double t = fma(ab.x, x2[r], ab.y);
-                            const double pm = (on && ex[r] == 0) ? p1[r] : 0.0;
-                            v[4 * i + 0] = fma(pm, gere[r], v[4 * i + 0]);
-                            v[4 * i + 1] = fma(pm, geim[r], v[4 * i + 1]);
-                            v[4 * i + 2] = fma(pm, gore[r], v[4 * i + 2]);
-                            v[4 * i + 3] = fma(pm, goim[r], v[4 * i + 3]);
-                            if (on) {
-                                const double pn = fma(t, p1[r], p0[r]);
-                                p0[r] = p1[r];
-                                p1[r] = pn;
-                            }
-                        }
+                    for (int r = 0; r < R; ++r) {
+                        const double t = fma(ab.x, x2[r], ab.y);
+                        v[4 * i + 0] = fma(p1[r], gere[r], v[4 * i + 0]);
+                        v[4 * i + 1] = fma(p1[r], geim[r], v[4 * i + 1]);
+                        v[4 * i + 2] = fma(p1[r], gore[r], v[4 * i + 2]);
+                        v[4 * i + 3] = fma(p1[r], goim[r], v[4 * i + 3]);
+                        const double pn = fma(t, p1[r], p0[r]);
+                        p0[r] = p1[r];
+                        p1[r] = pn;
                     }
                 }
-                const double tot = warp_transpose_reduce16(v, lane);
-                const int q = lane >> 1;          // value index 4 * step + component
-                if (!(lane & 1) && (q >> 2) < ns)
-                    atomicAdd(reinterpret_cast<double*>(eo + o + (int64_t)tile * ADJ_TN + i0) + q, tot);
+                // cross-lane sums: transpose through shared memory (value q of lane l at s_tr[q][l]);
+                // lane l then adds 16 entries of row l & 15, and the two halves are combined by a shuffle
+#pragma unroll
+                for (int q = 0; q < 4 * ADJ_CHUNK; ++q) s_tr[q][lane] = v[q];
+                __syncwarp();
+                const double* src = &s_tr[lane & 15][16 * (lane >> 4)];
+                double tot = 0.0, tot2 = 0.0;
+#pragma unroll
+                for (int k = 0; k < 16; k += 2) {
+                    tot += src[k];
+                    tot2 += src[k + 1];
+                }
+                tot += tot2;
+                tot += shfl_xor_d(tot, 16);
+                __syncwarp();
+                if (lane < 16 && (lane >> 2) < ns)      // lane = 4 * step + component
+                    atomicAdd(reinterpret_cast<double*>(eo + o + (int64_t)tile * ADJ_TN + i0) + lane, tot);
             } else {
                 for (int i = 0; i < ns; ++i) {
                     const double2 ab = s_ab[st][i0 + i];
@@ -637,6 +635,7 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
                         p1[r] *= SCALE_DOWN;
                         p0[r] *= SCALE_DOWN;
                         ex[r] -= 1;
+                        if (ex[r] == 0) load_g(jb + r * 32 + lane, gere[r], geim[r], gore[r], goim[r]);
                     }
                 }
             }
