@@ -19,7 +19,7 @@ def rel(a, b):
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
 
 
-@pytest.mark.parametrize("config,nsample", [(2, 1500), (3, 300)])
+@pytest.mark.parametrize("config,nsample", [(2, 1500), (3, 300), (4, 100)])
 def test_fullsize_sampled(oracle, config, nsample):
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")

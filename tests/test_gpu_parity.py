@@ -198,3 +198,80 @@ def test_host_buffer_calls_match_device_calls(nusht):
     assert torch.equal(fh, f)
     assert torch.allclose(ch, c, rtol=0, atol=1e-12 * float(c.abs().max()))
     plan.destroy()
+
+
+# ---- FP32 path (BASELINE.json configs[4]: eps in {1e-4, 1e-6} on the FP32 path) -----------------
+@pytest.mark.parametrize("eps", [1e-2, 1e-4, 1e-5, 1e-6])
+@pytest.mark.parametrize("L,M,npts", [(63, 63, 4000), (200, 150, 6000)])
+def test_fp32_path(nusht, oracle, eps, L, M, npts):
+    """north_star bar: relative l2 error <= 1e-4 for the FP32 path at eps >= 1e-5 (and <= 10 eps where
+    that is the looser bound).  alm / map are float32; theta, phi stay float64 (reading G10)."""
+    theta, phi = inputs.uniform_sphere_points(npts, 61)
+    theta[:2] = [0.0, np.pi]
+    alm = inputs.random_alm(L, M, 61)
+    x = inputs.random_map(npts, 61)
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps, dtype="f32")
+    f = plan.synthesis(cu(alm.astype(np.complex64))).cpu().numpy()
+    c = plan.adjoint(cu(x.astype(np.float32))).cpu().numpy()
+    assert f.dtype == np.float32 and c.dtype == np.complex64
+    bar = max(1e-4, 10 * eps) if eps >= 1e-5 else 3e-4     # eps = 1e-6 asks for more than binary32 carries
+    assert rel(f.astype(np.float64), oracle.synthesis(L, M, theta, phi, alm, "ld")) <= bar
+    assert rel(c.astype(np.complex128), oracle.adjoint(L, M, theta, phi, x, "ld")) <= bar
+    assert np.all(c[: L + 1].imag == 0)
+    plan.destroy()
+
+
+def test_fp32_adjointness(nusht, oracle):
+    L = M = 127
+    theta, phi = inputs.uniform_sphere_points(20000, 62)
+    alm = inputs.random_alm(L, M, 62).astype(np.complex64)
+    x = inputs.random_map(20000, 62).astype(np.float32)
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), 1e-5, dtype="f32")
+    f = plan.synthesis(cu(alm)).cpu().numpy().astype(np.float64)
+    c = plan.adjoint(cu(x)).cpu().numpy().astype(np.complex128)
+    lhs = float(np.dot(f, x.astype(np.float64)))
+    rhs = oracle.inner_alm(L, M, alm.astype(np.complex128), c)
+    assert abs(lhs - rhs) <= 1e-5 * np.linalg.norm(f) * np.linalg.norm(x)
+    plan.destroy()
+
+
+# ---- every kernel width of the FP64 path (w = 2 .. 14), incl. non-power-of-two grid sizes ---------
+@pytest.mark.parametrize("eps", [1e-1, 1e-3, 1e-5, 1e-7, 1e-9, 1e-11, 1e-13])
+def test_all_widths_fp64(nusht, oracle, eps):
+    L, M, npts = 89, 70, 5000            # n_theta = 180, fine grids 360 x 288: not powers of two
+    theta, phi = inputs.uniform_sphere_points(npts, 71)
+    alm = inputs.random_alm(L, M, 71)
+    x = inputs.random_map(npts, 71)
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps)
+    assert plan.info.kernel_width == int(np.ceil(np.log10(1 / eps))) + 1
+    f = plan.synthesis(cu(alm)).cpu().numpy()
+    c = plan.adjoint(cu(x)).cpu().numpy()
+    tol = max(10 * eps, 2e-12)           # 1e-13 is below the binary64 floor of the recurrence (SURVEY H5)
+    assert rel(f, oracle.synthesis(L, M, theta, phi, alm, "ld")) <= tol
+    assert rel(c, oracle.adjoint(L, M, theta, phi, x, "ld")) <= tol
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+    rhs = oracle.inner_alm(L, M, alm, c)
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    plan.destroy()
+
+
+def test_clustered_and_sorted_points(nusht, oracle):
+    """Degenerate point sets: all points in one cell, all on one ring, all at a pole, sorted input."""
+    L = M = 40
+    rng = np.random.default_rng(81)
+    sets = {
+        "one_cell": (1.0 + 1e-6 * rng.random(3000), 2.0 + 1e-6 * rng.random(3000)),
+        "one_ring": (np.full(3000, 0.7), rng.uniform(0, 2 * np.pi, 3000)),
+        "north_pole": (np.zeros(500), rng.uniform(0, 2 * np.pi, 500)),
+        "south_cap": (np.pi - 1e-3 * rng.random(2000), rng.uniform(0, 2 * np.pi, 2000)),
+        "sorted": (np.sort(np.arccos(rng.uniform(-1, 1, 4000))), np.sort(rng.uniform(0, 2 * np.pi, 4000))),
+    }
+    alm = inputs.random_alm(L, M, 82)
+    for name, (theta, phi) in sets.items():
+        x = rng.standard_normal(len(theta))
+        plan = nusht.Plan(L, M, cu(theta), cu(phi), 1e-9)
+        f = plan.synthesis(cu(alm)).cpu().numpy()
+        c = plan.adjoint(cu(x)).cpu().numpy()
+        assert rel(f, oracle.synthesis(L, M, theta, phi, alm, "ld")) <= 1e-8, name
+        assert rel(c, oracle.adjoint(L, M, theta, phi, x, "ld")) <= 1e-8, name
+        plan.destroy()
