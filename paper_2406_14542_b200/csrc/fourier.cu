@@ -73,6 +73,65 @@ __global__ void k_deconv_trunc(int L, int M, int nth2, int nth, const typename C
     ft[(int64_t)m * nth2 + r] = out;
 }
 
+// a5 / a9 layout change between the theta pass (H[m][a], a contiguous) and the phi pass
+// (Ht[a][m], m contiguous, row length mp = n_phi/2 + 1): 32 x 32 tiles through shared memory.
+// Only rows a <= n_theta/2 (theta in [0, pi]) and columns m <= mmax are moved.
+template <typename C>
+__global__ void __launch_bounds__(256)
+k_h_to_ht(int M, int nth, int nrow_half, int mp, const C* __restrict__ h, C* __restrict__ ht) {
+    __shared__ C tile[32][33];
+    const int a0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int m = m0 + r, a = a0 + tx;
+        if (m <= M && a < nrow_half) tile[r][tx] = h[(int64_t)m * nth + a];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int a = a0 + r, m = m0 + tx;
+        if (m <= M && a < nrow_half) ht[(int64_t)a * mp + m] = tile[tx][r];
+    }
+}
+
+// transpose back, fused with the zero-extension of the theta axis to the full period (the
+// transpose of "keep rows 0 .. n_theta/2"): H[m][a] = Ht[a][m] for a <= n_theta/2, 0 beyond
+template <typename C>
+__global__ void __launch_bounds__(256)
+k_ht_to_h(int M, int nth, int nrow_half, int mp, const C* __restrict__ ht, C* __restrict__ h) {
+    __shared__ C tile[32][33];
+    const int a0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    if (a0 < nrow_half) {
+#pragma unroll
+        for (int r = ty; r < 32; r += 8) {
+            const int a = a0 + r, m = m0 + tx;
+            if (m <= M && a < nrow_half) tile[r][tx] = ht[(int64_t)a * mp + m];
+        }
+    }
+    __syncthreads();
+    C zero;
+    zero.x = 0;
+    zero.y = 0;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int m = m0 + r, a = a0 + tx;
+        if (m <= M && a < nth) h[(int64_t)m * nth + a] = (a < nrow_half) ? tile[tx][r] : zero;
+    }
+}
+
+// plan-time probe: does any word of columns m > M of Ht differ from zero?
+__global__ void k_tail_nonzero(int M, int nrow_half, int mp, int words_per_elem, const unsigned long long* __restrict__ ht,
+                               int* __restrict__ flag) {
+    const int64_t tail = (int64_t)(mp - M - 1) * words_per_elem;
+    const int64_t total = (int64_t)nrow_half * tail;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t a = i / tail, q = i - a * tail;
+        if (ht[(a * mp + M + 1) * words_per_elem + q] != 0ull) *flag = 1;
+    }
+}
+
 }  // namespace
 
 template <typename T>
@@ -103,11 +162,16 @@ int fourier_build(nusht_plan_s* p) {
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_pth, pth.data(), sizeof(double) * (2 * L + 1), cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_pph, pph.data(), sizeof(double) * (M + 1), cudaMemcpyHostToDevice));
 
-    const size_t hbytes = (size_t)(g.nph / 2 + 1) * (size_t)g.nth * csz;
+    const int mp = g.nph / 2 + 1;
+    const size_t hbytes = (size_t)(M + 1) * (size_t)g.nth * csz;
+    const size_t htbytes = (size_t)g.nrow_half * (size_t)mp * csz;
     const size_t gbytes = (size_t)g.nrow_half * (size_t)g.nph * rsz;
     NUSHT_TRY(f_alloc(&p->d_h, hbytes, p));
+    NUSHT_TRY(f_alloc(&p->d_ht, htbytes, p));
+    NUSHT_TRY(f_alloc(&p->d_ht_adj, htbytes, p));   // R2C output of the adjoint (fills columns m > mmax too)
     NUSHT_TRY(f_alloc(&p->d_grid, gbytes, p));
     NUSHT_CUDA_TRY(cudaMemset(p->d_h, 0, hbytes));
+    NUSHT_CUDA_TRY(cudaMemset(p->d_ht, 0, htbytes));
     NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
 
     // cuFFT plans
@@ -127,16 +191,38 @@ int fourier_build(nusht_plan_s* p) {
         wtot += ws;
     }
     {
+        // phi pass on the transposed buffer Ht[a][m]: contiguous rows of mp complex <-> n_phi reals
         int n[1] = {g.nph};
-        int inembed[1] = {g.nph / 2 + 1}, onembed[1] = {g.nph};
+        int inembed[1] = {mp}, onembed[1] = {g.nph};
         NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi_c2r));
-        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_c2r, 1, n, inembed, g.nth, 1, onembed, 1, g.nph,
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_c2r, 1, n, inembed, 1, mp, onembed, 1, g.nph,
                                           f64 ? CUFFT_Z2D : CUFFT_C2R, g.nrow_half, &ws));
         wtot += ws;
         NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi_r2c));
-        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_r2c, 1, n, onembed, 1, g.nph, inembed, g.nth, 1,
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_r2c, 1, n, onembed, 1, g.nph, inembed, 1, mp,
                                           f64 ? CUFFT_D2Z : CUFFT_R2C, g.nrow_half, &ws));
         wtot += ws;
+    }
+    // Columns m > mmax of Ht are zero and must stay so for the C2R.  cuFFT is allowed to overwrite the
+    // input of an out-of-place C2R: probe once whether this plan does; if it does, they are re-zeroed
+    // on every synthesis, otherwise never again.
+    p->c2r_clobbers_input = false;
+    if (mp - M - 1 > 0) {
+        int* d_flag = nullptr;
+        NUSHT_CUDA_TRY(cudaMalloc((void**)&d_flag, sizeof(int)));
+        NUSHT_CUDA_TRY(cudaMemset(d_flag, 0, sizeof(int)));
+        NUSHT_CUDA_TRY(cudaMemset2D(p->d_ht, (size_t)mp * csz, 0x3c, (size_t)(M + 1) * csz, (size_t)g.nrow_half));
+        if (f64)
+            NUSHT_CUFFT_TRY(cufftExecZ2D(p->fft_phi_c2r, (cufftDoubleComplex*)p->d_ht, (cufftDoubleReal*)p->d_grid));
+        else
+            NUSHT_CUFFT_TRY(cufftExecC2R(p->fft_phi_c2r, (cufftComplex*)p->d_ht, (cufftReal*)p->d_grid));
+        k_tail_nonzero<<<1024, 256>>>(M, g.nrow_half, mp, (int)(csz / 8), (const unsigned long long*)p->d_ht, d_flag);
+        int flag = 0;
+        NUSHT_CUDA_TRY(cudaMemcpy(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost));
+        cudaFree(d_flag);
+        p->c2r_clobbers_input = flag != 0;
+        NUSHT_CUDA_TRY(cudaMemset(p->d_ht, 0, htbytes));
+        NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
     }
     p->workspace_bytes += (int64_t)wtot;
     p->have_fft = true;
@@ -168,9 +254,6 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
         else
             k_deconv_pad<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, p->d_ft, p->d_pth, p->d_pph, (float2*)p->d_h);
         NUSHT_CUDA_TRY(cudaGetLastError());
-        // rows m > mmax of H must be zero for the C2R; cuFFT may clobber its input, so re-zero them
-        const size_t tail = (size_t)(g.nph / 2 - M) * (size_t)g.nth * csz;
-        NUSHT_CUDA_TRY(cudaMemsetAsync((char*)p->d_h + (size_t)(M + 1) * g.nth * csz, 0, tail, s));
     }
     REC(2);
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_fine, s));
@@ -180,11 +263,24 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     else
         NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_theta_fine, (cufftComplex*)p->d_h, (cufftComplex*)p->d_h, CUFFT_INVERSE));
     REC(3);
+    {
+        // H[m][a] -> Ht[a][m] (rows theta in [0, pi] only), then the phi C2R on contiguous rows
+        const int mp = g.nph / 2 + 1;
+        dim3 grid((g.nrow_half + 31) / 32, (M + 32) / 32);
+        if (f64)
+            k_h_to_ht<double2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, mp, (const double2*)p->d_h, (double2*)p->d_ht);
+        else
+            k_h_to_ht<float2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, mp, (const float2*)p->d_h, (float2*)p->d_ht);
+        NUSHT_CUDA_TRY(cudaGetLastError());
+        if (p->c2r_clobbers_input && mp - M - 1 > 0)
+            NUSHT_CUDA_TRY(cudaMemset2DAsync((char*)p->d_ht + (size_t)(M + 1) * csz, (size_t)mp * csz, 0,
+                                             (size_t)(mp - M - 1) * csz, (size_t)g.nrow_half, s));
+    }
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi_c2r, s));
     if (f64)
-        NUSHT_CUFFT_TRY(cufftExecZ2D(p->fft_phi_c2r, (cufftDoubleComplex*)p->d_h, (cufftDoubleReal*)p->d_grid));
+        NUSHT_CUFFT_TRY(cufftExecZ2D(p->fft_phi_c2r, (cufftDoubleComplex*)p->d_ht, (cufftDoubleReal*)p->d_grid));
     else
-        NUSHT_CUFFT_TRY(cufftExecC2R(p->fft_phi_c2r, (cufftComplex*)p->d_h, (cufftReal*)p->d_grid));
+        NUSHT_CUFFT_TRY(cufftExecC2R(p->fft_phi_c2r, (cufftComplex*)p->d_ht, (cufftReal*)p->d_grid));
     REC(4);
     return NUSHT_OK;
 }
@@ -200,13 +296,19 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     REC(0);
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi_r2c, s));
     if (f64)
-        NUSHT_CUFFT_TRY(cufftExecD2Z(p->fft_phi_r2c, (cufftDoubleReal*)p->d_grid, (cufftDoubleComplex*)p->d_h));
+        NUSHT_CUFFT_TRY(cufftExecD2Z(p->fft_phi_r2c, (cufftDoubleReal*)p->d_grid, (cufftDoubleComplex*)p->d_ht_adj));
     else
-        NUSHT_CUFFT_TRY(cufftExecR2C(p->fft_phi_r2c, (cufftReal*)p->d_grid, (cufftComplex*)p->d_h));
-    // transpose of "keep rows 0..n_theta/2 of the theta FFT output": zero-extend to the full period
-    if (g.nth - g.nrow_half > 0)
-        NUSHT_CUDA_TRY(cudaMemset2DAsync((char*)p->d_h + (size_t)g.nrow_half * csz, (size_t)g.nth * csz, 0,
-                                         (size_t)(g.nth - g.nrow_half) * csz, (size_t)(M + 1), s));
+        NUSHT_CUFFT_TRY(cufftExecR2C(p->fft_phi_r2c, (cufftReal*)p->d_grid, (cufftComplex*)p->d_ht_adj));
+    {
+        // Ht[a][m] -> H[m][a] for m <= mmax, zero-extended in theta to the full period
+        const int mp = g.nph / 2 + 1;
+        dim3 grid((g.nth + 31) / 32, (M + 32) / 32);
+        if (f64)
+            k_ht_to_h<double2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, mp, (const double2*)p->d_ht_adj, (double2*)p->d_h);
+        else
+            k_ht_to_h<float2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, mp, (const float2*)p->d_ht_adj, (float2*)p->d_h);
+        NUSHT_CUDA_TRY(cudaGetLastError());
+    }
     REC(1);
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_fine, s));
     if (f64)
@@ -240,7 +342,7 @@ void fourier_free(nusht_plan_s* p) {
     if (p->fft_phi_c2r) cufftDestroy(p->fft_phi_c2r);
     if (p->fft_phi_r2c) cufftDestroy(p->fft_phi_r2c);
     p->fft_theta_coarse = p->fft_theta_fine = p->fft_phi_c2r = p->fft_phi_r2c = 0;
-    cudaFree(p->d_pth); cudaFree(p->d_pph); cudaFree(p->d_h); cudaFree(p->d_grid);
+    cudaFree(p->d_pth); cudaFree(p->d_pph); cudaFree(p->d_h); cudaFree(p->d_ht); cudaFree(p->d_ht_adj); cudaFree(p->d_grid);
     p->d_pth = p->d_pph = nullptr;
-    p->d_h = p->d_grid = nullptr;
+    p->d_h = p->d_ht = p->d_ht_adj = p->d_grid = nullptr;
 }
