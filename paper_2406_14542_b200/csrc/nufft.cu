@@ -612,6 +612,8 @@ __device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, do
 __host__ __device__ constexpr int mma_nt(int w) { return w <= 8 ? 2 : 3; }                 // n-tiles per strip
 __host__ __device__ constexpr int mma_ks(int w) { return w <= 6 ? 2 : (w <= 10 ? 3 : (w <= 14 ? 4 : 5)); }
 __host__ __device__ constexpr int mma_mt(int w) { return w <= 6 ? 1 : (w <= 14 ? 2 : 3); }
+// warps (work items) per CTA of the interpolation kernel: static shared memory stays below 48 KB
+__host__ __device__ constexpr int mma_interp_warps(int w) { return w <= 11 ? 4 : 2; }
 __host__ __device__ constexpr int mma_th_stride(int s) { return s <= 8 ? 12 : (s <= 16 ? 20 : 36); }  // = 4 or 12 mod 16
 
 template <int W, int S>
@@ -656,63 +658,86 @@ __device__ __forceinline__ int64_t grid_row(const NufftGeom& g, int a, bool& mir
     return (int64_t)(mirror ? g.nth - am : am) * g.nph;
 }
 
+// cp.async helpers (SASS LDGSTS): global -> shared without a register round trip, completion per thread
+__device__ __forceinline__ void cp_async_8(void* dst_smem, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_4(void* dst_smem, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// as grid_row, for any row (look-ahead staging may run past the last row a point can touch)
+__device__ __forceinline__ int64_t grid_row_any(const NufftGeom& g, int a, bool& mirror) {
+    int am = a % g.nth;
+    if (am < 0) am += g.nth;
+    mirror = am > g.nth / 2;
+    return (int64_t)(mirror ? g.nth - am : am) * g.nph;
+}
+
+constexpr int NU_RING_ROWS = 16;   // rows of the strip staged ahead of the register window
+constexpr int NU_RING_CHUNK = 8;   // rows staged per top-up
+
+template <int NT>
+struct StripRing {
+    double rows[NU_RING_ROWS][8 * NT];   // row r of the strip lives in rows[(r + 32) & 15]
+    double sx[32], sy[32];               // coordinates of the next batch of points
+    int sperm[32];
+};
+
 // ---------------------------------------------------------------------------------------------
 // a7: type-2 interpolation, FP64 / DMMA
+// Memory latency is taken off the critical path with cp.async: the strip's grid rows are staged
+// 8-16 rows ahead of the register window into a per-warp shared-memory ring, and the coordinates of
+// the next batch of 32 points are staged while the current batch is processed.
 // ---------------------------------------------------------------------------------------------
 template <int W>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(32 * mma_interp_warps(W))
 k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<double> kp,
              const double* __restrict__ grid, double* __restrict__ map) {
-    constexpr int NT = mma_nt(W), KS = mma_ks(W), S = 4 * KS, SPAN = S - W, OFF = 2 * S;
+    constexpr int NT = mma_nt(W), KS = mma_ks(W), S = 4 * KS, SPAN = S - W, OFF = 2 * S, NC = 8 * NT;
+    constexpr int RB = NU_RING_ROWS, CH = NU_RING_CHUNK;
     using WS = MmaScratch<W, S>;
-    __shared__ __align__(16) WS s_ws[4];
+    constexpr int NW = mma_interp_warps(W);
+    __shared__ __align__(16) WS s_ws[NW];
+    __shared__ __align__(16) StripRing<NT> s_ring[NW];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int item = blockIdx.x * 4 + warp;
+    const int item = blockIdx.x * NW + warp;
     if (item >= P.n_items) return;
     const int start = P.item_off[item], end = P.item_off[item + 1];
     if (start >= end) return;
     WS& ws = s_ws[warp];
+    StripRing<NT>& ring = s_ring[warp];
     const NufftGeom& g = P.g;
     const int strip = item % g.nstrip;
     const int c0 = strip * g.mb - g.fl;   // global column of strip column 0
     const int gq = lane >> 2, t = lane & 3;
-    int colb_n[NT], colb_m[NT];           // global columns (plain / mirrored) of this lane's B elements
-#pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
-        int c = (c0 + NT * gq + nt) % g.nph;
+    int cols_n, cols_m;                   // staging: lane < NC copies strip column `lane` of a row
+    {
+        int c = (c0 + min(lane, NC - 1)) % g.nph;
         if (c < 0) c += g.nph;
-        colb_n[nt] = c;
+        cols_n = c;
         c += g.nph / 2;
-        colb_m[nt] = (c >= g.nph) ? c - g.nph : c;
+        cols_m = (c >= g.nph) ? c - g.nph : c;
     }
     double win[KS][NT];                   // win[ks][nt]: row in slot 4 ks + t, strip column NT g + nt
 #pragma unroll
     for (int ks = 0; ks < KS; ++ks)
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) win[ks][nt] = 0.0;
-    int loaded_hi = INT_MIN;              // rows [loaded_hi - S, loaded_hi) are resident
-    int pf_hi = INT_MIN;                  // rows below pf_hi have been prefetched into L1
-    constexpr int PF_AHEAD = 8;
-    int colp_n, colp_m;                   // prefetch: lane covers strip columns 3 (lane & 7) ..
-    {
-        int c = (c0 + min(3 * (lane & 7), 8 * NT - 1)) % g.nph;
-        if (c < 0) c += g.nph;
-        colp_n = c;
-        c += g.nph / 2;
-        colp_m = (c >= g.nph) ? c - g.nph : c;
-    }
+    int loaded_hi = INT_MIN;              // rows [loaded_hi - S, loaded_hi) are in the register window
+    int staged_hi = INT_MIN;              // cp.async issued for rows below staged_hi (those >= loaded_hi are in the ring)
+    int landed_hi = INT_MIN;              // rows below landed_hi are known to have arrived
 
-    // group q = rows 4q .. 4q+3 (offset by OFF); lane t loads row 4q + t if it lies in [rb, re)
-    auto load_group = [&](int q, int rb, int re, double (&v)[NT]) -> bool {
-        const int rr = 4 * q + t;
-        const bool in = rr >= rb && rr < re;
-        if (in) {
+    auto stage_rows = [&](int r0, int r1) {
+#pragma unroll 1
+        for (int r = r0; r < r1; ++r) {
             bool mirror;
-            const int64_t ro = grid_row(g, rr - OFF, mirror);
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) v[nt] = grid[ro + (mirror ? colb_m[nt] : colb_n[nt])];
+            const int64_t ro = grid_row_any(g, r, mirror);
+            if (lane < NC) cp_async_8(&ring.rows[(r + 32) & (RB - 1)][lane], grid + ro + (mirror ? cols_m : cols_n));
         }
-        return in;
     };
     // static register indices + predicates only (a run-time index would put the window in local memory)
     auto commit_group = [&](int q, bool in, const double (&v)[NT]) {
@@ -723,20 +748,25 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             for (int nt = 0; nt < NT; ++nt) win[ksi][nt] = (in && ks == ksi) ? v[nt] : win[ksi][nt];
     };
 
-    double Xn = 0.0, Yn = 0.0;
     if (start + lane < end) {
-        Xn = P.px[start + lane];
-        Yn = P.py[start + lane];
+        cp_async_8(&ring.sx[lane], P.px + start + lane);
+        cp_async_8(&ring.sy[lane], P.py + start + lane);
+        cp_async_4(&ring.sperm[lane], P.perm + start + lane);
     }
     for (int batch = start; batch < end; batch += 32) {
         const int idx = batch + lane;
         const bool has = idx < end;
-        const double X = Xn, Y = Yn;
+        cp_async_wait_all();
+        __syncwarp();
+        landed_hi = staged_hi;
+        const double X = has ? ring.sx[lane] : 0.0, Y = has ? ring.sy[lane] : 0.0;
+        const int dst = has ? ring.sperm[lane] : 0;
+        __syncwarp();
         if (idx + 32 < end) {
-            Xn = P.px[idx + 32];
-            Yn = P.py[idx + 32];
+            cp_async_8(&ring.sx[lane], P.px + idx + 32);
+            cp_async_8(&ring.sy[lane], P.py + idx + 32);
+            cp_async_4(&ring.sperm[lane], P.perm + idx + 32);
         }
-        const int dst = has ? P.perm[idx] : 0;
         const int a0 = mma_publish<W, S>(ws, kp, lane, X, Y, has ? 1.0 : 0.0, c0);
         __syncwarp();
         const int npt = min(32, end - batch);
@@ -746,24 +776,35 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             const int row0 = __shfl_sync(0xffffffffu, a0, j0);
             const unsigned fit = __ballot_sync(0xffffffffu, has && lane >= j0 && a0 - row0 <= SPAN);
             const int cnt = min(8, __popc(fit));
-            // ---- L1 prefetch of the rows coming up: one instruction covers 4 rows (lane = row r4, 24-byte
-            //      chunk c8: every 32-byte sector of a <= 256-byte strip row is touched) ----
-            if (pf_hi < row0 + S + PF_AHEAD) {
-                if (pf_hi < row0 + S) pf_hi = row0 + S;
-                bool mirror;
-                const int64_t ro = grid_row(g, min(pf_hi + (lane >> 3), g.nth / 2), mirror);   // clamped: stays inside the grid
-                asm volatile("prefetch.global.L1 [%0];" ::"l"(grid + ro + (mirror ? colp_m : colp_n)));
-                pf_hi += 4;
-            }
-            // ---- make rows [row0, row0 + S) resident (circular slots) ----
-            if (loaded_hi < row0 + S) {
-                const int rb = max(loaded_hi, row0) + OFF, re = row0 + S + OFF;
+            const int need_hi = row0 + S;
+            // ---- rows [row0, need_hi) must be in the register window; they come from the ring ----
+            if (loaded_hi < need_hi) {
+                if (staged_hi < need_hi) {          // first tile of the item, or a jump past the look-ahead
+                    stage_rows(max(staged_hi, row0), need_hi);
+                    staged_hi = need_hi;
+                }
+                if (landed_hi < need_hi) {
+                    cp_async_wait_all();
+                    __syncwarp();
+                    landed_hi = staged_hi;
+                }
+                const int rb = max(loaded_hi, row0) + OFF, re = need_hi + OFF;
                 for (int q = rb >> 2; q <= (re - 1) >> 2; ++q) {
+                    const int rr = 4 * q + t;
+                    const bool in = rr >= rb && rr < re;
                     double v[NT];
-                    const bool in = load_group(q, rb, re, v);
+                    const double* src = &ring.rows[(rr - OFF + 32) & (RB - 1)][NT * gq];
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) v[nt] = src[nt];
                     commit_group(q, in, v);
                 }
-                loaded_hi = row0 + S;
+                loaded_hi = need_hi;
+                __syncwarp();                       // ring rows below loaded_hi may now be overwritten
+            }
+            // ---- keep the ring CH .. RB rows ahead of the window ----
+            if (staged_hi + CH <= loaded_hi + RB) {
+                stage_rows(staged_hi, staged_hi + CH);
+                staged_hi += CH;
             }
             // ---- A fragments: theta weights of point j0 + g in circular slot order ----
             const int jp = min(j0 + gq, 31);
@@ -938,7 +979,8 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
 template <int W>
 int launch_interp_mma(const NufftParams& P, const KernelHost& h, const void* grid, void* map, cudaStream_t s) {
     const KernelPoly<double> kp = make_device_poly<double>(h);
-    k_interp_mma<W><<<(P.n_items + 3) / 4, 128, 0, s>>>(P, kp, (const double*)grid, (double*)map);
+    constexpr int NW = mma_interp_warps(W);
+    k_interp_mma<W><<<(P.n_items + NW - 1) / NW, 32 * NW, 0, s>>>(P, kp, (const double*)grid, (double*)map);
     NUSHT_CUDA_TRY(cudaGetLastError());
     return NUSHT_OK;
 }
