@@ -47,6 +47,7 @@ constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
 
 struct LegParams {
     int lmax, mmax, nr, nth2, npairs, has_equator;
+    int nblk, rem;   // main blocks of 32 R pairs per m; left-over pairs handled by the remainder blocks
     const int64_t* eoff;
     const double2* ab;
     const double* x2;
@@ -273,12 +274,131 @@ __device__ __forceinline__ void seed_pair(const LegParams& P, int m, int j, bool
     e = ee;
 }
 
+// a2 for one ring pair: north = E + x O, south = E - x O; mirror rows carry (-1)^m (phi -> phi + pi)
+// (Fig. 1)
+__device__ __forceinline__ void write_pair(const LegParams& P, double2* row, double sgn, int j, double ere,
+                                           double eim, double ore_, double oim) {
+    const double x = P.x[j];
+    const double2 nv = make_double2(fma(x, ore_, ere), fma(x, oim, eim));
+    const double2 sv = make_double2(fma(-x, ore_, ere), fma(-x, oim, eim));
+    const int ks = P.nr - 1 - j;   // south ring index
+    row[j] = nv;
+    if (j != 0) row[P.nth2 - j] = make_double2(sgn * nv.x, sgn * nv.y);
+    if (ks != j) {
+        row[ks] = sv;
+        if (j != 0) row[P.nth2 - ks] = make_double2(sgn * sv.x, sgn * sv.y);
+    }
+}
+
+// a10 for one ring pair (D^T): G[k] = Gt[k] + (-1)^m Gt[Ntheta-k] away from the poles, then the even /
+// odd (in l - m) combinations of the north and south ring
+__device__ __forceinline__ void fold_pair(const LegParams& P, const double2* __restrict__ row, double sgn, int j,
+                                          double& ere, double& eim, double& ore_, double& oim) {
+    const int kn = j, ks = P.nr - 1 - j;
+    double2 gn = row[kn];
+    if (kn != 0) {
+        const double2 t = row[P.nth2 - kn];
+        gn.x = fma(sgn, t.x, gn.x);
+        gn.y = fma(sgn, t.y, gn.y);
+    }
+    double2 gs = make_double2(0.0, 0.0);
+    if (ks != kn) {
+        gs = row[ks];
+        if (kn != 0) {
+            const double2 t = row[P.nth2 - ks];
+            gs.x = fma(sgn, t.x, gs.x);
+            gs.y = fma(sgn, t.y, gs.y);
+        }
+    }
+    const double x = P.x[j];
+    ere = gn.x + gs.x;
+    eim = gn.y + gs.y;
+    ore_ = x * (gn.x - gs.x);
+    oim = x * (gn.y - gs.y);
+}
+
+// Remainder ring pairs.  With N_r = 2^k + 1 rings there are 2^(k-1) + 1 pairs: one more than a whole
+// number of 32 R blocks.  Rather than a 17th warp per m with a single busy lane, the last block
+// column of the grid takes the `rem` left-over pairs of 32/rem different m per warp, one (m, pair)
+// per lane, each lane streaming its own coefficient column from global memory.
+__device__ void synth_remainder(const LegParams& P, const double4* __restrict__ aeo, double2* __restrict__ ft, int j0,
+                                int rem) {
+    const int gid = blockIdx.y * 32 + threadIdx.x;
+    const int m = gid / rem, j = j0 + gid % rem;
+    if (m > P.mmax) return;
+    const int ne = (P.lmax - m) / 2 + 1;
+    const int64_t o = P.eoff[m];
+    double p0 = 0.0, p1;
+    int ex;
+    seed_pair(P, m, j, true, p1, ex);
+    const double x2 = P.x2[j];
+    double ere = 0.0, eim = 0.0, ore_ = 0.0, oim = 0.0;
+    for (int n = 0; n < ne; ++n) {
+        const double2 ab = P.ab[o + n];
+        const double t = fma(ab.x, x2, ab.y);
+        if (ex == 0) {
+            const double4 c = aeo[o + n];
+            ere = fma(c.x, p1, ere);
+            eim = fma(c.y, p1, eim);
+            ore_ = fma(c.z, p1, ore_);
+            oim = fma(c.w, p1, oim);
+        }
+        const double pn = fma(t, p1, p0);
+        p0 = p1;
+        p1 = pn;
+        if (ex > 0 && (n & 7) == 7 && fabs(p1) > SCALE_UP_LIMIT) {
+            p1 *= SCALE_DOWN;
+            p0 *= SCALE_DOWN;
+            ex -= 1;
+        }
+    }
+    write_pair(P, ft + (int64_t)m * P.nth2, (m & 1) ? -1.0 : 1.0, j, ere, eim, ore_, oim);
+}
+
+__device__ void adjoint_remainder(const LegParams& P, const double2* __restrict__ gt, double4* __restrict__ eo, int j0,
+                                  int rem) {
+    const int gid = blockIdx.y * 32 + threadIdx.x;
+    const int m = gid / rem, j = j0 + gid % rem;
+    if (m > P.mmax) return;
+    const int ne = (P.lmax - m) / 2 + 1;
+    const int64_t o = P.eoff[m];
+    double p0 = 0.0, p1;
+    int ex;
+    seed_pair(P, m, j, true, p1, ex);
+    const double x2 = P.x2[j];
+    double ere, eim, ore_, oim;
+    fold_pair(P, gt + (int64_t)m * P.nth2, (m & 1) ? -1.0 : 1.0, j, ere, eim, ore_, oim);
+    for (int n = 0; n < ne; ++n) {
+        const double2 ab = P.ab[o + n];
+        const double t = fma(ab.x, x2, ab.y);
+        if (ex == 0) {
+            double* out = reinterpret_cast<double*>(eo + o + n);
+            atomicAdd(out + 0, p1 * ere);
+            atomicAdd(out + 1, p1 * eim);
+            atomicAdd(out + 2, p1 * ore_);
+            atomicAdd(out + 3, p1 * oim);
+        }
+        const double pn = fma(t, p1, p0);
+        p0 = p1;
+        p1 = pn;
+        if (ex > 0 && (n & 3) == 3 && fabs(p1) > SCALE_UP_LIMIT) {
+            p1 *= SCALE_DOWN;
+            p0 *= SCALE_DOWN;
+            ex -= 1;
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // a1 + a2: Legendre synthesis with fused DFS doubling.  grid = (pair blocks, m).
 // ---------------------------------------------------------------------------------------------
 template <int R>
 __global__ void __launch_bounds__(SYN_THREADS)
 k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restrict__ ft) {
+    if (P.rem > 0 && blockIdx.x == P.nblk) {
+        synth_remainder(P, aeo, ft, P.nblk * (32 * R), P.rem);
+        return;
+    }
     __shared__ __align__(16) double2 s_ab[2][SYN_TN];
     __shared__ __align__(32) double4 s_aeo[2][SYN_TN];
     __shared__ __align__(8) uint64_t s_bar[2];
@@ -423,25 +543,12 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
     }
 
     if (!warp_has_work) return;
-    // a2: fused DFS doubling (Fig. 1): north = E + x O, south = E - x O;
-    // mirror rows carry (-1)^m (phi -> phi + pi).
+    // a2: fused DFS doubling
     const double sgn = (m & 1) ? -1.0 : 1.0;
     double2* row = ft + (int64_t)m * P.nth2;
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int j = jb + r * 32 + lane;
-        if (!valid[r]) continue;
-        const double x = P.x[j];
-        const double2 nv = make_double2(fma(x, ore_[r], ere[r]), fma(x, oim[r], eim[r]));
-        const double2 sv = make_double2(fma(-x, ore_[r], ere[r]), fma(-x, oim[r], eim[r]));
-        const int ks = P.nr - 1 - j;   // south ring index
-        row[j] = nv;
-        if (j != 0) row[P.nth2 - j] = make_double2(sgn * nv.x, sgn * nv.y);
-        if (ks != j) {
-            row[ks] = sv;
-            if (j != 0) row[P.nth2 - ks] = make_double2(sgn * sv.x, sgn * sv.y);
-        }
-    }
+    for (int r = 0; r < R; ++r)
+        if (valid[r]) write_pair(P, row, sgn, jb + r * 32 + lane, ere[r], eim[r], ore_[r], oim[r]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -494,6 +601,10 @@ __device__ __forceinline__ double warp_transpose_reduce16(double (&v)[16], int l
 template <int R>
 __global__ void __launch_bounds__(32)
 k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restrict__ eo) {
+    if (P.rem > 0 && blockIdx.x == P.nblk) {
+        adjoint_remainder(P, gt, eo, P.nblk * (32 * R), P.rem);
+        return;
+    }
     __shared__ __align__(16) double2 s_ab[2][ADJ_TN];
     __shared__ __align__(16) double s_tr[4 * ADJ_CHUNK][33];
     __shared__ __align__(8) uint64_t s_bar[2];
@@ -528,30 +639,8 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
     double x2[R], p0[R], p1[R], gere[R], geim[R], gore[R], goim[R];
     int ex[R];
     bool valid[R];
-    // a10 fold (D^T) of ring pair j: G[k] = Gt[k] + (-1)^m Gt[Ntheta-k] away from the poles, then the
-    // even / odd (in l - m) combinations of the north and south ring
     auto load_g = [&](int j, double& ere, double& eim, double& ore_, double& oim) {
-        const int kn = j, ks = P.nr - 1 - j;
-        double2 gn = row[kn];
-        if (kn != 0) {
-            const double2 t = row[P.nth2 - kn];
-            gn.x = fma(sgn, t.x, gn.x);
-            gn.y = fma(sgn, t.y, gn.y);
-        }
-        double2 gs = make_double2(0.0, 0.0);
-        if (ks != kn) {
-            gs = row[ks];
-            if (kn != 0) {
-                const double2 t = row[P.nth2 - ks];
-                gs.x = fma(sgn, t.x, gs.x);
-                gs.y = fma(sgn, t.y, gs.y);
-            }
-        }
-        const double x = P.x[j];
-        ere = gn.x + gs.x;
-        eim = gn.y + gs.y;
-        ore_ = x * (gn.x - gs.x);
-        oim = x * (gn.y - gs.y);
+        fold_pair(P, row, sgn, j, ere, eim, ore_, oim);
     };
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -650,8 +739,25 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
 // =============================================================================================
 // host side
 // =============================================================================================
+// grid decomposition of the ring pairs for R pairs per thread (see synth_remainder)
+static dim3 leg_grid(const nusht_plan_s* p, int R, LegParams& P) {
+    const int per = 32 * R;
+    int nblk = p->lg.npairs / per, rem = p->lg.npairs - nblk * per;
+    if (rem == 0 || rem > 8 || nblk == 0) {
+        nblk = (p->lg.npairs + per - 1) / per;
+        rem = 0;
+    }
+    P.nblk = nblk;
+    P.rem = rem;
+    const int need_y = rem ? ((p->mmax + 1) * rem + 31) / 32 : 0;   // remainder warps; they fit: rem <= 8
+    (void)need_y;
+    return dim3(nblk + (rem ? 1 : 0), p->mmax + 1);
+}
+
 static LegParams make_params(const nusht_plan_s* p) {
     LegParams P;
+    P.nblk = 0;
+    P.rem = 0;
     P.lmax = p->lmax;
     P.mmax = p->mmax;
     P.nr = p->lg.nr;
@@ -754,9 +860,9 @@ int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s) {
 }
 
 int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s) {
-    const int pairs_per_cta = SYN_THREADS * LEG_R;
-    dim3 grid((p->lg.npairs + pairs_per_cta - 1) / pairs_per_cta, p->mmax + 1);
-    k_legendre_synth<LEG_R><<<grid, SYN_THREADS, 0, s>>>(make_params(p), p->d_aeo, ft);
+    LegParams P = make_params(p);
+    const dim3 grid = leg_grid(p, LEG_R, P);
+    k_legendre_synth<LEG_R><<<grid, SYN_THREADS, 0, s>>>(P, p->d_aeo, ft);
     NUSHT_CUDA_TRY(cudaGetLastError());
     return NUSHT_OK;
 }
@@ -764,9 +870,9 @@ int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s) {
 int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
     // the kernel accumulates with global reductions
     NUSHT_CUDA_TRY(cudaMemsetAsync(p->d_aeo, 0, sizeof(double4) * (size_t)p->n_e_total, s));
-    const int pairs_per_cta = 32 * ADJ_R;
-    dim3 grid((p->lg.npairs + pairs_per_cta - 1) / pairs_per_cta, p->mmax + 1);
-    k_legendre_adjoint<ADJ_R><<<grid, 32, 0, s>>>(make_params(p), gt, p->d_aeo);
+    LegParams P = make_params(p);
+    const dim3 grid = leg_grid(p, ADJ_R, P);
+    k_legendre_adjoint<ADJ_R><<<grid, 32, 0, s>>>(P, gt, p->d_aeo);
     NUSHT_CUDA_TRY(cudaGetLastError());
     return NUSHT_OK;
 }
