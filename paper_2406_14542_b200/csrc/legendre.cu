@@ -48,6 +48,11 @@ constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
 struct LegParams {
     int lmax, mmax, nr, nth2, npairs, has_equator;
     int nblk, rem;   // main blocks of 32 R pairs per m; left-over pairs handled by the remainder blocks
+    // fast-forward table (plan time): for warp (m, block) the first n-step (multiple of LEG_CHUNK) at which
+    // one of its ring pairs is in range, and the scaled recurrence state of its pairs at that step
+    const int* ff_n;
+    const double2* ff_p;   // (p0, p1) per (m, block, r, lane)
+    const int* ff_e;       // exponent counter
     const int64_t* eoff;
     const double2* ab;
     const double* x2;
@@ -390,6 +395,67 @@ __device__ void adjoint_remainder(const LegParams& P, const double2* __restrict_
 }
 
 // ---------------------------------------------------------------------------------------------
+// plan time: fast-forward table.  While every ring pair of a warp is still below range (Pbar_mm ~
+// sin^m theta underflows for most (m, ring)), the transform kernels would only advance the
+// recurrence.  That part does not depend on the data, so it is run once here: the warp advances
+// chunk by chunk exactly as the transform kernels do, stops at the first chunk boundary where a
+// pair is in range, and stores the step and the state.  The transforms start from there; a warp
+// whose pairs never come into range before lmax does no work at all.
+// ---------------------------------------------------------------------------------------------
+template <int R>
+__global__ void __launch_bounds__(32)
+k_legendre_fastforward(LegParams P, int* __restrict__ ff_n, double2* __restrict__ ff_p, int* __restrict__ ff_e) {
+    const int m = blockIdx.y, lane = threadIdx.x;
+    const int ne = (P.lmax - m) / 2 + 1;
+    const int64_t o = P.eoff[m];
+    const int jb = blockIdx.x * (32 * R);
+    double x2[R], p0[R], p1[R];
+    int ex[R];
+    bool valid[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int j = jb + r * 32 + lane;
+        valid[r] = j < P.npairs;
+        x2[r] = valid[r] ? P.x2[j] : 0.0;
+        seed_pair(P, m, j, valid[r], p1[r], ex[r]);
+        p0[r] = 0.0;
+    }
+    int n = 0;
+    for (; n < ne; n += LEG_CHUNK) {
+        bool any_live = false;
+#pragma unroll
+        for (int r = 0; r < R; ++r) any_live |= (valid[r] && ex[r] == 0);
+        if (__any_sync(0xffffffffu, any_live)) break;
+        const int ns = min(LEG_CHUNK, ne - n);
+        for (int i = 0; i < ns; ++i) {
+            const double2 ab = P.ab[o + n + i];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double t = fma(ab.x, x2[r], ab.y);
+                const double pn = fma(t, p1[r], p0[r]);
+                p0[r] = p1[r];
+                p1[r] = pn;
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (ex[r] > 0 && fabs(p1[r]) > SCALE_UP_LIMIT) {
+                p1[r] *= SCALE_DOWN;
+                p0[r] *= SCALE_DOWN;
+                ex[r] -= 1;
+            }
+        }
+    }
+    const int64_t w = (int64_t)m * P.nblk + blockIdx.x;
+    if (lane == 0) ff_n[w] = min(n, ne);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        ff_p[(w * R + r) * 32 + lane] = make_double2(p0[r], p1[r]);
+        ff_e[(w * R + r) * 32 + lane] = ex[r];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // a1 + a2: Legendre synthesis with fused DFS doubling.  grid = (pair blocks, m).
 // ---------------------------------------------------------------------------------------------
 template <int R>
@@ -410,6 +476,9 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int jb = (blockIdx.x * SYN_WARPS + warp) * (32 * R);
     const int ntiles = (ne + SYN_TN - 1) / SYN_TN;
+    const int64_t wff = (int64_t)m * P.nblk + blockIdx.x;
+    const int n_start = P.ff_n[wff];          // first step at which a pair of this warp is in range
+    const int tile0 = n_start / SYN_TN;
 
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
@@ -418,15 +487,15 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
     }
     __syncthreads();
     auto issue = [&](int tile) {
-        const int st = tile & 1;
+        const int st = (tile - tile0) & 1;
         const int cnt = min(SYN_TN, ne - tile * SYN_TN);
         mbar_expect_tx(&s_bar[st], (uint32_t)cnt * 48u);
         bulk_g2s(&s_ab[st][0], P.ab + o + (int64_t)tile * SYN_TN, (uint32_t)cnt * 16u, &s_bar[st]);
         bulk_g2s(&s_aeo[st][0], aeo + o + (int64_t)tile * SYN_TN, (uint32_t)cnt * 32u, &s_bar[st]);
     };
-    if (tid == 0) {
-        issue(0);
-        if (ntiles > 1) issue(1);
+    if (tid == 0 && n_start < ne) {
+        issue(tile0);
+        if (tile0 + 1 < ntiles) issue(tile0 + 1);
     }
 
     double x2[R], p0[R], p1[R], ere[R], eim[R], ore_[R], oim[R];
@@ -437,18 +506,20 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
         const int j = jb + r * 32 + lane;
         valid[r] = j < P.npairs;
         x2[r] = valid[r] ? P.x2[j] : 0.0;
-        seed_pair(P, m, j, valid[r], p1[r], ex[r]);
-        p0[r] = 0.0;
+        const double2 pp = P.ff_p[(wff * R + r) * 32 + lane];   // state at n_start (plan-time fast-forward)
+        p0[r] = pp.x;
+        p1[r] = pp.y;
+        ex[r] = P.ff_e[(wff * R + r) * 32 + lane];
         ere[r] = eim[r] = ore_[r] = oim[r] = 0.0;
     }
     const bool warp_has_work = jb < P.npairs;
 
-    for (int tile = 0; tile < ntiles; ++tile) {
-        const int st = tile & 1;
+    for (int tile = tile0; tile < ntiles && n_start < ne; ++tile) {
+        const int st = (tile - tile0) & 1;
         const int cnt = min(SYN_TN, ne - tile * SYN_TN);
-        mbar_wait(&s_bar[st], (uint32_t)((tile >> 1) & 1));
+        mbar_wait(&s_bar[st], (uint32_t)(((tile - tile0) >> 1) & 1));
         if (warp_has_work) {
-            for (int i0 = 0; i0 < cnt; i0 += LEG_CHUNK) {
+            for (int i0 = (tile == tile0) ? n_start - tile0 * SYN_TN : 0; i0 < cnt; i0 += LEG_CHUNK) {
                 const int ns = min(LEG_CHUNK, cnt - i0);
                 bool any_dead = false, any_live = false;
 #pragma unroll
@@ -618,6 +689,10 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
     const int ntiles = (ne + ADJ_TN - 1) / ADJ_TN;
     const double sgn = (m & 1) ? -1.0 : 1.0;
     const double2* row = gt + (int64_t)m * P.nth2;
+    const int64_t wff = (int64_t)m * P.nblk + blockIdx.x;
+    const int n_start = P.ff_n[wff];          // first step at which a pair of this warp is in range
+    if (n_start >= ne) return;                // never before lmax: this warp contributes nothing
+    const int tile0 = n_start / ADJ_TN;
 
     if (lane == 0) {
         mbar_init(&s_bar[0], 1);
@@ -626,14 +701,14 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
     }
     __syncwarp();
     auto issue = [&](int tile) {
-        const int st = tile & 1;
+        const int st = (tile - tile0) & 1;
         const int cnt = min(ADJ_TN, ne - tile * ADJ_TN);
         mbar_expect_tx(&s_bar[st], (uint32_t)cnt * 16u);
         bulk_g2s(&s_ab[st][0], P.ab + o + (int64_t)tile * ADJ_TN, (uint32_t)cnt * 16u, &s_bar[st]);
     };
     if (lane == 0) {
-        issue(0);
-        if (ntiles > 1) issue(1);
+        issue(tile0);
+        if (tile0 + 1 < ntiles) issue(tile0 + 1);
     }
 
     double x2[R], p0[R], p1[R], gere[R], geim[R], gore[R], goim[R];
@@ -647,17 +722,19 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
         const int j = jb + r * 32 + lane;
         valid[r] = j < P.npairs;
         x2[r] = valid[r] ? P.x2[j] : 0.0;
-        seed_pair(P, m, j, valid[r], p1[r], ex[r]);
-        p0[r] = 0.0;
+        const double2 pp = P.ff_p[(wff * R + r) * 32 + lane];   // state at n_start (plan-time fast-forward)
+        p0[r] = pp.x;
+        p1[r] = pp.y;
+        ex[r] = P.ff_e[(wff * R + r) * 32 + lane];
         gere[r] = geim[r] = gore[r] = goim[r] = 0.0;
         if (valid[r] && ex[r] == 0) load_g(j, gere[r], geim[r], gore[r], goim[r]);
     }
 
-    for (int tile = 0; tile < ntiles; ++tile) {
-        const int st = tile & 1;
+    for (int tile = tile0; tile < ntiles; ++tile) {
+        const int st = (tile - tile0) & 1;
         const int cnt = min(ADJ_TN, ne - tile * ADJ_TN);
-        mbar_wait(&s_bar[st], (uint32_t)((tile >> 1) & 1));
-        for (int i0 = 0; i0 < cnt; i0 += ADJ_CHUNK) {
+        mbar_wait(&s_bar[st], (uint32_t)(((tile - tile0) >> 1) & 1));
+        for (int i0 = (tile == tile0) ? n_start - tile0 * ADJ_TN : 0; i0 < cnt; i0 += ADJ_CHUNK) {
             const int ns = min(ADJ_CHUNK, cnt - i0);
             bool any_dead = false, any_live = false;
 #pragma unroll
@@ -770,6 +847,9 @@ static LegParams make_params(const nusht_plan_s* p) {
     P.x = p->d_x;
     P.logsin = p->d_logsin;
     P.logkap = p->d_logkap;
+    P.ff_n = p->d_ff_n;
+    P.ff_p = p->d_ff_p;
+    P.ff_e = p->d_ff_e;
     return P;
 }
 
@@ -843,6 +923,19 @@ int legendre_build_tables(nusht_plan_s* p) {
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_x, x.data(), sizeof(double) * g.npairs, cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_logsin, ls.data(), sizeof(double2) * g.npairs, cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_logkap, lk.data(), sizeof(double2) * (M + 1), cudaMemcpyHostToDevice));
+    // fast-forward table (synthesis and adjoint use the same decomposition: LEG_R == ADJ_R pairs per thread)
+    {
+        static_assert(LEG_R == ADJ_R, "the fast-forward table is shared by both Legendre kernels");
+        LegParams P = make_params(p);
+        const dim3 grid = leg_grid(p, LEG_R, P);
+        const size_t nw = (size_t)(M + 1) * (size_t)P.nblk;
+        NUSHT_TRY(dev_alloc(&p->d_ff_n, nw, p));
+        NUSHT_TRY(dev_alloc(&p->d_ff_p, nw * LEG_R * 32, p));
+        NUSHT_TRY(dev_alloc(&p->d_ff_e, nw * LEG_R * 32, p));
+        k_legendre_fastforward<LEG_R><<<dim3(P.nblk, M + 1), 32>>>(P, p->d_ff_n, p->d_ff_p, p->d_ff_e);
+        NUSHT_CUDA_TRY(cudaGetLastError());
+        (void)grid;
+    }
     NUSHT_CUDA_TRY(cudaDeviceSynchronize());
     return NUSHT_OK;
 }
@@ -893,6 +986,8 @@ void legendre_free(nusht_plan_s* p) {
     cudaFree(p->d_eoff); cudaFree(p->d_ab); cudaFree(p->d_sig); cudaFree(p->d_sodd); cudaFree(p->d_rho);
     cudaFree(p->d_aeo); cudaFree(p->d_ft); cudaFree(p->d_x2); cudaFree(p->d_x); cudaFree(p->d_logsin);
     cudaFree(p->d_logkap);
+    cudaFree(p->d_ff_n); cudaFree(p->d_ff_p); cudaFree(p->d_ff_e);
+    p->d_ff_n = nullptr; p->d_ff_p = nullptr; p->d_ff_e = nullptr;
     p->d_eoff = nullptr; p->d_ab = nullptr; p->d_sig = p->d_sodd = p->d_rho = nullptr; p->d_aeo = nullptr;
     p->d_ft = nullptr; p->d_x2 = p->d_x = nullptr; p->d_logsin = p->d_logkap = nullptr;
 }

@@ -81,6 +81,9 @@ struct nusht_plan_s {
     double* d_x = nullptr;          // cos(theta_j)
     double2* d_logsin = nullptr;    // log2 sin(theta_j) as (hi, lo)
     double2* d_logkap = nullptr;    // log2 |Pbar_mm| prefactor per m as (hi, lo)
+    int* d_ff_n = nullptr;          // fast-forward table: first in-range step per (m, block of ring pairs)
+    double2* d_ff_p = nullptr;      //   recurrence state (p0, p1) per pair at that step
+    int* d_ff_e = nullptr;          //   exponent counter per pair at that step
     // --- Legendre work buffers ---
     double4* d_aeo = nullptr;       // scaled coefficients per (m,n): (ae.re, ae.im, ao.re, ao.im)
     double2* d_ft = nullptr;        // Ftilde / Gtilde: [mmax+1][nth2] complex128
