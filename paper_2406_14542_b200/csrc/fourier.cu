@@ -25,34 +25,46 @@ template <typename T> struct Cplx;
 template <> struct Cplx<double> { using type = double2; };
 template <> struct Cplx<float> { using type = float2; };
 
-// a4: one thread per fine-grid theta frequency slot k' of column m
+// The fine theta transform of length n_theta has at most n_theta/2 - 1 non-zero inputs (|k| <= lmax,
+// n_theta >= 4 lmax + 4), so it is done as TWO transforms of length nh = n_theta/2, each of which cuFFT
+// does in one pass through shared memory at the sizes of interest (a 16384-point FP64 transform is two
+// passes over HBM):  y[2a'] = sum_k B[k] e^{2 pi i k a'/nh},  y[2a'+1] = sum_k (B[k] e^{2 pi i k/n_theta}) e^{2 pi i k a'/nh}.
+// Buffer layout H[m][parity][nh]; rows a = 2a' + parity are re-interleaved by the transposes below.
+
+// a4: deconvolve + wrap into the two length-nh spectra; one thread per slot k' of column m
 template <typename T>
-__global__ void k_deconv_pad(int L, int M, int nth2, int nth, const double2* __restrict__ ft,
+__global__ void k_deconv_pad(int L, int M, int nth2, int nh, const double2* __restrict__ ft,
                              const double* __restrict__ pth, const double* __restrict__ pph,
                              typename Cplx<T>::type* __restrict__ h) {
     const int kp = blockIdx.x * blockDim.x + threadIdx.x;
     const int m = blockIdx.y;
-    if (kp >= nth) return;
+    if (kp >= nh) return;
     int k;
     bool in = true;
     if (kp <= L) k = kp;
-    else if (kp >= nth - L) k = kp - nth;
+    else if (kp >= nh - L) k = kp - nh;
     else { k = 0; in = false; }
-    typename Cplx<T>::type out;
-    out.x = 0;
-    out.y = 0;
+    typename Cplx<T>::type e, o;
+    e.x = e.y = o.x = o.y = 0;
     if (in) {
         const double2 c = ft[(int64_t)m * nth2 + (k >= 0 ? k : k + nth2)];
         const double f = pth[k + L] * pph[m];
-        out.x = (T)(c.x * f);
-        out.y = (T)(c.y * f);
+        const double cr = c.x * f, ci = c.y * f;
+        double sn, cs;
+        sincospi((double)k / (double)nh, &sn, &cs);      // e^{2 pi i k / n_theta}
+        e.x = (T)cr;
+        e.y = (T)ci;
+        o.x = (T)(cr * cs - ci * sn);
+        o.y = (T)(cr * sn + ci * cs);
     }
-    h[(int64_t)m * nth + kp] = out;
+    h[((int64_t)m * 2 + 0) * nh + kp] = e;
+    h[((int64_t)m * 2 + 1) * nh + kp] = o;
 }
 
-// a9: truncate to |k| <= lmax and deconvolve; one thread per slot r of the doubled-ring spectrum
+// a9: combine the two forward transforms (transpose of the above), truncate to |k| <= lmax and
+// deconvolve; one thread per slot r of the doubled-ring spectrum
 template <typename T>
-__global__ void k_deconv_trunc(int L, int M, int nth2, int nth, const typename Cplx<T>::type* __restrict__ h,
+__global__ void k_deconv_trunc(int L, int M, int nth2, int nh, const typename Cplx<T>::type* __restrict__ h,
                                const double* __restrict__ pth, const double* __restrict__ pph,
                                double2* __restrict__ ft) {
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
@@ -65,50 +77,55 @@ __global__ void k_deconv_trunc(int L, int M, int nth2, int nth, const typename C
     else { k = 0; in = false; }
     double2 out = make_double2(0.0, 0.0);
     if (in) {
-        const typename Cplx<T>::type c = h[(int64_t)m * nth + (k >= 0 ? k : k + nth)];
+        const int kp = k >= 0 ? k : k + nh;
+        const typename Cplx<T>::type e = h[((int64_t)m * 2 + 0) * nh + kp];
+        const typename Cplx<T>::type o = h[((int64_t)m * 2 + 1) * nh + kp];
+        double sn, cs;
+        sincospi((double)k / (double)nh, &sn, &cs);      // conj twiddle e^{-2 pi i k / n_theta}
         const double f = pth[k + L] * pph[m];
-        out.x = (double)c.x * f;
-        out.y = (double)c.y * f;
+        out.x = ((double)e.x + (double)o.x * cs + (double)o.y * sn) * f;
+        out.y = ((double)e.y + (double)o.y * cs - (double)o.x * sn) * f;
     }
     ft[(int64_t)m * nth2 + r] = out;
 }
 
-// a5 / a9 layout change between the theta pass (H[m][a], a contiguous) and the phi pass
+// a5 / a9 layout change between the theta pass (H[m][parity][a'], a = 2a' + parity) and the phi pass
 // (Ht[a][m], m contiguous, row length mp = n_phi/2 + 1): 32 x 32 tiles through shared memory.
 // Only rows a <= n_theta/2 (theta in [0, pi]) and columns m <= mmax are moved.
 template <typename C>
 __global__ void __launch_bounds__(256)
-k_h_to_ht(int M, int nth, int nrow_half, int mp, const C* __restrict__ h, C* __restrict__ ht) {
+k_h_to_ht(int M, int nh, int nrow_half, int mp, const C* __restrict__ h, C* __restrict__ ht) {
     __shared__ C tile[32][33];
-    const int a0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    // blockIdx.x enumerates (parity, 32 values of a')
+    const int nblk = (nh + 31) / 32;
+    const int par = blockIdx.x / nblk, ap0 = (blockIdx.x % nblk) * 32, m0 = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
 #pragma unroll
     for (int r = ty; r < 32; r += 8) {
-        const int m = m0 + r, a = a0 + tx;
-        if (m <= M && a < nrow_half) tile[r][tx] = h[(int64_t)m * nth + a];
+        const int m = m0 + r, ap = ap0 + tx;
+        if (m <= M && ap < nh && 2 * ap + par < nrow_half) tile[r][tx] = h[((int64_t)m * 2 + par) * nh + ap];
     }
     __syncthreads();
 #pragma unroll
     for (int r = ty; r < 32; r += 8) {
-        const int a = a0 + r, m = m0 + tx;
-        if (m <= M && a < nrow_half) ht[(int64_t)a * mp + m] = tile[tx][r];
+        const int a = 2 * (ap0 + r) + par, m = m0 + tx;
+        if (m <= M && ap0 + r < nh && a < nrow_half) ht[(int64_t)a * mp + m] = tile[tx][r];
     }
 }
 
 // transpose back, fused with the zero-extension of the theta axis to the full period (the
-// transpose of "keep rows 0 .. n_theta/2"): H[m][a] = Ht[a][m] for a <= n_theta/2, 0 beyond
+// transpose of "keep rows 0 .. n_theta/2"): H[m][parity][a'] = Ht[2a' + parity][m] for rows <= n_theta/2, 0 beyond
 template <typename C>
 __global__ void __launch_bounds__(256)
-k_ht_to_h(int M, int nth, int nrow_half, int mp, const C* __restrict__ ht, C* __restrict__ h) {
+k_ht_to_h(int M, int nh, int nrow_half, int mp, const C* __restrict__ ht, C* __restrict__ h) {
     __shared__ C tile[32][33];
-    const int a0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    const int nblk = (nh + 31) / 32;
+    const int par = blockIdx.x / nblk, ap0 = (blockIdx.x % nblk) * 32, m0 = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    if (a0 < nrow_half) {
 #pragma unroll
-        for (int r = ty; r < 32; r += 8) {
-            const int a = a0 + r, m = m0 + tx;
-            if (m <= M && a < nrow_half) tile[r][tx] = ht[(int64_t)a * mp + m];
-        }
+    for (int r = ty; r < 32; r += 8) {
+        const int a = 2 * (ap0 + r) + par, m = m0 + tx;
+        if (m <= M && a < nrow_half) tile[r][tx] = ht[(int64_t)a * mp + m];
     }
     __syncthreads();
     C zero;
@@ -116,8 +133,8 @@ k_ht_to_h(int M, int nth, int nrow_half, int mp, const C* __restrict__ ht, C* __
     zero.y = 0;
 #pragma unroll
     for (int r = ty; r < 32; r += 8) {
-        const int m = m0 + r, a = a0 + tx;
-        if (m <= M && a < nth) h[(int64_t)m * nth + a] = (a < nrow_half) ? tile[tx][r] : zero;
+        const int m = m0 + r, ap = ap0 + tx;
+        if (m <= M && ap < nh) h[((int64_t)m * 2 + par) * nh + ap] = (2 * ap + par < nrow_half) ? tile[tx][r] : zero;
     }
 }
 
@@ -184,10 +201,10 @@ int fourier_build(nusht_plan_s* p) {
         wtot += ws;
     }
     {
-        int n[1] = {g.nth};
+        int n[1] = {g.nth / 2};   // two half-length transforms per m (see k_deconv_pad)
         NUSHT_CUFFT_TRY(cufftCreate(&p->fft_theta_fine));
-        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_fine, 1, n, nullptr, 1, g.nth, nullptr, 1, g.nth,
-                                          f64 ? CUFFT_Z2Z : CUFFT_C2C, M + 1, &ws));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_fine, 1, n, nullptr, 1, g.nth / 2, nullptr, 1, g.nth / 2,
+                                          f64 ? CUFFT_Z2Z : CUFFT_C2C, 2 * (M + 1), &ws));
         wtot += ws;
     }
     {
@@ -248,11 +265,11 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
                                  CUFFT_FORWARD));
     REC(1);
     {
-        dim3 grid((g.nth + 255) / 256, M + 1);
+        dim3 grid((g.nth / 2 + 255) / 256, M + 1);
         if (f64)
-            k_deconv_pad<double><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, p->d_ft, p->d_pth, p->d_pph, (double2*)p->d_h);
+            k_deconv_pad<double><<<grid, 256, 0, s>>>(L, M, nth2, g.nth / 2, p->d_ft, p->d_pth, p->d_pph, (double2*)p->d_h);
         else
-            k_deconv_pad<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, p->d_ft, p->d_pth, p->d_pph, (float2*)p->d_h);
+            k_deconv_pad<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth / 2, p->d_ft, p->d_pth, p->d_pph, (float2*)p->d_h);
         NUSHT_CUDA_TRY(cudaGetLastError());
     }
     REC(2);
@@ -266,11 +283,11 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     {
         // H[m][a] -> Ht[a][m] (rows theta in [0, pi] only), then the phi C2R on contiguous rows
         const int mp = g.nph / 2 + 1;
-        dim3 grid((g.nrow_half + 31) / 32, (M + 32) / 32);
+        dim3 grid(2 * ((g.nth / 2 + 31) / 32), (M + 32) / 32);
         if (f64)
-            k_h_to_ht<double2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, mp, (const double2*)p->d_h, (double2*)p->d_ht);
+            k_h_to_ht<double2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, mp, (const double2*)p->d_h, (double2*)p->d_ht);
         else
-            k_h_to_ht<float2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, mp, (const float2*)p->d_h, (float2*)p->d_ht);
+            k_h_to_ht<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, mp, (const float2*)p->d_h, (float2*)p->d_ht);
         NUSHT_CUDA_TRY(cudaGetLastError());
         if (p->c2r_clobbers_input && mp - M - 1 > 0)
             NUSHT_CUDA_TRY(cudaMemset2DAsync((char*)p->d_ht + (size_t)(M + 1) * csz, (size_t)mp * csz, 0,
@@ -302,11 +319,11 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     {
         // Ht[a][m] -> H[m][a] for m <= mmax, zero-extended in theta to the full period
         const int mp = g.nph / 2 + 1;
-        dim3 grid((g.nth + 31) / 32, (M + 32) / 32);
+        dim3 grid(2 * ((g.nth / 2 + 31) / 32), (M + 32) / 32);
         if (f64)
-            k_ht_to_h<double2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, mp, (const double2*)p->d_ht_adj, (double2*)p->d_h);
+            k_ht_to_h<double2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, mp, (const double2*)p->d_ht_adj, (double2*)p->d_h);
         else
-            k_ht_to_h<float2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, mp, (const float2*)p->d_ht_adj, (float2*)p->d_h);
+            k_ht_to_h<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, mp, (const float2*)p->d_ht_adj, (float2*)p->d_h);
         NUSHT_CUDA_TRY(cudaGetLastError());
     }
     REC(1);
@@ -320,10 +337,10 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     {
         dim3 grid((nth2 + 255) / 256, M + 1);
         if (f64)
-            k_deconv_trunc<double><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, (const double2*)p->d_h, p->d_pth, p->d_pph,
+            k_deconv_trunc<double><<<grid, 256, 0, s>>>(L, M, nth2, g.nth / 2, (const double2*)p->d_h, p->d_pth, p->d_pph,
                                                         p->d_ft);
         else
-            k_deconv_trunc<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, (const float2*)p->d_h, p->d_pth, p->d_pph,
+            k_deconv_trunc<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth / 2, (const float2*)p->d_h, p->d_pth, p->d_pph,
                                                        p->d_ft);
         NUSHT_CUDA_TRY(cudaGetLastError());
     }
