@@ -99,18 +99,19 @@ def oracle_sample(cfg, theta, phi, alm, x, seconds):
     from oracle import oracle as o
     L, M = cfg["lmax"], cfg["mmax"]
     nlm = inputs.nlm(L, M)
-    steps_per_s = 3.0e8 * max(1, o.num_threads()) / 8.0      # rough prior, refined by a probe
-    probe = max(8, min(len(theta), int(0.5 * steps_per_s / nlm)))
-    t0 = time.perf_counter()
-    o.synthesis(L, M, theta[:probe], phi[:probe], alm)
-    dt = max(time.perf_counter() - t0, 1e-4)
-    n = int(max(8, min(len(theta), probe * (seconds / 2.0) / dt)))
-    t0 = time.perf_counter()
-    o.synthesis(L, M, theta[:n], phi[:n], alm)
-    t_syn = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    o.adjoint(L, M, theta[:n], phi[:n], x[:n])
-    t_adj = time.perf_counter() - t0
+    # grow the sample until synthesis + adjoint take about `seconds` of wall time (bounded by the sample given)
+    n = max(8, min(len(theta), int(2.0e8 * max(1, o.num_threads()) * 0.25 / nlm)))
+    while True:
+        t0 = time.perf_counter()
+        o.synthesis(L, M, theta[:n], phi[:n], alm)
+        t_syn = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        o.adjoint(L, M, theta[:n], phi[:n], x[:n])
+        t_adj = time.perf_counter() - t0
+        tot = t_syn + t_adj
+        if tot >= 0.5 * seconds or n >= len(theta):
+            break
+        n = int(min(len(theta), max(2 * n, n * 0.9 * seconds / max(tot, 1e-3))))
     scale = len(theta) / n
     ms_full = (t_syn + t_adj) * scale * 1e3
     return ms_full, {"value": ms_full, "unit": "ms", "cores": o.num_threads(), "kind": "oracle",
@@ -167,6 +168,18 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
 
 
+def ncu_traffic(cfg, npts):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of our kernels from the committed
+    `ncu --set full` capture (profiles/ncu_traffic.json); only valid for the workload it was captured on."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(path):
+        return {}
+    d = json.load(open(path))
+    if d.get("lmax") != cfg["lmax"] or d.get("npts") != npts or d.get("eps") != cfg["eps"]:
+        return {}
+    return d.get("bytes_per_launch", {})
+
+
 def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz):
     """Algorithmic work per stage over its CUDA-event time."""
     hbm, hbm_src, sm_max = measured_peaks()
@@ -192,6 +205,8 @@ def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz):
         out[name] = {"bound": "hbm", "achieved": a, "peak": hbm, "unit": "GB/s", "frac": a / hbm, "traffic": None,
                      "ms": ms, "peak_source": hbm_src, "algorithmic_bytes": nbytes}
 
+    traffic = ncu_traffic(cfg, npts)
+
     alu("legendre_synthesis", syn_ms["legendre"])
     alu("legendre_adjoint", adj_ms["legendre"])
     mem("interp", syn_ms["interp"], nu_bytes)
@@ -202,6 +217,20 @@ def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz):
     mem("fourier_synthesis", fft_ms, fft_bytes)
     fft_ms_a = adj_ms["fft_theta"] + adj_ms["deconv_trunc"] + adj_ms["fft_fine_theta"] + adj_ms["fft_fine_phi"]
     mem("fourier_adjoint", fft_ms_a, fft_bytes)
+    for k in out:
+        out[k]["traffic"] = traffic.get(k)
+    # interpolation / spreading at w >= 9 in FP64 are bound by the FP64 pipe (DMMA + kernel evaluation), not by
+    # HBM: report that fraction too.  Executed FMA per point: 4 KS NT 256/8 (interp) or
+    # 2 MT NT 256/4 (spread) tensor-core FMA + 2 (w/2)(deg+1) evaluation FMA.
+    w = info.kernel_width
+    nt = 2 if w <= 8 else 3
+    ks = 2 if w <= 6 else (3 if w <= 10 else (4 if w <= 14 else 5))
+    mt = 1 if w <= 6 else (2 if w <= 14 else 3)
+    ev = 2 * ((w + 1) // 2) * (max(w, 5) + 1)
+    for name, fma in (("interp", ks * nt * 256 / 8 + ev), ("spread", mt * nt * 256 / 4 + ev)):
+        tf = 2.0 * fma * npts / (out[name]["ms"] * 1e-3) / 1e12
+        out[name]["fp64_executed_tflops"] = tf
+        out[name]["fp64_frac"] = tf / fp64_peak
     return out
 
 
@@ -300,7 +329,10 @@ def run_b200(args, rank, world):
         "synthesis_ms": sum(syn_acc.values()), "adjoint_ms": sum(adj_acc.values()),
         "stage_ms": {"synthesis": syn_acc, "adjoint": adj_acc},
         "roofline": roof, "stage_rooflines": roofs, "clocks": clocks, "e2e": e2e,
-        "gpu_launches": 8 * args.steps,      # our kernels per step: 4 per transform (cuFFT/memset not counted)
+        # our kernels per step (cuFFT kernels and memsets not counted): synthesis k_alm_prep, k_legendre_synth,
+        # k_deconv_pad, k_h_to_ht, k_interp_mma; adjoint k_spread_mma, k_ht_to_h, k_deconv_trunc,
+        # k_legendre_adjoint, k_alm_post
+        "gpu_launches": 10 * args.steps,
         "plan": {"ms": plan.info.plan_ms, "workspace_gb": plan.info.workspace_bytes / 1e9,
                  "n_rings": plan.info.n_rings, "n_theta": plan.info.n_theta, "n_theta_fine": plan.info.n_theta_fine,
                  "n_phi_fine": plan.info.n_phi_fine, "kernel_width": plan.info.kernel_width},
