@@ -620,7 +620,7 @@ template <int W, int S>
 struct MmaScratch {
     static constexpr int STH = mma_th_stride(S);
     static constexpr int SP = W | 1;
-    double th[32][STH];   // per point: theta weights, zero-padded to S slots
+    double th[33][STH];   // per point: theta weights, zero-padded to S slots; row 32 stays zero (absent points)
     double ph[32][SP];    // per point: phi weights
     double res[32];       // interp: per point result
     int oy[32];           // per point: strip column of the first footprint column
@@ -710,6 +710,7 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
     if (start >= end) return;
     WS& ws = s_ws[warp];
     StripRing<NT>& ring = s_ring[warp];
+    if (lane < WS::STH) ws.th[32][lane] = 0.0;
     const NufftGeom& g = P.g;
     const int strip = item % g.nstrip;
     const int c0 = strip * g.mb - g.fl;   // global column of strip column 0
@@ -731,21 +732,25 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
     int staged_hi = INT_MIN;              // cp.async issued for rows below staged_hi (those >= loaded_hi are in the ring)
     int landed_hi = INT_MIN;              // rows below landed_hi are known to have arrived
 
+    const int r_limit = g.nth / 2 + 1 + S;   // no point touches a row >= r_limit (< 2 n_theta: grid_row is enough)
     auto stage_rows = [&](int r0, int r1) {
+        r1 = min(r1, r_limit);
 #pragma unroll 1
         for (int r = r0; r < r1; ++r) {
             bool mirror;
-            const int64_t ro = grid_row_any(g, r, mirror);
+            const int64_t ro = grid_row(g, r, mirror);
             if (lane < NC) cp_async_8(&ring.rows[(r + 32) & (RB - 1)][lane], grid + ro + (mirror ? cols_m : cols_n));
         }
     };
     // static register indices + predicates only (a run-time index would put the window in local memory)
     auto commit_group = [&](int q, bool in, const double (&v)[NT]) {
-        const int ks = q % KS;
+        const int ks = q % KS;        // warp-uniform: a branch per k-step, selects only inside it
 #pragma unroll
         for (int ksi = 0; ksi < KS; ++ksi)
+            if (ks == ksi) {
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt) win[ksi][nt] = (in && ks == ksi) ? v[nt] : win[ksi][nt];
+                for (int nt = 0; nt < NT; ++nt) win[ksi][nt] = in ? v[nt] : win[ksi][nt];
+            }
     };
 
     if (start + lane < end) {
@@ -780,6 +785,10 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             // ---- rows [row0, need_hi) must be in the register window; they come from the ring ----
             if (loaded_hi < need_hi) {
                 if (staged_hi < need_hi) {          // first tile of the item, or a jump past the look-ahead
+                    if (row0 > staged_hi) {         // discontinuity: older copies in flight may target the same ring slots
+                        cp_async_wait_all();
+                        __syncwarp();
+                    }
                     stage_rows(max(staged_hi, row0), need_hi);
                     staged_hi = need_hi;
                 }
@@ -811,14 +820,16 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             const int a0p = __shfl_sync(0xffffffffu, a0, jp);
             const int sp = (a0p + OFF) % S;
             const bool live = gq < cnt;
+            const double* thp = &ws.th[live ? jp : 32][0];      // row 32 is all zero
             double d[NT][2];
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt) d[nt][0] = d[nt][1] = 0.0;
 #pragma unroll
             for (int ks = 0; ks < KS; ++ks) {
                 int i = 4 * ks + t - sp;
-                if (i < 0) i += S;
-                const double a = live ? ws.th[jp][i] : 0.0;
+                if ((S & (S - 1)) == 0) i &= S - 1;
+                else if (i < 0) i += S;
+                const double a = thp[i];
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) dmma_m8n8k4(d[nt][0], d[nt][1], a, win[ks][nt]);
             }
@@ -860,6 +871,7 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
     const int start = P.item_off[item], end = P.item_off[item + 1];
     if (start >= end) return;
     WS& ws = s_ws[warp];
+    if (lane < WS::STH) ws.th[32][lane] = 0.0;
     const NufftGeom& g = P.g;
     const int strip = item % g.nstrip;
     const int c0 = strip * g.mb - g.fl;
@@ -950,12 +962,14 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             const int sp = (a0p + OFF) % S;
             const int oy = ws.oy[jp];
             const bool live = t < cnt;
+            const double* thp = &ws.th[live ? jp : 32][0];      // row 32 is all zero
             double a[MT], b[NT];
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) {
                 int i = 8 * mt + gq - sp;
-                if (i < 0) i += S;
-                a[mt] = live ? ws.th[jp][i] : 0.0;
+                if ((S & (S - 1)) == 0) i &= S - 1;
+                else if (i < 0) i += S;
+                a[mt] = thp[i];
             }
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt) {

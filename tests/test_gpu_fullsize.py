@@ -46,4 +46,8 @@ def test_fullsize_sampled(oracle, config, nsample):
     lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
     rhs = oracle.inner_alm(L, M, alm, cd)
     assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    # the same identity with x = S a (inner product ||f||^2, no cancellation): a bar on the operator pair
+    cf = plan.adjoint(cu(f)).cpu().numpy()
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(f)))
+    assert abs(lhs - oracle.inner_alm(L, M, alm, cf)) <= 1e-12 * lhs
     plan.destroy()

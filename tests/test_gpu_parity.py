@@ -26,6 +26,15 @@ def cu(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
+def strong_adjointness(plan, oracle, L, M, alm, f):
+    """<S a, x> = <a, S^T x> with x = S a itself: the inner product is ||f||^2 (no cancellation), so the
+    1e-12 bar relative to the norms is a bar on the operator pair, not on a lucky small inner product."""
+    c = plan.adjoint(torch.from_numpy(f).cuda()).cpu().numpy()
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(f)))
+    rhs = oracle.inner_alm(L, M, alm, c)
+    return abs(lhs - rhs) / lhs
+
+
 def ring_reference(oracle, L, M, alm, nr, nth2, prec="ld"):
     """Doubled ring map from the oracle's ring_sum (a1 + a2 by their definition)."""
     th = np.pi * np.arange(nr) / (nr - 1)
@@ -136,6 +145,7 @@ def test_config1_full(nusht, oracle):
     lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
     rhs = oracle.inner_alm(L, M, alm, c)
     assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    assert strong_adjointness(plan, oracle, L, M, alm, f) <= 1e-12
     plan.destroy()
 
 
@@ -252,6 +262,7 @@ def test_all_widths_fp64(nusht, oracle, eps):
     lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
     rhs = oracle.inner_alm(L, M, alm, c)
     assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    assert strong_adjointness(plan, oracle, L, M, alm, f) <= 1e-12
     plan.destroy()
 
 
@@ -275,3 +286,23 @@ def test_clustered_and_sorted_points(nusht, oracle):
         assert rel(f, oracle.synthesis(L, M, theta, phi, alm, "ld")) <= 1e-8, name
         assert rel(c, oracle.adjoint(L, M, theta, phi, x, "ld")) <= 1e-8, name
         plan.destroy()
+
+
+@pytest.mark.parametrize("L,npts,eps", [(1023, 3000, 1e-8), (1023, 3000, 1e-10), (511, 200000, 1e-6),
+                                        (2047, 50000, 1e-12)])
+def test_sparse_points_large_grid(nusht, oracle, L, npts, eps):
+    """Few points on a large grid: every tile jumps past the staged look-ahead rows of the interpolation
+    ring and past the accumulator window of the spreading kernel."""
+    theta, phi = inputs.uniform_sphere_points(npts, 91)
+    alm = inputs.random_alm(L, L, 91, "inv_l2")
+    x = inputs.random_map(npts, 91)
+    plan = nusht.Plan(L, L, cu(theta), cu(phi), eps)
+    f = plan.synthesis(cu(alm)).cpu().numpy()
+    c = plan.adjoint(cu(x)).cpu().numpy()
+    ns = min(npts, 1500)
+    assert rel(f[:ns], oracle.synthesis(L, L, theta[:ns], phi[:ns], alm, "ld")) <= 10 * eps
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+    rhs = oracle.inner_alm(L, L, alm, c)
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    assert strong_adjointness(plan, oracle, L, L, alm, f) <= 1e-12
+    plan.destroy()
