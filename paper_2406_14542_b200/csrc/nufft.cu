@@ -610,7 +610,7 @@ __device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, do
 }
 
 __host__ __device__ constexpr int mma_nt(int w) { return w <= 8 ? 2 : 3; }                 // n-tiles per strip
-__host__ __device__ constexpr int mma_ks(int w) { return w <= 6 ? 2 : (w <= 10 ? 3 : (w <= 14 ? 4 : 5)); }
+__host__ __device__ constexpr int mma_ks(int w) { return w <= 6 ? 2 : (w <= 11 ? 3 : (w <= 14 ? 4 : 5)); }
 __host__ __device__ constexpr int mma_mt(int w) { return w <= 6 ? 1 : (w <= 14 ? 2 : 3); }
 // warps (work items) per CTA of the interpolation kernel: static shared memory stays below 48 KB
 __host__ __device__ constexpr int mma_interp_warps(int w) { return w <= 11 ? 4 : 2; }
