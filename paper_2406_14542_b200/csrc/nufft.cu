@@ -614,7 +614,7 @@ __host__ __device__ constexpr int mma_ks(int w) { return w <= 6 ? 2 : (w <= 11 ?
 __host__ __device__ constexpr int mma_mt(int w) { return w <= 6 ? 1 : (w <= 14 ? 2 : 3); }
 // warps (work items) per CTA of the interpolation kernel: static shared memory stays below 48 KB
 __host__ __device__ constexpr int mma_interp_warps(int w) { return w <= 11 ? 4 : 2; }
-__host__ __device__ constexpr int mma_th_stride(int s) { return s <= 8 ? 12 : (s <= 16 ? 20 : 36); }  // = 4 or 12 mod 16
+__host__ __device__ constexpr int mma_th_stride(int s) { return s <= 12 ? 12 : (s <= 16 ? 20 : 36); }  // = 4 or 12 mod 16
 
 template <int W, int S>
 struct MmaScratch {
@@ -694,7 +694,7 @@ struct StripRing {
 // the next batch of 32 points are staged while the current batch is processed.
 // ---------------------------------------------------------------------------------------------
 template <int W>
-__global__ void __launch_bounds__(32 * mma_interp_warps(W))
+__global__ void __launch_bounds__(32 * mma_interp_warps(W), mma_interp_warps(W) == 4 ? 5 : 1)
 k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<double> kp,
              const double* __restrict__ grid, double* __restrict__ map) {
     constexpr int NT = mma_nt(W), KS = mma_ks(W), S = 4 * KS, SPAN = S - W, OFF = 2 * S, NC = 8 * NT;
