@@ -622,7 +622,6 @@ struct MmaScratch {
     static constexpr int SP = W | 1;
     double th[33][STH];   // per point: theta weights, zero-padded to S slots; row 32 stays zero (absent points)
     double ph[32][SP];    // per point: phi weights
-    double res[32];       // interp: per point result
     int oy[32];           // per point: strip column of the first footprint column
 };
 
@@ -680,9 +679,9 @@ __device__ __forceinline__ int64_t grid_row_any(const NufftGeom& g, int a, bool&
 constexpr int NU_RING_ROWS = 16;   // rows of the strip staged ahead of the register window
 constexpr int NU_RING_CHUNK = 8;   // rows staged per top-up
 
-template <int NT>
+template <int NT, int RB>
 struct StripRing {
-    double rows[NU_RING_ROWS][8 * NT];   // row r of the strip lives in rows[(r + 32) & 15]
+    double rows[RB][8 * NT];             // row r of the strip lives in rows[(r + 48) % RB]
     double sx[32], sy[32];               // coordinates of the next batch of points
     int sperm[32];
 };
@@ -694,22 +693,22 @@ struct StripRing {
 // the next batch of 32 points are staged while the current batch is processed.
 // ---------------------------------------------------------------------------------------------
 template <int W>
-__global__ void __launch_bounds__(32 * mma_interp_warps(W), mma_interp_warps(W) == 4 ? 5 : 1)
+__global__ void __launch_bounds__(32 * mma_interp_warps(W), mma_interp_warps(W) == 4 ? 6 : 1)
 k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<double> kp,
              const double* __restrict__ grid, double* __restrict__ map) {
     constexpr int NT = mma_nt(W), KS = mma_ks(W), S = 4 * KS, SPAN = S - W, OFF = 2 * S, NC = 8 * NT;
-    constexpr int RB = NU_RING_ROWS, CH = NU_RING_CHUNK;
+    constexpr int RB = S <= 12 ? 12 : NU_RING_ROWS, CH = S <= 12 ? 4 : NU_RING_CHUNK;   // ring rows >= window slots
     using WS = MmaScratch<W, S>;
     constexpr int NW = mma_interp_warps(W);
     __shared__ __align__(16) WS s_ws[NW];
-    __shared__ __align__(16) StripRing<NT> s_ring[NW];
+    __shared__ __align__(16) StripRing<NT, RB> s_ring[NW];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int item = blockIdx.x * NW + warp;
     if (item >= P.n_items) return;
     const int start = P.item_off[item], end = P.item_off[item + 1];
     if (start >= end) return;
     WS& ws = s_ws[warp];
-    StripRing<NT>& ring = s_ring[warp];
+    StripRing<NT, RB>& ring = s_ring[warp];
     if (lane < WS::STH) ws.th[32][lane] = 0.0;
     const NufftGeom& g = P.g;
     const int strip = item % g.nstrip;
@@ -739,7 +738,7 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
         for (int r = r0; r < r1; ++r) {
             bool mirror;
             const int64_t ro = grid_row(g, r, mirror);
-            if (lane < NC) cp_async_8(&ring.rows[(r + 32) & (RB - 1)][lane], grid + ro + (mirror ? cols_m : cols_n));
+            if (lane < NC) cp_async_8(&ring.rows[(r + 48) % RB][lane], grid + ro + (mirror ? cols_m : cols_n));
         }
     };
     // static register indices + predicates only (a run-time index would put the window in local memory)
@@ -802,7 +801,7 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
                     const int rr = 4 * q + t;
                     const bool in = rr >= rb && rr < re;
                     double v[NT];
-                    const double* src = &ring.rows[(rr - OFF + 32) & (RB - 1)][NT * gq];
+                    const double* src = &ring.rows[(rr - OFF + 48) % RB][NT * gq];
 #pragma unroll
                     for (int nt = 0; nt < NT; ++nt) v[nt] = src[nt];
                     commit_group(q, in, v);
@@ -846,11 +845,10 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
                 }
             sum += __shfl_xor_sync(0xffffffffu, sum, 1);
             sum += __shfl_xor_sync(0xffffffffu, sum, 2);
-            if (t == 0 && live) ws.res[jp] = sum;
+            const int dstp = __shfl_sync(0xffffffffu, dst, jp);   // caller index of point j0 + g
+            if (t == 0 && live) map[dstp] = sum;
             j0 += cnt;
         }
-        __syncwarp();
-        if (has) map[dst] = ws.res[lane];
         __syncwarp();
     }
 }
