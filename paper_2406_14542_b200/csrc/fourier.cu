@@ -89,14 +89,21 @@ __global__ void k_deconv_trunc(int L, int M, int nth2, int nh, const typename Cp
     ft[(int64_t)m * nth2 + r] = out;
 }
 
-// a5 / a9 layout change between the theta pass (H[m][parity][a'], a = 2a' + parity) and the phi pass
-// (Ht[a][m], m contiguous, row length mp = n_phi/2 + 1): 32 x 32 tiles through shared memory.
-// Only rows a <= n_theta/2 (theta in [0, pi]) and columns m <= mmax are moved.
+// a5 / a9, phi pass.  The real transform of length N = n_phi on row a is done as ONE complex transform of
+// length N/2 on the row itself (the real row viewed as N/2 complex numbers x[2j] + i x[2j+1]), with the
+// usual pre-/post-processing of a real FFT fused into the transposes between the theta-pass layout
+// H[m][parity][a'] (a = 2a' + parity) and the grid rows:
+//   synthesis:  Z[k] = (X[k] + conj X[N/2-k]) + i W^k (X[k] - conj X[N/2-k]),  W = e^{2 pi i/N},  X[k] = H_a[k] for
+//               k <= mmax < N/4 and 0 otherwise, so Z[m] = X[m] (1 + i W^m), Z[N/2-m] = conj(X[m]) (1 - i W^{N/2-m});
+//               the inverse transform of Z is x[2j] + i x[2j+1] with x[n] = sum_m w_m Re(X[m] W^{mn}).
+//   adjoint:    Zf = forward transform of the row;  Y[m] = (Zf[m] + conj Zf[N/2-m])/2 - (i/2) W^{-m} (Zf[m] - conj Zf[N/2-m])
+//               = sum_n x[n] W^{-mn}  for m <= mmax.
+// 32 x 32 tiles through shared memory; only rows a <= n_theta/2 (theta in [0, pi]) and columns m <= mmax.
 template <typename C>
 __global__ void __launch_bounds__(256)
-k_h_to_ht(int M, int nh, int nrow_half, int mp, const C* __restrict__ h, C* __restrict__ ht) {
+k_h_to_z(int M, int nh, int nrow_half, int nz, const double2* __restrict__ tw, const C* __restrict__ h,
+         C* __restrict__ z) {
     __shared__ C tile[32][33];
-    // blockIdx.x enumerates (parity, 32 values of a')
     const int nblk = (nh + 31) / 32;
     const int par = blockIdx.x / nblk, ap0 = (blockIdx.x % nblk) * 32, m0 = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
@@ -109,23 +116,53 @@ k_h_to_ht(int M, int nh, int nrow_half, int mp, const C* __restrict__ h, C* __re
 #pragma unroll
     for (int r = ty; r < 32; r += 8) {
         const int a = 2 * (ap0 + r) + par, m = m0 + tx;
-        if (m <= M && ap0 + r < nh && a < nrow_half) ht[(int64_t)a * mp + m] = tile[tx][r];
+        if (ap0 + r >= nh || a >= nrow_half) continue;
+        C* row = z + (int64_t)a * nz;
+        if (m <= M) {
+            const C x = tile[tx][r];
+            const double2 w = tw[m];      // W^m = (cos, sin)
+            const double xr = x.x, xi = x.y;
+            C v;
+            if (m == 0) {                 // X[0] is real for a real row; its imaginary part is ignored
+                v.x = x.x;
+                v.y = x.x;
+                row[0] = v;
+            } else {
+                v.x = xr * (1.0 - w.y) - xi * w.x;
+                v.y = xr * w.x + xi * (1.0 - w.y);
+                row[m] = v;
+                v.x = xr * (1.0 + w.y) + xi * w.x;
+                v.y = xr * w.x - xi * (1.0 + w.y);
+                row[nz - m] = v;
+            }
+        }
+        if (blockIdx.y == 0) {            // columns mmax+1 .. N/2-mmax-1 carry no mode
+            C zero;
+            zero.x = 0;
+            zero.y = 0;
+            for (int k = M + 1 + tx; k <= nz - M - 1; k += 32) row[k] = zero;
+        }
     }
 }
 
-// transpose back, fused with the zero-extension of the theta axis to the full period (the
-// transpose of "keep rows 0 .. n_theta/2"): H[m][parity][a'] = Ht[2a' + parity][m] for rows <= n_theta/2, 0 beyond
+// adjoint: post-processing of the forward transform + transpose + zero-extension of the theta axis to the
+// full period (the transpose of "keep rows 0 .. n_theta/2")
 template <typename C>
 __global__ void __launch_bounds__(256)
-k_ht_to_h(int M, int nh, int nrow_half, int mp, const C* __restrict__ ht, C* __restrict__ h) {
-    __shared__ C tile[32][33];
+k_z_to_h(int M, int nh, int nrow_half, int nz, const double2* __restrict__ tw, const C* __restrict__ z,
+         C* __restrict__ h) {
+    __shared__ C ta[32][33], tb[32][33];
     const int nblk = (nh + 31) / 32;
     const int par = blockIdx.x / nblk, ap0 = (blockIdx.x % nblk) * 32, m0 = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
 #pragma unroll
     for (int r = ty; r < 32; r += 8) {
         const int a = 2 * (ap0 + r) + par, m = m0 + tx;
-        if (m <= M && a < nrow_half) tile[r][tx] = ht[(int64_t)a * mp + m];
+        if (m <= M && a < nrow_half) {
+            const C* row = z + (int64_t)a * nz;
+            ta[r][tx] = row[m];
+            tb[r][tx] = row[m == 0 ? 0 : nz - m];
+        }
     }
     __syncthreads();
     C zero;
@@ -134,18 +171,17 @@ k_ht_to_h(int M, int nh, int nrow_half, int mp, const C* __restrict__ ht, C* __r
 #pragma unroll
     for (int r = ty; r < 32; r += 8) {
         const int m = m0 + r, ap = ap0 + tx;
-        if (m <= M && ap < nh) h[((int64_t)m * 2 + par) * nh + ap] = (2 * ap + par < nrow_half) ? tile[tx][r] : zero;
-    }
-}
-
-// plan-time probe: does any word of columns m > M of Ht differ from zero?
-__global__ void k_tail_nonzero(int M, int nrow_half, int mp, int words_per_elem, const unsigned long long* __restrict__ ht,
-                               int* __restrict__ flag) {
-    const int64_t tail = (int64_t)(mp - M - 1) * words_per_elem;
-    const int64_t total = (int64_t)nrow_half * tail;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t a = i / tail, q = i - a * tail;
-        if (ht[(a * mp + M + 1) * words_per_elem + q] != 0ull) *flag = 1;
+        if (m > M || ap >= nh) continue;
+        C out = zero;
+        if (2 * ap + par < nrow_half) {
+            const C A = ta[tx][r], Bc = tb[tx][r];
+            const double2 w = tw[m];
+            const double bx = Bc.x, by = -(double)Bc.y;          // B = conj Zf[N/2 - m]
+            const double dx = (double)A.x - bx, dy = (double)A.y - by;
+            out.x = 0.5 * (((double)A.x + bx) + (w.x * dy - w.y * dx));
+            out.y = 0.5 * (((double)A.y + by) - (w.x * dx + w.y * dy));
+        }
+        h[((int64_t)m * 2 + par) * nh + ap] = out;
     }
 }
 
@@ -179,16 +215,11 @@ int fourier_build(nusht_plan_s* p) {
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_pth, pth.data(), sizeof(double) * (2 * L + 1), cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_pph, pph.data(), sizeof(double) * (M + 1), cudaMemcpyHostToDevice));
 
-    const int mp = g.nph / 2 + 1;
     const size_t hbytes = (size_t)(M + 1) * (size_t)g.nth * csz;
-    const size_t htbytes = (size_t)g.nrow_half * (size_t)mp * csz;
     const size_t gbytes = (size_t)g.nrow_half * (size_t)g.nph * rsz;
     NUSHT_TRY(f_alloc(&p->d_h, hbytes, p));
-    NUSHT_TRY(f_alloc(&p->d_ht, htbytes, p));
-    NUSHT_TRY(f_alloc(&p->d_ht_adj, htbytes, p));   // R2C output of the adjoint (fills columns m > mmax too)
     NUSHT_TRY(f_alloc(&p->d_grid, gbytes, p));
     NUSHT_CUDA_TRY(cudaMemset(p->d_h, 0, hbytes));
-    NUSHT_CUDA_TRY(cudaMemset(p->d_ht, 0, htbytes));
     NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
 
     // cuFFT plans
@@ -208,38 +239,20 @@ int fourier_build(nusht_plan_s* p) {
         wtot += ws;
     }
     {
-        // phi pass on the transposed buffer Ht[a][m]: contiguous rows of mp complex <-> n_phi reals
-        int n[1] = {g.nph};
-        int inembed[1] = {mp}, onembed[1] = {g.nph};
-        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi_c2r));
-        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_c2r, 1, n, inembed, 1, mp, onembed, 1, g.nph,
-                                          f64 ? CUFFT_Z2D : CUFFT_C2R, g.nrow_half, &ws));
+        // phi pass: one complex transform of length n_phi/2 per grid row, in place (see k_h_to_z)
+        int n[1] = {g.nph / 2};
+        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi, 1, n, nullptr, 1, g.nph / 2, nullptr, 1, g.nph / 2,
+                                          f64 ? CUFFT_Z2Z : CUFFT_C2C, g.nrow_half, &ws));
         wtot += ws;
-        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi_r2c));
-        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_r2c, 1, n, onembed, 1, g.nph, inembed, 1, mp,
-                                          f64 ? CUFFT_D2Z : CUFFT_R2C, g.nrow_half, &ws));
-        wtot += ws;
-    }
-    // Columns m > mmax of Ht are zero and must stay so for the C2R.  cuFFT is allowed to overwrite the
-    // input of an out-of-place C2R: probe once whether this plan does; if it does, they are re-zeroed
-    // on every synthesis, otherwise never again.
-    p->c2r_clobbers_input = false;
-    if (mp - M - 1 > 0) {
-        int* d_flag = nullptr;
-        NUSHT_CUDA_TRY(cudaMalloc((void**)&d_flag, sizeof(int)));
-        NUSHT_CUDA_TRY(cudaMemset(d_flag, 0, sizeof(int)));
-        NUSHT_CUDA_TRY(cudaMemset2D(p->d_ht, (size_t)mp * csz, 0x3c, (size_t)(M + 1) * csz, (size_t)g.nrow_half));
-        if (f64)
-            NUSHT_CUFFT_TRY(cufftExecZ2D(p->fft_phi_c2r, (cufftDoubleComplex*)p->d_ht, (cufftDoubleReal*)p->d_grid));
-        else
-            NUSHT_CUFFT_TRY(cufftExecC2R(p->fft_phi_c2r, (cufftComplex*)p->d_ht, (cufftReal*)p->d_grid));
-        k_tail_nonzero<<<1024, 256>>>(M, g.nrow_half, mp, (int)(csz / 8), (const unsigned long long*)p->d_ht, d_flag);
-        int flag = 0;
-        NUSHT_CUDA_TRY(cudaMemcpy(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost));
-        cudaFree(d_flag);
-        p->c2r_clobbers_input = flag != 0;
-        NUSHT_CUDA_TRY(cudaMemset(p->d_ht, 0, htbytes));
-        NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
+        std::vector<double2> tw(M + 1);
+        const long double PI_L = 3.14159265358979323846264338327950288L;
+        for (int m = 0; m <= M; ++m) {
+            const long double ang = 2.0L * PI_L * (long double)m / (long double)g.nph;
+            tw[m] = make_double2((double)cosl(ang), (double)sinl(ang));
+        }
+        NUSHT_TRY(f_alloc(&p->d_twz, sizeof(double2) * (M + 1), p));
+        NUSHT_CUDA_TRY(cudaMemcpy(p->d_twz, tw.data(), sizeof(double2) * (M + 1), cudaMemcpyHostToDevice));
     }
     p->workspace_bytes += (int64_t)wtot;
     p->have_fft = true;
@@ -281,23 +294,23 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
         NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_theta_fine, (cufftComplex*)p->d_h, (cufftComplex*)p->d_h, CUFFT_INVERSE));
     REC(3);
     {
-        // H[m][a] -> Ht[a][m] (rows theta in [0, pi] only), then the phi C2R on contiguous rows
-        const int mp = g.nph / 2 + 1;
+        // H -> pre-processed rows of the grid buffer, then one in-place complex transform per row
+        const int nz = g.nph / 2;
         dim3 grid(2 * ((g.nth / 2 + 31) / 32), (M + 32) / 32);
         if (f64)
-            k_h_to_ht<double2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, mp, (const double2*)p->d_h, (double2*)p->d_ht);
+            k_h_to_z<double2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, p->d_twz, (const double2*)p->d_h,
+                                                    (double2*)p->d_grid);
         else
-            k_h_to_ht<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, mp, (const float2*)p->d_h, (float2*)p->d_ht);
+            k_h_to_z<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, p->d_twz, (const float2*)p->d_h,
+                                                   (float2*)p->d_grid);
         NUSHT_CUDA_TRY(cudaGetLastError());
-        if (p->c2r_clobbers_input && mp - M - 1 > 0)
-            NUSHT_CUDA_TRY(cudaMemset2DAsync((char*)p->d_ht + (size_t)(M + 1) * csz, (size_t)mp * csz, 0,
-                                             (size_t)(mp - M - 1) * csz, (size_t)g.nrow_half, s));
     }
-    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi_c2r, s));
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi, s));
     if (f64)
-        NUSHT_CUFFT_TRY(cufftExecZ2D(p->fft_phi_c2r, (cufftDoubleComplex*)p->d_ht, (cufftDoubleReal*)p->d_grid));
+        NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_phi, (cufftDoubleComplex*)p->d_grid, (cufftDoubleComplex*)p->d_grid,
+                                     CUFFT_INVERSE));
     else
-        NUSHT_CUFFT_TRY(cufftExecC2R(p->fft_phi_c2r, (cufftComplex*)p->d_ht, (cufftReal*)p->d_grid));
+        NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_phi, (cufftComplex*)p->d_grid, (cufftComplex*)p->d_grid, CUFFT_INVERSE));
     REC(4);
     return NUSHT_OK;
 }
@@ -311,19 +324,22 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     const bool f64 = p->dtype == NUSHT_F64;
     const size_t csz = f64 ? 16 : 8;
     REC(0);
-    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi_r2c, s));
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi, s));
     if (f64)
-        NUSHT_CUFFT_TRY(cufftExecD2Z(p->fft_phi_r2c, (cufftDoubleReal*)p->d_grid, (cufftDoubleComplex*)p->d_ht_adj));
+        NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_phi, (cufftDoubleComplex*)p->d_grid, (cufftDoubleComplex*)p->d_grid,
+                                     CUFFT_FORWARD));
     else
-        NUSHT_CUFFT_TRY(cufftExecR2C(p->fft_phi_r2c, (cufftReal*)p->d_grid, (cufftComplex*)p->d_ht_adj));
+        NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_phi, (cufftComplex*)p->d_grid, (cufftComplex*)p->d_grid, CUFFT_FORWARD));
     {
-        // Ht[a][m] -> H[m][a] for m <= mmax, zero-extended in theta to the full period
-        const int mp = g.nph / 2 + 1;
+        // post-processing + transpose to H[m][parity][a'], zero-extended in theta to the full period
+        const int nz = g.nph / 2;
         dim3 grid(2 * ((g.nth / 2 + 31) / 32), (M + 32) / 32);
         if (f64)
-            k_ht_to_h<double2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, mp, (const double2*)p->d_ht_adj, (double2*)p->d_h);
+            k_z_to_h<double2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, p->d_twz, (const double2*)p->d_grid,
+                                                    (double2*)p->d_h);
         else
-            k_ht_to_h<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, mp, (const float2*)p->d_ht_adj, (float2*)p->d_h);
+            k_z_to_h<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, p->d_twz, (const float2*)p->d_grid,
+                                                   (float2*)p->d_h);
         NUSHT_CUDA_TRY(cudaGetLastError());
     }
     REC(1);
@@ -356,10 +372,10 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
 void fourier_free(nusht_plan_s* p) {
     if (p->fft_theta_coarse) cufftDestroy(p->fft_theta_coarse);
     if (p->fft_theta_fine) cufftDestroy(p->fft_theta_fine);
-    if (p->fft_phi_c2r) cufftDestroy(p->fft_phi_c2r);
-    if (p->fft_phi_r2c) cufftDestroy(p->fft_phi_r2c);
-    p->fft_theta_coarse = p->fft_theta_fine = p->fft_phi_c2r = p->fft_phi_r2c = 0;
-    cudaFree(p->d_pth); cudaFree(p->d_pph); cudaFree(p->d_h); cudaFree(p->d_ht); cudaFree(p->d_ht_adj); cudaFree(p->d_grid);
+    if (p->fft_phi) cufftDestroy(p->fft_phi);
+    p->fft_theta_coarse = p->fft_theta_fine = p->fft_phi = 0;
+    cudaFree(p->d_pth); cudaFree(p->d_pph); cudaFree(p->d_h); cudaFree(p->d_twz); cudaFree(p->d_grid);
     p->d_pth = p->d_pph = nullptr;
-    p->d_h = p->d_ht = p->d_ht_adj = p->d_grid = nullptr;
+    p->d_h = p->d_grid = nullptr;
+    p->d_twz = nullptr;
 }

@@ -91,14 +91,11 @@ struct nusht_plan_s {
     double* d_pth = nullptr;        // deconvolution factors p_theta(k), k = -lmax..lmax
     double* d_pph = nullptr;        // p_phi(m), m = 0..mmax
     void* d_h = nullptr;            // theta-pass buffer H[m][a]: [mmax+1][nth] complex (dtype)
-    void* d_ht = nullptr;           // phi-pass buffer Ht[a][m]: [nth/2+1][nph/2+1] complex (dtype), columns m > mmax zero
-    void* d_ht_adj = nullptr;       // same shape: R2C output of the adjoint
-    bool c2r_clobbers_input = false;   // plan-time probe of the cuFFT C2R plan
+    double2* d_twz = nullptr;       // W^m = e^{2 pi i m / n_phi}, m = 0..mmax (real-FFT pre/post-processing)
     void* d_grid = nullptr;         // fine real grid [nth/2+1][nph] (dtype)
     cufftHandle fft_theta_coarse = 0;  // Z2Z, length nth2, batch mmax+1
     cufftHandle fft_theta_fine = 0;    // C2C (dtype), length nth, batch mmax+1
-    cufftHandle fft_phi_c2r = 0;       // C2R (dtype), length nph, batch nth/2+1, contiguous rows of Ht
-    cufftHandle fft_phi_r2c = 0;       // R2C (dtype), contiguous rows of Ht
+    cufftHandle fft_phi = 0;           // C2C (dtype), length nph/2, batch nth/2+1, in place on the grid rows
     bool have_fft = false;
     // --- points ---
     double* d_px = nullptr;         // sorted theta in fine-grid units
