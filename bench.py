@@ -46,6 +46,10 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--eps-sweep", action="store_true",
+                    help="BASELINE.json configs[4]: lmax=4095 on 67M points, eps in {1e-4, 1e-6} FP32 and "
+                         "{1e-8, 1e-10, 1e-12} FP64; one JSON line per eps (accuracy on an oracle subset + timing)")
+    ap.add_argument("--sweep-subset", type=int, default=1500, help="points of the oracle subset of the sweep")
     return ap.parse_args()
 
 
@@ -359,8 +363,61 @@ def run_b200(args, rank, world):
         dist.destroy_process_group()
 
 
+def run_eps_sweep(args):
+    """Config 5: accuracy (Eq. 9-10 against the long-double oracle on a seeded subset of the points; the
+    paper's own subset is 1e6 points, which a direct sum cannot afford here) and throughput per eps."""
+    import torch
+    from oracle import oracle as o
+    from paper_2406_14542_b200 import nusht
+    torch.cuda.set_device(0)
+    cfg, theta, phi, alm, x = inputs.make_config(args.config, npts=args.npts)
+    L, M, npts = cfg["lmax"], cfg["mmax"], len(theta)
+    rng = np.random.default_rng(12345)
+    sub = np.sort(rng.choice(npts, min(args.sweep_subset, npts), replace=False))
+    f_ref = o.synthesis(L, M, theta[sub], phi[sub], alm, "ld")
+    xs = np.zeros(npts)
+    xs[sub] = x[sub]
+    c_ref = o.adjoint(L, M, theta[sub], phi[sub], x[sub], "ld")
+    d_theta, d_phi = torch.from_numpy(theta).cuda(), torch.from_numpy(phi).cuda()
+    for dtype, eps in (("f32", 1e-4), ("f32", 1e-6), ("f64", 1e-8), ("f64", 1e-10), ("f64", 1e-12)):
+        plan = nusht.Plan(L, M, d_theta, d_phi, eps, dtype)
+        rd, cd = (np.float32, np.complex64) if dtype == "f32" else (np.float64, np.complex128)
+        d_alm, d_x, d_xs = (torch.from_numpy(alm.astype(cd)).cuda(), torch.from_numpy(x.astype(rd)).cuda(),
+                            torch.from_numpy(xs.astype(rd)).cuda())
+        f = plan.synthesis(d_alm)
+        c = plan.adjoint(d_xs)
+        e_syn = float(np.linalg.norm(f[torch.from_numpy(sub).cuda()].cpu().numpy().astype(np.float64) - f_ref)
+                      / np.linalg.norm(f_ref))
+        e_adj = float(np.linalg.norm(c.cpu().numpy().astype(np.complex128) - c_ref) / np.linalg.norm(c_ref))
+        d_map = torch.empty_like(f)
+        d_out = torch.empty_like(c)
+        plan.set_stage_timing(True)
+        for _ in range(3):
+            plan.synthesis(d_alm, d_map)
+            plan.adjoint(d_x, d_out)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            plan.synthesis(d_alm, d_map)
+            plan.adjoint(d_x, d_out)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        print(json.dumps({"metric": METRIC, "value": ms, "unit": "ms", "dtype": dtype, "eps": eps,
+                          "kernel_width": plan.info.kernel_width, "eps_eff_synthesis": e_syn, "eps_eff_adjoint": e_adj,
+                          "subset_points": int(len(sub)), "points_per_s": 2.0 * npts / (ms * 1e-3),
+                          "stage_ms": {"synthesis": plan.stage_times("synthesis"), "adjoint": plan.stage_times("adjoint")},
+                          "config": workload_config(dict(cfg, eps=eps), npts)}))
+        plan.destroy()
+        del d_alm, d_x, d_xs, f, c, d_map, d_out
+
+
 def main():
     args = parse()
+    if args.eps_sweep:
+        run_eps_sweep(args)
+        return
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
     if args.impl == "reference":
