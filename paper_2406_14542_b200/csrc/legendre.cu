@@ -670,7 +670,7 @@ __device__ __forceinline__ double warp_transpose_reduce16(double (&v)[16], int l
 // (scaled value below range) keeps G = 0 in registers, so the inner loop needs no masks; its folded
 // G values are loaded when the pair comes into range.
 template <int R>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32, 18)
 k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restrict__ eo) {
     if (P.rem > 0 && blockIdx.x == P.nblk) {
         adjoint_remainder(P, gt, eo, P.nblk * (32 * R), P.rem);
