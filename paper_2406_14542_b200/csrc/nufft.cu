@@ -938,7 +938,7 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
         const int npt = min(32, end - batch);
         int j0 = 0;
         while (j0 < npt) {
-            // ---- tile: up to 4 consecutive points within SPAN rows of the first ----
+            // ---- tile: up to 8 consecutive points whose origins lie within SPAN rows of the window base ----
             const int row0 = __shfl_sync(0xffffffffu, a0, j0);
             // ---- rows below row0 are complete: flush them FG at a time (slots hold [a_lo, a_lo + S)) ----
             if (a_lo == INT_MIN) a_lo = row0;
@@ -953,31 +953,35 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
                 a_lo += FG;
             }
             const unsigned fit = __ballot_sync(0xffffffffu, has && lane >= j0 && a0 - a_lo <= SPAN);
-            const int cnt = min(4, __popc(fit));
-            // ---- fragments: A[slot][point t] and B[point t][column], point = j0 + t ----
-            const int jp = min(j0 + t, 31);
-            const int a0p = __shfl_sync(0xffffffffu, a0, jp);
-            const int sp = (a0p + OFF) % S;
-            const int oy = ws.oy[jp];
-            const bool live = t < cnt;
-            const double* thp = &ws.th[live ? jp : 32][0];      // row 32 is all zero
-            double a[MT], b[NT];
+            const int cnt = min(8, __popc(fit));
+            // ---- two k-steps of 4 points each; fragments A[slot][point t], B[point t][column], point = j0 + 4 kk + t ----
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) {
-                int i = 8 * mt + gq - sp;
-                if ((S & (S - 1)) == 0) i &= S - 1;
-                else if (i < 0) i += S;
-                a[mt] = thp[i];
+            for (int kk = 0; kk < 2; ++kk) {
+                if (4 * kk >= cnt) break;                          // warp-uniform
+                const int jp = min(j0 + 4 * kk + t, 31);
+                const int a0p = __shfl_sync(0xffffffffu, a0, jp);
+                const int sp = (a0p + OFF) % S;
+                const int oy = ws.oy[jp];
+                const bool live = 4 * kk + t < cnt;
+                const double* thp = &ws.th[live ? jp : 32][0];      // row 32 is all zero
+                double a[MT], b[NT];
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) {
+                    int i = 8 * mt + gq - sp;
+                    if ((S & (S - 1)) == 0) i &= S - 1;
+                    else if (i < 0) i += S;
+                    a[mt] = thp[i];
+                }
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const unsigned ip = (unsigned)(NT * gq + nt - oy);
+                    b[nt] = (ip < (unsigned)W) ? ws.ph[jp][ip] : 0.0;
+                }
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) dmma_m8n8k4(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
             }
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) {
-                const unsigned ip = (unsigned)(NT * gq + nt - oy);
-                b[nt] = (ip < (unsigned)W) ? ws.ph[jp][ip] : 0.0;
-            }
-#pragma unroll
-            for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-                for (int nt = 0; nt < NT; ++nt) dmma_m8n8k4(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
             j0 += cnt;
         }
         __syncwarp();
