@@ -322,7 +322,7 @@ def run_b200(args, rank, world):
         for _ in range(args.steps):
             plan.synthesis_host(h_alm, h_map, stream)
             plan.adjoint_host(h_x, h_out, stream)
-            stream.synchronize()
+            plan.host_sync()          # both results are in host memory
         barrier()
         e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
         e2e_ms = max_over_ranks(e2e_ms, world, "cuda")

@@ -117,11 +117,17 @@ NUSHT_API int nusht_adjoint(nusht_plan_t* plan, const void* map, void* alm, void
 /* Free the plan and everything it owns.  NULL is accepted. */
 NUSHT_API int nusht_destroy(nusht_plan_t* plan);
 
-/* Same transforms with HOST buffers (pinned or pageable): the call copies the input to a
- * plan-owned device buffer, runs the transform, copies the result back, all on `stream`, and
- * returns without synchronising (the caller synchronises the stream before reading the output). */
+/* Same transforms with HOST buffers (pinned for overlap; pageable works but serialises): the call
+ * uploads the input on a plan-owned copy stream, runs the transform on `stream`, downloads the result on
+ * a second plan-owned copy stream, and returns without synchronising.  Uploads, kernels and downloads of
+ * consecutive calls overlap (each direction has its own device staging buffers, allocated on first use).
+ * The outputs are valid after nusht_host_sync(plan) (or a device-wide synchronisation); synchronising
+ * `stream` alone is NOT enough.  The host buffers must stay untouched until then. */
 NUSHT_API int nusht_synthesis_host(nusht_plan_t* plan, const void* alm_host, void* map_host, void* stream);
 NUSHT_API int nusht_adjoint_host(nusht_plan_t* plan, const void* map_host, void* alm_host, void* stream);
+/* Block the calling thread until every host-buffer transform issued so far on this plan has delivered
+ * its output. */
+NUSHT_API int nusht_host_sync(nusht_plan_t* plan);
 
 /* Stage entry points (tests and per-stage measurement).
  * Legendre synthesis + DFS doubling alone: alm -> Ftilde, DEVICE complex128

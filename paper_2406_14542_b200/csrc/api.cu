@@ -54,8 +54,14 @@ static void plan_release(nusht_plan_s* p) {
     legendre_free(p);
     fourier_free(p);
     nufft_free(p);
-    cudaFree(p->d_stage_alm);
-    cudaFree(p->d_stage_map);
+    cudaFree(p->d_in_alm); cudaFree(p->d_out_alm); cudaFree(p->d_in_map); cudaFree(p->d_out_map);
+    if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
+    if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
+    for (int k = 0; k < 2; ++k) {
+        if (p->ev_in[k]) cudaEventDestroy(p->ev_in[k]);
+        if (p->ev_cdone[k]) cudaEventDestroy(p->ev_cdone[k]);
+        if (p->ev_out[k]) cudaEventDestroy(p->ev_out[k]);
+    }
     for (int k = 0; k < 2; ++k)
         for (int i = 0; i <= NUSHT_NUM_STAGES; ++i)
             if (p->ev[k][i]) cudaEventDestroy(p->ev[k][i]);
@@ -204,15 +210,46 @@ extern "C" int nusht_adjoint(nusht_plan_t* p, const void* map, void* alm, void* 
     return NUSHT_OK;
 }
 
+// Host-buffer transforms.  Copies run on two plan-owned streams (host->device, device->host) and are
+// ordered against the compute on `stream` with events, so that with pinned host memory the upload of
+// the next input and the download of the previous result overlap the kernels of the current call
+// (PCIe is full duplex).  Each direction has its own input and output staging buffer.
+static int host_setup(nusht_plan_s* p) {
+    if (p->s_h2d) return NUSHT_OK;
+    const size_t abytes = (size_t)p->nlm * 2 * real_size(p), mbytes = (size_t)p->npts * real_size(p);
+    NUSHT_CUDA_TRY(cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
+    NUSHT_CUDA_TRY(cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
+    for (int k = 0; k < 2; ++k) {
+        NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_in[k], cudaEventDisableTiming));
+        NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_cdone[k], cudaEventDisableTiming));
+        NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_out[k], cudaEventDisableTiming));
+    }
+    NUSHT_CUDA_TRY(cudaMalloc(&p->d_in_alm, abytes ? abytes : 16));
+    NUSHT_CUDA_TRY(cudaMalloc(&p->d_out_alm, abytes ? abytes : 16));
+    NUSHT_CUDA_TRY(cudaMalloc(&p->d_in_map, mbytes ? mbytes : 16));
+    NUSHT_CUDA_TRY(cudaMalloc(&p->d_out_map, mbytes ? mbytes : 16));
+    p->workspace_bytes += (int64_t)(2 * abytes + 2 * mbytes);
+    return NUSHT_OK;
+}
+
 extern "C" int nusht_synthesis_host(nusht_plan_t* p, const void* alm_host, void* map_host, void* stream) {
     if (!p || !alm_host || (!map_host && p->npts > 0)) return NUSHT_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     const size_t abytes = (size_t)p->nlm * 2 * real_size(p), mbytes = (size_t)p->npts * real_size(p);
-    if (!p->d_stage_alm) NUSHT_CUDA_TRY(cudaMalloc(&p->d_stage_alm, abytes ? abytes : 16));
-    if (!p->d_stage_map) NUSHT_CUDA_TRY(cudaMalloc(&p->d_stage_map, mbytes ? mbytes : 16));
-    NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_stage_alm, alm_host, abytes, cudaMemcpyHostToDevice, s));
-    NUSHT_TRY(nusht_synthesis(p, p->d_stage_alm, p->d_stage_map, stream));
-    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(map_host, p->d_stage_map, mbytes, cudaMemcpyDeviceToHost, s));
+    NUSHT_TRY(host_setup(p));
+    // upload: the input staging buffer is free once the previous synthesis has consumed it
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_h2d, p->ev_cdone[0], 0));
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_in_alm, alm_host, abytes, cudaMemcpyHostToDevice, p->s_h2d));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_in[0], p->s_h2d));
+    // compute: needs the input, and the output staging buffer back from the previous download
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_in[0], 0));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_out[0], 0));
+    NUSHT_TRY(nusht_synthesis(p, p->d_in_alm, p->d_out_map, stream));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_cdone[0], s));
+    // download
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_d2h, p->ev_cdone[0], 0));
+    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(map_host, p->d_out_map, mbytes, cudaMemcpyDeviceToHost, p->s_d2h));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_out[0], p->s_d2h));
     return NUSHT_OK;
 }
 
@@ -220,11 +257,24 @@ extern "C" int nusht_adjoint_host(nusht_plan_t* p, const void* map_host, void* a
     if (!p || !alm_host || (!map_host && p->npts > 0)) return NUSHT_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     const size_t abytes = (size_t)p->nlm * 2 * real_size(p), mbytes = (size_t)p->npts * real_size(p);
-    if (!p->d_stage_alm) NUSHT_CUDA_TRY(cudaMalloc(&p->d_stage_alm, abytes ? abytes : 16));
-    if (!p->d_stage_map) NUSHT_CUDA_TRY(cudaMalloc(&p->d_stage_map, mbytes ? mbytes : 16));
-    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_stage_map, map_host, mbytes, cudaMemcpyHostToDevice, s));
-    NUSHT_TRY(nusht_adjoint(p, p->d_stage_map, p->d_stage_alm, stream));
-    NUSHT_CUDA_TRY(cudaMemcpyAsync(alm_host, p->d_stage_alm, abytes, cudaMemcpyDeviceToHost, s));
+    NUSHT_TRY(host_setup(p));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_h2d, p->ev_cdone[1], 0));
+    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_in_map, map_host, mbytes, cudaMemcpyHostToDevice, p->s_h2d));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_in[1], p->s_h2d));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_in[1], 0));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_out[1], 0));
+    NUSHT_TRY(nusht_adjoint(p, p->d_in_map, p->d_out_alm, stream));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_cdone[1], s));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_d2h, p->ev_cdone[1], 0));
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(alm_host, p->d_out_alm, abytes, cudaMemcpyDeviceToHost, p->s_d2h));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_out[1], p->s_d2h));
+    return NUSHT_OK;
+}
+
+extern "C" int nusht_host_sync(nusht_plan_t* p) {
+    if (!p) return NUSHT_ERR_INVALID_ARG;
+    if (!p->s_d2h) return NUSHT_OK;
+    NUSHT_CUDA_TRY(cudaStreamSynchronize(p->s_d2h));   // downloads are ordered after their compute and upload
     return NUSHT_OK;
 }
 

@@ -106,8 +106,9 @@ struct nusht_plan_s {
     int n_items = 0;
     void* kernel_host = nullptr;    // nufft.cu: host model of the kernel polynomial
     // --- host-buffer staging (allocated on first use of *_host) ---
-    void* d_stage_alm = nullptr;
-    void* d_stage_map = nullptr;
+    void *d_in_alm = nullptr, *d_out_alm = nullptr, *d_in_map = nullptr, *d_out_map = nullptr;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    cudaEvent_t ev_in[2] = {}, ev_cdone[2] = {}, ev_out[2] = {};   // [0] synthesis, [1] adjoint
     // --- stage timing ---
     int timing = 0;
     cudaEvent_t ev[2][NUSHT_NUM_STAGES + 1] = {};

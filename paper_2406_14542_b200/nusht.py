@@ -20,7 +20,7 @@ SYN_STAGES = ["alm_prep", "legendre", "fft_theta", "deconv_pad", "fft_fine_theta
 ADJ_STAGES = ["spread", "fft_fine_phi", "fft_fine_theta", "deconv_trunc", "fft_theta", "legendre", "alm_post"]
 EXPORTS = [
     "nusht_plan", "nusht_synthesis", "nusht_adjoint", "nusht_destroy", "nusht_synthesis_host",
-    "nusht_adjoint_host", "nusht_stage_legendre_synthesis", "nusht_stage_legendre_adjoint",
+    "nusht_adjoint_host", "nusht_host_sync", "nusht_stage_legendre_synthesis", "nusht_stage_legendre_adjoint",
     "nusht_stage_interp", "nusht_stage_spread", "nusht_set_stage_timing", "nusht_stage_times",
     "nusht_plan_info", "nusht_strerror", "nusht_version",
 ]
@@ -58,6 +58,8 @@ def _load():
     lib.nusht_plan.restype = ip
     lib.nusht_destroy.argtypes = [vp]
     lib.nusht_destroy.restype = ip
+    lib.nusht_host_sync.argtypes = [vp]
+    lib.nusht_host_sync.restype = ip
     lib.nusht_set_stage_timing.argtypes = [vp, ip]
     lib.nusht_set_stage_timing.restype = ip
     lib.nusht_stage_times.argtypes = [vp, ip, ctypes.POINTER(ctypes.c_float), ip]
@@ -155,6 +157,10 @@ class Plan:
         _check(lib.nusht_adjoint_host(self._h, self._map_arg(x_host, False), self._alm_arg(out_host, False),
                                       _stream_ptr(stream)))
         return out_host
+
+    def host_sync(self):
+        """Wait until every host-buffer transform issued so far has delivered its output."""
+        _check(lib.nusht_host_sync(self._h))
 
     # ---- stages ----
     def stage_legendre_synthesis(self, alm, stream=None):
