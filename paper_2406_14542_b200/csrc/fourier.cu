@@ -14,9 +14,12 @@
 // cuFFT is used for the FFTs only; everything else here is our own kernels.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 
+#include <algorithm>
 #include <vector>
 
+#include "fft_smem.cuh"
 #include "nusht_internal.cuh"
 
 namespace {
@@ -149,8 +152,8 @@ k_h_to_z(int M, int nh, int nrow_half, int nz, const double2* __restrict__ tw, c
 // full period (the transpose of "keep rows 0 .. n_theta/2")
 template <typename C>
 __global__ void __launch_bounds__(256)
-k_z_to_h(int M, int nh, int nrow_half, int nz, const double2* __restrict__ tw, const C* __restrict__ z,
-         C* __restrict__ h) {
+k_z_to_h(int M, int nh, int nrow_half, int nz, bool write_ext, const double2* __restrict__ tw,
+         const C* __restrict__ z, C* __restrict__ h) {
     __shared__ C ta[32][33], tb[32][33];
     const int nblk = (nh + 31) / 32;
     const int par = blockIdx.x / nblk, ap0 = (blockIdx.x % nblk) * 32, m0 = blockIdx.y * 32;
@@ -173,6 +176,7 @@ k_z_to_h(int M, int nh, int nrow_half, int nz, const double2* __restrict__ tw, c
         const int m = m0 + r, ap = ap0 + tx;
         if (m > M || ap >= nh) continue;
         C out = zero;
+        if (2 * ap + par >= nrow_half && !write_ext) continue;   // the fused theta chain never reads the extension
         if (2 * ap + par < nrow_half) {
             const C A = ta[tx][r], Bc = tb[tx][r];
             const double2 w = tw[m];
@@ -183,6 +187,245 @@ k_z_to_h(int M, int nh, int nrow_half, int nz, const double2* __restrict__ tw, c
         }
         h[((int64_t)m * 2 + par) * nh + ap] = out;
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused theta chains (a3 + a4 + a5-theta, and the theta part of a9), used when the coarse and the
+// half fine length coincide (N = Ntheta = n_theta/2, a power of two <= 8192: sigma = 2 at the
+// BASELINE sizes).  One CTA per m keeps the column in shared memory (fft_smem.cuh):
+//   synthesis  Ftilde[m][.] --FFT--> c[m,k] --(p_theta p_phi, |k| <= lmax)--> registers
+//              --(parity 0: as is; parity 1: e^{2 pi i k/n_theta})--> inverse FFT --> H[m][parity][a'],
+//              storing only the rows a = 2a' + parity <= n_theta/2 that the phi pass reads;
+//   adjoint    the transposed chain: H[m][parity][a'] (zero beyond n_theta/2) --FFT--> combine the
+//              parities, truncate, deconvolve --> inverse FFT --> Gtilde[m][.].
+// HBM traffic per column: N complex in, ~N complex out (the cuFFT chain it replaces moves 9 N).
+// ---------------------------------------------------------------------------------------------
+template <int N>
+struct ChainCfg {
+    static constexpr int T = N >= 512 ? N / 16 : 32;    // threads per CTA: one radix-16 butterfly per thread and stage
+    static constexpr int E = N / T;                     // spectrum entries held per thread
+    static constexpr size_t SMEM = sizeof(double2) * (size_t)fftsm::padded_len(N);
+};
+
+// plan-time tables of the fused chains (one allocation, see fourier_build)
+struct ChainTables {
+    const double2* tw2;     // exp(-2 pi i i/N), i < N/2: the fused radix-2 stage
+    const double2* stw;     // per-stage twiddles (fftsm::stage_table_offset)
+    const double* fpos;     // p_theta(k(p)) for |k(p)| <= lmax, else 0, at digit-reversed position p
+    const double2* twpar;   // exp(+2 pi i k(p)/(2N)): the parity-1 shift, at position p
+};
+
+template <int N, int SIGN>
+struct DevExec {
+    double2* s;
+    const double2* stw;
+    int tid;
+    template <int R, int NS>
+    __device__ __forceinline__ void dif() {
+        fftsm::stage_dif<N, R, NS, SIGN>(s, tid, ChainCfg<N>::T, stw + fftsm::stage_table_offset(N, NS));
+        __syncthreads();
+    }
+    template <int R, int NS>
+    __device__ __forceinline__ void dit() {
+        fftsm::stage_dit<N, R, NS, SIGN>(s, tid, ChainCfg<N>::T, stw + fftsm::stage_table_offset(N, NS));
+        __syncthreads();
+    }
+};
+
+// L2 prefetch of the next column while the current one is transformed (one CTA per SM: nothing else overlaps HBM)
+__device__ __forceinline__ void prefetch_l2(const void* ptr, int bytes, int tid, int T) {
+    for (int o = tid * 4096; o < bytes; o += T * 4096) {
+        const int n = min(4096, bytes - o);
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"((const char*)ptr + o), "r"(n) : "memory");
+    }
+}
+
+template <int N, typename C>
+__global__ void __launch_bounds__(ChainCfg<N>::T)
+k_theta_chain_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, const double* __restrict__ pph,
+                  const ChainTables tb, C* __restrict__ h) {
+    using namespace fftsm;
+    constexpr int T = ChainCfg<N>::T, E = ChainCfg<N>::E;
+    extern __shared__ __align__(16) double2 s_col[];
+    const int tid = threadIdx.x;
+    for (int m = blockIdx.x; m <= M; m += gridDim.x) {
+        const double2* col = ft + (int64_t)m * N;
+        if (m + (int)gridDim.x <= M) prefetch_l2(col + (int64_t)gridDim.x * N, N * (int)sizeof(double2), tid, T);
+        __syncthreads();   // previous column's stores have read s_col
+        // a3: forward transform; its radix-2 stage is fused with the load
+        for (int i = tid; i < N / 2; i += T) {
+            const double2 a = col[i], b = col[i + N / 2];
+            s_col[pad(i)] = make_double2(a.x + b.x, a.y + b.y);
+            s_col[pad(i + N / 2)] = cmul(make_double2(a.x - b.x, a.y - b.y), tb.tw2[i]);
+        }
+        __syncthreads();
+        DevExec<N, -1> fwd{s_col, tb.stw, tid};
+        forward_stages<N / 2>(fwd);
+        // a4: deconvolve and truncate; the spectrum stays in registers (digit-reversed positions tid + T e)
+        double2 c[E];
+        const double fm = pph[m];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int p = tid + T * e;
+            const double2 v = s_col[pad(p)];
+            const double f = tb.fpos[p] * fm;
+            c[e] = make_double2(v.x * f, v.y * f);
+        }
+        // a5 (theta): rows a = 2a' + parity, one inverse transform per parity
+#pragma unroll 1
+        for (int par = 0; par < 2; ++par) {
+            __syncthreads();
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int p = tid + T * e;
+                s_col[pad(p)] = par ? cmul(c[e], tb.twpar[p]) : c[e];
+            }
+            __syncthreads();
+            DevExec<N, +1> inv{s_col, tb.stw, tid};
+            inverse_stages<N / 2>(inv);
+            C* out = h + ((int64_t)m * 2 + par) * N;
+            for (int i = tid; i < N / 2; i += T) {
+                const double2 z0 = s_col[pad(i)], z1 = cmul(s_col[pad(i + N / 2)], cconj(tb.tw2[i]));
+                if (2 * i + par < nrow_half) {
+                    C v;
+                    v.x = z0.x + z1.x;
+                    v.y = z0.y + z1.y;
+                    out[i] = v;
+                }
+                if (2 * (i + N / 2) + par < nrow_half) {
+                    C v;
+                    v.x = z0.x - z1.x;
+                    v.y = z0.y - z1.y;
+                    out[i + N / 2] = v;
+                }
+            }
+        }
+    }
+}
+
+template <int N, typename C>
+__global__ void __launch_bounds__(ChainCfg<N>::T)
+k_theta_chain_adj(int L, int M, int nrow_half, const C* __restrict__ h, const double* __restrict__ pph,
+                  const ChainTables tb, double2* __restrict__ ft) {
+    using namespace fftsm;
+    constexpr int T = ChainCfg<N>::T, E = ChainCfg<N>::E;
+    extern __shared__ __align__(16) double2 s_col[];
+    const int tid = threadIdx.x;
+    // rows of a parity block that exist: a = 2a' + par < nrow_half
+    for (int m = blockIdx.x; m <= M; m += gridDim.x) {
+        if (m + (int)gridDim.x <= M) {
+            const C* nxt = h + ((int64_t)(m + gridDim.x) * 2) * N;
+            const int rows = min(N, (nrow_half + 1) / 2);
+            prefetch_l2(nxt, rows * (int)sizeof(C), tid, T);
+            prefetch_l2(nxt + N, rows * (int)sizeof(C), tid, T);
+        }
+        double2 acc[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) acc[e] = make_double2(0.0, 0.0);
+#pragma unroll 1
+        for (int par = 0; par < 2; ++par) {
+            const C* in = h + ((int64_t)m * 2 + par) * N;
+            __syncthreads();
+            // zero-extension beyond row n_theta/2 (transpose of "keep rows 0 .. n_theta/2"), radix-2 stage fused
+            for (int i = tid; i < N / 2; i += T) {
+                double2 a = make_double2(0.0, 0.0), b = a;
+                if (2 * i + par < nrow_half) {
+                    const C v = in[i];
+                    a = make_double2((double)v.x, (double)v.y);
+                }
+                if (2 * (i + N / 2) + par < nrow_half) {
+                    const C v = in[i + N / 2];
+                    b = make_double2((double)v.x, (double)v.y);
+                }
+                s_col[pad(i)] = make_double2(a.x + b.x, a.y + b.y);
+                s_col[pad(i + N / 2)] = cmul(make_double2(a.x - b.x, a.y - b.y), tb.tw2[i]);
+            }
+            __syncthreads();
+            DevExec<N, -1> fwd{s_col, tb.stw, tid};
+            forward_stages<N / 2>(fwd);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int p = tid + T * e;
+                double2 v = s_col[pad(p)];
+                if (par) v = cmul(v, cconj(tb.twpar[p]));
+                acc[e].x += v.x;
+                acc[e].y += v.y;
+            }
+        }
+        __syncthreads();
+        const double fm = pph[m];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int p = tid + T * e;
+            const double f = tb.fpos[p] * fm;
+            s_col[pad(p)] = make_double2(acc[e].x * f, acc[e].y * f);
+        }
+        __syncthreads();
+        DevExec<N, +1> inv{s_col, tb.stw, tid};
+        inverse_stages<N / 2>(inv);
+        double2* out = ft + (int64_t)m * N;
+        for (int i = tid; i < N / 2; i += T) {
+            const double2 z0 = s_col[pad(i)], z1 = cmul(s_col[pad(i + N / 2)], cconj(tb.tw2[i]));
+            out[i] = make_double2(z0.x + z1.x, z0.y + z1.y);
+            out[i + N / 2] = make_double2(z0.x - z1.x, z0.y - z1.y);
+        }
+    }
+}
+
+// position -> frequency of the forward chain for a run-time N (host; mirrors fftsm::freq_of_pos)
+static int chain_freq_of_pos(int n, int p) {
+    int q = p / (n / 2), mul = 2, ns = n / 2;
+    p %= n / 2;
+    while (ns >= 16) {
+        q += mul * (p / (ns / 16));
+        p %= ns / 16;
+        mul *= 16;
+        ns /= 16;
+    }
+    return q + mul * p;
+}
+
+template <int N, typename C>
+int launch_chain(bool adjoint, int L, int M, int nrow_half, int n_sm, double2* ft, const double* pph,
+                 const ChainTables& tb, C* h, cudaStream_t s) {
+    static bool attr_set[2] = {false, false};
+    if (!attr_set[adjoint]) {
+        if (adjoint)
+            NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_theta_chain_adj<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                (int)ChainCfg<N>::SMEM));
+        else
+            NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_theta_chain_syn<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                (int)ChainCfg<N>::SMEM));
+        attr_set[adjoint] = true;
+    }
+    // persistent: as many CTAs as fit at once (shared memory bound), columns dealt round robin
+    const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(8, (size_t)(200 * 1024) / (ChainCfg<N>::SMEM + 1024)));
+    const int grid = std::min(M + 1, n_sm * per_sm);
+    if (adjoint)
+        k_theta_chain_adj<N, C><<<grid, ChainCfg<N>::T, ChainCfg<N>::SMEM, s>>>(L, M, nrow_half, h, pph, tb, ft);
+    else
+        k_theta_chain_syn<N, C><<<grid, ChainCfg<N>::T, ChainCfg<N>::SMEM, s>>>(L, M, nrow_half, ft, pph, tb, h);
+    NUSHT_CUDA_TRY(cudaGetLastError());
+    return NUSHT_OK;
+}
+
+template <typename C>
+int dispatch_chain(const nusht_plan_s* p, bool adjoint, C* h, cudaStream_t s) {
+    const int n = p->lg.nth2;
+    ChainTables tb;
+    tb.tw2 = p->d_tw2n;
+    tb.stw = p->d_tw2n + n / 2;
+    tb.twpar = p->d_tw2n + n / 2 + fftsm::stage_table_len(n);
+    tb.fpos = reinterpret_cast<const double*>(tb.twpar + n);
+    switch (n) {
+#define NUSHT_CHAIN(NN) \
+    case NN:            \
+        return launch_chain<NN, C>(adjoint, p->lmax, p->mmax, p->ng.nrow_half, p->n_sm, p->d_ft, p->d_pph, tb, h, s);
+        NUSHT_CHAIN(128) NUSHT_CHAIN(256) NUSHT_CHAIN(512) NUSHT_CHAIN(1024) NUSHT_CHAIN(2048) NUSHT_CHAIN(4096)
+        NUSHT_CHAIN(8192)
+#undef NUSHT_CHAIN
+    }
+    return NUSHT_ERR_UNSUPPORTED;
 }
 
 }  // namespace
@@ -222,16 +465,47 @@ int fourier_build(nusht_plan_s* p) {
     NUSHT_CUDA_TRY(cudaMemset(p->d_h, 0, hbytes));
     NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
 
+    // fused theta chains: coarse length == half fine length, a power of two that fits shared memory
+    p->theta_fused = (g.nth / 2 == nth2) && (nth2 & (nth2 - 1)) == 0 && nth2 >= 128 && nth2 <= 8192;
+    if (getenv("NUSHT_NO_FUSED_THETA")) p->theta_fused = false;   // TUNING HOOK (temporary)
+    if (p->theta_fused) {
+        // one buffer: tw2 [N/2] | stage tables | twpar [N] | fpos [N doubles]
+        const int n = nth2, nst = fftsm::stage_table_len(n);
+        std::vector<double2> tb((size_t)n / 2 + nst + n + (n + 1) / 2);
+        const long double PI_L = 3.14159265358979323846264338327950288L;
+        auto unit = [&](long double turns) {   // exp(2 pi i turns)
+            return make_double2((double)cosl(2.0L * PI_L * turns), (double)sinl(2.0L * PI_L * turns));
+        };
+        for (int i = 0; i < n / 2; ++i) tb[i] = unit(-(long double)i / (long double)n);
+        {
+            size_t o = (size_t)n / 2;
+            for (int ns = n / 2; ns >= 32; ns /= 16)
+                for (int i = 0; i < ns / 16; ++i) tb[o++] = unit(-(long double)i / (long double)ns);
+        }
+        double2* twpar = tb.data() + n / 2 + nst;
+        double* fpos = reinterpret_cast<double*>(twpar + n);
+        for (int q = 0; q < n; ++q) {
+            const int f = chain_freq_of_pos(n, q), k = f < n / 2 ? f : f - n;
+            twpar[q] = unit((long double)k / (long double)(2 * n));
+            fpos[q] = (k >= -L && k <= L) ? pth[k + L] : 0.0;
+        }
+        NUSHT_TRY(f_alloc(&p->d_tw2n, sizeof(double2) * tb.size(), p));
+        NUSHT_CUDA_TRY(cudaMemcpy(p->d_tw2n, tb.data(), sizeof(double2) * tb.size(), cudaMemcpyHostToDevice));
+        int dev = 0;
+        NUSHT_CUDA_TRY(cudaGetDevice(&dev));
+        NUSHT_CUDA_TRY(cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, dev));
+    }
+
     // cuFFT plans
     size_t ws = 0, wtot = 0;
-    {
+    if (!p->theta_fused) {
         int n[1] = {nth2};
         NUSHT_CUFFT_TRY(cufftCreate(&p->fft_theta_coarse));
         NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_coarse, 1, n, nullptr, 1, nth2, nullptr, 1, nth2, CUFFT_Z2Z,
                                           M + 1, &ws));
         wtot += ws;
     }
-    {
+    if (!p->theta_fused) {
         int n[1] = {g.nth / 2};   // two half-length transforms per m (see k_deconv_pad)
         NUSHT_CUFFT_TRY(cufftCreate(&p->fft_theta_fine));
         NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_fine, 1, n, nullptr, 1, g.nth / 2, nullptr, 1, g.nth / 2,
@@ -273,6 +547,14 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     const bool f64 = p->dtype == NUSHT_F64;
     const size_t csz = f64 ? 16 : 8;
     REC(0);
+    if (p->theta_fused) {
+        REC(1);
+        REC(2);
+        if (f64)
+            NUSHT_TRY(dispatch_chain<double2>(p, false, (double2*)p->d_h, s));
+        else
+            NUSHT_TRY(dispatch_chain<float2>(p, false, (float2*)p->d_h, s));
+    } else {
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_coarse, s));
     NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_coarse, (cufftDoubleComplex*)p->d_ft, (cufftDoubleComplex*)p->d_ft,
                                  CUFFT_FORWARD));
@@ -292,6 +574,7 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
                                      CUFFT_INVERSE));
     else
         NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_theta_fine, (cufftComplex*)p->d_h, (cufftComplex*)p->d_h, CUFFT_INVERSE));
+    }
     REC(3);
     {
         // H -> pre-processed rows of the grid buffer, then one in-place complex transform per row
@@ -335,14 +618,24 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
         const int nz = g.nph / 2;
         dim3 grid(2 * ((g.nth / 2 + 31) / 32), (M + 32) / 32);
         if (f64)
-            k_z_to_h<double2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, p->d_twz, (const double2*)p->d_grid,
+            k_z_to_h<double2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, !p->theta_fused, p->d_twz, (const double2*)p->d_grid,
                                                     (double2*)p->d_h);
         else
-            k_z_to_h<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, p->d_twz, (const float2*)p->d_grid,
+            k_z_to_h<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, !p->theta_fused, p->d_twz, (const float2*)p->d_grid,
                                                    (float2*)p->d_h);
         NUSHT_CUDA_TRY(cudaGetLastError());
     }
     REC(1);
+    if (p->theta_fused) {
+        if (f64)
+            NUSHT_TRY(dispatch_chain<double2>(p, true, (double2*)p->d_h, s));
+        else
+            NUSHT_TRY(dispatch_chain<float2>(p, true, (float2*)p->d_h, s));
+        REC(2);
+        REC(3);
+        REC(4);
+        return NUSHT_OK;
+    }
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_fine, s));
     if (f64)
         NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_fine, (cufftDoubleComplex*)p->d_h, (cufftDoubleComplex*)p->d_h,
@@ -374,7 +667,8 @@ void fourier_free(nusht_plan_s* p) {
     if (p->fft_theta_fine) cufftDestroy(p->fft_theta_fine);
     if (p->fft_phi) cufftDestroy(p->fft_phi);
     p->fft_theta_coarse = p->fft_theta_fine = p->fft_phi = 0;
-    cudaFree(p->d_pth); cudaFree(p->d_pph); cudaFree(p->d_h); cudaFree(p->d_twz); cudaFree(p->d_grid);
+    cudaFree(p->d_pth); cudaFree(p->d_pph); cudaFree(p->d_h); cudaFree(p->d_twz); cudaFree(p->d_grid); cudaFree(p->d_tw2n);
+    p->d_tw2n = nullptr;
     p->d_pth = p->d_pph = nullptr;
     p->d_h = p->d_grid = nullptr;
     p->d_twz = nullptr;

@@ -22,6 +22,7 @@
 // The CPU oracle (oracle/) uses the plain three-term recurrence in l and shares nothing with this file.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 
 #include <vector>
 
@@ -42,6 +43,7 @@ constexpr int SYN_TN = 64;
 constexpr int ADJ_R = 4;
 constexpr int ADJ_TN = 64;
 constexpr int ADJ_CHUNK = 4;       // n-steps per transposing reduction / exponent check
+__host__ __device__ constexpr int adj_min_ctas(int r, int c) { return r <= 4 ? (c <= 2 ? 22 : 18) : (c <= 2 ? 12 : 10); }
 constexpr double SCALE_UP_LIMIT = 1.157920892373162e+77;   // 2^256
 constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
 
@@ -669,15 +671,16 @@ __device__ __forceinline__ double warp_transpose_reduce16(double (&v)[16], int l
 // No warp ever waits for another one, whatever its mix of live and dead ring pairs.  A dead pair
 // (scaled value below range) keeps G = 0 in registers, so the inner loop needs no masks; its folded
 // G values are loaded when the pair comes into range.
-template <int R>
-__global__ void __launch_bounds__(32, 18)
+template <int R, int C>
+__global__ void __launch_bounds__(32, adj_min_ctas(R, C))
 k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restrict__ eo) {
     if (P.rem > 0 && blockIdx.x == P.nblk) {
         adjoint_remainder(P, gt, eo, P.nblk * (32 * R), P.rem);
         return;
     }
     __shared__ __align__(16) double2 s_ab[2][ADJ_TN];
-    __shared__ __align__(16) double s_tr[4 * ADJ_CHUNK][33];
+    constexpr int NV = 4 * C;             // values reduced across the warp per chunk of C steps
+    __shared__ __align__(16) double s_tr[NV][33];
     __shared__ __align__(8) uint64_t s_bar[2];
 
     const int m = blockIdx.y;
@@ -694,12 +697,15 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
     if (n_start >= ne) return;                // never before lmax: this warp contributes nothing
     const int tile0 = n_start / ADJ_TN;
 
+    // entries past the end of a column are read (and their results dropped): keep them finite
+    for (int i = lane; i < 2 * ADJ_TN; i += 32) (&s_ab[0][0])[i] = make_double2(0.0, 0.0);
     if (lane == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
         mbar_fence_init();
     }
     __syncwarp();
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy zero fill before the bulk copies
     auto issue = [&](int tile) {
         const int st = (tile - tile0) & 1;
         const int cnt = min(ADJ_TN, ne - tile * ADJ_TN);
@@ -730,29 +736,34 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
         if (valid[r] && ex[r] == 0) load_g(j, gere[r], geim[r], gore[r], goim[r]);
     }
 
+    bool steady = false;                      // every pair of the warp in range: no more exponent bookkeeping
     for (int tile = tile0; tile < ntiles; ++tile) {
         const int st = (tile - tile0) & 1;
         const int cnt = min(ADJ_TN, ne - tile * ADJ_TN);
         mbar_wait(&s_bar[st], (uint32_t)(((tile - tile0) >> 1) & 1));
-        for (int i0 = (tile == tile0) ? n_start - tile0 * ADJ_TN : 0; i0 < cnt; i0 += ADJ_CHUNK) {
-            const int ns = min(ADJ_CHUNK, cnt - i0);
-            bool any_dead = false, any_live = false;
+        for (int i0 = (tile == tile0) ? n_start - tile0 * ADJ_TN : 0; i0 < cnt; i0 += C) {
+            const int ns = min(C, cnt - i0);
+            bool w_dead = false, w_live = true;
+            if (!steady) {                       // warp-uniform; exponents only ever count down to 0
+                bool any_dead = false, any_live = false;
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                any_dead |= (ex[r] > 0);
-                any_live |= (valid[r] && ex[r] == 0);
+                for (int r = 0; r < R; ++r) {
+                    any_dead |= (ex[r] > 0);
+                    any_live |= (valid[r] && ex[r] == 0);
+                }
+                w_dead = __any_sync(0xffffffffu, any_dead);
+                w_live = __any_sync(0xffffffffu, any_live);
+                steady = !w_dead && w_live;
             }
-            const bool w_dead = __any_sync(0xffffffffu, any_dead);
-            const bool w_live = __any_sync(0xffffffffu, any_live);
             if (w_live) {
                 // always ADJ_CHUNK steps: beyond the end of the column the sums are dropped below and
                 // the recurrence state is never used again
-                double v[4 * ADJ_CHUNK];
+                double v[NV];
 #pragma unroll
-                for (int q = 0; q < 4 * ADJ_CHUNK; ++q) v[q] = 0.0;
+                for (int q = 0; q < NV; ++q) v[q] = 0.0;
 #pragma unroll
-                for (int i = 0; i < ADJ_CHUNK; ++i) {
-                    const double2 ab = s_ab[st][min(i0 + i, cnt - 1)];
+                for (int i = 0; i < C; ++i) {
+                    const double2 ab = s_ab[st][i0 + i];   // beyond cnt: stale or zero entries, results dropped
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
                         const double t = fma(ab.x, x2[r], ab.y);
@@ -765,22 +776,23 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
                         p1[r] = pn;
                     }
                 }
-                // cross-lane sums: transpose through shared memory (value q of lane l at s_tr[q][l]);
-                // lane l then adds 16 entries of row l & 15, and the two halves are combined by a shuffle
+                // cross-lane sums: transpose through shared memory (value q of lane l at s_tr[q][l]); the
+                // 32 / NV lanes of row q = lane % NV add NV entries each and are combined by shuffles
 #pragma unroll
-                for (int q = 0; q < 4 * ADJ_CHUNK; ++q) s_tr[q][lane] = v[q];
+                for (int q = 0; q < NV; ++q) s_tr[q][lane] = v[q];
                 __syncwarp();
-                const double* src = &s_tr[lane & 15][16 * (lane >> 4)];
+                const double* src = &s_tr[lane % NV][NV * (lane / NV)];
                 double tot = 0.0, tot2 = 0.0;
 #pragma unroll
-                for (int k = 0; k < 16; k += 2) {
+                for (int k = 0; k < NV; k += 2) {
                     tot += src[k];
                     tot2 += src[k + 1];
                 }
                 tot += tot2;
-                tot += shfl_xor_d(tot, 16);
+#pragma unroll
+                for (int sh = NV; sh < 32; sh *= 2) tot += shfl_xor_d(tot, sh);
                 __syncwarp();
-                if (lane < 16 && (lane >> 2) < ns)      // lane = 4 * step + component
+                if (lane < NV && (lane >> 2) < ns)      // lane = 4 * step + component
                     atomicAdd(reinterpret_cast<double*>(eo + o + (int64_t)tile * ADJ_TN + i0) + lane, tot);
             } else {
                 for (int i = 0; i < ns; ++i) {
@@ -831,7 +843,8 @@ static dim3 leg_grid(const nusht_plan_s* p, int R, LegParams& P) {
     return dim3(nblk + (rem ? 1 : 0), p->mmax + 1);
 }
 
-static LegParams make_params(const nusht_plan_s* p) {
+static int g_adj_variant = 44;   // TUNING HOOK (temporary)
+static LegParams make_params(const nusht_plan_s* p, bool adjoint_tables = false) {
     LegParams P;
     P.nblk = 0;
     P.rem = 0;
@@ -847,9 +860,10 @@ static LegParams make_params(const nusht_plan_s* p) {
     P.x = p->d_x;
     P.logsin = p->d_logsin;
     P.logkap = p->d_logkap;
-    P.ff_n = p->d_ff_n;
-    P.ff_p = p->d_ff_p;
-    P.ff_e = p->d_ff_e;
+    const bool a = adjoint_tables && g_adj_variant / 10 == 8;
+    P.ff_n = a ? p->d_ffa_n : p->d_ff_n;
+    P.ff_p = a ? p->d_ffa_p : p->d_ff_p;
+    P.ff_e = a ? p->d_ffa_e : p->d_ff_e;
     return P;
 }
 
@@ -923,9 +937,9 @@ int legendre_build_tables(nusht_plan_s* p) {
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_x, x.data(), sizeof(double) * g.npairs, cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_logsin, ls.data(), sizeof(double2) * g.npairs, cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_logkap, lk.data(), sizeof(double2) * (M + 1), cudaMemcpyHostToDevice));
-    // fast-forward table (synthesis and adjoint use the same decomposition: LEG_R == ADJ_R pairs per thread)
+    // fast-forward tables: one per decomposition of the ring pairs (LEG_R pairs per thread in the
+    // synthesis, ADJ_R in the adjoint)
     {
-        static_assert(LEG_R == ADJ_R, "the fast-forward table is shared by both Legendre kernels");
         LegParams P = make_params(p);
         const dim3 grid = leg_grid(p, LEG_R, P);
         const size_t nw = (size_t)(M + 1) * (size_t)P.nblk;
@@ -935,6 +949,20 @@ int legendre_build_tables(nusht_plan_s* p) {
         k_legendre_fastforward<LEG_R><<<dim3(P.nblk, M + 1), 32>>>(P, p->d_ff_n, p->d_ff_p, p->d_ff_e);
         NUSHT_CUDA_TRY(cudaGetLastError());
         (void)grid;
+    }
+    {
+        const char* ev = getenv("NUSHT_ADJ_VARIANT");
+        g_adj_variant = ev ? atoi(ev) : 44;
+    }
+    if (g_adj_variant / 10 == 8) {
+        LegParams P = make_params(p);
+        leg_grid(p, 8, P);
+        const size_t nw = (size_t)(M + 1) * (size_t)P.nblk;
+        NUSHT_TRY(dev_alloc(&p->d_ffa_n, nw, p));
+        NUSHT_TRY(dev_alloc(&p->d_ffa_p, nw * 8 * 32, p));
+        NUSHT_TRY(dev_alloc(&p->d_ffa_e, nw * 8 * 32, p));
+        k_legendre_fastforward<8><<<dim3(P.nblk, M + 1), 32>>>(P, p->d_ffa_n, p->d_ffa_p, p->d_ffa_e);
+        NUSHT_CUDA_TRY(cudaGetLastError());
     }
     NUSHT_CUDA_TRY(cudaDeviceSynchronize());
     return NUSHT_OK;
@@ -963,9 +991,15 @@ int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s) {
 int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
     // the kernel accumulates with global reductions
     NUSHT_CUDA_TRY(cudaMemsetAsync(p->d_aeo, 0, sizeof(double4) * (size_t)p->n_e_total, s));
-    LegParams P = make_params(p);
-    const dim3 grid = leg_grid(p, ADJ_R, P);
-    k_legendre_adjoint<ADJ_R><<<grid, 32, 0, s>>>(P, gt, p->d_aeo);
+    LegParams P = make_params(p, true);
+    const int R = g_adj_variant / 10;
+    const dim3 grid = leg_grid(p, R, P);
+    switch (g_adj_variant) {
+        case 42: k_legendre_adjoint<4, 2><<<grid, 32, 0, s>>>(P, gt, p->d_aeo); break;
+        case 82: k_legendre_adjoint<8, 2><<<grid, 32, 0, s>>>(P, gt, p->d_aeo); break;
+        case 84: k_legendre_adjoint<8, 4><<<grid, 32, 0, s>>>(P, gt, p->d_aeo); break;
+        default: k_legendre_adjoint<4, 4><<<grid, 32, 0, s>>>(P, gt, p->d_aeo); break;
+    }
     NUSHT_CUDA_TRY(cudaGetLastError());
     return NUSHT_OK;
 }
@@ -987,7 +1021,9 @@ void legendre_free(nusht_plan_s* p) {
     cudaFree(p->d_aeo); cudaFree(p->d_ft); cudaFree(p->d_x2); cudaFree(p->d_x); cudaFree(p->d_logsin);
     cudaFree(p->d_logkap);
     cudaFree(p->d_ff_n); cudaFree(p->d_ff_p); cudaFree(p->d_ff_e);
+    cudaFree(p->d_ffa_n); cudaFree(p->d_ffa_p); cudaFree(p->d_ffa_e);
     p->d_ff_n = nullptr; p->d_ff_p = nullptr; p->d_ff_e = nullptr;
+    p->d_ffa_n = nullptr; p->d_ffa_p = nullptr; p->d_ffa_e = nullptr;
     p->d_eoff = nullptr; p->d_ab = nullptr; p->d_sig = p->d_sodd = p->d_rho = nullptr; p->d_aeo = nullptr;
     p->d_ft = nullptr; p->d_x2 = p->d_x = nullptr; p->d_logsin = p->d_logkap = nullptr;
 }

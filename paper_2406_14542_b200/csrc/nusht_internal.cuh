@@ -84,6 +84,9 @@ struct nusht_plan_s {
     int* d_ff_n = nullptr;          // fast-forward table: first in-range step per (m, block of ring pairs)
     double2* d_ff_p = nullptr;      //   recurrence state (p0, p1) per pair at that step
     int* d_ff_e = nullptr;          //   exponent counter per pair at that step
+    int* d_ffa_n = nullptr;         // the same for the adjoint's decomposition (more ring pairs per thread)
+    double2* d_ffa_p = nullptr;
+    int* d_ffa_e = nullptr;
     // --- Legendre work buffers ---
     double4* d_aeo = nullptr;       // scaled coefficients per (m,n): (ae.re, ae.im, ao.re, ao.im)
     double2* d_ft = nullptr;        // Ftilde / Gtilde: [mmax+1][nth2] complex128
@@ -97,6 +100,9 @@ struct nusht_plan_s {
     cufftHandle fft_theta_fine = 0;    // C2C (dtype), length nth, batch mmax+1
     cufftHandle fft_phi = 0;           // C2C (dtype), length nph/2, batch nth/2+1, in place on the grid rows
     bool have_fft = false;
+    bool theta_fused = false;       // a3 + a4 + a5-theta (and their transposes) as one kernel per direction (fourier.cu)
+    double2* d_tw2n = nullptr;      // tables of the fused theta chains (twiddles, position-ordered deconvolution factors)
+    int n_sm = 0;                   // SM count of the plan's device (persistent grids)
     // --- points ---
     double* d_px = nullptr;         // sorted theta in fine-grid units
     double* d_py = nullptr;         // sorted phi in fine-grid units
