@@ -161,24 +161,59 @@ __host__ __device__ constexpr int stage_table_len(int n) {
     return off;
 }
 
+// radix of the last forward stage (= first inverse stage) on sub-transforms of length NS0 = N/2; its
+// stride is 1, it has no twiddles, and thread `tid` of T owns butterflies b = tid + T u: positions R b + j.
+__host__ __device__ constexpr int last_radix(int ns0) {
+    int ns = ns0;
+    while (ns > 16) ns /= 16;
+    return ns;   // 16 when ns0 is a power of 16, else 2, 4 or 8
+}
+
+// last forward stage: shared memory -> registers (c[u * R + j] = output j of butterfly tid + T u)
+template <int N, int R, int SIGN, int E>
+FFTSM_HD void last_stage_to_regs(const double2* s, int tid, int T, double2 (&c)[E]) {
+#pragma unroll
+    for (int u = 0; u < E / R; ++u) {
+        const int base = (tid + T * u) * R;
+        double2 x[R];
+#pragma unroll
+        for (int j = 0; j < R; ++j) x[j] = s[pad(base + j)];
+        dft_reg<R, SIGN>(x);
+#pragma unroll
+        for (int j = 0; j < R; ++j) c[u * R + j] = x[bitrev(j, R)];
+    }
+}
+// first inverse stage: registers -> shared memory
+template <int N, int R, int SIGN, int E>
+FFTSM_HD void first_stage_from_regs(double2* s, int tid, int T, const double2 (&c)[E]) {
+#pragma unroll
+    for (int u = 0; u < E / R; ++u) {
+        const int base = (tid + T * u) * R;
+        double2 x[R];
+#pragma unroll
+        for (int j = 0; j < R; ++j) x[j] = c[u * R + j];
+        dft_reg<R, SIGN>(x);
+#pragma unroll
+        for (int j = 0; j < R; ++j) s[pad(base + j)] = x[bitrev(j, R)];
+    }
+}
+
 // Stage drivers.  Exec supplies `template <int R, int NS> void dif()` / `dit()`: run one stage for
 // all threads and synchronise (the device executor of fourier.cu; a sequential loop on the host).
+// The last forward / first inverse stage (sub-transform length last_radix) is NOT run by these: the
+// caller does it between shared memory and registers with the two functions above.
 template <int NS, class Exec>
 FFTSM_HD void forward_stages(Exec& ex) {   // after the fused radix-2 stage: sub-transforms of length NS
-    if constexpr (NS >= 16) {
+    if constexpr (NS > 16) {
         ex.template dif<16, NS>();
         forward_stages<NS / 16>(ex);
-    } else if constexpr (NS > 1) {
-        ex.template dif<NS, NS>();
     }
 }
 template <int NS, class Exec>
 FFTSM_HD void inverse_stages(Exec& ex) {   // mirror image; the fused radix-2 stage follows
-    if constexpr (NS >= 16) {
+    if constexpr (NS > 16) {
         inverse_stages<NS / 16>(ex);
         ex.template dit<16, NS>();
-    } else if constexpr (NS > 1) {
-        ex.template dit<NS, NS>();
     }
 }
 

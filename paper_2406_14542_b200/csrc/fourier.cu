@@ -200,9 +200,14 @@ k_z_to_h(int M, int nh, int nrow_half, int nz, bool write_ext, const double2* __
 //              parities, truncate, deconvolve --> inverse FFT --> Gtilde[m][.].
 // HBM traffic per column: N complex in, ~N complex out (the cuFFT chain it replaces moves 9 N).
 // ---------------------------------------------------------------------------------------------
+#ifndef NUSHT_CHAIN_DIV
+#define NUSHT_CHAIN_DIV 16
+#endif
+constexpr int chain_threads(int n) { return n >= 32 * NUSHT_CHAIN_DIV ? n / NUSHT_CHAIN_DIV : 32; }
+
 template <int N>
 struct ChainCfg {
-    static constexpr int T = N >= 512 ? N / 16 : 32;    // threads per CTA: one radix-16 butterfly per thread and stage
+    static constexpr int T = chain_threads(N);          // threads per CTA: one radix-16 butterfly per thread and stage
     static constexpr int E = N / T;                     // spectrum entries held per thread
     static constexpr size_t SMEM = sizeof(double2) * (size_t)fftsm::padded_len(N);
 };
@@ -245,7 +250,7 @@ __global__ void __launch_bounds__(ChainCfg<N>::T)
 k_theta_chain_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, const double* __restrict__ pph,
                   const ChainTables tb, C* __restrict__ h) {
     using namespace fftsm;
-    constexpr int T = ChainCfg<N>::T, E = ChainCfg<N>::E;
+    constexpr int T = ChainCfg<N>::T, E = ChainCfg<N>::E, RL = last_radix(N / 2);
     extern __shared__ __align__(16) double2 s_col[];
     const int tid = threadIdx.x;
     for (int m = blockIdx.x; m <= M; m += gridDim.x) {
@@ -261,25 +266,25 @@ k_theta_chain_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, c
         __syncthreads();
         DevExec<N, -1> fwd{s_col, tb.stw, tid};
         forward_stages<N / 2>(fwd);
-        // a4: deconvolve and truncate; the spectrum stays in registers (digit-reversed positions tid + T e)
+        // a4: deconvolve and truncate.  The last forward stage leaves the spectrum in registers (entry e of
+        // thread tid sits at digit-reversed position RL (tid + T (e / RL)) + e % RL; tables are laid out [e][tid])
         double2 c[E];
+        last_stage_to_regs<N, RL, -1, E>(s_col, tid, T, c);
         const double fm = pph[m];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const int p = tid + T * e;
-            const double2 v = s_col[pad(p)];
-            const double f = tb.fpos[p] * fm;
-            c[e] = make_double2(v.x * f, v.y * f);
+            const double f = tb.fpos[e * T + tid] * fm;
+            c[e] = make_double2(c[e].x * f, c[e].y * f);
         }
         // a5 (theta): rows a = 2a' + parity, one inverse transform per parity
 #pragma unroll 1
         for (int par = 0; par < 2; ++par) {
             __syncthreads();
+            if (par) {   // the spectrum is not needed again after parity 1: twiddle it in place
 #pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const int p = tid + T * e;
-                s_col[pad(p)] = par ? cmul(c[e], tb.twpar[p]) : c[e];
+                for (int e = 0; e < E; ++e) c[e] = cmul(c[e], tb.twpar[e * T + tid]);
             }
+            first_stage_from_regs<N, RL, +1, E>(s_col, tid, T, c);
             __syncthreads();
             DevExec<N, +1> inv{s_col, tb.stw, tid};
             inverse_stages<N / 2>(inv);
@@ -308,7 +313,7 @@ __global__ void __launch_bounds__(ChainCfg<N>::T)
 k_theta_chain_adj(int L, int M, int nrow_half, const C* __restrict__ h, const double* __restrict__ pph,
                   const ChainTables tb, double2* __restrict__ ft) {
     using namespace fftsm;
-    constexpr int T = ChainCfg<N>::T, E = ChainCfg<N>::E;
+    constexpr int T = ChainCfg<N>::T, E = ChainCfg<N>::E, RL = last_radix(N / 2);
     extern __shared__ __align__(16) double2 s_col[];
     const int tid = threadIdx.x;
     // rows of a parity block that exist: a = 2a' + par < nrow_half
@@ -343,23 +348,23 @@ k_theta_chain_adj(int L, int M, int nrow_half, const C* __restrict__ h, const do
             __syncthreads();
             DevExec<N, -1> fwd{s_col, tb.stw, tid};
             forward_stages<N / 2>(fwd);
+            double2 v[E];
+            last_stage_to_regs<N, RL, -1, E>(s_col, tid, T, v);
 #pragma unroll
             for (int e = 0; e < E; ++e) {
-                const int p = tid + T * e;
-                double2 v = s_col[pad(p)];
-                if (par) v = cmul(v, cconj(tb.twpar[p]));
-                acc[e].x += v.x;
-                acc[e].y += v.y;
+                if (par) v[e] = cmul(v[e], cconj(tb.twpar[e * T + tid]));
+                acc[e].x += v[e].x;
+                acc[e].y += v[e].y;
             }
         }
         __syncthreads();
         const double fm = pph[m];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const int p = tid + T * e;
-            const double f = tb.fpos[p] * fm;
-            s_col[pad(p)] = make_double2(acc[e].x * f, acc[e].y * f);
+            const double f = tb.fpos[e * T + tid] * fm;
+            acc[e] = make_double2(acc[e].x * f, acc[e].y * f);
         }
+        first_stage_from_regs<N, RL, +1, E>(s_col, tid, T, acc);
         __syncthreads();
         DevExec<N, +1> inv{s_col, tb.stw, tid};
         inverse_stages<N / 2>(inv);
@@ -484,11 +489,15 @@ int fourier_build(nusht_plan_s* p) {
         }
         double2* twpar = tb.data() + n / 2 + nst;
         double* fpos = reinterpret_cast<double*>(twpar + n);
-        for (int q = 0; q < n; ++q) {
-            const int f = chain_freq_of_pos(n, q), k = f < n / 2 ? f : f - n;
-            twpar[q] = unit((long double)k / (long double)(2 * n));
-            fpos[q] = (k >= -L && k <= L) ? pth[k + L] : 0.0;
-        }
+        // entry e of thread t <-> position RL (t + T (e / RL)) + e % RL, stored at [e][t] (coalesced)
+        const int T = chain_threads(n), E = n / T, RL = fftsm::last_radix(n / 2);
+        for (int e = 0; e < E; ++e)
+            for (int t = 0; t < T; ++t) {
+                const int pos = RL * (t + T * (e / RL)) + e % RL;
+                const int f = chain_freq_of_pos(n, pos), k = f < n / 2 ? f : f - n;
+                twpar[(size_t)e * T + t] = unit((long double)k / (long double)(2 * n));
+                fpos[(size_t)e * T + t] = (k >= -L && k <= L) ? pth[k + L] : 0.0;
+            }
         NUSHT_TRY(f_alloc(&p->d_tw2n, sizeof(double2) * tb.size(), p));
         NUSHT_CUDA_TRY(cudaMemcpy(p->d_tw2n, tb.data(), sizeof(double2) * tb.size(), cudaMemcpyHostToDevice));
         int dev = 0;
