@@ -15,6 +15,7 @@
 #include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
+#include <string.h>
 
 #include <algorithm>
 #include <vector>
@@ -472,7 +473,10 @@ int fourier_build(nusht_plan_s* p) {
 
     // fused theta chains: coarse length == half fine length, a power of two that fits shared memory
     p->theta_fused = (g.nth / 2 == nth2) && (nth2 & (nth2 - 1)) == 0 && nth2 >= 128 && nth2 <= 8192;
-    if (getenv("NUSHT_NO_FUSED_THETA")) p->theta_fused = false;   // TUNING HOOK (temporary)
+    {   // NUSHT_THETA_CHAIN=cufft keeps the cuFFT chain (tests compare the two; config 4 always uses it)
+        const char* ev = getenv("NUSHT_THETA_CHAIN");
+        if (ev && strcmp(ev, "cufft") == 0) p->theta_fused = false;
+    }
     if (p->theta_fused) {
         // one buffer: tw2 [N/2] | stage tables | twpar [N] | fpos [N doubles]
         const int n = nth2, nst = fftsm::stage_table_len(n);

@@ -22,7 +22,6 @@
 // The CPU oracle (oracle/) uses the plain three-term recurrence in l and shares nothing with this file.
 #include <math.h>
 #include <stdio.h>
-#include <stdlib.h>
 
 #include <vector>
 
@@ -843,7 +842,6 @@ static dim3 leg_grid(const nusht_plan_s* p, int R, LegParams& P) {
     return dim3(nblk + (rem ? 1 : 0), p->mmax + 1);
 }
 
-static int g_adj_variant = 44;   // TUNING HOOK (temporary)
 static LegParams make_params(const nusht_plan_s* p, bool adjoint_tables = false) {
     LegParams P;
     P.nblk = 0;
@@ -860,7 +858,7 @@ static LegParams make_params(const nusht_plan_s* p, bool adjoint_tables = false)
     P.x = p->d_x;
     P.logsin = p->d_logsin;
     P.logkap = p->d_logkap;
-    const bool a = adjoint_tables && g_adj_variant / 10 == 8;
+    const bool a = adjoint_tables && ADJ_R != LEG_R;
     P.ff_n = a ? p->d_ffa_n : p->d_ff_n;
     P.ff_p = a ? p->d_ffa_p : p->d_ff_p;
     P.ff_e = a ? p->d_ffa_e : p->d_ff_e;
@@ -950,18 +948,14 @@ int legendre_build_tables(nusht_plan_s* p) {
         NUSHT_CUDA_TRY(cudaGetLastError());
         (void)grid;
     }
-    {
-        const char* ev = getenv("NUSHT_ADJ_VARIANT");
-        g_adj_variant = ev ? atoi(ev) : 44;
-    }
-    if (g_adj_variant / 10 == 8) {
+    if (ADJ_R != LEG_R) {
         LegParams P = make_params(p);
-        leg_grid(p, 8, P);
+        leg_grid(p, ADJ_R, P);
         const size_t nw = (size_t)(M + 1) * (size_t)P.nblk;
         NUSHT_TRY(dev_alloc(&p->d_ffa_n, nw, p));
-        NUSHT_TRY(dev_alloc(&p->d_ffa_p, nw * 8 * 32, p));
-        NUSHT_TRY(dev_alloc(&p->d_ffa_e, nw * 8 * 32, p));
-        k_legendre_fastforward<8><<<dim3(P.nblk, M + 1), 32>>>(P, p->d_ffa_n, p->d_ffa_p, p->d_ffa_e);
+        NUSHT_TRY(dev_alloc(&p->d_ffa_p, nw * ADJ_R * 32, p));
+        NUSHT_TRY(dev_alloc(&p->d_ffa_e, nw * ADJ_R * 32, p));
+        k_legendre_fastforward<ADJ_R><<<dim3(P.nblk, M + 1), 32>>>(P, p->d_ffa_n, p->d_ffa_p, p->d_ffa_e);
         NUSHT_CUDA_TRY(cudaGetLastError());
     }
     NUSHT_CUDA_TRY(cudaDeviceSynchronize());
@@ -992,14 +986,8 @@ int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
     // the kernel accumulates with global reductions
     NUSHT_CUDA_TRY(cudaMemsetAsync(p->d_aeo, 0, sizeof(double4) * (size_t)p->n_e_total, s));
     LegParams P = make_params(p, true);
-    const int R = g_adj_variant / 10;
-    const dim3 grid = leg_grid(p, R, P);
-    switch (g_adj_variant) {
-        case 42: k_legendre_adjoint<4, 2><<<grid, 32, 0, s>>>(P, gt, p->d_aeo); break;
-        case 82: k_legendre_adjoint<8, 2><<<grid, 32, 0, s>>>(P, gt, p->d_aeo); break;
-        case 84: k_legendre_adjoint<8, 4><<<grid, 32, 0, s>>>(P, gt, p->d_aeo); break;
-        default: k_legendre_adjoint<4, 4><<<grid, 32, 0, s>>>(P, gt, p->d_aeo); break;
-    }
+    const dim3 grid = leg_grid(p, ADJ_R, P);
+    k_legendre_adjoint<ADJ_R, ADJ_CHUNK><<<grid, 32, 0, s>>>(P, gt, p->d_aeo);
     NUSHT_CUDA_TRY(cudaGetLastError());
     return NUSHT_OK;
 }

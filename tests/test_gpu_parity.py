@@ -307,3 +307,38 @@ def test_sparse_points_large_grid(nusht, oracle, L, npts, eps):
     assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
     assert strong_adjointness(plan, oracle, L, L, alm, f) <= 1e-12
     plan.destroy()
+
+
+# ---- Fourier stage: fused theta chains (own shared-memory FFT) vs the cuFFT chain ----------------
+@pytest.mark.parametrize("dtype,eps,tol", [("f64", 1e-10, 1e-13), ("f32", 1e-5, 2e-6)])
+@pytest.mark.parametrize("L,M", [(63, 63), (127, 100), (255, 255), (511, 300), (1023, 1023)])
+def test_fused_theta_chain_matches_cufft_chain(nusht, oracle, monkeypatch, dtype, eps, tol, L, M):
+    """Ntheta = 2 (L + 1) is a power of two here, so the default plan runs k_theta_chain_syn/adj;
+    NUSHT_THETA_CHAIN=cufft keeps the cuFFT chain (the path of non-power-of-two sizes and of config 4).
+    Both must agree to rounding, in both directions, and the fused pair must stay adjoint to 1e-12."""
+    npts = 20000
+    theta, phi = inputs.uniform_sphere_points(npts, 77)
+    alm = inputs.random_alm(L, M, 77)
+    x = inputs.random_map(npts, 77)
+    rd, cd = (np.float32, np.complex64) if dtype == "f32" else (np.float64, np.complex128)
+    res = {}
+    for mode in ("fused", "cufft"):
+        if mode == "cufft":
+            monkeypatch.setenv("NUSHT_THETA_CHAIN", "cufft")
+        else:
+            monkeypatch.delenv("NUSHT_THETA_CHAIN", raising=False)
+        plan = nusht.Plan(L, M, cu(theta), cu(phi), eps, dtype)
+        f = plan.synthesis(cu(alm.astype(cd))).cpu().numpy().astype(np.float64)
+        c = plan.adjoint(cu(x.astype(rd))).cpu().numpy().astype(np.complex128)
+        res[mode] = (f, c)
+        if mode == "fused" and dtype == "f64":
+            lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+            rhs = oracle.inner_alm(L, M, alm, c)
+            assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+        plan.destroy()
+    assert rel(res["fused"][0], res["cufft"][0]) <= tol
+    assert rel(res["fused"][1], res["cufft"][1]) <= tol
+    if L <= 255:
+        sub = slice(0, 2000)
+        f_ref = oracle.synthesis(L, M, theta[sub], phi[sub], alm, "ld")
+        assert rel(res["fused"][0][sub], f_ref) <= (10 * eps if dtype == "f64" else 1e-4)
