@@ -41,8 +41,8 @@ constexpr int SYN_TN = 64;
 // adjoint: one warp per CTA as well; more ring pairs per thread halve the cost of the cross-lane reduction
 constexpr int ADJ_R = 4;
 constexpr int ADJ_TN = 64;
-constexpr int ADJ_CHUNK = 4;       // n-steps per transposing reduction / exponent check
-__host__ __device__ constexpr int adj_min_ctas(int r, int c) { return r <= 4 ? (c <= 2 ? 22 : 18) : (c <= 2 ? 12 : 10); }
+constexpr int ADJ_CHUNK = 8;       // n-steps per transposing reduction / exponent check
+__host__ __device__ constexpr int adj_min_ctas(int r, int c) { return r <= 4 ? (c <= 2 ? 22 : (c <= 4 ? 18 : 16)) : (c <= 2 ? 12 : 10); }
 constexpr double SCALE_UP_LIMIT = 1.157920892373162e+77;   // 2^256
 constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
 
