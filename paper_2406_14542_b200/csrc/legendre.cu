@@ -679,7 +679,7 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
     }
     __shared__ __align__(16) double2 s_ab[2][ADJ_TN];
     constexpr int NV = 4 * C;             // values reduced across the warp per chunk of C steps
-    __shared__ __align__(16) double s_tr[NV][33];
+    __shared__ __align__(16) double s_tr[NV][34];   // row stride 272 B: 16-byte aligned rows, conflict-free LDS.128
     __shared__ __align__(8) uint64_t s_bar[2];
 
     const int m = blockIdx.y;
@@ -780,14 +780,17 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
 #pragma unroll
                 for (int q = 0; q < NV; ++q) s_tr[q][lane] = v[q];
                 __syncwarp();
-                const double* src = &s_tr[lane % NV][NV * (lane / NV)];
-                double tot = 0.0, tot2 = 0.0;
+                const double2* src = reinterpret_cast<const double2*>(&s_tr[lane % NV][NV * (lane / NV)]);
+                double ta = 0.0, tb2 = 0.0, tc = 0.0, td = 0.0;      // four short add chains
 #pragma unroll
-                for (int k = 0; k < NV; k += 2) {
-                    tot += src[k];
-                    tot2 += src[k + 1];
+                for (int k = 0; k < NV / 2; k += 2) {
+                    const double2 u = src[k], w = src[k + 1];
+                    ta += u.x;
+                    tb2 += u.y;
+                    tc += w.x;
+                    td += w.y;
                 }
-                tot += tot2;
+                double tot = (ta + tb2) + (tc + td);
 #pragma unroll
                 for (int sh = NV; sh < 32; sh *= 2) tot += shfl_xor_d(tot, sh);
                 __syncwarp();
