@@ -514,6 +514,7 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
         ere[r] = eim[r] = ore_[r] = oim[r] = 0.0;
     }
     const bool warp_has_work = jb < P.npairs;
+    bool steady = false;                      // every pair of the warp in range: no more exponent bookkeeping
 
     for (int tile = tile0; tile < ntiles && n_start < ne; ++tile) {
         const int st = (tile - tile0) & 1;
@@ -522,14 +523,18 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
         if (warp_has_work) {
             for (int i0 = (tile == tile0) ? n_start - tile0 * SYN_TN : 0; i0 < cnt; i0 += LEG_CHUNK) {
                 const int ns = min(LEG_CHUNK, cnt - i0);
-                bool any_dead = false, any_live = false;
+                bool w_dead = false, w_live = true;
+                if (!steady) {                   // warp-uniform; exponents only ever count down to 0
+                    bool any_dead = false, any_live = false;
 #pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    any_dead |= (ex[r] > 0);
-                    any_live |= (valid[r] && ex[r] == 0);
+                    for (int r = 0; r < R; ++r) {
+                        any_dead |= (ex[r] > 0);
+                        any_live |= (valid[r] && ex[r] == 0);
+                    }
+                    w_dead = __any_sync(0xffffffffu, any_dead);
+                    w_live = __any_sync(0xffffffffu, any_live);
+                    steady = !w_dead;
                 }
-                const bool w_dead = __any_sync(0xffffffffu, any_dead);
-                const bool w_live = __any_sync(0xffffffffu, any_live);
                 if (!w_dead) {
                     // all pairs live: 6 FMA per pair per step, no checks
                     if (ns == LEG_CHUNK) {
