@@ -535,8 +535,10 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
                     w_live = __any_sync(0xffffffffu, any_live);
                     steady = !w_dead;
                 }
-                if (!w_dead) {
-                    // all pairs live: 6 FMA per pair per step, no checks
+                if (w_live) {
+                    // some pair in range: 6 FMA per pair and step, no masks.  A pair still below range
+                    // accumulates finite garbage (|p1| <= 2^256 scaled); its sums are cleared when it comes
+                    // into range (below) or at the end, which drops exactly the terms < 2^-232 it stands for.
                     if (ns == LEG_CHUNK) {
 #pragma unroll
                         for (int i = 0; i < LEG_CHUNK; ++i) {
@@ -572,44 +574,29 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
                         }
                     }
                 } else {
-                    if (w_live) {
-                        // mixed: pairs that were live at the start of the chunk accumulate
-                        for (int i = 0; i < ns; ++i) {
-                            const double2 ab = s_ab[st][i0 + i];
-                            const double4 c = s_aeo[st][i0 + i];
+                    // every pair of the warp still below range: recurrence only (2 FMA)
+                    for (int i = 0; i < ns; ++i) {
+                        const double2 ab = s_ab[st][i0 + i];
 #pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                const double t = fma(ab.x, x2[r], ab.y);
-                                const double pm = (ex[r] == 0) ? p1[r] : 0.0;
-                                ere[r] = fma(c.x, pm, ere[r]);
-                                eim[r] = fma(c.y, pm, eim[r]);
-                                ore_[r] = fma(c.z, pm, ore_[r]);
-                                oim[r] = fma(c.w, pm, oim[r]);
-                                const double pn = fma(t, p1[r], p0[r]);
-                                p0[r] = p1[r];
-                                p1[r] = pn;
-                            }
-                        }
-                    } else {
-                        // every pair of the warp still below range: recurrence only (2 FMA)
-                        for (int i = 0; i < ns; ++i) {
-                            const double2 ab = s_ab[st][i0 + i];
-#pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                const double t = fma(ab.x, x2[r], ab.y);
-                                const double pn = fma(t, p1[r], p0[r]);
-                                p0[r] = p1[r];
-                                p1[r] = pn;
-                            }
+                        for (int r = 0; r < R; ++r) {
+                            const double t = fma(ab.x, x2[r], ab.y);
+                            const double pn = fma(t, p1[r], p0[r]);
+                            p0[r] = p1[r];
+                            p1[r] = pn;
                         }
                     }
+                }
+                if (w_dead) {
                     // exponent bookkeeping once per chunk: growth over 8 steps is < 2^32
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
-                        if (ex[r] > 0 && fabs(p1[r]) > SCALE_UP_LIMIT) {
-                            p1[r] *= SCALE_DOWN;
-                            p0[r] *= SCALE_DOWN;
-                            ex[r] -= 1;
+                        if (ex[r] > 0) {
+                            if (fabs(p1[r]) > SCALE_UP_LIMIT) {
+                                p1[r] *= SCALE_DOWN;
+                                p0[r] *= SCALE_DOWN;
+                                ex[r] -= 1;
+                            }
+                            ere[r] = eim[r] = ore_[r] = oim[r] = 0.0;   // nothing counted before the pair is in range
                         }
                     }
                 }
@@ -620,6 +607,9 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
     }
 
     if (!warp_has_work) return;
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+        if (ex[r] > 0) ere[r] = eim[r] = ore_[r] = oim[r] = 0.0;   // never came into range
     // a2: fused DFS doubling
     const double sgn = (m & 1) ? -1.0 : 1.0;
     double2* row = ft + (int64_t)m * P.nth2;
