@@ -17,7 +17,7 @@
 // One thread owns R north/south ring pairs (Pbar_lm(pi-theta) = (-1)^{l+m} Pbar_lm(theta)): per pair
 // and per two l it issues 2 FMA of recurrence and 4 FMA of accumulation.  Underflow of
 // Pbar_mm ~ sin^m(theta) is handled with a per-pair power-of-two exponent counter: while it is
-// positive the pair is "dead" (true value < 2^-232) and contributes nothing.
+// positive the pair is "dead" (true value < 2^-128, LIVE_BITS below) and contributes nothing.
 //
 // The CPU oracle (oracle/) uses the plain three-term recurrence in l and shares nothing with this file.
 #include <math.h>
@@ -43,7 +43,11 @@ constexpr int ADJ_R = 4;
 constexpr int ADJ_TN = 64;
 constexpr int ADJ_CHUNK = 8;       // n-steps per transposing reduction / exponent check
 __host__ __device__ constexpr int adj_min_ctas(int r, int c) { return r <= 4 ? (c <= 2 ? 22 : (c <= 4 ? 18 : 16)) : (c <= 2 ? 12 : 10); }
-constexpr double SCALE_UP_LIMIT = 1.157920892373162e+77;   // 2^256
+// A ring pair is "in range" once |Pbar_lm| >= 2^-LIVE_BITS; below that its terms are dropped (relative to
+// Pbar = O(1) that is 3e-39: no FP64 result can resolve it).  With the counter at 1 the stored value is the
+// true one times 2^512, so the pair comes into range when it passes 2^(512 - LIVE_BITS).
+constexpr int LIVE_BITS = 128;
+constexpr double SCALE_UP_LIMIT = 3.940200619639448e+115;   // 2^(512 - LIVE_BITS) = 2^384
 constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
 
 struct LegParams {
@@ -271,7 +275,7 @@ __device__ __forceinline__ void seed_pair(const LegParams& P, int m, int j, bool
     const double err2 = (mh - (s - bb)) + (lk.x - bb);
     const double low = err + err2 + fma(dm, ls.y, lk.y);
     int ee = 0;
-    if (s < -800.0) ee = (int)floor((-s + 256.0) * (1.0 / 512.0));
+    if (s < -(double)LIVE_BITS) ee = (int)floor((-s - (double)LIVE_BITS) * (1.0 / 512.0)) + 1;
     const double expo = s + 512.0 * (double)ee;      // exact: s has < 2^16 magnitude
     const double ip = rint(expo);
     const double fr = (expo - ip) + low;
@@ -537,8 +541,8 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
                 }
                 if (w_live) {
                     // some pair in range: 6 FMA per pair and step, no masks.  A pair still below range
-                    // accumulates finite garbage (|p1| <= 2^256 scaled); its sums are cleared when it comes
-                    // into range (below) or at the end, which drops exactly the terms < 2^-232 it stands for.
+                    // accumulates finite garbage (scaled |p1| stays below 2^416); its sums are cleared when it
+                    // comes into range (below) or at the end, which drops exactly the terms < 2^-LIVE_BITS.
                     if (ns == LEG_CHUNK) {
 #pragma unroll
                         for (int i = 0; i < LEG_CHUNK; ++i) {
