@@ -734,24 +734,22 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
     const int r_limit = g.nth / 2 + 1 + S;   // no point touches a row >= r_limit (< 2 n_theta: grid_row is enough)
     auto stage_rows = [&](int r0, int r1) {
         r1 = min(r1, r_limit);
+        int slot = (r0 + 48) % RB;
 #pragma unroll 1
         for (int r = r0; r < r1; ++r) {
-            bool mirror;
-            const int64_t ro = grid_row(g, r, mirror);
-            if (lane < NC) cp_async_8(&ring.rows[(r + 48) % RB][lane], grid + ro + (mirror ? cols_m : cols_n));
+            const double* src;
+            if ((unsigned)r <= (unsigned)(g.nth / 2)) {          // a stored row (all but the rows next to a pole)
+                src = grid + ((int64_t)r * g.nph + cols_n);
+            } else {
+                bool mirror;
+                const int64_t ro = grid_row(g, r, mirror);
+                src = grid + ro + (mirror ? cols_m : cols_n);
+            }
+            if (lane < NC) cp_async_8(&ring.rows[slot][lane], src);
+            slot = (slot + 1 == RB) ? 0 : slot + 1;
         }
     };
-    // static register indices + predicates only (a run-time index would put the window in local memory)
-    auto commit_group = [&](int q, bool in, const double (&v)[NT]) {
-        const int ks = q % KS;        // warp-uniform: a branch per k-step, selects only inside it
-#pragma unroll
-        for (int ksi = 0; ksi < KS; ++ksi)
-            if (ks == ksi) {
-#pragma unroll
-                for (int nt = 0; nt < NT; ++nt) win[ksi][nt] = in ? v[nt] : win[ksi][nt];
-            }
-    };
-
+    int w_tq = 0, w_ks = 0, w_slot = 0;   // window bookkeeping of row loaded_hi: (r & 3, (r >> 2) % KS, ring slot)
     if (start + lane < end) {
         cp_async_8(&ring.sx[lane], P.px + start + lane);
         cp_async_8(&ring.sy[lane], P.py + start + lane);
@@ -772,6 +770,7 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             cp_async_4(&ring.sperm[lane], P.perm + idx + 32);
         }
         const int a0 = mma_publish<W, S>(ws, kp, lane, X, Y, has ? 1.0 : 0.0, c0);
+        const int sp_own = (a0 + OFF) % S;      // window slot of the point's first row
         __syncwarp();
         const int npt = min(32, end - batch);
         int j0 = 0;
@@ -796,15 +795,32 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
                     __syncwarp();
                     landed_hi = staged_hi;
                 }
-                const int rb = max(loaded_hi, row0) + OFF, re = need_hi + OFF;
-                for (int q = rb >> 2; q <= (re - 1) >> 2; ++q) {
-                    const int rr = 4 * q + t;
-                    const bool in = rr >= rb && rr < re;
-                    double v[NT];
-                    const double* src = &ring.rows[(rr - OFF + 48) % RB][NT * gq];
+                // one row at a time: row r goes to slot 4 ks + (r & 3) of the circular register window, i.e. to the
+                // lanes with t == (r & 3); static register indices + predicates only (a run-time index would put the
+                // window in local memory)
+                int r = max(loaded_hi, row0);
+                if (r != loaded_hi) {               // jump: recompute the bookkeeping (OFF keeps the operands positive)
+                    w_tq = (r + OFF) & 3;
+                    w_ks = ((r + OFF) >> 2) % KS;
+                    w_slot = (r + 48) % RB;
+                }
+#pragma unroll 1
+                for (; r < need_hi; ++r) {
+                    const double* src = &ring.rows[w_slot][NT * gq];
+                    const bool mine = t == w_tq;
 #pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) v[nt] = src[nt];
-                    commit_group(q, in, v);
+                    for (int ksi = 0; ksi < KS; ++ksi)
+                        if (w_ks == ksi) {          // warp-uniform
+                            if (mine) {
+#pragma unroll
+                                for (int nt = 0; nt < NT; ++nt) win[ksi][nt] = src[nt];
+                            }
+                        }
+                    if (++w_tq == 4) {
+                        w_tq = 0;
+                        if (++w_ks == KS) w_ks = 0;
+                    }
+                    if (++w_slot == RB) w_slot = 0;
                 }
                 loaded_hi = need_hi;
                 __syncwarp();                       // ring rows below loaded_hi may now be overwritten
@@ -816,8 +832,7 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             }
             // ---- A fragments: theta weights of point j0 + g in circular slot order ----
             const int jp = min(j0 + gq, 31);
-            const int a0p = __shfl_sync(0xffffffffu, a0, jp);
-            const int sp = (a0p + OFF) % S;
+            const int sp = __shfl_sync(0xffffffffu, sp_own, jp);
             const bool live = gq < cnt;
             const double* thp = &ws.th[live ? jp : 32][0];      // row 32 is all zero
             double d[NT][2];
