@@ -22,6 +22,7 @@
 #include <math.h>
 #include <stdio.h>
 
+#include <type_traits>
 #include <vector>
 
 #include "nusht_internal.cuh"
@@ -931,7 +932,31 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
         }
     };
     constexpr int FG = SPAN >= 4 ? 4 : (SPAN >= 2 ? 2 : 1);   // rows flushed together
-
+    // The window base a_lo is kept a multiple of FG, so the FG rows of a regular flush sit in ONE group of 8
+    // slots: the m-tile is warp-uniform and only its 2 NT accumulators are touched.
+    auto flush_aligned = [&](int r0) {
+        const int s0 = (r0 + OFF) % S;    // multiple of FG
+        const int i = (gq - s0) & 7;
+        const bool rowhit = i < FG;
+        bool mirror;
+        const int64_t ro = grid_row(g, r0 + i, mirror);
+        auto body = [&](auto mtc) {       // compile-time m-tile: static register indices only
+            constexpr int mt = decltype(mtc)::value;
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const double v = acc[mt][nt][e];
+                    const int q = NT * e + nt;
+                    if (rowhit && v != 0.0) atomicAdd(&grid[ro + (mirror ? colc_m[q] : colc_n[q])], v);
+                    acc[mt][nt][e] = rowhit ? 0.0 : v;
+                }
+        };
+        const int mtu = s0 >> 3;          // warp-uniform
+        if (MT == 1 || mtu == 0) body(std::integral_constant<int, 0>{});
+        else if (MT == 2 || mtu == 1) body(std::integral_constant<int, MT >= 2 ? 1 : 0>{});
+        else body(std::integral_constant<int, MT >= 3 ? 2 : 0>{});
+    };
     double Xn = 0.0, Yn = 0.0, vn = 0.0;
     if (start + lane < end) {
         Xn = P.px[start + lane];
@@ -956,15 +981,15 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             // ---- tile: up to 8 consecutive points whose origins lie within SPAN rows of the window base ----
             const int row0 = __shfl_sync(0xffffffffu, a0, j0);
             // ---- rows below row0 are complete: flush them FG at a time (slots hold [a_lo, a_lo + S)) ----
-            if (a_lo == INT_MIN) a_lo = row0;
+            if (a_lo == INT_MIN) a_lo = row0 & ~(FG - 1);
             if (row0 - a_lo >= S) {
 #pragma unroll 1
                 for (int k = 0; k < S; k += 8) flush_group(a_lo + k, 8);
-                a_lo = row0;
+                a_lo = row0 & ~(FG - 1);
             }
 #pragma unroll 1
             while (row0 - a_lo >= FG) {
-                flush_group(a_lo, FG);
+                flush_aligned(a_lo);
                 a_lo += FG;
             }
             const unsigned fit = __ballot_sync(0xffffffffu, has && lane >= j0 && a0 - a_lo <= SPAN);
