@@ -683,8 +683,6 @@ constexpr int NU_RING_CHUNK = 8;   // rows staged per top-up
 template <int NT, int RB>
 struct StripRing {
     double rows[RB][8 * NT];             // row r of the strip lives in rows[(r + 48) % RB]
-    double sx[32], sy[32];               // coordinates of the next batch of points
-    int sperm[32];
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -751,24 +749,24 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
         }
     };
     int w_tq = 0, w_ks = 0, w_slot = 0;   // window bookkeeping of row loaded_hi: (r & 3, (r >> 2) % KS, ring slot)
+    // coordinates of the next batch travel in registers (plain loads issued one batch ahead), so that the only
+    // cp.async traffic is the row staging and no wait is needed at the top of a batch
+    double Xn = 0.0, Yn = 0.0;
+    int dn = 0;
     if (start + lane < end) {
-        cp_async_8(&ring.sx[lane], P.px + start + lane);
-        cp_async_8(&ring.sy[lane], P.py + start + lane);
-        cp_async_4(&ring.sperm[lane], P.perm + start + lane);
+        Xn = P.px[start + lane];
+        Yn = P.py[start + lane];
+        dn = P.perm[start + lane];
     }
     for (int batch = start; batch < end; batch += 32) {
         const int idx = batch + lane;
         const bool has = idx < end;
-        cp_async_wait_all();
-        __syncwarp();
-        landed_hi = staged_hi;
-        const double X = has ? ring.sx[lane] : 0.0, Y = has ? ring.sy[lane] : 0.0;
-        const int dst = has ? ring.sperm[lane] : 0;
-        __syncwarp();
+        const double X = has ? Xn : 0.0, Y = has ? Yn : 0.0;
+        const int dst = has ? dn : 0;
         if (idx + 32 < end) {
-            cp_async_8(&ring.sx[lane], P.px + idx + 32);
-            cp_async_8(&ring.sy[lane], P.py + idx + 32);
-            cp_async_4(&ring.sperm[lane], P.perm + idx + 32);
+            Xn = P.px[idx + 32];
+            Yn = P.py[idx + 32];
+            dn = P.perm[idx + 32];
         }
         const int a0 = mma_publish<W, S>(ws, kp, lane, X, Y, has ? 1.0 : 0.0, c0);
         const int sp_own = (a0 + OFF) % S;      // window slot of the point's first row
