@@ -20,6 +20,8 @@
 #include <algorithm>
 #include <vector>
 
+#include <cooperative_groups.h>
+
 #include "fft_smem.cuh"
 #include "nusht_internal.cuh"
 
@@ -378,6 +380,187 @@ k_theta_chain_adj(int L, int M, int nrow_half, const C* __restrict__ h, const do
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Cluster-pair variant of the fused chains.  After the radix-2 stage that is fused with the load, the even- and
+// the odd-frequency half of a column are independent transforms of length H = N/2 all the way to the last
+// (radix-2) stage of the inverse transform.  Two CTAs of a thread-block cluster take one half each (68 KB of
+// shared memory at N = 8192: two or three independent CTAs per SM whose load / stage / store phases overlap,
+// where the single-CTA kernel holds an SM alone; and a 16384-point FP64 column, which no single SM can hold,
+// fits as two halves), and combine the halves in that last stage through distributed shared memory.
+// ---------------------------------------------------------------------------------------------
+constexpr int half_threads(int h) { return h >= 512 ? h / 16 : 32; }
+
+template <int N>
+struct HalfCfg {
+    static constexpr int H = N / 2;
+    static constexpr int T = half_threads(H);
+    static constexpr int E = H / T;
+    static constexpr size_t SMEM = sizeof(double2) * (size_t)fftsm::padded_len(H);
+    static constexpr int CTAS = 512 / T > 8 ? 8 : 512 / T;   // CTAs per SM at 128 registers per thread
+};
+
+template <int N, int SIGN>
+struct HalfExec {   // stages on ONE half (array length N/2); stage tables are those of the full length N
+    double2* s;
+    const double2* stw;
+    int tid;
+    template <int R, int NS>
+    __device__ __forceinline__ void dif() {
+        fftsm::stage_dif<N / 2, R, NS, SIGN>(s, tid, HalfCfg<N>::T, stw + fftsm::stage_table_offset(N, NS));
+        __syncthreads();
+    }
+    template <int R, int NS>
+    __device__ __forceinline__ void dit() {
+        fftsm::stage_dit<N / 2, R, NS, SIGN>(s, tid, HalfCfg<N>::T, stw + fftsm::stage_table_offset(N, NS));
+        __syncthreads();
+    }
+};
+
+template <int N, typename C>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(HalfCfg<N>::T, HalfCfg<N>::CTAS)
+k_theta_chain2_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, const double* __restrict__ pph,
+                   const ChainTables tb, C* __restrict__ h) {
+    using namespace fftsm;
+    namespace cg = cooperative_groups;
+    constexpr int H = HalfCfg<N>::H, T = HalfCfg<N>::T, E = HalfCfg<N>::E, RL = last_radix(H);
+    extern __shared__ __align__(16) double2 s_col[];
+    cg::cluster_group cluster = cg::this_cluster();
+    const int d0 = (int)cluster.block_rank();          // 0: even frequencies, 1: odd frequencies
+    const double2* s_even = d0 == 0 ? s_col : cluster.map_shared_rank(s_col, 0);
+    const double2* s_odd = d0 == 1 ? s_col : cluster.map_shared_rank(s_col, 1);
+    const int tid = threadIdx.x;
+    const int ncl = gridDim.x / 2;
+    const double* fpos = tb.fpos + d0 * H;
+    const double2* twpar = tb.twpar + d0 * H;
+    for (int m = blockIdx.x / 2; m <= M; m += ncl) {
+        const double2* col = ft + (int64_t)m * N;
+        if (m + ncl <= M) prefetch_l2(col + (int64_t)ncl * N + d0 * H, H * (int)sizeof(double2), tid, T);
+        // a3: this CTA's half of the radix-2 stage, fused with the load
+        for (int i = tid; i < H; i += T) {
+            const double2 a = col[i], b = col[i + H];
+            s_col[pad(i)] = d0 ? cmul(make_double2(a.x - b.x, a.y - b.y), tb.tw2[i]) : make_double2(a.x + b.x, a.y + b.y);
+        }
+        __syncthreads();
+        HalfExec<N, -1> fwd{s_col, tb.stw, tid};
+        forward_stages<H>(fwd);
+        double2 c[E];
+        last_stage_to_regs<H, RL, -1, E>(s_col, tid, T, c);
+        const double fm = pph[m];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double f = fpos[e * T + tid] * fm;
+            c[e] = make_double2(c[e].x * f, c[e].y * f);
+        }
+#pragma unroll 1
+        for (int par = 0; par < 2; ++par) {
+            if (par) {
+#pragma unroll
+                for (int e = 0; e < E; ++e) c[e] = cmul(c[e], twpar[e * T + tid]);
+            }
+            // (own reads of s_col by last_stage_to_regs / the previous combine are ordered by the cluster.sync below
+            //  and by program order: a thread overwrites exactly the positions it read in the last forward stage)
+            first_stage_from_regs<H, RL, +1, E>(s_col, tid, T, c);
+            __syncthreads();
+            HalfExec<N, +1> inv{s_col, tb.stw, tid};
+            inverse_stages<H>(inv);
+            cluster.sync();                            // both halves complete
+            // last inverse stage across the pair; this CTA stores rows i in [d0 H/2, (d0+1) H/2) (and i + H)
+            C* out = h + ((int64_t)m * 2 + par) * N;
+            for (int i = d0 * (H / 2) + tid; i < (d0 + 1) * (H / 2); i += T) {
+                const double2 z0 = s_even[pad(i)], z1 = cmul(s_odd[pad(i)], cconj(tb.tw2[i]));
+                if (2 * i + par < nrow_half) {
+                    C v;
+                    v.x = z0.x + z1.x;
+                    v.y = z0.y + z1.y;
+                    out[i] = v;
+                }
+                if (2 * (i + H) + par < nrow_half) {
+                    C v;
+                    v.x = z0.x - z1.x;
+                    v.y = z0.y - z1.y;
+                    out[i + H] = v;
+                }
+            }
+            cluster.sync();                            // the peer has read this CTA's half
+        }
+    }
+}
+
+template <int N, typename C>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(HalfCfg<N>::T, HalfCfg<N>::CTAS)
+k_theta_chain2_adj(int L, int M, int nrow_half, const C* __restrict__ h, const double* __restrict__ pph,
+                   const ChainTables tb, double2* __restrict__ ft) {
+    using namespace fftsm;
+    namespace cg = cooperative_groups;
+    constexpr int H = HalfCfg<N>::H, T = HalfCfg<N>::T, E = HalfCfg<N>::E, RL = last_radix(H);
+    extern __shared__ __align__(16) double2 s_col[];
+    cg::cluster_group cluster = cg::this_cluster();
+    const int d0 = (int)cluster.block_rank();
+    const double2* s_even = d0 == 0 ? s_col : cluster.map_shared_rank(s_col, 0);
+    const double2* s_odd = d0 == 1 ? s_col : cluster.map_shared_rank(s_col, 1);
+    const int tid = threadIdx.x;
+    const int ncl = gridDim.x / 2;
+    const double* fpos = tb.fpos + d0 * H;
+    const double2* twpar = tb.twpar + d0 * H;
+    const int rows = min(N, (nrow_half + 1) / 2);      // rows of a parity block that exist
+    for (int m = blockIdx.x / 2; m <= M; m += ncl) {
+        if (m + ncl <= M && d0 == 0) {
+            const C* nxt = h + ((int64_t)(m + ncl) * 2) * N;
+            prefetch_l2(nxt, rows * (int)sizeof(C), tid, T);
+            prefetch_l2(nxt + N, rows * (int)sizeof(C), tid, T);
+        }
+        double2 acc[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) acc[e] = make_double2(0.0, 0.0);
+#pragma unroll 1
+        for (int par = 0; par < 2; ++par) {
+            const C* in = h + ((int64_t)m * 2 + par) * N;
+            if (par) __syncthreads();                  // the last forward stage of parity 0 has read s_col
+            for (int i = tid; i < H; i += T) {
+                double2 a = make_double2(0.0, 0.0), b = a;
+                if (2 * i + par < nrow_half) {
+                    const C v = in[i];
+                    a = make_double2((double)v.x, (double)v.y);
+                }
+                if (2 * (i + H) + par < nrow_half) {
+                    const C v = in[i + H];
+                    b = make_double2((double)v.x, (double)v.y);
+                }
+                s_col[pad(i)] = d0 ? cmul(make_double2(a.x - b.x, a.y - b.y), tb.tw2[i]) : make_double2(a.x + b.x, a.y + b.y);
+            }
+            __syncthreads();
+            HalfExec<N, -1> fwd{s_col, tb.stw, tid};
+            forward_stages<H>(fwd);
+            double2 v[E];
+            last_stage_to_regs<H, RL, -1, E>(s_col, tid, T, v);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                if (par) v[e] = cmul(v[e], cconj(twpar[e * T + tid]));
+                acc[e].x += v[e].x;
+                acc[e].y += v[e].y;
+            }
+        }
+        const double fm = pph[m];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const double f = fpos[e * T + tid] * fm;
+            acc[e] = make_double2(acc[e].x * f, acc[e].y * f);
+        }
+        first_stage_from_regs<H, RL, +1, E>(s_col, tid, T, acc);
+        __syncthreads();
+        HalfExec<N, +1> inv{s_col, tb.stw, tid};
+        inverse_stages<H>(inv);
+        cluster.sync();
+        double2* out = ft + (int64_t)m * N;
+        for (int i = d0 * (H / 2) + tid; i < (d0 + 1) * (H / 2); i += T) {
+            const double2 z0 = s_even[pad(i)], z1 = cmul(s_odd[pad(i)], cconj(tb.tw2[i]));
+            out[i] = make_double2(z0.x + z1.x, z0.y + z1.y);
+            out[i + H] = make_double2(z0.x - z1.x, z0.y - z1.y);
+        }
+        cluster.sync();
+    }
+}
+
 // position -> frequency of the forward chain for a run-time N (host; mirrors fftsm::freq_of_pos)
 static int chain_freq_of_pos(int n, int p) {
     int q = p / (n / 2), mul = 2, ns = n / 2;
@@ -415,6 +598,31 @@ int launch_chain(bool adjoint, int L, int M, int nrow_half, int n_sm, double2* f
     return NUSHT_OK;
 }
 
+template <int N, typename C>
+int launch_chain2(bool adjoint, int L, int M, int nrow_half, int n_sm, double2* ft, const double* pph,
+                  const ChainTables& tb, C* h, cudaStream_t s) {
+    static bool attr_set[2] = {false, false};
+    if (!attr_set[adjoint]) {
+        if (adjoint)
+            NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_theta_chain2_adj<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                (int)HalfCfg<N>::SMEM));
+        else
+            NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_theta_chain2_syn<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                (int)HalfCfg<N>::SMEM));
+        attr_set[adjoint] = true;
+    }
+    // persistent pairs: as many CTAs as fit at once (shared memory, 128 registers per thread), columns round robin
+    const size_t by_smem = (size_t)(200 * 1024) / (HalfCfg<N>::SMEM + 1024);
+    const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(HalfCfg<N>::CTAS, by_smem));
+    const int grid = 2 * std::max(1, std::min(M + 1, n_sm * per_sm / 2));
+    if (adjoint)
+        k_theta_chain2_adj<N, C><<<grid, HalfCfg<N>::T, HalfCfg<N>::SMEM, s>>>(L, M, nrow_half, h, pph, tb, ft);
+    else
+        k_theta_chain2_syn<N, C><<<grid, HalfCfg<N>::T, HalfCfg<N>::SMEM, s>>>(L, M, nrow_half, ft, pph, tb, h);
+    NUSHT_CUDA_TRY(cudaGetLastError());
+    return NUSHT_OK;
+}
+
 template <typename C>
 int dispatch_chain(const nusht_plan_s* p, bool adjoint, C* h, cudaStream_t s) {
     const int n = p->lg.nth2;
@@ -423,6 +631,16 @@ int dispatch_chain(const nusht_plan_s* p, bool adjoint, C* h, cudaStream_t s) {
     tb.stw = p->d_tw2n + n / 2;
     tb.twpar = p->d_tw2n + n / 2 + fftsm::stage_table_len(n);
     tb.fpos = reinterpret_cast<const double*>(tb.twpar + n);
+    if (p->theta_chain == 2) {
+        switch (n) {
+#define NUSHT_CHAIN2(NN) \
+    case NN:             \
+        return launch_chain2<NN, C>(adjoint, p->lmax, p->mmax, p->ng.nrow_half, p->n_sm, p->d_ft, p->d_pph, tb, h, s);
+            NUSHT_CHAIN2(2048) NUSHT_CHAIN2(4096) NUSHT_CHAIN2(8192) NUSHT_CHAIN2(16384)
+#undef NUSHT_CHAIN2
+        }
+        return NUSHT_ERR_UNSUPPORTED;
+    }
     switch (n) {
 #define NUSHT_CHAIN(NN) \
     case NN:            \
@@ -471,11 +689,21 @@ int fourier_build(nusht_plan_s* p) {
     NUSHT_CUDA_TRY(cudaMemset(p->d_h, 0, hbytes));
     NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
 
-    // fused theta chains: coarse length == half fine length, a power of two that fits shared memory
-    p->theta_fused = (g.nth / 2 == nth2) && (nth2 & (nth2 - 1)) == 0 && nth2 >= 128 && nth2 <= 8192;
-    {   // NUSHT_THETA_CHAIN=cufft keeps the cuFFT chain (tests compare the two; config 4 always uses it)
+    // fused theta chains: coarse length == half fine length, a power of two.  theta_chain = 1: one CTA per
+    // column (128 <= N <= 8192, the default there: 0.73 / 0.84 ms against 0.76 / 0.87 ms at N = 8192);
+    // 2: a cluster pair per column (2048 <= N <= 16384; the default at 16384, where one SM cannot hold a column)
+    {
+        const bool pow2 = (g.nth / 2 == nth2) && (nth2 & (nth2 - 1)) == 0;
+        p->theta_chain = 0;
+        if (pow2 && nth2 >= 128 && nth2 <= 8192) p->theta_chain = 1;
+        else if (pow2 && nth2 == 16384) p->theta_chain = 2;
+        // NUSHT_THETA_CHAIN = cufft | single | cluster overrides the choice where the variant exists (tests
+        // compare the three)
         const char* ev = getenv("NUSHT_THETA_CHAIN");
-        if (ev && strcmp(ev, "cufft") == 0) p->theta_fused = false;
+        if (ev && strcmp(ev, "cufft") == 0) p->theta_chain = 0;
+        if (ev && strcmp(ev, "single") == 0 && pow2 && nth2 >= 128 && nth2 <= 8192) p->theta_chain = 1;
+        if (ev && strcmp(ev, "cluster") == 0 && pow2 && nth2 >= 2048 && nth2 <= 16384) p->theta_chain = 2;
+        p->theta_fused = p->theta_chain != 0;
     }
     if (p->theta_fused) {
         // one buffer: tw2 [N/2] | stage tables | twpar [N] | fpos [N doubles]
@@ -494,14 +722,19 @@ int fourier_build(nusht_plan_s* p) {
         double2* twpar = tb.data() + n / 2 + nst;
         double* fpos = reinterpret_cast<double*>(twpar + n);
         // entry e of thread t <-> position RL (t + T (e / RL)) + e % RL, stored at [e][t] (coalesced)
-        const int T = chain_threads(n), E = n / T, RL = fftsm::last_radix(n / 2);
-        for (int e = 0; e < E; ++e)
-            for (int t = 0; t < T; ++t) {
-                const int pos = RL * (t + T * (e / RL)) + e % RL;
-                const int f = chain_freq_of_pos(n, pos), k = f < n / 2 ? f : f - n;
-                twpar[(size_t)e * T + t] = unit((long double)k / (long double)(2 * n));
-                fpos[(size_t)e * T + t] = (k >= -L && k <= L) ? pth[k + L] : 0.0;
-            }
+        // (cluster pair: the same per half d0, stored at [d0][e][t])
+        const int nhalf = p->theta_chain == 2 ? 2 : 1, len = n / nhalf;
+        const int T = p->theta_chain == 2 ? half_threads(len) : chain_threads(n), E = len / T;
+        const int RL = fftsm::last_radix(n / 2);
+        for (int d0 = 0; d0 < nhalf; ++d0)
+            for (int e = 0; e < E; ++e)
+                for (int t = 0; t < T; ++t) {
+                    const int pos = d0 * len + RL * (t + T * (e / RL)) + e % RL;
+                    const int f = chain_freq_of_pos(n, pos), k = f < n / 2 ? f : f - n;
+                    const size_t at = (size_t)d0 * len + (size_t)e * T + t;
+                    twpar[at] = unit((long double)k / (long double)(2 * n));
+                    fpos[at] = (k >= -L && k <= L) ? pth[k + L] : 0.0;
+                }
         NUSHT_TRY(f_alloc(&p->d_tw2n, sizeof(double2) * tb.size(), p));
         NUSHT_CUDA_TRY(cudaMemcpy(p->d_tw2n, tb.data(), sizeof(double2) * tb.size(), cudaMemcpyHostToDevice));
         int dev = 0;

@@ -781,10 +781,15 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             const int need_hi = row0 + S;
             // ---- rows [row0, need_hi) must be in the register window; they come from the ring ----
             if (loaded_hi < need_hi) {
-                if (staged_hi < need_hi) {          // first tile of the item, or a jump past the look-ahead
-                    if (row0 > staged_hi) {         // discontinuity: older copies in flight may target the same ring slots
+                if (staged_hi < need_hi) {          // first tile of the item, or the window outran the look-ahead
+                    // Copies still in flight (rows [landed_hi, staged_hi)) must not target a ring slot that is staged
+                    // again now: two asynchronous copies to one address may land in either order.  Row r and row
+                    // r + RB share a slot, so that is the case as soon as the rows staged now reach landed_hi + RB
+                    // (always, after a jump of the window past rows that were staged but never used).
+                    if (landed_hi < staged_hi && need_hi - RB > landed_hi) {
                         cp_async_wait_all();
                         __syncwarp();
+                        landed_hi = staged_hi;
                     }
                     stage_rows(max(staged_hi, row0), need_hi);
                     staged_hi = need_hi;

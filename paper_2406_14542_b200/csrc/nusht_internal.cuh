@@ -100,6 +100,7 @@ struct nusht_plan_s {
     cufftHandle fft_theta_fine = 0;    // C2C (dtype), length nth, batch mmax+1
     cufftHandle fft_phi = 0;           // C2C (dtype), length nph/2, batch nth/2+1, in place on the grid rows
     bool have_fft = false;
+    int theta_chain = 0;            // 0: cuFFT chain, 1: fused chain, one CTA per column, 2: fused chain, cluster pair per column
     bool theta_fused = false;       // a3 + a4 + a5-theta (and their transposes) as one kernel per direction (fourier.cu)
     double2* d_tw2n = nullptr;      // tables of the fused theta chains (twiddles, position-ordered deconvolution factors)
     int n_sm = 0;                   // SM count of the plan's device (persistent grids)
