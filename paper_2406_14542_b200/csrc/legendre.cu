@@ -37,10 +37,10 @@ constexpr int LEG_R = 4;           // ring pairs per thread
 // synthesis: one warp per CTA, so that warps with different live/dead histories never wait for each other
 constexpr int SYN_THREADS = 32;
 constexpr int SYN_WARPS = SYN_THREADS / 32;
-constexpr int SYN_TN = 64;
+constexpr int SYN_TN = 128;
 // adjoint: one warp per CTA as well; more ring pairs per thread halve the cost of the cross-lane reduction
 constexpr int ADJ_R = 4;
-constexpr int ADJ_TN = 64;
+constexpr int ADJ_TN = 128;
 constexpr int ADJ_CHUNK = 8;       // n-steps per transposing reduction / exponent check
 __host__ __device__ constexpr int adj_min_ctas(int r, int c) { return r <= 4 ? (c <= 2 ? 22 : (c <= 4 ? 18 : 16)) : (c <= 2 ? 12 : 10); }
 // A ring pair is "in range" once |Pbar_lm| >= 2^-LIVE_BITS; below that its terms are dropped (relative to
