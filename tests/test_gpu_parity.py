@@ -361,3 +361,17 @@ def test_synthesis_is_bitwise_reproducible(nusht, dtype, eps, L, M, npts):
     for _ in range(60):
         assert torch.equal(plan.synthesis(d_alm), f0)
     plan.destroy()
+
+
+@pytest.mark.parametrize("L,M,npts,eps", [(2047, 1500, 20000, 1e-10), (4095, 4095, 1500000, 1e-10), (255, 255, 50000, 1e-6)])
+def test_adjoint_is_reproducible_to_rounding(nusht, L, M, npts, eps):
+    """The adjoint accumulates with global FP64 reductions, so repeated runs differ in the last bits only: 40 repeats
+    must agree with the first to 1e-13 in norm (a lost or doubled update would be orders of magnitude above that)."""
+    theta, phi = inputs.uniform_sphere_points(npts, 79)
+    d_x = cu(inputs.random_map(npts, 79))
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps)
+    c0 = plan.adjoint(d_x).clone()
+    n0 = float(torch.linalg.vector_norm(c0))
+    for _ in range(40):
+        assert float(torch.linalg.vector_norm(plan.adjoint(d_x) - c0)) <= 1e-13 * n0
+    plan.destroy()
