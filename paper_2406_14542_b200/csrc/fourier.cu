@@ -791,7 +791,6 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     const NufftGeom& g = p->ng;
     const int nth2 = p->lg.nth2;
     const bool f64 = p->dtype == NUSHT_F64;
-    const size_t csz = f64 ? 16 : 8;
     REC(0);
     if (p->theta_fused) {
         REC(1);
@@ -851,7 +850,6 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     const NufftGeom& g = p->ng;
     const int nth2 = p->lg.nth2;
     const bool f64 = p->dtype == NUSHT_F64;
-    const size_t csz = f64 ? 16 : 8;
     REC(0);
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi, s));
     if (f64)

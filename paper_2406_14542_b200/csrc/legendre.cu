@@ -29,9 +29,6 @@
 
 namespace {
 
-constexpr int LEG_THREADS = 128;   // 4 warps
-constexpr int LEG_WARPS = LEG_THREADS / 32;
-constexpr int LEG_TN = 128;        // n-steps (pairs of l) per shared-memory tile
 constexpr int LEG_CHUNK = 8;       // n-steps between exponent checks
 constexpr int LEG_R = 4;           // ring pairs per thread
 // synthesis: one warp per CTA, so that warps with different live/dead histories never wait for each other
@@ -630,37 +627,6 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ double shfl_xor_d(double v, int mask) {
     return __shfl_xor_sync(0xffffffffu, v, mask);
-}
-
-// v[0..31] per lane -> lane l returns sum over lanes of v[l]
-__device__ __forceinline__ double warp_transpose_reduce32(double (&v)[32], int lane) {
-#pragma unroll
-    for (int half = 16; half >= 1; half >>= 1) {
-        const bool up = (lane & half) != 0;
-#pragma unroll
-        for (int i = 0; i < half; ++i) {
-            const double keep = up ? v[i + half] : v[i];
-            const double send = up ? v[i] : v[i + half];
-            v[i] = keep + shfl_xor_d(send, half);
-        }
-    }
-    return v[0];
-}
-
-// v[0..15] per lane -> returns, in lanes 2q and 2q+1, the sum over all lanes of v[q]
-__device__ __forceinline__ double warp_transpose_reduce16(double (&v)[16], int lane) {
-#pragma unroll
-    for (int half = 8; half >= 1; half >>= 1) {
-        const int mask = 2 * half;
-        const bool up = (lane & mask) != 0;
-#pragma unroll
-        for (int i = 0; i < half; ++i) {
-            const double keep = up ? v[i + half] : v[i];
-            const double send = up ? v[i] : v[i + half];
-            v[i] = keep + shfl_xor_d(send, mask);
-        }
-    }
-    return v[0] + shfl_xor_d(v[0], 1);
 }
 
 // One warp per CTA: the warp owns 32 R ring pairs of one m for all n, forms the 4 partial sums of

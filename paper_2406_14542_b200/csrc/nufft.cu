@@ -663,19 +663,7 @@ __device__ __forceinline__ void cp_async_8(void* dst_smem, const void* src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
                  : "memory");
 }
-__device__ __forceinline__ void cp_async_4(void* dst_smem, const void* src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
-                 : "memory");
-}
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
-// as grid_row, for any row (look-ahead staging may run past the last row a point can touch)
-__device__ __forceinline__ int64_t grid_row_any(const NufftGeom& g, int a, bool& mirror) {
-    int am = a % g.nth;
-    if (am < 0) am += g.nth;
-    mirror = am > g.nth / 2;
-    return (int64_t)(mirror ? g.nth - am : am) * g.nph;
-}
 
 constexpr int NU_RING_ROWS = 16;   // rows of the strip staged ahead of the register window
 constexpr int NU_RING_CHUNK = 8;   // rows staged per top-up
