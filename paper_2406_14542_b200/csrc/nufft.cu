@@ -627,7 +627,7 @@ struct MmaScratch {
 };
 
 // lane `lane` evaluates the weights of its own point and publishes them; returns a0 of the point
-template <int W, int S>
+template <int W, int S, bool SCALE>
 __device__ __forceinline__ int mma_publish(MmaScratch<W, S>& ws, const KernelPoly<double>& kp, int lane, double X,
                                            double Y, double val, int c0) {
     const double a0d = ceil(X - 0.5 * W), b0d = ceil(Y - 0.5 * W);
@@ -638,8 +638,8 @@ __device__ __forceinline__ int mma_publish(MmaScratch<W, S>& ws, const KernelPol
 #pragma unroll
     for (int i = 0; i < S; i += 2) {
         double2 v;
-        v.x = (i < W) ? val * k[i < W ? i : 0] : 0.0;
-        v.y = (i + 1 < W) ? val * k[i + 1 < W ? i + 1 : 0] : 0.0;
+        v.x = (i < W) ? (SCALE ? val * k[i < W ? i : 0] : k[i < W ? i : 0]) : 0.0;
+        v.y = (i + 1 < W) ? (SCALE ? val * k[i + 1 < W ? i + 1 : 0] : k[i + 1 < W ? i + 1 : 0]) : 0.0;
         *reinterpret_cast<double2*>(&ws.th[lane][i]) = v;
     }
     eval_taps<W, double>(kp, up, k);
@@ -756,7 +756,7 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             Yn = P.py[idx + 32];
             dn = P.perm[idx + 32];
         }
-        const int a0 = mma_publish<W, S>(ws, kp, lane, X, Y, has ? 1.0 : 0.0, c0);
+        const int a0 = mma_publish<W, S, false>(ws, kp, lane, X, Y, 1.0, c0);   // absent points: zero weight row (live)
         const int sp_own = (a0 + OFF) % S;      // window slot of the point's first row
         __syncwarp();
         const int npt = min(32, end - batch);
@@ -964,7 +964,7 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
             vn = map[P.perm[idx + 32]];
         }
         // the point's value rides on the theta weights
-        const int a0 = mma_publish<W, S>(ws, kp, lane, X, Y, val, c0);
+        const int a0 = mma_publish<W, S, true>(ws, kp, lane, X, Y, val, c0);
         __syncwarp();
         const int npt = min(32, end - batch);
         int j0 = 0;
