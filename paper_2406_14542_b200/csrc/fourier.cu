@@ -248,6 +248,17 @@ __device__ __forceinline__ void prefetch_l2(const void* ptr, int bytes, int tid,
     }
 }
 
+// Column pairs.  Ftilde_m has the DFS symmetry Ftilde_m[N - r] = (-1)^m Ftilde_m[r], which every step of the chain
+// preserves: c[m,-k] = (-1)^m c[m,k], and the fine rows obey g_m[-a] = (-1)^m g_m[a].  An even
+// column m and its odd neighbour m + 1 therefore go through the chain TOGETHER, as x = p_phi(m) Ftilde_m +
+// p_phi(m+1) Ftilde_{m+1} (one forward and two inverse transforms per PAIR instead of three per column), and are
+// separated at the end by their parity under a -> -a:  y_m = (u[a'] + u[mirror a']) / 2,  y_{m+1} = (u[a'] -
+// u[mirror a']) / 2, with mirror a' = N - a' on the even fine rows and N - 1 - a' on the odd ones.  No division by a
+// small number occurs anywhere (unlike the usual cosine-transform-by-FFT trick).  The adjoint kernel is the exact
+// transpose: it builds the full-length u from the two half-length inputs, and both output columns receive the same
+// transformed sequence (times their p_phi); the component of the neighbour it contains has the opposite symmetry
+// and cancels in the fold Gtilde[k] + (-1)^m Gtilde[N - k] that the adjoint Legendre kernel starts with (a10).
+// The factor 1/2 is folded into the deconvolution table.
 template <int N, typename C>
 __global__ void __launch_bounds__(ChainCfg<N>::T)
 k_theta_chain_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, const double* __restrict__ pph,
@@ -256,13 +267,23 @@ k_theta_chain_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, c
     constexpr int T = ChainCfg<N>::T, E = ChainCfg<N>::E, RL = last_radix(N / 2);
     extern __shared__ __align__(16) double2 s_col[];
     const int tid = threadIdx.x;
-    for (int m = blockIdx.x; m <= M; m += gridDim.x) {
-        const double2* col = ft + (int64_t)m * N;
-        if (m + (int)gridDim.x <= M) prefetch_l2(col + (int64_t)gridDim.x * N, N * (int)sizeof(double2), tid, T);
-        __syncthreads();   // previous column's stores have read s_col
-        // a3: forward transform; its radix-2 stage is fused with the load
+    const int npair = M / 2 + 1;
+    for (int mp = blockIdx.x; mp < npair; mp += gridDim.x) {
+        const int ma = 2 * mp, mb = 2 * mp + 1;
+        const bool has_b = mb <= M;
+        const double2* cola = ft + (int64_t)ma * N;
+        const double2* colb = ft + (int64_t)(has_b ? mb : ma) * N;
+        if (mp + (int)gridDim.x < npair) {
+            const int ncol = (2 * (mp + (int)gridDim.x) + 1 <= M) ? 2 : 1;
+            prefetch_l2(cola + 2 * (int64_t)gridDim.x * N, ncol * N * (int)sizeof(double2), tid, T);
+        }
+        const double pa = pph[ma], pb = has_b ? pph[mb] : 0.0;
+        __syncthreads();   // previous pair's stores have read s_col
+        // a3: forward transform of the pair; its radix-2 stage is fused with the load
         for (int i = tid; i < N / 2; i += T) {
-            const double2 a = col[i], b = col[i + N / 2];
+            const double2 a0 = cola[i], a1 = cola[i + N / 2], b0 = colb[i], b1 = colb[i + N / 2];
+            const double2 a = make_double2(fma(pb, b0.x, pa * a0.x), fma(pb, b0.y, pa * a0.y));
+            const double2 b = make_double2(fma(pb, b1.x, pa * a1.x), fma(pb, b1.y, pa * a1.y));
             s_col[pad(i)] = make_double2(a.x + b.x, a.y + b.y);
             s_col[pad(i + N / 2)] = cmul(make_double2(a.x - b.x, a.y - b.y), tb.tw2[i]);
         }
@@ -273,13 +294,12 @@ k_theta_chain_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, c
         // thread tid sits at digit-reversed position RL (tid + T (e / RL)) + e % RL; tables are laid out [e][tid])
         double2 c[E];
         last_stage_to_regs<N, RL, -1, E>(s_col, tid, T, c);
-        const double fm = pph[m];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const double f = tb.fpos[e * T + tid] * fm;
+            const double f = tb.fpos[e * T + tid];     // p_theta(k) / (2 Ntheta), zero outside |k| <= lmax
             c[e] = make_double2(c[e].x * f, c[e].y * f);
         }
-        // a5 (theta): rows a = 2a' + parity, one inverse transform per parity
+        // a5 (theta): rows a = 2a' + parity, one inverse transform of the pair per parity
 #pragma unroll 1
         for (int par = 0; par < 2; ++par) {
             __syncthreads();
@@ -291,21 +311,25 @@ k_theta_chain_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, c
             __syncthreads();
             DevExec<N, +1> inv{s_col, tb.stw, tid};
             inverse_stages<N / 2>(inv);
-            C* out = h + ((int64_t)m * 2 + par) * N;
-            for (int i = tid; i < N / 2; i += T) {
+            for (int i = tid; i < N / 2; i += T) {     // last inverse stage, in place (a thread owns its two slots)
                 const double2 z0 = s_col[pad(i)], z1 = cmul(s_col[pad(i + N / 2)], cconj(tb.tw2[i]));
-                if (2 * i + par < nrow_half) {
-                    C v;
-                    v.x = z0.x + z1.x;
-                    v.y = z0.y + z1.y;
-                    out[i] = v;
-                }
-                if (2 * (i + N / 2) + par < nrow_half) {
-                    C v;
-                    v.x = z0.x - z1.x;
-                    v.y = z0.y - z1.y;
-                    out[i + N / 2] = v;
-                }
+                s_col[pad(i)] = make_double2(z0.x + z1.x, z0.y + z1.y);
+                s_col[pad(i + N / 2)] = make_double2(z0.x - z1.x, z0.y - z1.y);
+            }
+            __syncthreads();
+            // separate the two columns by their mirror parity; only rows a = 2a' + par < nrow_half are stored
+            C* outa = h + ((int64_t)ma * 2 + par) * N;
+            C* outb = h + ((int64_t)mb * 2 + par) * N;
+            for (int ap = tid; 2 * ap + par < nrow_half && ap < N; ap += T) {
+                const int mir = par ? N - 1 - ap : (ap == 0 ? 0 : N - ap);
+                const double2 u = s_col[pad(ap)], v = s_col[pad(mir)];
+                C va, vb;
+                va.x = u.x + v.x;
+                va.y = u.y + v.y;
+                vb.x = u.x - v.x;
+                vb.y = u.y - v.y;
+                outa[ap] = va;
+                if (has_b) outb[ap] = vb;
             }
         }
     }
@@ -319,31 +343,44 @@ k_theta_chain_adj(int L, int M, int nrow_half, const C* __restrict__ h, const do
     constexpr int T = ChainCfg<N>::T, E = ChainCfg<N>::E, RL = last_radix(N / 2);
     extern __shared__ __align__(16) double2 s_col[];
     const int tid = threadIdx.x;
-    // rows of a parity block that exist: a = 2a' + par < nrow_half
-    for (int m = blockIdx.x; m <= M; m += gridDim.x) {
-        if (m + (int)gridDim.x <= M) {
-            const C* nxt = h + ((int64_t)(m + gridDim.x) * 2) * N;
+    const int npair = M / 2 + 1;
+    auto ld = [](const C* ptr, int idx) {
+        const C v = ptr[idx];
+        return make_double2((double)v.x, (double)v.y);
+    };
+    for (int mp = blockIdx.x; mp < npair; mp += gridDim.x) {
+        const int ma = 2 * mp, mb = 2 * mp + 1;
+        const bool has_b = mb <= M;
+        if (mp + (int)gridDim.x < npair) {
+            const C* nxt = h + ((int64_t)(ma + 2 * gridDim.x) * 2) * N;
             const int rows = min(N, (nrow_half + 1) / 2);
-            prefetch_l2(nxt, rows * (int)sizeof(C), tid, T);
-            prefetch_l2(nxt + N, rows * (int)sizeof(C), tid, T);
+            const int nblk = (ma + 2 * (int)gridDim.x + 1 <= M) ? 4 : 2;
+            for (int q = 0; q < nblk; ++q) prefetch_l2(nxt + (int64_t)q * N, rows * (int)sizeof(C), tid, T);
         }
         double2 acc[E];
 #pragma unroll
         for (int e = 0; e < E; ++e) acc[e] = make_double2(0.0, 0.0);
 #pragma unroll 1
         for (int par = 0; par < 2; ++par) {
-            const C* in = h + ((int64_t)m * 2 + par) * N;
+            const C* ina = h + ((int64_t)ma * 2 + par) * N;
+            const C* inb = h + ((int64_t)(has_b ? mb : ma) * 2 + par) * N;
+            const double sb = has_b ? 1.0 : 0.0;
             __syncthreads();
-            // zero-extension beyond row n_theta/2 (transpose of "keep rows 0 .. n_theta/2"), radix-2 stage fused
+            // transpose of the separation: u[j] = ha[j] + hb[j] (j below the mirror point), ha[mirror j] - hb[mirror j]
+            // above it, 2 ha at the self-mirrored rows 0 and N/2 of parity 0; rows beyond nrow_half do not exist (N is
+            // the half fine length, nrow_half = N + 1).  The radix-2 stage of the forward transform is fused in.
             for (int i = tid; i < N / 2; i += T) {
-                double2 a = make_double2(0.0, 0.0), b = a;
-                if (2 * i + par < nrow_half) {
-                    const C v = in[i];
-                    a = make_double2((double)v.x, (double)v.y);
-                }
-                if (2 * (i + N / 2) + par < nrow_half) {
-                    const C v = in[i + N / 2];
-                    b = make_double2((double)v.x, (double)v.y);
+                double2 a, b;
+                if (par == 0) {
+                    const double2 xa = ld(ina, i), xb = ld(inb, i);
+                    const double2 ya = ld(ina, N / 2 - i), yb = ld(inb, N / 2 - i);
+                    a = i == 0 ? make_double2(2.0 * xa.x, 2.0 * xa.y) : make_double2(fma(sb, xb.x, xa.x), fma(sb, xb.y, xa.y));
+                    b = i == 0 ? make_double2(2.0 * ya.x, 2.0 * ya.y) : make_double2(fma(-sb, yb.x, ya.x), fma(-sb, yb.y, ya.y));
+                } else {
+                    const double2 xa = ld(ina, i), xb = ld(inb, i);
+                    const double2 ya = ld(ina, N / 2 - 1 - i), yb = ld(inb, N / 2 - 1 - i);
+                    a = make_double2(fma(sb, xb.x, xa.x), fma(sb, xb.y, xa.y));
+                    b = make_double2(fma(-sb, yb.x, ya.x), fma(-sb, yb.y, ya.y));
                 }
                 s_col[pad(i)] = make_double2(a.x + b.x, a.y + b.y);
                 s_col[pad(i + N / 2)] = cmul(make_double2(a.x - b.x, a.y - b.y), tb.tw2[i]);
@@ -361,21 +398,27 @@ k_theta_chain_adj(int L, int M, int nrow_half, const C* __restrict__ h, const do
             }
         }
         __syncthreads();
-        const double fm = pph[m];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const double f = tb.fpos[e * T + tid] * fm;
+            const double f = tb.fpos[e * T + tid];
             acc[e] = make_double2(acc[e].x * f, acc[e].y * f);
         }
         first_stage_from_regs<N, RL, +1, E>(s_col, tid, T, acc);
         __syncthreads();
         DevExec<N, +1> inv{s_col, tb.stw, tid};
         inverse_stages<N / 2>(inv);
-        double2* out = ft + (int64_t)m * N;
+        const double pa = pph[ma], pb = has_b ? pph[mb] : 0.0;
+        double2* outa = ft + (int64_t)ma * N;
+        double2* outb = ft + (int64_t)mb * N;
         for (int i = tid; i < N / 2; i += T) {
             const double2 z0 = s_col[pad(i)], z1 = cmul(s_col[pad(i + N / 2)], cconj(tb.tw2[i]));
-            out[i] = make_double2(z0.x + z1.x, z0.y + z1.y);
-            out[i + N / 2] = make_double2(z0.x - z1.x, z0.y - z1.y);
+            const double2 x0 = make_double2(z0.x + z1.x, z0.y + z1.y), x1 = make_double2(z0.x - z1.x, z0.y - z1.y);
+            outa[i] = make_double2(pa * x0.x, pa * x0.y);
+            outa[i + N / 2] = make_double2(pa * x1.x, pa * x1.y);
+            if (has_b) {
+                outb[i] = make_double2(pb * x0.x, pb * x0.y);
+                outb[i + N / 2] = make_double2(pb * x1.x, pb * x1.y);
+            }
         }
     }
 }
@@ -589,7 +632,7 @@ int launch_chain(bool adjoint, int L, int M, int nrow_half, int n_sm, double2* f
     }
     // persistent: as many CTAs as fit at once (shared memory bound), columns dealt round robin
     const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(8, (size_t)(200 * 1024) / (ChainCfg<N>::SMEM + 1024)));
-    const int grid = std::min(M + 1, n_sm * per_sm);
+    const int grid = std::min(M / 2 + 1, n_sm * per_sm);   // one CTA iteration per column pair
     if (adjoint)
         k_theta_chain_adj<N, C><<<grid, ChainCfg<N>::T, ChainCfg<N>::SMEM, s>>>(L, M, nrow_half, h, pph, tb, ft);
     else
@@ -733,7 +776,8 @@ int fourier_build(nusht_plan_s* p) {
                     const int f = chain_freq_of_pos(n, pos), k = f < n / 2 ? f : f - n;
                     const size_t at = (size_t)d0 * len + (size_t)e * T + t;
                     twpar[at] = unit((long double)k / (long double)(2 * n));
-                    fpos[at] = (k >= -L && k <= L) ? pth[k + L] : 0.0;
+                    // (single-CTA variant: column pairs, the 1/2 of their separation is folded in here)
+                    fpos[at] = (k >= -L && k <= L) ? pth[k + L] * (p->theta_chain == 1 ? 0.5 : 1.0) : 0.0;
                 }
         NUSHT_TRY(f_alloc(&p->d_tw2n, sizeof(double2) * tb.size(), p));
         NUSHT_CUDA_TRY(cudaMemcpy(p->d_tw2n, tb.data(), sizeof(double2) * tb.size(), cudaMemcpyHostToDevice));
