@@ -36,10 +36,10 @@ constexpr int SYN_THREADS = 32;
 constexpr int SYN_WARPS = SYN_THREADS / 32;
 constexpr int SYN_TN = 128;
 // adjoint: one warp per CTA as well; more ring pairs per thread halve the cost of the cross-lane reduction
-constexpr int ADJ_R = 4;
+constexpr int ADJ_R = 5;           // adjoint: 5 pairs per thread amortise the cross-lane reduction (still 128 registers, 16 warps/SM)
 constexpr int ADJ_TN = 128;
 constexpr int ADJ_CHUNK = 8;       // n-steps per transposing reduction / exponent check
-__host__ __device__ constexpr int adj_min_ctas(int r, int c) { return r <= 4 ? (c <= 2 ? 22 : (c <= 4 ? 18 : 16)) : (c <= 2 ? 12 : 10); }
+__host__ __device__ constexpr int adj_min_ctas(int r, int c) { return r <= 4 ? (c <= 2 ? 22 : (c <= 4 ? 18 : 16)) : (r == 5 ? 13 : (r == 6 ? 12 : (c <= 2 ? 12 : 10))); }
 // A ring pair is "in range" once |Pbar_lm| >= 2^-LIVE_BITS; below that its terms are dropped (relative to
 // Pbar = O(1) that is 3e-39: no FP64 result can resolve it).  With the counter at 1 the stored value is the
 // true one times 2^512, so the pair comes into range when it passes 2^(512 - LIVE_BITS).
