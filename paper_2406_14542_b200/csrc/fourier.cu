@@ -469,18 +469,28 @@ k_theta_chain2_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, 
     extern __shared__ __align__(16) double2 s_col[];
     cg::cluster_group cluster = cg::this_cluster();
     const int d0 = (int)cluster.block_rank();          // 0: even frequencies, 1: odd frequencies
-    const double2* s_even = d0 == 0 ? s_col : cluster.map_shared_rank(s_col, 0);
-    const double2* s_odd = d0 == 1 ? s_col : cluster.map_shared_rank(s_col, 1);
+    double2* s_even = d0 == 0 ? s_col : cluster.map_shared_rank(s_col, 0);
+    double2* s_odd = d0 == 1 ? s_col : cluster.map_shared_rank(s_col, 1);
     const int tid = threadIdx.x;
     const int ncl = gridDim.x / 2;
     const double* fpos = tb.fpos + d0 * H;
     const double2* twpar = tb.twpar + d0 * H;
-    for (int m = blockIdx.x / 2; m <= M; m += ncl) {
-        const double2* col = ft + (int64_t)m * N;
-        if (m + ncl <= M) prefetch_l2(col + (int64_t)ncl * N + d0 * H, H * (int)sizeof(double2), tid, T);
-        // a3: this CTA's half of the radix-2 stage, fused with the load
+    const int npair = M / 2 + 1;                       // even / odd column pairs, as in k_theta_chain_syn
+    for (int mp = blockIdx.x / 2; mp < npair; mp += ncl) {
+        const int ma = 2 * mp, mb = 2 * mp + 1;
+        const bool has_b = mb <= M;
+        const double2* cola = ft + (int64_t)ma * N;
+        const double2* colb = ft + (int64_t)(has_b ? mb : ma) * N;
+        if (mp + ncl < npair) {
+            const int64_t nxt = (int64_t)(ma + 2 * ncl + ((2 * (mp + ncl) + 1 <= M) ? d0 : 0)) * N;
+            prefetch_l2(ft + nxt, N * (int)sizeof(double2), tid, T);
+        }
+        const double pa = pph[ma], pb = has_b ? pph[mb] : 0.0;
+        // a3: this CTA's half of the radix-2 stage, fused with the load of the pair
         for (int i = tid; i < H; i += T) {
-            const double2 a = col[i], b = col[i + H];
+            const double2 a0 = cola[i], a1 = cola[i + H], b0 = colb[i], b1 = colb[i + H];
+            const double2 a = make_double2(fma(pb, b0.x, pa * a0.x), fma(pb, b0.y, pa * a0.y));
+            const double2 b = make_double2(fma(pb, b1.x, pa * a1.x), fma(pb, b1.y, pa * a1.y));
             s_col[pad(i)] = d0 ? cmul(make_double2(a.x - b.x, a.y - b.y), tb.tw2[i]) : make_double2(a.x + b.x, a.y + b.y);
         }
         __syncthreads();
@@ -488,10 +498,9 @@ k_theta_chain2_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, 
         forward_stages<H>(fwd);
         double2 c[E];
         last_stage_to_regs<H, RL, -1, E>(s_col, tid, T, c);
-        const double fm = pph[m];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const double f = fpos[e * T + tid] * fm;
+            const double f = fpos[e * T + tid];
             c[e] = make_double2(c[e].x * f, c[e].y * f);
         }
 #pragma unroll 1
@@ -500,29 +509,46 @@ k_theta_chain2_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, 
 #pragma unroll
                 for (int e = 0; e < E; ++e) c[e] = cmul(c[e], twpar[e * T + tid]);
             }
-            // (own reads of s_col by last_stage_to_regs / the previous combine are ordered by the cluster.sync below
-            //  and by program order: a thread overwrites exactly the positions it read in the last forward stage)
+            // (a thread overwrites exactly the positions it read in the last forward stage; for parity 1 the
+            //  cluster.sync that ends parity 0 orders it after every read of this buffer)
             first_stage_from_regs<H, RL, +1, E>(s_col, tid, T, c);
             __syncthreads();
             HalfExec<N, +1> inv{s_col, tb.stw, tid};
             inverse_stages<H>(inv);
             cluster.sync();                            // both halves complete
-            // last inverse stage across the pair; this CTA stores rows i in [d0 H/2, (d0+1) H/2) (and i + H)
-            C* out = h + ((int64_t)m * 2 + par) * N;
+            // last inverse stage across the pair, in place: u[i] goes to the even CTA's slot i, u[i + H] to the odd
+            // CTA's slot i; this CTA does i in [d0 H/2, (d0+1) H/2), nobody else touches those slots
             for (int i = d0 * (H / 2) + tid; i < (d0 + 1) * (H / 2); i += T) {
                 const double2 z0 = s_even[pad(i)], z1 = cmul(s_odd[pad(i)], cconj(tb.tw2[i]));
-                if (2 * i + par < nrow_half) {
-                    C v;
-                    v.x = z0.x + z1.x;
-                    v.y = z0.y + z1.y;
-                    out[i] = v;
-                }
-                if (2 * (i + H) + par < nrow_half) {
-                    C v;
-                    v.x = z0.x - z1.x;
-                    v.y = z0.y - z1.y;
-                    out[i + H] = v;
-                }
+                s_even[pad(i)] = make_double2(z0.x + z1.x, z0.y + z1.y);
+                s_odd[pad(i)] = make_double2(z0.x - z1.x, z0.y - z1.y);
+            }
+            cluster.sync();
+            // separate the two columns by mirror parity: the mirror of row a' is u[N - a'] = odd slot H - a' on the
+            // even fine rows, u[N - 1 - a'] = odd slot H - 1 - a' on the odd ones
+            C* outa = h + ((int64_t)ma * 2 + par) * N;
+            C* outb = h + ((int64_t)mb * 2 + par) * N;
+            for (int ap = d0 * (H / 2) + tid; ap < (d0 + 1) * (H / 2); ap += T) {
+                if (2 * ap + par >= nrow_half) break;
+                const double2 u = s_even[pad(ap)];
+                const double2 v = par ? s_odd[pad(H - 1 - ap)] : (ap == 0 ? u : s_odd[pad(H - ap)]);
+                C va, vb;
+                va.x = u.x + v.x;
+                va.y = u.y + v.y;
+                vb.x = u.x - v.x;
+                vb.y = u.y - v.y;
+                outa[ap] = va;
+                if (has_b) outb[ap] = vb;
+            }
+            if (par == 0 && d0 == 0 && tid == 0 && 2 * H < nrow_half) {   // row a' = H = N/2 mirrors onto itself
+                const double2 u = s_odd[pad(0)];
+                C va, vb;
+                va.x = 2.0 * u.x;
+                va.y = 2.0 * u.y;
+                vb.x = 0;
+                vb.y = 0;
+                outa[H] = va;
+                if (has_b) outb[H] = vb;
             }
             cluster.sync();                            // the peer has read this CTA's half
         }
@@ -545,29 +571,36 @@ k_theta_chain2_adj(int L, int M, int nrow_half, const C* __restrict__ h, const d
     const int ncl = gridDim.x / 2;
     const double* fpos = tb.fpos + d0 * H;
     const double2* twpar = tb.twpar + d0 * H;
-    const int rows = min(N, (nrow_half + 1) / 2);      // rows of a parity block that exist
-    for (int m = blockIdx.x / 2; m <= M; m += ncl) {
-        if (m + ncl <= M && d0 == 0) {
-            const C* nxt = h + ((int64_t)(m + ncl) * 2) * N;
-            prefetch_l2(nxt, rows * (int)sizeof(C), tid, T);
-            prefetch_l2(nxt + N, rows * (int)sizeof(C), tid, T);
-        }
+    const int npair = M / 2 + 1;
+    auto ld = [](const C* ptr, int idx) {
+        const C v = ptr[idx];
+        return make_double2((double)v.x, (double)v.y);
+    };
+    for (int mp = blockIdx.x / 2; mp < npair; mp += ncl) {
+        const int ma = 2 * mp, mb = 2 * mp + 1;
+        const bool has_b = mb <= M;
+        const double sb = has_b ? 1.0 : 0.0;
         double2 acc[E];
 #pragma unroll
         for (int e = 0; e < E; ++e) acc[e] = make_double2(0.0, 0.0);
 #pragma unroll 1
         for (int par = 0; par < 2; ++par) {
-            const C* in = h + ((int64_t)m * 2 + par) * N;
+            const C* ina = h + ((int64_t)ma * 2 + par) * N;
+            const C* inb = h + ((int64_t)(has_b ? mb : ma) * 2 + par) * N;
             if (par) __syncthreads();                  // the last forward stage of parity 0 has read s_col
+            // transpose of the separation (see k_theta_chain_adj), this CTA's half of the radix-2 stage fused in
             for (int i = tid; i < H; i += T) {
-                double2 a = make_double2(0.0, 0.0), b = a;
-                if (2 * i + par < nrow_half) {
-                    const C v = in[i];
-                    a = make_double2((double)v.x, (double)v.y);
-                }
-                if (2 * (i + H) + par < nrow_half) {
-                    const C v = in[i + H];
-                    b = make_double2((double)v.x, (double)v.y);
+                double2 a, b;
+                if (par == 0) {
+                    const double2 xa = ld(ina, i), xb = ld(inb, i);
+                    const double2 ya = ld(ina, H - i), yb = ld(inb, H - i);
+                    a = i == 0 ? make_double2(2.0 * xa.x, 2.0 * xa.y) : make_double2(fma(sb, xb.x, xa.x), fma(sb, xb.y, xa.y));
+                    b = i == 0 ? make_double2(2.0 * ya.x, 2.0 * ya.y) : make_double2(fma(-sb, yb.x, ya.x), fma(-sb, yb.y, ya.y));
+                } else {
+                    const double2 xa = ld(ina, i), xb = ld(inb, i);
+                    const double2 ya = ld(ina, H - 1 - i), yb = ld(inb, H - 1 - i);
+                    a = make_double2(fma(sb, xb.x, xa.x), fma(sb, xb.y, xa.y));
+                    b = make_double2(fma(-sb, yb.x, ya.x), fma(-sb, yb.y, ya.y));
                 }
                 s_col[pad(i)] = d0 ? cmul(make_double2(a.x - b.x, a.y - b.y), tb.tw2[i]) : make_double2(a.x + b.x, a.y + b.y);
             }
@@ -583,10 +616,9 @@ k_theta_chain2_adj(int L, int M, int nrow_half, const C* __restrict__ h, const d
                 acc[e].y += v[e].y;
             }
         }
-        const double fm = pph[m];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const double f = fpos[e * T + tid] * fm;
+            const double f = fpos[e * T + tid];
             acc[e] = make_double2(acc[e].x * f, acc[e].y * f);
         }
         first_stage_from_regs<H, RL, +1, E>(s_col, tid, T, acc);
@@ -594,11 +626,18 @@ k_theta_chain2_adj(int L, int M, int nrow_half, const C* __restrict__ h, const d
         HalfExec<N, +1> inv{s_col, tb.stw, tid};
         inverse_stages<H>(inv);
         cluster.sync();
-        double2* out = ft + (int64_t)m * N;
+        const double pa = pph[ma], pb = has_b ? pph[mb] : 0.0;
+        double2* outa = ft + (int64_t)ma * N;
+        double2* outb = ft + (int64_t)mb * N;
         for (int i = d0 * (H / 2) + tid; i < (d0 + 1) * (H / 2); i += T) {
             const double2 z0 = s_even[pad(i)], z1 = cmul(s_odd[pad(i)], cconj(tb.tw2[i]));
-            out[i] = make_double2(z0.x + z1.x, z0.y + z1.y);
-            out[i + H] = make_double2(z0.x - z1.x, z0.y - z1.y);
+            const double2 x0 = make_double2(z0.x + z1.x, z0.y + z1.y), x1 = make_double2(z0.x - z1.x, z0.y - z1.y);
+            outa[i] = make_double2(pa * x0.x, pa * x0.y);
+            outa[i + H] = make_double2(pa * x1.x, pa * x1.y);
+            if (has_b) {
+                outb[i] = make_double2(pb * x0.x, pb * x0.y);
+                outb[i + H] = make_double2(pb * x1.x, pb * x1.y);
+            }
         }
         cluster.sync();
     }
@@ -657,7 +696,7 @@ int launch_chain2(bool adjoint, int L, int M, int nrow_half, int n_sm, double2* 
     // persistent pairs: as many CTAs as fit at once (shared memory, 128 registers per thread), columns round robin
     const size_t by_smem = (size_t)(200 * 1024) / (HalfCfg<N>::SMEM + 1024);
     const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(HalfCfg<N>::CTAS, by_smem));
-    const int grid = 2 * std::max(1, std::min(M + 1, n_sm * per_sm / 2));
+    const int grid = 2 * std::max(1, std::min(M / 2 + 1, n_sm * per_sm / 2));   // one cluster iteration per column pair
     if (adjoint)
         k_theta_chain2_adj<N, C><<<grid, HalfCfg<N>::T, HalfCfg<N>::SMEM, s>>>(L, M, nrow_half, h, pph, tb, ft);
     else
@@ -776,8 +815,8 @@ int fourier_build(nusht_plan_s* p) {
                     const int f = chain_freq_of_pos(n, pos), k = f < n / 2 ? f : f - n;
                     const size_t at = (size_t)d0 * len + (size_t)e * T + t;
                     twpar[at] = unit((long double)k / (long double)(2 * n));
-                    // (single-CTA variant: column pairs, the 1/2 of their separation is folded in here)
-                    fpos[at] = (k >= -L && k <= L) ? pth[k + L] * (p->theta_chain == 1 ? 0.5 : 1.0) : 0.0;
+                    // (column pairs: the 1/2 of their separation is folded in here)
+                    fpos[at] = (k >= -L && k <= L) ? 0.5 * pth[k + L] : 0.0;
                 }
         NUSHT_TRY(f_alloc(&p->d_tw2n, sizeof(double2) * tb.size(), p));
         NUSHT_CUDA_TRY(cudaMemcpy(p->d_tw2n, tb.data(), sizeof(double2) * tb.size(), cudaMemcpyHostToDevice));
