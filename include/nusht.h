@@ -64,7 +64,11 @@ enum {
     NUSHT_ERR_BAD_POINTS = -6   /* NaN/Inf coordinates or theta outside [0, pi] */
 };
 
-/* Stage slots reported by nusht_stage_times. */
+/* Stage slots reported by nusht_stage_times.
+ * When the plan uses a fused theta chain (Ntheta a power of two <= 16384: one kernel does a3 + a4 + the
+ * theta pass of a5, and one its transpose in a9) the whole chain is reported in the *_FFT_FINE_THETA slot
+ * and the *_FFT_THETA / *_DECONV_* slots read ~0.  The environment variable NUSHT_THETA_CHAIN =
+ * cufft | single | cluster, read by nusht_plan, selects the chain variant where it exists (testing). */
 enum {
     NUSHT_SYN_ALM_PREP = 0,  /* a1 prologue: coefficient scaling + odd-class fold (O(lmax^2)) */
     NUSHT_SYN_LEGENDRE = 1,  /* a1 + a2: Legendre synthesis with fused DFS doubling */
