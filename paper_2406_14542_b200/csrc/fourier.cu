@@ -279,7 +279,8 @@ k_theta_chain_syn(int L, int M, int nrow_half, const double2* __restrict__ ft, c
         }
         const double pa = pph[ma], pb = has_b ? pph[mb] : 0.0;
         __syncthreads();   // previous pair's stores have read s_col
-        // a3: forward transform of the pair; its radix-2 stage is fused with the load
+        // a3: forward transform of the pair; its radix-2 stage is fused with the load (unrolled: 16 loads in flight)
+#pragma unroll 4
         for (int i = tid; i < N / 2; i += T) {
             const double2 a0 = cola[i], a1 = cola[i + N / 2], b0 = colb[i], b1 = colb[i + N / 2];
             const double2 a = make_double2(fma(pb, b0.x, pa * a0.x), fma(pb, b0.y, pa * a0.y));
@@ -369,6 +370,7 @@ k_theta_chain_adj(int L, int M, int nrow_half, const C* __restrict__ h, const do
             // transpose of the separation: u[j] = ha[j] + hb[j] (j below the mirror point), ha[mirror j] - hb[mirror j]
             // above it, 2 ha at the self-mirrored rows 0 and N/2 of parity 0; rows beyond nrow_half do not exist (N is
             // the half fine length, nrow_half = N + 1).  The radix-2 stage of the forward transform is fused in.
+#pragma unroll 4
             for (int i = tid; i < N / 2; i += T) {
                 double2 a, b;
                 if (par == 0) {
