@@ -375,3 +375,30 @@ def test_adjoint_is_reproducible_to_rounding(nusht, L, M, npts, eps):
     for _ in range(40):
         assert float(torch.linalg.vector_norm(plan.adjoint(d_x) - c0)) <= 1e-13 * n0
     plan.destroy()
+
+
+@pytest.mark.parametrize("mode", ["single", "cluster"])
+@pytest.mark.parametrize("L,M", [(63, 0), (63, 1), (255, 2), (1023, 0), (1023, 7), (2047, 4)])
+def test_fused_theta_chain_few_columns(nusht, oracle, monkeypatch, mode, L, M):
+    """Column pairing at its edges: a single column (mmax = 0: the pair has no odd partner), one pair, an odd
+    count; both fused variants against the oracle and for adjointness."""
+    if mode == "cluster" and 2 * (L + 1) < 2048:
+        pytest.skip("the cluster-pair chain starts at Ntheta = 2048")
+    monkeypatch.setenv("NUSHT_THETA_CHAIN", mode)
+    npts, eps = 4000, 1e-10
+    theta, phi = inputs.uniform_sphere_points(npts, 80)
+    theta[:2] = [0.0, np.pi]
+    alm = inputs.random_alm(L, M, 80)
+    x = inputs.random_map(npts, 80)
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps)
+    f = plan.synthesis(cu(alm)).cpu().numpy()
+    c = plan.adjoint(cu(x)).cpu().numpy()
+    sub = slice(0, 400)
+    assert rel(f[sub], oracle.synthesis(L, M, theta[sub], phi[sub], alm, "ld")) <= 10 * eps
+    xs = np.zeros(npts)
+    xs[sub] = x[sub]
+    cs = plan.adjoint(cu(xs)).cpu().numpy()
+    assert rel(cs, oracle.adjoint(L, M, theta[sub], phi[sub], x[sub], "ld")) <= 10 * eps
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+    assert abs(lhs - oracle.inner_alm(L, M, alm, c)) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    plan.destroy()
