@@ -21,6 +21,8 @@
 // rows beyond the poles are the DFS mirror  g[-a][b] = g[a][b + n_phi/2].
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
 
 #include <type_traits>
 #include <vector>
@@ -171,6 +173,76 @@ __global__ void k_scan_add(int* __restrict__ out, const int* __restrict__ totals
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// L2-blocked un-permutation (plan-time tables + one run-time copy kernel).
+// The transforms work on points in sorted order but `map` is in the caller's order, and the caller's
+// order is random with respect to the grid: writing f_j straight to map[perm[j]] is npts isolated
+// 4-byte stores, each a read-modify-write of a DRAM sector (1.8 ms at 67 M points in FP32, more than
+// the interpolation itself).  Instead the caller's index range is cut into n_buckets ranges small
+// enough to stay in the 126 MB L2 (2^23 elements); at plan time every sorted position gets a slot in
+// bucket-major order (stable inside a bucket, so a warp's 32 results go to n_buckets short
+// contiguous runs that L2 merges into full sectors), and at run time k_unpermute walks the slots
+// in order: coalesced reads, and the random writes of one bucket all land in an L2-resident range
+// whose sectors are complete before they are evicted.
+// ---------------------------------------------------------------------------------------------
+constexpr int BUCKET_SHIFT = 23;           // caller indices per bucket: 2^23 (32 MB of FP32)
+constexpr int BUCKET_MAX = 31;             // lane b of a warp keeps bucket b's counter
+constexpr int BUCKET_CHUNK = 1024;         // consecutive sorted positions per warp
+constexpr int BUCKET_WARPS = 4;
+
+__global__ void __launch_bounds__(32 * BUCKET_WARPS)
+k_bucket_count(const int* __restrict__ perm, int64_t npts, int shift, int nchunks, int* __restrict__ cnt) {
+    __shared__ int s_cnt[BUCKET_WARPS][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int chunk = blockIdx.x * BUCKET_WARPS + warp;
+    if (chunk >= nchunks) return;
+    s_cnt[warp][lane] = 0;
+    __syncwarp();
+    const int64_t base = (int64_t)chunk * BUCKET_CHUNK;
+    for (int r = 0; r < BUCKET_CHUNK; r += 32) {
+        const int64_t i = base + r + lane;
+        const int b = (i < npts) ? (perm[i] >> shift) : BUCKET_MAX;   // absent points: a bucket nobody uses
+        const unsigned mask = __match_any_sync(0xffffffffu, b);
+        if (lane == __ffs(mask) - 1) s_cnt[warp][b] += __popc(mask);
+        __syncwarp();
+    }
+    if (lane < BUCKET_MAX) cnt[(int64_t)lane * nchunks + chunk] = s_cnt[warp][lane];   // bucket-major matrix
+}
+
+__global__ void __launch_bounds__(32 * BUCKET_WARPS)
+k_bucket_place(const int* __restrict__ perm, int64_t npts, int shift, int nchunks, const int* __restrict__ off,
+               int* __restrict__ slot, int* __restrict__ dest) {
+    __shared__ int s_off[BUCKET_WARPS][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int chunk = blockIdx.x * BUCKET_WARPS + warp;
+    if (chunk >= nchunks) return;
+    s_off[warp][lane] = (lane < BUCKET_MAX) ? off[(int64_t)lane * nchunks + chunk] : 0;
+    __syncwarp();
+    const int64_t base = (int64_t)chunk * BUCKET_CHUNK;
+    for (int r = 0; r < BUCKET_CHUNK; r += 32) {
+        const int64_t i = base + r + lane;
+        const bool has = i < npts;
+        const int dst = has ? perm[i] : 0;
+        const int b = has ? (dst >> shift) : BUCKET_MAX;
+        const unsigned mask = __match_any_sync(0xffffffffu, b);
+        const int at = s_off[warp][b] + __popc(mask & ((1u << lane) - 1u));
+        __syncwarp();
+        if (lane == 31 - __clz(mask)) s_off[warp][b] = at + 1;     // last lane of the group
+        __syncwarp();
+        if (has) {
+            slot[i] = at;
+            dest[at] = dst;
+        }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_unpermute(const T* __restrict__ stage, const int* __restrict__ dest, int64_t npts, T* __restrict__ map) {
+    const int64_t e = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (e < npts) map[dest[e]] = stage[e];
+}
+
 __global__ void k_item_offsets(const int* __restrict__ bin_off, int* __restrict__ item_off, int n_items,
                                int npts) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -230,6 +302,7 @@ struct NufftParams {
     const int* perm;
     const int* item_off;
     int n_items;
+    int64_t npts;
 };
 
 // warps (= independent work items) per CTA; fewer for wide double-precision kernels so that the
@@ -246,6 +319,15 @@ struct WarpScratch {
     T part[32][SP];     // interp: per point, per active lane partial sums
     int oy[32];         // per point: lane of the first footprint column
 };
+
+// fine-grid row offset and mirror flag of logical row a (may lie beyond a pole)
+__device__ __forceinline__ int64_t grid_row(const NufftGeom& g, int a, bool& mirror) {
+    int am = a;
+    if (am < 0) am += g.nth;
+    if (am >= g.nth) am -= g.nth;
+    mirror = am > g.nth / 2;
+    return (int64_t)(mirror ? g.nth - am : am) * g.nph;
+}
 
 // fine-grid row/column of logical row a (may lie beyond a pole) for a lane
 __device__ __forceinline__ int64_t grid_index(const NufftGeom& g, int a, int col_n, int col_m) {
@@ -413,6 +495,69 @@ k_interp(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
 }
 
 // ---------------------------------------------------------------------------------------------
+// a7, FP32 path at small widths (eps >= 1e-6, W <= 8): one THREAD per point, the W x W footprint
+// gathered straight from the grid through L1.  The sorted order (segment, strip, row) keeps the 32
+// points of a warp inside about two grid rows of one strip, so each of the W^2 load instructions
+// touches two to four 128-byte lines that stay L1-resident across the footprint; per point the
+// warp issues about 5 instructions instead of the ~20 of the register-window kernel, which is
+// issue-bound at these widths (2.8 ms at W = 5, 7 for an HBM floor of 0.3 ms at config 5).
+// Same arithmetic as k_interp: weights from eval_taps, theta contraction innermost per column is
+// replaced by phi innermost per row (sum order differs: FP32 rounding only).
+// ---------------------------------------------------------------------------------------------
+constexpr int GATHER_THREADS = 256;
+
+template <int W>
+__global__ void __launch_bounds__(GATHER_THREADS)
+k_interp_gather(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<float> kp,
+                const float* __restrict__ grid, float* __restrict__ map) {
+    const int64_t idx = (int64_t)blockIdx.x * GATHER_THREADS + threadIdx.x;
+    if (idx >= P.npts) return;
+    const NufftGeom& g = P.g;
+    const double X = P.px[idx], Y = P.py[idx];
+    const int out = P.perm[idx];
+    const double a0d = ceil(X - 0.5 * W), b0d = ceil(Y - 0.5 * W);
+    const float ut = (float)(2.0 * ((a0d + 0.5 * W) - X) - 1.0);
+    const float up = (float)(2.0 * ((b0d + 0.5 * W) - Y) - 1.0);
+    float kt[W], kph[W];
+    eval_taps<W, float>(kp, ut, kt);
+    eval_taps<W, float>(kp, up, kph);
+    const int a0 = (int)a0d;
+    int b0 = (int)b0d;                       // in [-W/2, nph]
+    if (b0 < 0) b0 += g.nph;
+    if (b0 >= g.nph) b0 -= g.nph;
+    int bm = b0 + g.nph / 2;                 // first column on a mirrored row (beyond a pole)
+    if (bm >= g.nph) bm -= g.nph;
+    const bool interior = (a0 >= 0) && (a0 + W - 1 <= g.nth / 2) && (b0 + W <= g.nph);
+    float sum = 0.f;
+    if (interior) {
+        const float* src = grid + (int64_t)a0 * g.nph + b0;
+#pragma unroll
+        for (int i = 0; i < W; ++i) {
+            float r = 0.f;
+#pragma unroll
+            for (int j = 0; j < W; ++j) r = fmaf(kph[j], __ldg(src + j), r);
+            sum = fmaf(kt[i], r, sum);
+            src += g.nph;
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < W; ++i) {
+            bool mirror;
+            const int64_t base = grid_row(g, a0 + i, mirror);
+            int c = mirror ? bm : b0;
+            float r = 0.f;
+#pragma unroll
+            for (int j = 0; j < W; ++j) {
+                r = fmaf(kph[j], __ldg(grid + base + c), r);
+                c = (c + 1 == g.nph) ? 0 : c + 1;
+            }
+            sum = fmaf(kt[i], r, sum);
+        }
+    }
+    map[out] = sum;
+}
+
+// ---------------------------------------------------------------------------------------------
 // a8: type-1 spreading (grid must be zero on entry)
 // ---------------------------------------------------------------------------------------------
 template <int W, typename T>
@@ -556,6 +701,23 @@ int launch_spread(const NufftParams& P, const KernelHost& h, const void* map, vo
     return NUSHT_OK;
 }
 
+template <int W>
+int launch_interp_gather(const NufftParams& P, const KernelHost& h, const void* grid, void* map, cudaStream_t s) {
+    const KernelPoly<float> kp = make_device_poly<float>(h);
+    const unsigned blocks = (unsigned)((P.npts + GATHER_THREADS - 1) / GATHER_THREADS);
+    k_interp_gather<W><<<blocks, GATHER_THREADS, 0, s>>>(P, kp, (const float*)grid, (float*)map);
+    NUSHT_CUDA_TRY(cudaGetLastError());
+    return NUSHT_OK;
+}
+int dispatch_interp_gather(int w, const NufftParams& P, const KernelHost& h, const void* grid, void* map, cudaStream_t s) {
+    switch (w) {
+#define NUSHT_CASE(WW) case WW: return launch_interp_gather<WW>(P, h, grid, map, s);
+        NUSHT_CASE(2) NUSHT_CASE(3) NUSHT_CASE(4) NUSHT_CASE(5) NUSHT_CASE(6) NUSHT_CASE(7) NUSHT_CASE(8)
+#undef NUSHT_CASE
+    }
+    return NUSHT_ERR_UNSUPPORTED;
+}
+
 template <typename T>
 int dispatch_interp(int w, const NufftParams& P, const KernelHost& h, const void* grid, void* map, cudaStream_t s) {
     switch (w) {
@@ -647,15 +809,6 @@ __device__ __forceinline__ int mma_publish(MmaScratch<W, S>& ws, const KernelPol
     for (int i = 0; i < W; ++i) ws.ph[lane][i] = k[i];
     ws.oy[lane] = (int)b0d - c0;
     return (int)a0d;
-}
-
-// fine-grid row offset and mirror flag of logical row a (may lie beyond a pole)
-__device__ __forceinline__ int64_t grid_row(const NufftGeom& g, int a, bool& mirror) {
-    int am = a;
-    if (am < 0) am += g.nth;
-    if (am >= g.nth) am -= g.nth;
-    mirror = am > g.nth / 2;
-    return (int64_t)(mirror ? g.nth - am : am) * g.nph;
 }
 
 // cp.async helpers (SASS LDGSTS): global -> shared without a register round trip, completion per thread
@@ -1254,8 +1407,45 @@ int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi) {
         SORT_TRY(cudaGetLastError());
     }
     SORT_TRY(cudaDeviceSynchronize());
-#undef SORT_TRY
     cleanup();
+    d_keys = d_hist = d_off = d_tot = d_bad = nullptr;
+    // L2-blocked un-permutation tables (FP32 gather interpolation; see k_unpermute)
+    p->n_buckets = 1;
+    int bshift = BUCKET_SHIFT;
+    if (const char* ev = getenv("NUSHT_UNPERMUTE_SHIFT")) {      // tests: several buckets at small point counts
+        const int v = atoi(ev);
+        if (v >= 4 && v <= 30) bshift = v;
+    }
+    const int64_t nb64 = (n + ((int64_t)1 << bshift) - 1) >> bshift;
+    if (p->dtype == NUSHT_F32 && g.w <= 8 && nb64 > 1 && nb64 <= BUCKET_MAX) {
+        const int nb = (int)nb64;
+        const int nchunks = (int)((n + BUCKET_CHUNK - 1) / BUCKET_CHUNK);
+        const int ncnt = BUCKET_MAX * nchunks;
+        const int nt = (ncnt + SCAN_TILE - 1) / SCAN_TILE;
+        NUSHT_TRY(nu_alloc(&p->d_slot, (size_t)n, p));
+        NUSHT_TRY(nu_alloc(&p->d_dest, (size_t)n, p));
+        float* stage = nullptr;
+        NUSHT_TRY(nu_alloc(&stage, (size_t)n, p));
+        p->d_stage = stage;
+        SORT_TRY(cudaMalloc((void**)&d_hist, sizeof(int) * (size_t)ncnt));
+        SORT_TRY(cudaMalloc((void**)&d_off, sizeof(int) * (size_t)ncnt));
+        SORT_TRY(cudaMalloc((void**)&d_tot, sizeof(int) * (size_t)nt));
+        const int blocks = (nchunks + BUCKET_WARPS - 1) / BUCKET_WARPS;
+        k_bucket_count<<<blocks, 32 * BUCKET_WARPS>>>(p->d_perm, n, bshift, nchunks, d_hist);
+        SORT_TRY(cudaGetLastError());
+        k_scan_tiles<<<nt, SCAN_BLOCK>>>(d_hist, d_off, d_tot, ncnt);
+        SORT_TRY(cudaGetLastError());
+        k_scan_totals<<<1, 1024>>>(d_tot, nt);
+        SORT_TRY(cudaGetLastError());
+        k_scan_add<<<nt, SCAN_BLOCK>>>(d_off, d_tot, ncnt);
+        SORT_TRY(cudaGetLastError());
+        k_bucket_place<<<blocks, 32 * BUCKET_WARPS>>>(p->d_perm, n, bshift, nchunks, d_off, p->d_slot, p->d_dest);
+        SORT_TRY(cudaGetLastError());
+        SORT_TRY(cudaDeviceSynchronize());
+        cleanup();
+        p->n_buckets = nb;
+    }
+#undef SORT_TRY
     return status;
 }
 
@@ -1267,6 +1457,7 @@ static NufftParams make_nufft_params(const nusht_plan_s* p) {
     P.perm = p->d_perm;
     P.item_off = p->d_item_off;
     P.n_items = p->n_items;
+    P.npts = p->npts;
     return P;
 }
 
@@ -1275,6 +1466,20 @@ int nufft_interp(nusht_plan_s* p, const void* grid, void* map, cudaStream_t s) {
     const KernelHost* h = g_kernel_of(p);
     const NufftParams P = make_nufft_params(p);
     if (p->dtype == NUSHT_F64) return dispatch_interp_mma(p->ng.w, P, *h, grid, map, s);
+    // FP32: thread-per-point gather up to W = 8 (eps >= 1e-7); NUSHT_INTERP_F32=window keeps the register-window
+    // kernel for the tests, which compare the two
+    const char* ev = getenv("NUSHT_INTERP_F32");
+    const bool window = ev && strcmp(ev, "window") == 0;
+    if (p->ng.w <= 8 && !window) {
+        if (p->n_buckets <= 1) return dispatch_interp_gather(p->ng.w, P, *h, grid, map, s);
+        NufftParams Q = P;
+        Q.perm = p->d_slot;       // results go to their bucket-major slot, then to the caller's order
+        NUSHT_TRY(dispatch_interp_gather(p->ng.w, Q, *h, grid, p->d_stage, s));
+        k_unpermute<float><<<(unsigned)((p->npts + 255) / 256), 256, 0, s>>>((const float*)p->d_stage, p->d_dest,
+                                                                           p->npts, (float*)map);
+        NUSHT_CUDA_TRY(cudaGetLastError());
+        return NUSHT_OK;
+    }
     return dispatch_interp<float>(p->ng.w, P, *h, grid, map, s);
 }
 
@@ -1291,6 +1496,8 @@ int nufft_spread(nusht_plan_s* p, const void* map, void* grid, cudaStream_t s) {
 void nufft_free(nusht_plan_s* p) {
     cudaFree(p->d_px); cudaFree(p->d_py); cudaFree(p->d_perm); cudaFree(p->d_item_off);
     p->d_px = p->d_py = nullptr; p->d_perm = nullptr; p->d_item_off = nullptr;
+    cudaFree(p->d_slot); cudaFree(p->d_dest); cudaFree(p->d_stage);
+    p->d_slot = p->d_dest = nullptr; p->d_stage = nullptr;
     delete static_cast<KernelHost*>(p->kernel_host);
     p->kernel_host = nullptr;
 }

@@ -111,6 +111,11 @@ struct nusht_plan_s {
     int* d_item_off = nullptr;      // [nseg*nstrip + 1] start of each (segment, strip) work item
     int* d_item_order = nullptr;    // work items sorted by decreasing point count
     int n_items = 0;
+    // L2-blocked un-permutation of the FP32 interpolation result (nufft.cu): bucket-major slots
+    int n_buckets = 1;              // 1: results are scattered through d_perm directly
+    int* d_slot = nullptr;          // sorted position -> slot (bucket-major, stable inside a bucket)
+    int* d_dest = nullptr;          // slot -> caller index
+    void* d_stage = nullptr;        // [npts] results in slot order (dtype)
     void* kernel_host = nullptr;    // nufft.cu: host model of the kernel polynomial
     // --- host-buffer staging (allocated on first use of *_host) ---
     void *d_in_alm = nullptr, *d_out_alm = nullptr, *d_in_map = nullptr, *d_out_map = nullptr;

@@ -130,6 +130,54 @@ def test_spread_is_transpose_of_interp(nusht, eps):
     plan.destroy()
 
 
+@pytest.mark.parametrize("eps", [1e-1, 1e-2, 1e-3, 1e-4, 1e-5, 1e-6])
+def test_fp32_gather_interp_matches_window_kernel(nusht, monkeypatch, eps):
+    """FP32 interpolation runs the thread-per-point gather kernel (k_interp_gather, W <= 8) by default;
+    NUSHT_INTERP_F32=window selects the register-window kernel.  Same weights, different sum order: they must
+    agree to binary32 rounding, on pole and phi-wrap footprints as well, and the gather kernel must be the
+    transpose of the FP32 spreading kernel to binary32 rounding."""
+    L, npts = 60, 30000
+    theta, phi = inputs.uniform_sphere_points(npts, 33)
+    theta[:6] = [0.0, np.pi, 1e-9, np.pi - 1e-9, 0.01, np.pi - 0.01]
+    phi[:6] = [0.0, 2 * np.pi - 1e-12, 6.28, 1e-15, 2 * np.pi - 1e-3, 1e-3]
+    plan = nusht.Plan(L, L, cu(theta), cu(phi), eps, dtype="f32")
+    rng = np.random.default_rng(34)
+    g = rng.standard_normal(plan.grid_shape()).astype(np.float32)
+    x = rng.standard_normal(npts).astype(np.float32)
+    monkeypatch.setenv("NUSHT_INTERP_F32", "window")
+    f_win = plan.stage_interp(cu(g)).cpu().numpy().astype(np.float64)
+    monkeypatch.delenv("NUSHT_INTERP_F32")
+    f_gat = plan.stage_interp(cu(g)).cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(f_gat - f_win)) <= 4e-6 * np.max(np.abs(f_win))
+    assert not np.array_equal(f_gat, f_win) or plan.info.kernel_width <= 2   # two different kernels did run
+    gs = plan.stage_spread(cu(x)).cpu().numpy().astype(np.float64)
+    lhs, rhs = np.dot(f_gat, x.astype(np.float64)), np.sum(g.astype(np.float64) * gs)
+    assert abs(lhs - rhs) <= 2e-6 * np.linalg.norm(f_gat) * np.linalg.norm(x)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("shift,npts", [(10, 30000), (12, 100001), (9, 15000)])
+def test_fp32_l2_blocked_unpermute(nusht, monkeypatch, shift, npts):
+    """At large point counts the FP32 interpolation writes its results to bucket-major slots and k_unpermute
+    brings them to the caller's order (L2-blocked; nufft.cu).  NUSHT_UNPERMUTE_SHIFT (plan time) makes the
+    buckets small enough to exercise 8-30 of them here: pure data movement, so the result must be bitwise
+    the one of the direct scatter, ragged last chunk and last bucket included."""
+    L = 50
+    theta, phi = inputs.uniform_sphere_points(npts, 35)
+    rng = np.random.default_rng(36)
+    plan0 = nusht.Plan(L, L, cu(theta), cu(phi), 1e-4, dtype="f32")
+    g = cu(rng.standard_normal(plan0.grid_shape()).astype(np.float32))
+    f0 = plan0.stage_interp(g).cpu().numpy()
+    plan0.destroy()
+    monkeypatch.setenv("NUSHT_UNPERMUTE_SHIFT", str(shift))
+    plan1 = nusht.Plan(L, L, cu(theta), cu(phi), 1e-4, dtype="f32")
+    monkeypatch.delenv("NUSHT_UNPERMUTE_SHIFT")
+    assert plan1.info.workspace_bytes >= plan0.info.workspace_bytes + 12 * npts   # slot, dest, stage tables exist
+    f1 = plan1.stage_interp(g).cpu().numpy()
+    assert np.array_equal(f0, f1)
+    plan1.destroy()
+
+
 # ---- full transforms, config 1 (BASELINE.json configs[0]) in full ------------------------------
 def test_config1_full(nusht, oracle):
     cfg, theta, phi, alm, x = inputs.make_config(1)
