@@ -179,13 +179,13 @@ __global__ void k_scan_add(int* __restrict__ out, const int* __restrict__ totals
 // order is random with respect to the grid: writing f_j straight to map[perm[j]] is npts isolated
 // 4-byte stores, each a read-modify-write of a DRAM sector (1.8 ms at 67 M points in FP32, more than
 // the interpolation itself).  Instead the caller's index range is cut into n_buckets ranges small
-// enough to stay in the 126 MB L2 (2^23 elements); at plan time every sorted position gets a slot in
+// enough to stay in the 126 MB L2 (2^22 elements); at plan time every sorted position gets a slot in
 // bucket-major order (stable inside a bucket, so a warp's 32 results go to n_buckets short
 // contiguous runs that L2 merges into full sectors), and at run time k_unpermute walks the slots
 // in order: coalesced reads, and the random writes of one bucket all land in an L2-resident range
 // whose sectors are complete before they are evicted.
 // ---------------------------------------------------------------------------------------------
-constexpr int BUCKET_SHIFT = 23;           // caller indices per bucket: 2^23 (32 MB of FP32)
+constexpr int BUCKET_SHIFT = 22;           // caller indices per bucket: 2^22 (16 MB of FP32; measured best of 2^22..2^24), more if that gives over 31 buckets
 constexpr int BUCKET_MAX = 31;             // lane b of a warp keeps bucket b's counter
 constexpr int BUCKET_CHUNK = 1024;         // consecutive sorted positions per warp
 constexpr int BUCKET_WARPS = 4;
@@ -1412,6 +1412,7 @@ int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi) {
     // L2-blocked un-permutation tables (FP32 gather interpolation; see k_unpermute)
     p->n_buckets = 1;
     int bshift = BUCKET_SHIFT;
+    while (((n + ((int64_t)1 << bshift) - 1) >> bshift) > BUCKET_MAX) ++bshift;
     if (const char* ev = getenv("NUSHT_UNPERMUTE_SHIFT")) {      // tests: several buckets at small point counts
         const int v = atoi(ev);
         if (v >= 4 && v <= 30) bshift = v;
