@@ -23,6 +23,8 @@
 #include <math.h>
 #include <stdio.h>
 
+#include <algorithm>
+#include <utility>
 #include <vector>
 
 #include "nusht_internal.cuh"
@@ -55,6 +57,8 @@ struct LegParams {
     const int* ff_n;
     const double2* ff_p;   // (p0, p1) per (m, block, r, lane)
     const int* ff_e;       // exponent counter
+    // work list of the synthesis (plan time): CTA i takes items[i] = (block of ring pairs, m), longest first
+    const int2* items;
     const int64_t* eoff;
     const double2* ab;
     const double* x2;
@@ -329,8 +333,8 @@ __device__ __forceinline__ void fold_pair(const LegParams& P, const double2* __r
 // column of the grid takes the `rem` left-over pairs of 32/rem different m per warp, one (m, pair)
 // per lane, each lane streaming its own coefficient column from global memory.
 __device__ void synth_remainder(const LegParams& P, const double4* __restrict__ aeo, double2* __restrict__ ft, int j0,
-                                int rem) {
-    const int gid = blockIdx.y * 32 + threadIdx.x;
+                                int rem, int by) {
+    const int gid = by * 32 + threadIdx.x;
     const int m = gid / rem, j = j0 + gid % rem;
     if (m > P.mmax) return;
     const int ne = (P.lmax - m) / 2 + 1;
@@ -363,8 +367,8 @@ __device__ void synth_remainder(const LegParams& P, const double4* __restrict__ 
 }
 
 __device__ void adjoint_remainder(const LegParams& P, const double2* __restrict__ gt, double4* __restrict__ eo, int j0,
-                                  int rem) {
-    const int gid = blockIdx.y * 32 + threadIdx.x;
+                                  int rem, int by) {
+    const int gid = by * 32 + threadIdx.x;
     const int m = gid / rem, j = j0 + gid % rem;
     if (m > P.mmax) return;
     const int ne = (P.lmax - m) / 2 + 1;
@@ -463,22 +467,24 @@ k_legendre_fastforward(LegParams P, int* __restrict__ ff_n, double2* __restrict_
 template <int R>
 __global__ void __launch_bounds__(SYN_THREADS)
 k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restrict__ ft) {
-    if (P.rem > 0 && blockIdx.x == P.nblk) {
-        synth_remainder(P, aeo, ft, P.nblk * (32 * R), P.rem);
+    const int2 item = P.items[blockIdx.x];
+    const int bx = item.x, by = item.y;
+    if (P.rem > 0 && bx == P.nblk) {
+        synth_remainder(P, aeo, ft, P.nblk * (32 * R), P.rem, by);
         return;
     }
     __shared__ __align__(16) double2 s_ab[2][SYN_TN];
     __shared__ __align__(32) double4 s_aeo[2][SYN_TN];
     __shared__ __align__(8) uint64_t s_bar[2];
 
-    const int m = blockIdx.y;
+    const int m = by;
     const int L = P.lmax;
     const int ne = (L - m) / 2 + 1;
     const int64_t o = P.eoff[m];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int jb = (blockIdx.x * SYN_WARPS + warp) * (32 * R);
+    const int jb = (bx * SYN_WARPS + warp) * (32 * R);
     const int ntiles = (ne + SYN_TN - 1) / SYN_TN;
-    const int64_t wff = (int64_t)m * P.nblk + blockIdx.x;
+    const int64_t wff = (int64_t)m * P.nblk + bx;
     const int n_start = P.ff_n[wff];          // first step at which a pair of this warp is in range
     const int tile0 = n_start / SYN_TN;
 
@@ -638,8 +644,11 @@ __device__ __forceinline__ double shfl_xor_d(double v, int mask) {
 template <int R, int C>
 __global__ void __launch_bounds__(32, adj_min_ctas(R, C))
 k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restrict__ eo) {
-    if (P.rem > 0 && blockIdx.x == P.nblk) {
-        adjoint_remainder(P, gt, eo, P.nblk * (32 * R), P.rem);
+    // plain 2-D grid (block of ring pairs, m): the blocks of one m run together and add into the same eo[m]
+    // column while it is L2-resident; a work list as in the synthesis was tried (see build_work_list)
+    const int bx = blockIdx.x, by = blockIdx.y;
+    if (P.rem > 0 && bx == P.nblk) {
+        adjoint_remainder(P, gt, eo, P.nblk * (32 * R), P.rem, by);
         return;
     }
     __shared__ __align__(16) double2 s_ab[2][ADJ_TN];
@@ -647,16 +656,16 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
     __shared__ __align__(16) double s_tr[NV][34];   // row stride 272 B: 16-byte aligned rows, conflict-free LDS.128
     __shared__ __align__(8) uint64_t s_bar[2];
 
-    const int m = blockIdx.y;
+    const int m = by;
     const int L = P.lmax;
     const int ne = (L - m) / 2 + 1;
     const int64_t o = P.eoff[m];
     const int lane = threadIdx.x;
-    const int jb = blockIdx.x * (32 * R);
+    const int jb = bx * (32 * R);
     const int ntiles = (ne + ADJ_TN - 1) / ADJ_TN;
     const double sgn = (m & 1) ? -1.0 : 1.0;
     const double2* row = gt + (int64_t)m * P.nth2;
-    const int64_t wff = (int64_t)m * P.nblk + blockIdx.x;
+    const int64_t wff = (int64_t)m * P.nblk + bx;
     const int n_start = P.ff_n[wff];          // first step at which a pair of this warp is in range
     if (n_start >= ne) return;                // never before lmax: this warp contributes nothing
     const int tile0 = n_start / ADJ_TN;
@@ -830,6 +839,7 @@ static LegParams make_params(const nusht_plan_s* p, bool adjoint_tables = false)
     P.ff_n = a ? p->d_ffa_n : p->d_ff_n;
     P.ff_p = a ? p->d_ffa_p : p->d_ff_p;
     P.ff_e = a ? p->d_ffa_e : p->d_ff_e;
+    P.items = p->d_items_syn;
     return P;
 }
 
@@ -839,6 +849,44 @@ static int dev_alloc(T** ptr, size_t count, nusht_plan_s* p) {
     if (bytes == 0) bytes = sizeof(T);
     NUSHT_CUDA_TRY(cudaMalloc((void**)ptr, bytes));
     p->workspace_bytes += (int64_t)bytes;
+    return NUSHT_OK;
+}
+
+// Work list of the synthesis kernel: one entry (block of ring pairs, m) per CTA.  A block's cost is the number of
+// n-steps from its first in-range step to the end of the column, known from the fast-forward table.  The
+// remainder CTAs (one lane per (m, pair), dependent global loads: long latency chains) come first, then the
+// blocks by decreasing cost, so the grid drains evenly (3.07 -> 2.95 ms at lmax = 4095); blocks that never come
+// into range go last and only write their zeros.  The adjoint kernel keeps its 2-D grid: it sits exactly at
+// 128 registers and the list lookup made it spill (4.2 -> 4.9 ms), and its blocks of one m should run together
+// anyway (they add into the same eo[m] column while it is L2-resident).
+static int build_work_list(nusht_plan_s* p, int R, const int* d_ff_n, int2** d_items, int* n_items) {
+    LegParams P = make_params(p);
+    leg_grid(p, R, P);
+    const int M = p->mmax, L = p->lmax;
+    std::vector<int> ffn((size_t)(M + 1) * P.nblk);
+    NUSHT_CUDA_TRY(cudaMemcpy(ffn.data(), d_ff_n, sizeof(int) * ffn.size(), cudaMemcpyDeviceToHost));
+    std::vector<int2> items;
+    items.reserve(ffn.size() + (size_t)M + 1);
+    if (P.rem > 0) {
+        const int ny = ((M + 1) * P.rem + 31) / 32;
+        for (int y = 0; y < ny; ++y) items.push_back(make_int2(P.nblk, y));
+    }
+    std::vector<std::pair<int, int64_t>> order;     // (cost, m * nblk + block)
+    order.reserve(ffn.size());
+    for (int m = 0; m <= M; ++m) {
+        const int ne = (L - m) / 2 + 1;
+        for (int b = 0; b < P.nblk; ++b) {
+            const int cost = ne - ffn[(size_t)m * P.nblk + b];
+            order.push_back(std::make_pair(cost > 0 ? cost : 0, (int64_t)m * P.nblk + b));
+        }
+    }
+    std::stable_sort(order.begin(), order.end(),
+                     [](const std::pair<int, int64_t>& a, const std::pair<int, int64_t>& b) { return a.first > b.first; });
+    for (const auto& e : order) items.push_back(make_int2((int)(e.second % P.nblk), (int)(e.second / P.nblk)));
+    *n_items = (int)items.size();
+    NUSHT_TRY(dev_alloc(d_items, items.size(), p));
+    if (!items.empty())
+        NUSHT_CUDA_TRY(cudaMemcpy(*d_items, items.data(), sizeof(int2) * items.size(), cudaMemcpyHostToDevice));
     return NUSHT_OK;
 }
 
@@ -927,6 +975,7 @@ int legendre_build_tables(nusht_plan_s* p) {
         NUSHT_CUDA_TRY(cudaGetLastError());
     }
     NUSHT_CUDA_TRY(cudaDeviceSynchronize());
+    NUSHT_TRY(build_work_list(p, LEG_R, p->d_ff_n, &p->d_items_syn, &p->n_items_syn));
     return NUSHT_OK;
 }
 
@@ -944,8 +993,9 @@ int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s) {
 
 int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s) {
     LegParams P = make_params(p);
-    const dim3 grid = leg_grid(p, LEG_R, P);
-    k_legendre_synth<LEG_R><<<grid, SYN_THREADS, 0, s>>>(P, p->d_aeo, ft);
+    leg_grid(p, LEG_R, P);
+    if (p->n_items_syn == 0) return NUSHT_OK;
+    k_legendre_synth<LEG_R><<<p->n_items_syn, SYN_THREADS, 0, s>>>(P, p->d_aeo, ft);
     NUSHT_CUDA_TRY(cudaGetLastError());
     return NUSHT_OK;
 }
@@ -973,6 +1023,8 @@ int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s) {
 }
 
 void legendre_free(nusht_plan_s* p) {
+    cudaFree(p->d_items_syn);
+    p->d_items_syn = nullptr;
     cudaFree(p->d_eoff); cudaFree(p->d_ab); cudaFree(p->d_sig); cudaFree(p->d_sodd); cudaFree(p->d_rho);
     cudaFree(p->d_aeo); cudaFree(p->d_ft); cudaFree(p->d_x2); cudaFree(p->d_x); cudaFree(p->d_logsin);
     cudaFree(p->d_logkap);

@@ -302,7 +302,6 @@ struct NufftParams {
     const int* perm;
     const int* item_off;
     int n_items;
-    int64_t npts;
 };
 
 // warps (= independent work items) per CTA; fewer for wide double-precision kernels so that the
@@ -508,10 +507,10 @@ constexpr int GATHER_THREADS = 256;
 
 template <int W>
 __global__ void __launch_bounds__(GATHER_THREADS)
-k_interp_gather(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<float> kp,
+k_interp_gather(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<float> kp, int64_t npts,
                 const float* __restrict__ grid, float* __restrict__ map) {
     const int64_t idx = (int64_t)blockIdx.x * GATHER_THREADS + threadIdx.x;
-    if (idx >= P.npts) return;
+    if (idx >= npts) return;
     const NufftGeom& g = P.g;
     const double X = P.px[idx], Y = P.py[idx];
     const int out = P.perm[idx];
@@ -702,16 +701,18 @@ int launch_spread(const NufftParams& P, const KernelHost& h, const void* map, vo
 }
 
 template <int W>
-int launch_interp_gather(const NufftParams& P, const KernelHost& h, const void* grid, void* map, cudaStream_t s) {
+int launch_interp_gather(const NufftParams& P, const KernelHost& h, int64_t npts, const void* grid, void* map,
+                         cudaStream_t s) {
     const KernelPoly<float> kp = make_device_poly<float>(h);
-    const unsigned blocks = (unsigned)((P.npts + GATHER_THREADS - 1) / GATHER_THREADS);
-    k_interp_gather<W><<<blocks, GATHER_THREADS, 0, s>>>(P, kp, (const float*)grid, (float*)map);
+    const unsigned blocks = (unsigned)((npts + GATHER_THREADS - 1) / GATHER_THREADS);
+    k_interp_gather<W><<<blocks, GATHER_THREADS, 0, s>>>(P, kp, npts, (const float*)grid, (float*)map);
     NUSHT_CUDA_TRY(cudaGetLastError());
     return NUSHT_OK;
 }
-int dispatch_interp_gather(int w, const NufftParams& P, const KernelHost& h, const void* grid, void* map, cudaStream_t s) {
+int dispatch_interp_gather(int w, const NufftParams& P, const KernelHost& h, int64_t npts, const void* grid, void* map,
+                           cudaStream_t s) {
     switch (w) {
-#define NUSHT_CASE(WW) case WW: return launch_interp_gather<WW>(P, h, grid, map, s);
+#define NUSHT_CASE(WW) case WW: return launch_interp_gather<WW>(P, h, npts, grid, map, s);
         NUSHT_CASE(2) NUSHT_CASE(3) NUSHT_CASE(4) NUSHT_CASE(5) NUSHT_CASE(6) NUSHT_CASE(7) NUSHT_CASE(8)
 #undef NUSHT_CASE
     }
@@ -1458,7 +1459,6 @@ static NufftParams make_nufft_params(const nusht_plan_s* p) {
     P.perm = p->d_perm;
     P.item_off = p->d_item_off;
     P.n_items = p->n_items;
-    P.npts = p->npts;
     return P;
 }
 
@@ -1472,10 +1472,10 @@ int nufft_interp(nusht_plan_s* p, const void* grid, void* map, cudaStream_t s) {
     const char* ev = getenv("NUSHT_INTERP_F32");
     const bool window = ev && strcmp(ev, "window") == 0;
     if (p->ng.w <= 8 && !window) {
-        if (p->n_buckets <= 1) return dispatch_interp_gather(p->ng.w, P, *h, grid, map, s);
+        if (p->n_buckets <= 1) return dispatch_interp_gather(p->ng.w, P, *h, p->npts, grid, map, s);
         NufftParams Q = P;
         Q.perm = p->d_slot;       // results go to their bucket-major slot, then to the caller's order
-        NUSHT_TRY(dispatch_interp_gather(p->ng.w, Q, *h, grid, p->d_stage, s));
+        NUSHT_TRY(dispatch_interp_gather(p->ng.w, Q, *h, p->npts, grid, p->d_stage, s));
         k_unpermute<float><<<(unsigned)((p->npts + 255) / 256), 256, 0, s>>>((const float*)p->d_stage, p->d_dest,
                                                                            p->npts, (float*)map);
         NUSHT_CUDA_TRY(cudaGetLastError());

@@ -87,6 +87,8 @@ struct nusht_plan_s {
     int* d_ffa_n = nullptr;         // the same for the adjoint's decomposition (more ring pairs per thread)
     double2* d_ffa_p = nullptr;
     int* d_ffa_e = nullptr;
+    int2* d_items_syn = nullptr;    // work list of the Legendre synthesis: (block of ring pairs, m) per CTA, longest first
+    int n_items_syn = 0;
     // --- Legendre work buffers ---
     double4* d_aeo = nullptr;       // scaled coefficients per (m,n): (ae.re, ae.im, ao.re, ao.im)
     double2* d_ft = nullptr;        // Ftilde / Gtilde: [mmax+1][nth2] complex128
