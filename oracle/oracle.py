@@ -162,3 +162,35 @@ def inner_alm(lmax: int, mmax: int, a, c) -> float:
     prod = np.longdouble(a[n0:].real) * np.longdouble(c[n0:].real) + \
         np.longdouble(a[n0:].imag) * np.longdouble(c[n0:].imag)
     return s0 + 2.0 * float(np.sum(prod))
+
+
+def pointing(theta, phi, alpha_theta, alpha_phi):
+    """Deflected positions of arXiv 2406.14542 Eq. C1, written out in numpy long double:
+
+        n' = cos(a) n + (sin(a)/a) (a_theta e_theta + a_phi e_phi),   a = sqrt(a_theta^2 + a_phi^2),
+
+    with n = (sin t cos p, sin t sin p, cos t) and the right-handed basis e_theta = dn/dtheta =
+    (cos t cos p, cos t sin p, -sin t), e_phi = (-sin p, cos p, 0).  Returns the angles of n':
+    theta' = atan2(|n'_xy|, n'_z) in [0, pi] (the polar angle, written so that it keeps its accuracy next to the
+    poles, where arccos does not) and phi' = atan2(n'_y, n'_x) mod 2 pi; sin(a)/a := 1 at a = 0.
+    Pins (tests/test_oracle_pins.py): a = 0 is the identity, a_phi = 0 moves along the meridian by a_theta,
+    on the equator a_theta = 0 moves along the equator by a_phi, |n'| = 1 and the angle between n and n' is a,
+    and the spherical-triangle cosine rule for theta'."""
+    ld = np.longdouble
+    t, p = np.asarray(theta, dtype=ld), np.asarray(phi, dtype=ld)
+    at, ap = np.asarray(alpha_theta, dtype=ld), np.asarray(alpha_phi, dtype=ld)
+    a = np.sqrt(at * at + ap * ap)
+    st, ct, sp, cp = np.sin(t), np.cos(t), np.sin(p), np.cos(p)
+    n = (st * cp, st * sp, ct)
+    e_t = (ct * cp, ct * sp, -st)
+    e_p = (-sp, cp, np.zeros_like(sp))
+    with np.errstate(invalid="ignore", divide="ignore"):
+        sinc = np.where(a > 0, np.sin(a) / np.where(a > 0, a, ld(1)), ld(1))
+    ca = np.cos(a)
+    nx, ny, nz = (ca * n[k] + sinc * (at * e_t[k] + ap * e_p[k]) for k in range(3))
+    two_pi = 2 * np.arctan2(ld(0), ld(-1))
+    theta2 = np.arctan2(np.sqrt(nx * nx + ny * ny), nz)
+    phi2 = np.arctan2(ny, nx)
+    phi2 = np.where(phi2 < 0, phi2 + two_pi, phi2)
+    phi2 = np.where(phi2 >= two_pi, phi2 - two_pi, phi2)
+    return theta2, phi2

@@ -258,3 +258,50 @@ def test_large_lmax_rescaling_synthesis_vs_mpmath(oracle):
         y = mp.spherharm(l, m, mp.mpf(float(th[j])), mp.mpf(float(ph[j])), maxprec=400000)
         ref = 2 * float(mp.re(mp.mpc(1.0, 0.5) * y))
         assert abs(f[j] - ref) < 5e-12 * max(abs(ref), 1e-30) + 1e-300
+
+
+# ---- pointing (Eq. C1) ---------------------------------------------------------
+def _unit(theta, phi):
+    return np.stack([np.sin(theta) * np.cos(phi), np.sin(theta) * np.sin(phi), np.cos(theta)])
+
+
+def test_pointing_zero_deflection_is_identity(oracle):
+    rng = np.random.default_rng(5)
+    th, ph = np.arccos(rng.uniform(-1, 1, 1000)), rng.uniform(0, 2 * np.pi, 1000)
+    t2, p2 = oracle.pointing(th, ph, np.zeros(1000), np.zeros(1000))
+    assert np.max(np.abs(t2 - th)) < 1e-17 + 2e-19 * 10 and np.max(np.abs(np.asarray(p2, dtype=np.float64) - ph)) < 1e-15
+
+
+def test_pointing_along_the_meridian_and_along_the_equator(oracle):
+    """Closed forms: alpha_phi = 0 is a rotation about e_phi, i.e. theta' = theta + alpha_theta at the same phi
+    (fixes the sign and direction of e_theta); on the equator alpha_theta = 0 is a rotation about the z axis,
+    phi' = phi + alpha_phi at theta' = pi/2 (fixes e_phi)."""
+    rng = np.random.default_rng(6)
+    th, ph = rng.uniform(0.3, 2.8, 500), rng.uniform(0.3, 6.0, 500)
+    a = rng.uniform(-0.2, 0.2, 500)
+    t2, p2 = oracle.pointing(th, ph, a, np.zeros(500))
+    assert np.max(np.abs(np.asarray(t2 - (np.longdouble(1) * th + a), dtype=np.float64))) < 1e-17
+    assert np.max(np.abs(np.asarray(p2, dtype=np.float64) - ph)) < 1e-15
+    t3, p3 = oracle.pointing(np.full(500, np.pi / 2), ph, np.zeros(500), a)
+    assert np.max(np.abs(np.asarray(t3, dtype=np.float64) - np.pi / 2)) < 1e-15     # pi/2 itself is rounded in binary64
+    assert np.max(np.abs(np.asarray(p3, dtype=np.float64) - (ph + a))) < 1e-15
+
+
+def test_pointing_moves_by_alpha_on_a_great_circle_and_obeys_the_cosine_rule(oracle):
+    """Invariants: n' is the unit vector at angular distance alpha from n, and with psi the angle of the
+    deflection from e_theta (alpha_theta = alpha cos psi) the spherical triangle (pole, n, n') gives
+    cos theta' = cos alpha cos theta - sin alpha sin theta cos psi."""
+    rng = np.random.default_rng(7)
+    n = 2000
+    th, ph = np.arccos(rng.uniform(-1, 1, n)), rng.uniform(0, 2 * np.pi, n)
+    alpha, psi = rng.uniform(1e-6, 0.5, n), rng.uniform(0, 2 * np.pi, n)
+    t2, p2 = oracle.pointing(th, ph, alpha * np.cos(psi), alpha * np.sin(psi))
+    t2, p2 = np.asarray(t2, dtype=np.float64), np.asarray(p2, dtype=np.float64)
+    assert np.all((t2 >= 0) & (t2 <= np.pi) & (p2 >= 0) & (p2 < 2 * np.pi))
+    cosd = np.sum(_unit(th, ph) * _unit(t2, p2), axis=0)
+    assert np.max(np.abs(cosd - np.cos(alpha))) < 5e-16
+    assert np.max(np.abs(np.cos(t2) - (np.cos(alpha) * np.cos(th) - np.sin(alpha) * np.sin(th) * np.cos(psi)))) < 5e-16
+    # a deflection with a positive alpha_phi moves east: the z component of n x n' is positive
+    t4, p4 = oracle.pointing(th, ph, np.zeros(n), alpha)
+    u, v = _unit(th, ph), _unit(np.asarray(t4, dtype=np.float64), np.asarray(p4, dtype=np.float64))
+    assert np.all((u[0] * v[1] - u[1] * v[0])[np.sin(th) > 1e-3] > 0)
