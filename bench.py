@@ -333,6 +333,32 @@ def run_b200(args, rank, world):
         nb = plan.nlm * 16 + npts * 8
         e2e = {"value": job_value(e2e_ms, world), "unit": "ms", "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb,
                "checksum": float(h_map[:1024].double().sum().item())}
+    # pointing (Eq. C1): not part of a step; timed on its own over the same number of points
+    pointing = None
+    if rank == 0:
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(1234)
+        sig = 2.5 * np.pi / (180 * 60)
+        p_t = torch.from_numpy(theta).cuda()
+        p_p = torch.from_numpy(phi).cuda()
+        a_t = sig * torch.randn(npts, dtype=torch.float64, device="cuda", generator=gen)
+        a_p = sig * torch.randn(npts, dtype=torch.float64, device="cuda", generator=gen)
+        for _ in range(3):
+            nusht.nusht_pointing(p_t, p_p, a_t, a_p, stream)
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        p0.record(stream)
+        for _ in range(args.steps):
+            nusht.nusht_pointing(p_t, p_p, a_t, a_p, stream)
+        p1.record(stream)
+        torch.cuda.synchronize()
+        pt_ms = p0.elapsed_time(p1) / args.steps
+        peak, src, _ = measured_peaks()
+        pointing = {"kernel": "k_pointing", "npts": npts, "ms": pt_ms, "bound": "hbm", "algorithmic_bytes": 48 * npts,
+                    "achieved": 48 * npts / (pt_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                    "frac": 48 * npts / (pt_ms * 1e-3) / 1e9 / peak, "peak_source": src,
+                    "note": "outside the timed step; output allocation (2 x npts x 8 B) inside the timed calls"}
+        del p_t, p_p, a_t, a_p
     if rank != 0:
         return
     roofs = stage_rooflines(cfg, plan.info, npts, syn_acc, adj_acc, clocks.get("sm_mhz"))
@@ -352,6 +378,7 @@ def run_b200(args, rank, world):
         # k_deconv_pad, k_h_to_ht, k_interp_mma; adjoint k_spread_mma, k_ht_to_h, k_deconv_trunc,
         # k_legendre_adjoint, k_alm_post
         "gpu_launches": 10 * args.steps,
+        "pointing": pointing,
         "plan": {"ms": plan.info.plan_ms, "workspace_gb": plan.info.workspace_bytes / 1e9,
                  "n_rings": plan.info.n_rings, "n_theta": plan.info.n_theta, "n_theta_fine": plan.info.n_theta_fine,
                  "n_phi_fine": plan.info.n_phi_fine, "kernel_width": plan.info.kernel_width},

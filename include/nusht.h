@@ -152,6 +152,17 @@ NUSHT_API int nusht_stage_spread(nusht_plan_t* plan, const void* map, void* grid
 NUSHT_API int nusht_set_stage_timing(nusht_plan_t* plan, int enable);
 NUSHT_API int nusht_stage_times(nusht_plan_t* plan, int which, float* ms, int n);
 
+/* Pointing for CMB weak lensing (Appendix C, Eq. C1): the positions reached from
+ * (theta_i, phi_i) by the deflection (alpha_theta_i, alpha_phi_i), components along e_theta and e_phi in radians,
+ *   n' = cos(a) n + (sin(a)/a) (alpha_theta e_theta + alpha_phi e_phi),  a = |(alpha_theta, alpha_phi)|,
+ * returned as theta' in [0, pi] and phi' in [0, 2 pi): the point set to hand to nusht_plan.  All six arrays are
+ * DEVICE FP64 of length npts, caller-owned; the outputs may alias the inputs element for element (theta_out ==
+ * theta is fine).  No plan is involved; the kernel is enqueued on `stream` and the call returns without
+ * synchronising.  npts == 0 is a no-op; npts < 0 or a NULL array gives NUSHT_ERR_INVALID_ARG.  The deflection
+ * field itself (Eq. C2, a spin-1 transform of the lensing potential) is an input, not computed here. */
+NUSHT_API int nusht_pointing(int64_t npts, const double* theta, const double* phi, const double* alpha_theta,
+                             const double* alpha_phi, double* theta_out, double* phi_out, void* stream);
+
 NUSHT_API int nusht_plan_info(const nusht_plan_t* plan, nusht_info_t* info);
 NUSHT_API const char* nusht_strerror(int code);
 /* Library version string, e.g. "nusht-b200 0.1 (sm_100a)". */

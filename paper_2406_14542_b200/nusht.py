@@ -22,7 +22,7 @@ EXPORTS = [
     "nusht_plan", "nusht_synthesis", "nusht_adjoint", "nusht_destroy", "nusht_synthesis_host",
     "nusht_adjoint_host", "nusht_host_sync", "nusht_stage_legendre_synthesis", "nusht_stage_legendre_adjoint",
     "nusht_stage_interp", "nusht_stage_spread", "nusht_set_stage_timing", "nusht_stage_times",
-    "nusht_plan_info", "nusht_strerror", "nusht_version",
+    "nusht_plan_info", "nusht_strerror", "nusht_version", "nusht_pointing",
 ]
 
 
@@ -66,6 +66,8 @@ def _load():
     lib.nusht_stage_times.restype = ip
     lib.nusht_plan_info.argtypes = [vp, ctypes.POINTER(NushtInfo)]
     lib.nusht_plan_info.restype = ip
+    lib.nusht_pointing.argtypes = [ctypes.c_int64, vp, vp, vp, vp, vp, vp, vp]
+    lib.nusht_pointing.restype = ip
     lib.nusht_strerror.argtypes = [ip]
     lib.nusht_strerror.restype = ctypes.c_char_p
     lib.nusht_version.restype = ctypes.c_char_p
@@ -217,3 +219,16 @@ def nusht_adjoint(plan, x, alm_out=None, stream=None):
 
 def nusht_destroy(plan):
     plan.destroy()
+
+
+def nusht_pointing(theta, phi, alpha_theta, alpha_phi, stream=None):
+    """Eq. C1: deflected positions (theta', phi') of CUDA float64 points; argument marshalling
+    only, the arithmetic is k_pointing (csrc/pointing.cu)."""
+    n = theta.numel()
+    for a in (theta, phi, alpha_theta, alpha_phi):
+        if not a.is_cuda or a.dtype != torch.float64 or a.numel() != n or not a.is_contiguous():
+            raise TypeError("theta, phi, alpha_theta, alpha_phi must be contiguous CUDA float64 of one length")
+    t2, p2 = torch.empty_like(theta), torch.empty_like(phi)
+    _check(lib.nusht_pointing(n, theta.data_ptr(), phi.data_ptr(), alpha_theta.data_ptr(), alpha_phi.data_ptr(),
+                              t2.data_ptr(), p2.data_ptr(), _stream_ptr(stream)))
+    return t2, p2
