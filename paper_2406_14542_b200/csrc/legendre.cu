@@ -17,7 +17,7 @@
 // One thread owns R north/south ring pairs (Pbar_lm(pi-theta) = (-1)^{l+m} Pbar_lm(theta)): per pair
 // and per two l it issues 2 FMA of recurrence and 4 FMA of accumulation.  Underflow of
 // Pbar_mm ~ sin^m(theta) is handled with a per-pair power-of-two exponent counter: while it is
-// positive the pair is "dead" (true value < 2^-128, LIVE_BITS below) and contributes nothing.
+// positive the pair is "dead" (true value < 2^-96, LIVE_BITS below) and contributes nothing.
 //
 // The CPU oracle (oracle/) uses the plain three-term recurrence in l and shares nothing with this file.
 #include <math.h>
@@ -42,11 +42,14 @@ constexpr int ADJ_R = 5;           // adjoint: 5 pairs per thread amortise the c
 constexpr int ADJ_TN = 128;
 constexpr int ADJ_CHUNK = 8;       // n-steps per transposing reduction / exponent check
 __host__ __device__ constexpr int adj_min_ctas(int r, int c) { return r <= 4 ? (c <= 2 ? 22 : (c <= 4 ? 18 : 16)) : (r == 5 ? 13 : (r == 6 ? 12 : (c <= 2 ? 12 : 10))); }
-// A ring pair is "in range" once |Pbar_lm| >= 2^-LIVE_BITS; below that its terms are dropped (relative to
-// Pbar = O(1) that is 3e-39: no FP64 result can resolve it).  With the counter at 1 the stored value is the
-// true one times 2^512, so the pair comes into range when it passes 2^(512 - LIVE_BITS).
-constexpr int LIVE_BITS = 128;
-constexpr double SCALE_UP_LIMIT = 3.940200619639448e+115;   // 2^(512 - LIVE_BITS) = 2^384
+// A ring pair is "in range" once |Pbar_lm| >= 2^-LIVE_BITS; below that its terms are dropped.  The test runs once
+// per chunk of 8 n-steps, over which Pbar grows by less than 2^32, so the largest dropped term is below
+// 2^(32 - LIVE_BITS) = 2^-64 = 5e-20 relative to Pbar = O(1): no FP64 result can resolve it (LIVE_BITS = 64
+// would drop terms up to 2^-32 and fails the stage test; 128 costs 0.07 ms per direction at lmax = 4095).  With
+// the counter at 1 the stored value is the true one times 2^512, so the pair comes into range when it passes
+// 2^(512 - LIVE_BITS).
+constexpr int LIVE_BITS = 96;
+constexpr double SCALE_UP_LIMIT = 1.6923032801030364e+125;   // 2^(512 - LIVE_BITS) = 2^416
 constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
 
 struct LegParams {
@@ -544,7 +547,7 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
                 }
                 if (w_live) {
                     // some pair in range: 6 FMA per pair and step, no masks.  A pair still below range
-                    // accumulates finite garbage (scaled |p1| stays below 2^416); its sums are cleared when it
+                    // accumulates finite garbage (scaled |p1| stays below 2^448); its sums are cleared when it
                     // comes into range (below) or at the end, which drops exactly the terms < 2^-LIVE_BITS.
                     if (ns == LEG_CHUNK) {
 #pragma unroll
