@@ -51,3 +51,39 @@ def test_fullsize_sampled(oracle, config, nsample):
     lhs = float(np.sum(np.longdouble(f) * np.longdouble(f)))
     assert abs(lhs - oracle.inner_alm(L, M, alm, cf)) <= 1e-12 * lhs
     plan.destroy()
+
+
+@pytest.mark.parametrize("eps", [1e-4, 1e-6])
+def test_fullsize_fp32_sampled(oracle, monkeypatch, eps):
+    """BASELINE.json configs[4], FP32 rows: lmax = 4095 on 67 M points, in the configuration bench.py --eps-sweep
+    times: the gather interpolation with the L2-blocked un-permutation at its default bucket size (16 buckets
+    here).  Sampled outputs against the long-double oracle at the north_star bar for the FP32 path (1e-4 at
+    eps >= 1e-5; at 1e-6 binary32 itself limits the result, 3e-4 as in test_fp32_path), the whole map against the
+    register-window kernel with its direct scatter to binary32 rounding, and every output written exactly once."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2406_14542_b200 import nusht
+    cfg, theta, phi, alm, x = inputs.make_config(3)
+    L, M, npts = cfg["lmax"], cfg["mmax"], cfg["npts"]
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps, dtype="f32")
+    d_alm = cu(alm.astype(np.complex64))
+    f = plan.synthesis(d_alm)
+    rng = np.random.default_rng(98)
+    idx = np.sort(rng.choice(npts, 200, replace=False))
+    idx = np.unique(np.concatenate([idx, [0, npts - 1, np.argmin(theta), np.argmax(theta)]]))
+    f_ref = oracle.synthesis(L, M, theta[idx], phi[idx], alm, "ld")
+    bar = 1e-4 if eps >= 1e-5 else 3e-4
+    assert rel(f[torch.from_numpy(idx).cuda()].cpu().numpy().astype(np.float64), f_ref) <= bar
+    # same plan, register-window kernel with the direct scatter map[perm[j]]: same grid, same weights
+    g = torch.randn(plan.grid_shape(), dtype=torch.float32, device="cuda")
+    f_blocked = plan.stage_interp(g)
+    monkeypatch.setenv("NUSHT_INTERP_F32", "window")
+    f_window = plan.stage_interp(g)
+    monkeypatch.delenv("NUSHT_INTERP_F32")
+    assert float((f_blocked - f_window).abs().max()) <= 4e-6 * float(f_window.abs().max())
+    # every output was written exactly once: no element keeps the sentinel
+    out = torch.full((npts,), float("nan"), dtype=torch.float32, device="cuda")
+    plan.synthesis(d_alm, out)
+    assert not bool(torch.isnan(out).any())
+    assert torch.equal(out, f)
+    plan.destroy()
