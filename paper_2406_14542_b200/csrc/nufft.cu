@@ -526,17 +526,34 @@ k_interp_gather(const __grid_constant__ NufftParams P, const __grid_constant__ K
     if (b0 >= g.nph) b0 -= g.nph;
     int bm = b0 + g.nph / 2;                 // first column on a mirrored row (beyond a pole)
     if (bm >= g.nph) bm -= g.nph;
-    const bool interior = (a0 >= 0) && (a0 + W - 1 <= g.nth / 2) && (b0 + W <= g.nph);
+    // Interior footprints (no pole, no phi wrap) are read as NV aligned column PAIRS per row (64-bit loads:
+    // n_phi is even, so every row starts 8-byte aligned): the W weights are shifted by the parity of b0 into
+    // a (2 NV)-entry row with zeros at the ends, once per point, instead of W 32-bit loads per row.
+    constexpr int NV = W / 2 + 1;
+    const int q = b0 & 1, ba = b0 - q;
+    const bool interior = (a0 >= 0) && (a0 + W - 1 <= g.nth / 2) && (ba + 2 * NV <= g.nph) && ((g.nph & 1) == 0);
     float sum = 0.f;
     if (interior) {
-        const float* src = grid + (int64_t)a0 * g.nph + b0;
+        float ks[2 * NV];
+#pragma unroll
+        for (int j = 0; j < 2 * NV; ++j) {
+            const float lo = (j < W) ? kph[j < W ? j : 0] : 0.f;                  // q = 0: weight j
+            const float hi = (j >= 1 && j - 1 < W) ? kph[(j >= 1 && j - 1 < W) ? j - 1 : 0] : 0.f;   // q = 1: weight j - 1
+            ks[j] = q ? hi : lo;
+        }
+        const float2* src = reinterpret_cast<const float2*>(grid + (int64_t)a0 * g.nph + ba);
+        const int64_t stride2 = g.nph / 2;
 #pragma unroll
         for (int i = 0; i < W; ++i) {
-            float r = 0.f;
+            float r0 = 0.f, r1 = 0.f;
 #pragma unroll
-            for (int j = 0; j < W; ++j) r = fmaf(kph[j], __ldg(src + j), r);
-            sum = fmaf(kt[i], r, sum);
-            src += g.nph;
+            for (int j = 0; j < NV; ++j) {
+                const float2 v = __ldg(src + j);
+                r0 = fmaf(ks[2 * j], v.x, r0);
+                r1 = fmaf(ks[2 * j + 1], v.y, r1);
+            }
+            sum = fmaf(kt[i], r0 + r1, sum);
+            src += stride2;
         }
     } else {
 #pragma unroll
