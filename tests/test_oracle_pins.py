@@ -305,3 +305,92 @@ def test_pointing_moves_by_alpha_on_a_great_circle_and_obeys_the_cosine_rule(ora
     t4, p4 = oracle.pointing(th, ph, np.zeros(n), alpha)
     u, v = _unit(th, ph), _unit(np.asarray(t4, dtype=np.float64), np.asarray(p4, dtype=np.float64))
     assert np.all((u[0] * v[1] - u[1] * v[0])[np.sin(th) > 1e-3] > 0)
+
+
+# ---- the exponent-rescaling regime (O2): where the full-size GPU tests use the oracle as truth ----------------
+# At lmax >= ~1000 most (m, theta) start with Pbar_mm ~ sin^m(theta) far below binary64 range; the value comes back
+# into range through the `renorm` / `sc` refresh inside each copy of the l loop (ring_sum, synthesis,
+# adjoint_columns).  The pins above run at lmax <= 63 (or through oracle_plm / oracle_synthesis only), so a slip in
+# the ring_sum or adjoint copy of that bookkeeping would go unseen; these run every copy in that regime.
+def _near_pole_points(n, seed):
+    rng = np.random.default_rng(seed)
+    th = np.arccos(rng.uniform(-1, 1, n))
+    k = n // 2
+    cap = rng.uniform(0.02, 0.6, k)
+    th[:k] = np.where(rng.random(k) < 0.5, cap, np.pi - cap)
+    th[k] = 1e-3
+    return th, rng.uniform(0, 2 * np.pi, n)
+
+
+@pytest.mark.parametrize("prec,tol", [("d", 1e-14), ("ld", 1e-14)])
+def test_adjoint_identity_rescaling_regime(oracle, prec, tol):
+    """P4 at lmax = mmax = 1500 with half of the points at theta in [0.02, 0.6] and the mirrored cap: sin^m theta
+    leaves the binary64 range for most m there and returns through the sc refresh of BOTH loops (synthesis,
+    adjoint_columns).  <S a, x> = <a, S^T x> in the G3 inner product (Eq. 2-3)."""
+    L = M = 1500
+    th, ph = _near_pole_points(100, 17)
+    a = inputs.random_alm(L, M, 17)
+    x = inputs.random_map(100, 17)
+    f = oracle.synthesis(L, M, th, ph, a, prec)
+    c = oracle.adjoint(L, M, th, ph, x, prec)
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+    rhs = oracle.inner_alm(L, M, a, c)
+    assert abs(lhs - rhs) <= tol * np.linalg.norm(f) * np.linalg.norm(x)
+
+
+@pytest.mark.parametrize("l,m,theta", [(2100, 2000, 0.4), (2100, 300, 0.05), (2100, 2100, 2.9)])
+def test_single_point_adjoint_columns_vs_mpmath_rescaling(oracle, l, m, theta):
+    """Eq. 2 for one point is c_lm = x conj(Y_lm(theta, phi)); Y_lm from the library routine mpmath.spherharm.
+    The seeds are sin(0.4)^2000 ~ 1e-820, sin(0.05)^300 ~ 1e-390 and sin(2.9)^2100 ~ 1e-1300: the value only
+    exists through the rescaling of oracle_adjoint_columns (both precisions)."""
+    mp = pytest.importorskip("mpmath")
+    mp.mp.dps = 40
+    phi, xval = 2.2, 1.7
+    y = mp.spherharm(l, m, mp.mpf(float(theta)), mp.mpf(float(phi)), maxprec=400000)
+    ref = xval * complex(float(mp.re(y)), -float(mp.im(y)))
+    for prec, tol in (("d", 5e-12), ("ld", 5e-13)):
+        col = oracle.adjoint_columns(l, [m], np.array([theta]), np.array([phi]), np.array([xval]), prec)
+        assert abs(col[0, l] - ref) <= tol * abs(ref), (prec, col[0, l], ref)
+        # a column of the full adjoint is the same numbers
+        assert np.all(col[0, :m] == 0)
+
+
+@pytest.mark.parametrize("m", [300, 900, 1500])
+def test_ring_sum_matches_synthesis_rescaling_regime(oracle, m):
+    """ring_sum (the truth of the Legendre stage tests at lmax = 4095 / 8191) against the synthesis entry point
+    (itself pinned to mpmath in that regime above) at lmax = 1500 on rings that include the neighbourhood of both
+    poles: f = 2 Re(F_m e^{i m phi}) for a_lm supported on one m."""
+    L = M = 1500
+    a = inputs.random_alm(L, M, 18)
+    lo = inputs.lm_index(L, m, m)
+    am = a[lo: lo + L - m + 1]
+    th = np.concatenate([np.pi * np.arange(0, 1502, 7) / 1501, [0.02, 0.05, 0.3, np.pi - 0.02, np.pi - 0.3]])
+    only = np.zeros_like(a)
+    only[lo: lo + L - m + 1] = am
+    ph = np.full_like(th, 0.37)
+    for prec in ("d", "ld"):
+        F = oracle.ring_sum(L, m, th, am, prec)
+        f = oracle.synthesis(L, M, th, ph, only, prec)
+        ref = 2 * np.real(F * np.exp(1j * np.asarray(np.longdouble(m) * np.longdouble(ph), dtype=np.float64)))
+        assert np.max(np.abs(f - ref)) <= 2e-13 * np.max(np.abs(f)), (m, prec)
+        assert np.max(np.abs(F)) > 0.1      # the column is not all underflow
+
+
+def test_ring_sum_single_coefficient_vs_mpmath_golden(oracle):
+    """ring_sum with one non-zero a_lm must return a Pbar_lm(theta): against the stored mpmath values at l = 4095
+    and 8191 (tests/golden/plm_mpmath.txt) wherever the value is representable in binary64.  Seeds: sin(1)^2000 ~
+    1e-150, sin(0.08)^300 ~ 1e-330, sin(1)^4000 ~ 1e-300, sin(1.2)^8000 ~ 1e-245, sin(0.02)^100 ~ 1e-170."""
+    a = 1.3 - 0.4j
+    n = 0
+    for l, m, th, frac, ex in _golden():
+        if l < 4095 or ex < -1000:
+            continue
+        am = np.zeros(l - m + 1, dtype=np.complex128)
+        am[-1] = a
+        ref = a * frac * 2.0 ** ex
+        for prec, eps in (("d", 2.0 ** -53), ("ld", 2.0 ** -64)):
+            F = oracle.ring_sum(l, m, np.array([th]), am, prec)[0]
+            tol = eps * (2000.0 + 8.0 * l / max(np.sin(th), 1e-3)) + 2.0 ** -52
+            assert abs(F - ref) <= tol * abs(ref), (l, m, th, prec, F, ref)
+        n += 1
+    assert n >= 8
