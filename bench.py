@@ -103,8 +103,11 @@ def oracle_sample(cfg, theta, phi, alm, x, seconds):
     from oracle import oracle as o
     L, M = cfg["lmax"], cfg["mmax"]
     nlm = inputs.nlm(L, M)
-    # grow the sample until synthesis + adjoint take about `seconds` of wall time (bounded by the sample given)
-    n = max(8, min(len(theta), int(2.0e8 * max(1, o.num_threads()) * 0.25 / nlm)))
+    # One sampling rule for both legs (cpu_baseline and --impl reference): at least 64 points per OpenMP thread (the
+    # oracle's synthesis loop hands out chunks of 64 points: fewer leaves threads idle and under-reports it), then
+    # grown until synthesis + adjoint take about `seconds` of wall time (bounded by the sample given).
+    n = max(64 * max(1, o.num_threads()), int(2.0e8 * max(1, o.num_threads()) * 0.25 / nlm))
+    n = min(len(theta), n)
     while True:
         t0 = time.perf_counter()
         o.synthesis(L, M, theta[:n], phi[:n], alm)
@@ -184,7 +187,7 @@ def ncu_traffic(cfg, npts):
     return d.get("bytes_per_launch", {})
 
 
-def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz):
+def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz, probe):
     """Algorithmic work per stage over its CUDA-event time."""
     hbm, hbm_src, sm_max = measured_peaks()
     L, M = cfg["lmax"], cfg["mmax"]
@@ -197,11 +200,22 @@ def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz):
     nu_bytes = npts * (16 + 8) + grid_bytes
     out = {}
 
-    def alu(name, ms):
-        a = leg_flop / (ms * 1e-3) / 1e12
+    def alu(name, ms, fma_executed):
+        # `achieved` / `frac`: the FP64 FMAs the launch EXECUTES (nusht_plan_info: the (l, m, ring pair) steps left
+        # after the plan-time fast-forward x 3) over its CUDA-event time: at most 1 by construction.  `nominal`: the
+        # SURVEY.md 8(d) count nlm x ceil(N_r/2) x 3 FMA, which includes the below-range steps the kernel skips, so
+        # its ratio to the peak is a speed-up over the plain loop, not a pipe fraction (it exceeds 1 at lmax = 8191).
+        a = 2.0 * fma_executed / (ms * 1e-3) / 1e12
+        an = leg_flop / (ms * 1e-3) / 1e12
         out[name] = {"bound": "alu", "achieved": a, "peak": fp64_peak, "unit": "TFLOP/s", "frac": a / fp64_peak,
                      "traffic": None, "ms": ms,
                      "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x %.0f MHz (max SM clock)" % sm_max,
+                     "peak_measured_dfma": probe.get("dfma"), "peak_measured_dmma": probe.get("dmma"),
+                     "frac_of_measured_dfma": (a / probe["dfma"]) if probe.get("dfma") else None,
+                     "frac_executed": a / fp64_peak,
+                     "executed_fma_per_launch": int(fma_executed),
+                     "nominal": {"fma_per_launch": leg_flop / 2.0, "tflops": an, "ratio_to_peak": an / fp64_peak,
+                                 "note": "SURVEY 8(d) count incl. the below-range steps the kernel skips"},
                      "frac_at_sampled_clock": (a / (fp64_peak * sm_mhz / sm_max)) if sm_mhz else None}
 
     def mem(name, ms, nbytes):
@@ -211,8 +225,8 @@ def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz):
 
     traffic = ncu_traffic(cfg, npts)
 
-    alu("legendre_synthesis", syn_ms["legendre"])
-    alu("legendre_adjoint", adj_ms["legendre"])
+    alu("legendre_synthesis", syn_ms["legendre"], info.legendre_fma_synthesis)
+    alu("legendre_adjoint", adj_ms["legendre"], info.legendre_fma_adjoint)
     mem("interp", syn_ms["interp"], nu_bytes)
     mem("spread", adj_ms["spread"], nu_bytes + grid_bytes)      # + zeroing the grid
     fft_ms = syn_ms["fft_theta"] + syn_ms["deconv_pad"] + syn_ms["fft_fine_theta"] + syn_ms["fft_fine_phi"]
@@ -235,6 +249,7 @@ def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz):
         tf = 2.0 * fma * npts / (out[name]["ms"] * 1e-3) / 1e12
         out[name]["fp64_executed_tflops"] = tf
         out[name]["fp64_frac"] = tf / fp64_peak
+        out[name]["fp64_frac_of_measured_dmma"] = (tf / probe["dmma"]) if probe.get("dmma") else None
     return out
 
 
@@ -284,6 +299,8 @@ def run_b200(args, rank, world):
             dist.barrier()
         torch.cuda.synchronize()
 
+    # FP64 throughput of this device (denominator of the Legendre / nuFFT rooflines), outside the timed region
+    probe = {"dfma": nusht.probe_fp64("dfma"), "dmma": nusht.probe_fp64("dmma")}
     plan.set_stage_timing(False)
     for _ in range(max(args.warmup, 3)):
         step()
@@ -292,10 +309,12 @@ def run_b200(args, rank, world):
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    launches0 = nusht.launch_count()
     e0.record(stream)
     for _ in range(args.steps):                 # the timed region: exactly K steps, nothing else
         step()
     e1.record(stream)
+    launches = nusht.launch_count() - launches0   # kernels of libnusht.so launched inside the timed region (counted)
     barrier()
     ms = e0.elapsed_time(e1) / args.steps
     ms = max_over_ranks(ms, world, "cuda")
@@ -361,7 +380,7 @@ def run_b200(args, rank, world):
         del p_t, p_p, a_t, a_p
     if rank != 0:
         return
-    roofs = stage_rooflines(cfg, plan.info, npts, syn_acc, adj_acc, clocks.get("sm_mhz"))
+    roofs = stage_rooflines(cfg, plan.info, npts, syn_acc, adj_acc, clocks.get("sm_mhz"), probe)
     own = ["legendre_synthesis", "legendre_adjoint", "interp", "spread"]
     dominant = max(own, key=lambda k: roofs[k]["ms"])
     roof = dict(roofs[dominant])
@@ -374,12 +393,18 @@ def run_b200(args, rank, world):
         "synthesis_ms": sum(syn_acc.values()), "adjoint_ms": sum(adj_acc.values()),
         "stage_ms": {"synthesis": syn_acc, "adjoint": adj_acc},
         "roofline": roof, "stage_rooflines": roofs, "clocks": clocks, "e2e": e2e,
-        # our kernels per step (cuFFT kernels and memsets not counted): synthesis k_alm_prep, k_legendre_synth,
-        # k_deconv_pad, k_h_to_ht, k_interp_mma; adjoint k_spread_mma, k_ht_to_h, k_deconv_trunc,
-        # k_legendre_adjoint, k_alm_post
-        "gpu_launches": 10 * args.steps,
+        # kernels of libnusht.so launched inside the timed region, counted by the library (nusht_launch_count);
+        # cuFFT's kernels and memsets are not included
+        "gpu_launches": int(launches),
+        "fp64_probe": {"dfma_tflops": probe["dfma"], "dmma_tflops": probe["dmma"],
+                       "how": "nusht_probe_fp64: dependent-free DFMA / mma.sync.m8n8k4.f64 streams on every SM, CUDA "
+                              "events, best of 10, measured in this run before the timed region"},
         "pointing": pointing,
         "plan": {"ms": plan.info.plan_ms, "workspace_gb": plan.info.workspace_bytes / 1e9,
+                 "sort_ms": plan.info.sort_ms, "sort_algorithmic_bytes": 60 * npts,
+                 "sort_gbs": (60 * npts / (plan.info.sort_ms * 1e-3) / 1e9) if plan.info.sort_ms > 0 else None,
+                 "sort_frac_of_hbm": (60 * npts / (plan.info.sort_ms * 1e-3) / 1e9 / measured_peaks()[0])
+                 if plan.info.sort_ms > 0 else None,
                  "n_rings": plan.info.n_rings, "n_theta": plan.info.n_theta, "n_theta_fine": plan.info.n_theta_fine,
                  "n_phi_fine": plan.info.n_phi_fine, "kernel_width": plan.info.kernel_width},
     }

@@ -101,12 +101,16 @@ typedef struct {
     double sigma;       /* up-sampling factor */
     int64_t workspace_bytes; /* device memory owned by the plan */
     double plan_ms;     /* wall time of nusht_plan (sort + tables + cuFFT plans) */
+    double sort_ms;     /* a6 alone: point keys + histogram, scan, scatter (CUDA events inside nusht_plan) */
+    int64_t legendre_fma_synthesis; /* FP64 FMAs ONE launch of the Legendre synthesis kernel executes: the (l, m, ring */
+    int64_t legendre_fma_adjoint;   /* pair) steps left after the plan-time fast-forward x 3 (measurement: the roofline's
+                                       executed fraction); the adjoint's cross-lane adds are not counted */
 } nusht_info_t;
 
 /* Build a plan: choose grid sizes / kernel width from (lmax, mmax, eps), build recurrence and
  * deconvolution tables, counting-sort the points into strips (planning is done
  * before, and excluded from, the transforms).  Synchronous; may synchronise the device.
- *   lmax >= 0, 0 <= mmax <= lmax, 0 <= npts < 2^31, dtype NUSHT_F64 | NUSHT_F32,
+ *   0 <= lmax <= 32000 (larger: NUSHT_ERR_UNSUPPORTED), 0 <= mmax <= lmax, 0 <= npts < 2^31, dtype NUSHT_F64 | NUSHT_F32,
  *   eps in [1e-13, 1e-1] (F64) or [1e-6, 1e-1] (F32); theta/phi DEVICE pointers (may be NULL iff npts == 0). */
 NUSHT_API int nusht_plan(nusht_plan_t** out, int lmax, int mmax, int64_t npts, const double* theta,
                const double* phi, double eps, int dtype);
@@ -132,6 +136,9 @@ NUSHT_API int nusht_adjoint_host(nusht_plan_t* plan, const void* map_host, void*
 /* Block the calling thread until every host-buffer transform issued so far on this plan has delivered
  * its output. */
 NUSHT_API int nusht_host_sync(nusht_plan_t* plan);
+/* Allocate the device staging buffers and copy streams of the host-buffer calls now (2 x alm + 2 x map of device
+ * memory), so that the first nusht_*_host call allocates nothing either.  Idempotent. */
+NUSHT_API int nusht_host_reserve(nusht_plan_t* plan);
 
 /* Stage entry points (tests and per-stage measurement).
  * Legendre synthesis + DFS doubling alone: alm -> Ftilde, DEVICE complex128
@@ -140,6 +147,15 @@ NUSHT_API int nusht_host_sync(nusht_plan_t* plan);
  * Its transpose (a10-a11): Gtilde (same layout) -> alm. */
 NUSHT_API int nusht_stage_legendre_synthesis(nusht_plan_t* plan, const void* alm, void* ftilde, void* stream);
 NUSHT_API int nusht_stage_legendre_adjoint(nusht_plan_t* plan, const void* gtilde, void* alm, void* stream);
+/* Fourier stage alone (a3 + a4 + a5, and a9): Ftilde (layout above) -> the plan's half fine grid, DEVICE real
+ * [n_theta_fine/2 + 1][n_phi_fine] of the plan's dtype, i.e. the coarse theta FFT, deconvolution by the kernel's
+ * Fourier transform, zero-padding and the fine inverse FFT; and its transpose grid -> Gtilde.
+ * Ftilde must carry the DFS symmetry Ftilde[m][n_theta - r] = (-1)^m Ftilde[m][r] that a2 produces (the fused chains
+ * transform even/odd column pairs together and separate them by it); likewise the Gtilde returned by the transpose
+ * is defined up to components that cancel in the fold of a10, G[k] = Gtilde[k] + (-1)^m Gtilde[n_theta - k].  Both
+ * calls copy through the plan's own buffers (tests and per-stage measurement only). */
+NUSHT_API int nusht_stage_fourier_synthesis(nusht_plan_t* plan, const void* ftilde, void* grid, void* stream);
+NUSHT_API int nusht_stage_fourier_adjoint(nusht_plan_t* plan, const void* grid, void* gtilde, void* stream);
 /* nuFFT stages alone (a7 / a8) on the plan's half fine grid: DEVICE real [n_theta_fine/2 + 1][n_phi_fine]
  * of the plan's dtype; rows outside [0, pi] are reached through the DFS mirror symmetry.
  * interp reads `grid`, writes `map`; spread zeroes `grid` then accumulates `map` into it. */
@@ -164,6 +180,13 @@ NUSHT_API int nusht_pointing(int64_t npts, const double* theta, const double* ph
                              const double* alpha_phi, double* theta_out, double* phi_out, void* stream);
 
 NUSHT_API int nusht_plan_info(const nusht_plan_t* plan, nusht_info_t* info);
+/* Number of kernels of THIS library launched by the process so far (cuFFT's kernels and memsets are not counted);
+ * bench.py reports the difference over its timed region as `gpu_launches`. */
+NUSHT_API int64_t nusht_launch_count(void);
+/* Measurement aid (not part of any transform): FP64 throughput of the current device in TFLOP/s, measured with a
+ * dependent-free instruction stream on every SM, CUDA events, best of 10 launches.  kind 0: DFMA chains (the
+ * instruction of the Legendre kernels); kind 1: DMMA, mma.sync.m8n8k4.f64 (interpolation / spreading).  Synchronous. */
+NUSHT_API int nusht_probe_fp64(int kind, double* tflops);
 NUSHT_API const char* nusht_strerror(int code);
 /* Library version string, e.g. "nusht-b200 0.1 (sm_100a)". */
 NUSHT_API const char* nusht_version(void);

@@ -5,6 +5,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <atomic>
 #include <chrono>
 #include <new>
 
@@ -18,6 +19,13 @@ void nusht_note_cuda_error(cudaError_t e, const char* what, const char* file, in
     if (getenv("NUSHT_VERBOSE")) fprintf(stderr, "[nusht] %s\n", g_last_error);
     cudaGetLastError();   // clear the sticky-free error state
 }
+static std::atomic<long long> g_launches{0};
+cudaError_t nusht_launched() {
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return cudaGetLastError();
+}
+extern "C" int64_t nusht_launch_count(void) { return (int64_t)g_launches.load(std::memory_order_relaxed); }
+
 void nusht_note_cufft_error(int r, const char* what, const char* file, int line) {
     snprintf(g_last_error, sizeof(g_last_error), "cuFFT error %d at %s:%d: %s", r, file, line, what);
     if (getenv("NUSHT_VERBOSE")) fprintf(stderr, "[nusht] %s\n", g_last_error);
@@ -158,6 +166,9 @@ extern "C" int nusht_plan_info(const nusht_plan_t* p, nusht_info_t* info) {
     info->sigma = p->sigma;
     info->workspace_bytes = p->workspace_bytes;
     info->plan_ms = p->plan_ms;
+    info->sort_ms = p->sort_ms;
+    info->legendre_fma_synthesis = p->leg_fma_syn;
+    info->legendre_fma_adjoint = p->leg_fma_adj;
     return NUSHT_OK;
 }
 
@@ -232,6 +243,11 @@ static int host_setup(nusht_plan_s* p) {
     return NUSHT_OK;
 }
 
+extern "C" int nusht_host_reserve(nusht_plan_t* p) {
+    if (!p) return NUSHT_ERR_INVALID_ARG;
+    return host_setup(p);
+}
+
 extern "C" int nusht_synthesis_host(nusht_plan_t* p, const void* alm_host, void* map_host, void* stream) {
     if (!p || !alm_host || (!map_host && p->npts > 0)) return NUSHT_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
@@ -293,6 +309,28 @@ extern "C" int nusht_stage_legendre_adjoint(nusht_plan_t* p, const void* gtilde,
     cudaStream_t s = (cudaStream_t)stream;
     NUSHT_TRY(legendre_adjoint(p, (const double2*)gtilde, s));
     return legendre_alm_post(p, alm, s);
+}
+
+extern "C" int nusht_stage_fourier_synthesis(nusht_plan_t* p, const void* ftilde, void* grid, void* stream) {
+    if (!p || !ftilde || !grid) return NUSHT_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t fbytes = sizeof(double2) * (size_t)(p->mmax + 1) * (size_t)p->lg.nth2;
+    const size_t gbytes = (size_t)p->ng.nrow_half * (size_t)p->ng.nph * real_size(p);
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_ft, ftilde, fbytes, cudaMemcpyDeviceToDevice, s));
+    NUSHT_TRY(fourier_synthesis(p, s, nullptr));
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(grid, p->d_grid, gbytes, cudaMemcpyDeviceToDevice, s));
+    return NUSHT_OK;
+}
+
+extern "C" int nusht_stage_fourier_adjoint(nusht_plan_t* p, const void* grid, void* gtilde, void* stream) {
+    if (!p || !gtilde || !grid) return NUSHT_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t fbytes = sizeof(double2) * (size_t)(p->mmax + 1) * (size_t)p->lg.nth2;
+    const size_t gbytes = (size_t)p->ng.nrow_half * (size_t)p->ng.nph * real_size(p);
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_grid, grid, gbytes, cudaMemcpyDeviceToDevice, s));
+    NUSHT_TRY(fourier_adjoint(p, s, nullptr));
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(gtilde, p->d_ft, fbytes, cudaMemcpyDeviceToDevice, s));
+    return NUSHT_OK;
 }
 
 extern "C" int nusht_stage_interp(nusht_plan_t* p, const void* grid, void* map, void* stream) {

@@ -659,9 +659,9 @@ static int chain_freq_of_pos(int n, int p) {
 }
 
 template <int N, typename C>
-int launch_chain(bool adjoint, int L, int M, int nrow_half, int n_sm, double2* ft, const double* pph,
+int launch_chain(bool* attr_set, bool adjoint, int L, int M, int nrow_half, int n_sm, double2* ft, const double* pph,
                  const ChainTables& tb, C* h, cudaStream_t s) {
-    static bool attr_set[2] = {false, false};
+    // the attribute is per device: the flag lives in the plan (one device), not in the process
     if (!attr_set[adjoint]) {
         if (adjoint)
             NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_theta_chain_adj<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -678,14 +678,13 @@ int launch_chain(bool adjoint, int L, int M, int nrow_half, int n_sm, double2* f
         k_theta_chain_adj<N, C><<<grid, ChainCfg<N>::T, ChainCfg<N>::SMEM, s>>>(L, M, nrow_half, h, pph, tb, ft);
     else
         k_theta_chain_syn<N, C><<<grid, ChainCfg<N>::T, ChainCfg<N>::SMEM, s>>>(L, M, nrow_half, ft, pph, tb, h);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 
 template <int N, typename C>
-int launch_chain2(bool adjoint, int L, int M, int nrow_half, int n_sm, double2* ft, const double* pph,
+int launch_chain2(bool* attr_set, bool adjoint, int L, int M, int nrow_half, int n_sm, double2* ft, const double* pph,
                   const ChainTables& tb, C* h, cudaStream_t s) {
-    static bool attr_set[2] = {false, false};
     if (!attr_set[adjoint]) {
         if (adjoint)
             NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_theta_chain2_adj<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -703,12 +702,12 @@ int launch_chain2(bool adjoint, int L, int M, int nrow_half, int n_sm, double2* 
         k_theta_chain2_adj<N, C><<<grid, HalfCfg<N>::T, HalfCfg<N>::SMEM, s>>>(L, M, nrow_half, h, pph, tb, ft);
     else
         k_theta_chain2_syn<N, C><<<grid, HalfCfg<N>::T, HalfCfg<N>::SMEM, s>>>(L, M, nrow_half, ft, pph, tb, h);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 
 template <typename C>
-int dispatch_chain(const nusht_plan_s* p, bool adjoint, C* h, cudaStream_t s) {
+int dispatch_chain(nusht_plan_s* p, bool adjoint, C* h, cudaStream_t s) {
     const int n = p->lg.nth2;
     ChainTables tb;
     tb.tw2 = p->d_tw2n;
@@ -719,7 +718,7 @@ int dispatch_chain(const nusht_plan_s* p, bool adjoint, C* h, cudaStream_t s) {
         switch (n) {
 #define NUSHT_CHAIN2(NN) \
     case NN:             \
-        return launch_chain2<NN, C>(adjoint, p->lmax, p->mmax, p->ng.nrow_half, p->n_sm, p->d_ft, p->d_pph, tb, h, s);
+        return launch_chain2<NN, C>(p->chain_attr_set, adjoint, p->lmax, p->mmax, p->ng.nrow_half, p->n_sm, p->d_ft, p->d_pph, tb, h, s);
             NUSHT_CHAIN2(2048) NUSHT_CHAIN2(4096) NUSHT_CHAIN2(8192) NUSHT_CHAIN2(16384)
 #undef NUSHT_CHAIN2
         }
@@ -728,7 +727,7 @@ int dispatch_chain(const nusht_plan_s* p, bool adjoint, C* h, cudaStream_t s) {
     switch (n) {
 #define NUSHT_CHAIN(NN) \
     case NN:            \
-        return launch_chain<NN, C>(adjoint, p->lmax, p->mmax, p->ng.nrow_half, p->n_sm, p->d_ft, p->d_pph, tb, h, s);
+        return launch_chain<NN, C>(p->chain_attr_set, adjoint, p->lmax, p->mmax, p->ng.nrow_half, p->n_sm, p->d_ft, p->d_pph, tb, h, s);
         NUSHT_CHAIN(128) NUSHT_CHAIN(256) NUSHT_CHAIN(512) NUSHT_CHAIN(1024) NUSHT_CHAIN(2048) NUSHT_CHAIN(4096)
         NUSHT_CHAIN(8192)
 #undef NUSHT_CHAIN
@@ -895,7 +894,7 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
             k_deconv_pad<double><<<grid, 256, 0, s>>>(L, M, nth2, g.nth / 2, p->d_ft, p->d_pth, p->d_pph, (double2*)p->d_h);
         else
             k_deconv_pad<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth / 2, p->d_ft, p->d_pth, p->d_pph, (float2*)p->d_h);
-        NUSHT_CUDA_TRY(cudaGetLastError());
+        NUSHT_CUDA_TRY(nusht_launched());
     }
     REC(2);
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_fine, s));
@@ -916,7 +915,7 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
         else
             k_h_to_z<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, p->d_twz, (const float2*)p->d_h,
                                                    (float2*)p->d_grid);
-        NUSHT_CUDA_TRY(cudaGetLastError());
+        NUSHT_CUDA_TRY(nusht_launched());
     }
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi, s));
     if (f64)
@@ -952,7 +951,7 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
         else
             k_z_to_h<float2><<<grid, 256, 0, s>>>(M, g.nth / 2, g.nrow_half, nz, !p->theta_fused, p->d_twz, (const float2*)p->d_grid,
                                                    (float2*)p->d_h);
-        NUSHT_CUDA_TRY(cudaGetLastError());
+        NUSHT_CUDA_TRY(nusht_launched());
     }
     REC(1);
     if (p->theta_fused) {
@@ -980,7 +979,7 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
         else
             k_deconv_trunc<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth / 2, (const float2*)p->d_h, p->d_pth, p->d_pph,
                                                        p->d_ft);
-        NUSHT_CUDA_TRY(cudaGetLastError());
+        NUSHT_CUDA_TRY(nusht_launched());
     }
     REC(3);
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_coarse, s));

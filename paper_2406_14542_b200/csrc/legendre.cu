@@ -11,6 +11,11 @@
 // c_l^2 = (l^2-m^2)/(4 l^2-1):
 //   even class  q_n = Pbar_{m+2n}:   q_{n+1} = A_n (x^2 - D_n) q_n - C_n q_{n-1}
 //   scaled      q_n = sigma_n qh_n:  qh_{n+1} = (alpha_n x^2 + beta_n) qh_n + qh_{n-1}      (2 FMA)
+//               evaluated as  t_n = (alpha_n + beta_n) - alpha_n sin^2(theta):  next to the poles x^2 = cos^2(theta)
+//               rounds with an absolute error of 1e-16, the SAME error for every n of a ring, i.e. a coherent
+//               shift of theta by 1e-16 / sin(2 theta) that grows to l * shift in the phase of Pbar_lm; sin^2 is
+//               small there and carries a relative error instead.  The tables hold
+//               (-alpha_n, alpha_n + beta_n) and sin^2(theta_j), the kernels do one FMA as before.
 //   odd class   Pbar_{m+2n+1} = (x q_n - c_{m+2n} Pbar_{m+2n-1})/c_{m+2n+1}  is folded into the
 //               coefficients once per transform (O(lmax^2)):  sum_n b_n Pbar_{m+2n+1} =
 //               x sum_j (r_j/c_{m+2j+1}) q_j,  r_j = b_j - rho_j r_{j+1},  rho_j = c_{m+2j+2}/c_{m+2j+3}.
@@ -64,7 +69,7 @@ struct LegParams {
     const int2* items;
     const int64_t* eoff;
     const double2* ab;
-    const double* x2;
+    const double* x2;      // sin^2(theta_j) per ring pair (the operand of the x^2-stepping recurrence, header)
     const double* x;
     const double2* logsin;
     const double2* logkap;
@@ -127,7 +132,7 @@ __global__ void k_legendre_tables(int L, int M, const int64_t* __restrict__ eoff
         const double C = sqrt(c2l * c2lm1) * A;
         const double sg_next = (n == 0) ? 1.0 : -C * sg_prev;
         const double alpha = A * sg / sg_next;
-        ab[o + n] = make_double2(alpha, -alpha * D);
+        ab[o + n] = make_double2(-alpha, alpha * (1.0 - D));   // t_n = ab.y + ab.x sin^2(theta) = alpha (x^2 - D)
         sig[o + n] = sg;
         sodd[o + n] = sg / sqrt(c2l1);
         rho[o + n] = sqrt(c2l2 / c2l3);
@@ -862,12 +867,36 @@ static int dev_alloc(T** ptr, size_t count, nusht_plan_s* p) {
 // into range go last and only write their zeros.  The adjoint kernel keeps its 2-D grid: it sits exactly at
 // 128 registers and the list lookup made it spill (4.2 -> 4.9 ms), and its blocks of one m should run together
 // anyway (they add into the same eo[m] column while it is L2-resident).
+// FP64 FMAs one launch executes with R ring pairs per thread: every warp runs 6 FMA (2 recurrence + 4 accumulation)
+// per lane, ring pair and n-step from its fast-forward step to the end of the column (pairs of a live warp that are
+// still below range execute them too); the remainder pairs run whole columns.
+static int64_t executed_fma(const nusht_plan_s* p, int R, const LegParams& P, const std::vector<int>& ffn) {
+    const int M = p->mmax, L = p->lmax;
+    int64_t steps = 0;
+    for (int m = 0; m <= M; ++m) {
+        const int ne = (L - m) / 2 + 1;
+        for (int b = 0; b < P.nblk; ++b) steps += (int64_t)std::max(0, ne - ffn[(size_t)m * P.nblk + b]) * 32 * R;
+        steps += (int64_t)ne * P.rem;
+    }
+    return 6 * steps;
+}
+
 static int build_work_list(nusht_plan_s* p, int R, const int* d_ff_n, int2** d_items, int* n_items) {
     LegParams P = make_params(p);
     leg_grid(p, R, P);
     const int M = p->mmax, L = p->lmax;
     std::vector<int> ffn((size_t)(M + 1) * P.nblk);
     NUSHT_CUDA_TRY(cudaMemcpy(ffn.data(), d_ff_n, sizeof(int) * ffn.size(), cudaMemcpyDeviceToHost));
+    p->leg_fma_syn = executed_fma(p, R, P, ffn);
+    if (ADJ_R != LEG_R) {
+        LegParams Pa = make_params(p, true);
+        leg_grid(p, ADJ_R, Pa);
+        std::vector<int> ffa((size_t)(M + 1) * Pa.nblk);
+        NUSHT_CUDA_TRY(cudaMemcpy(ffa.data(), p->d_ffa_n, sizeof(int) * ffa.size(), cudaMemcpyDeviceToHost));
+        p->leg_fma_adj = executed_fma(p, ADJ_R, Pa, ffa);
+    } else {
+        p->leg_fma_adj = p->leg_fma_syn;
+    }
     std::vector<int2> items;
     items.reserve(ffn.size() + (size_t)M + 1);
     if (P.rem > 0) {
@@ -917,7 +946,7 @@ int legendre_build_tables(nusht_plan_s* p) {
         const int threads = 32;
         k_legendre_tables<<<(M + 1 + threads - 1) / threads, threads>>>(L, M, p->d_eoff, p->d_ab, p->d_sig,
                                                                          p->d_sodd, p->d_rho);
-        NUSHT_CUDA_TRY(cudaGetLastError());
+        NUSHT_CUDA_TRY(nusht_launched());
     }
     // ring tables in extended precision on the host: theta_j = pi j/(nr-1)
     const long double PI_L = 3.14159265358979323846264338327950288L;
@@ -928,7 +957,8 @@ int legendre_build_tables(nusht_plan_s* p) {
         long double c = cosl(th), s = sinl(th);
         if (g.has_equator && j == g.npairs - 1) c = 0.0L;
         x[j] = (double)c;
-        x2[j] = (double)(c * c);
+        x2[j] = (double)(s * s);          // the kernels' "x2" operand is sin^2(theta): see the header
+        if (g.has_equator && j == g.npairs - 1) x2[j] = 1.0;
         if (j == 0) {
             ls[j] = make_double2(0.0, 0.0);   // unused: poles are special-cased
         } else {
@@ -964,7 +994,7 @@ int legendre_build_tables(nusht_plan_s* p) {
         NUSHT_TRY(dev_alloc(&p->d_ff_p, nw * LEG_R * 32, p));
         NUSHT_TRY(dev_alloc(&p->d_ff_e, nw * LEG_R * 32, p));
         k_legendre_fastforward<LEG_R><<<dim3(P.nblk, M + 1), 32>>>(P, p->d_ff_n, p->d_ff_p, p->d_ff_e);
-        NUSHT_CUDA_TRY(cudaGetLastError());
+        NUSHT_CUDA_TRY(nusht_launched());
         (void)grid;
     }
     if (ADJ_R != LEG_R) {
@@ -975,7 +1005,7 @@ int legendre_build_tables(nusht_plan_s* p) {
         NUSHT_TRY(dev_alloc(&p->d_ffa_p, nw * ADJ_R * 32, p));
         NUSHT_TRY(dev_alloc(&p->d_ffa_e, nw * ADJ_R * 32, p));
         k_legendre_fastforward<ADJ_R><<<dim3(P.nblk, M + 1), 32>>>(P, p->d_ffa_n, p->d_ffa_p, p->d_ffa_e);
-        NUSHT_CUDA_TRY(cudaGetLastError());
+        NUSHT_CUDA_TRY(nusht_launched());
     }
     NUSHT_CUDA_TRY(cudaDeviceSynchronize());
     NUSHT_TRY(build_work_list(p, LEG_R, p->d_ff_n, &p->d_items_syn, &p->n_items_syn));
@@ -990,7 +1020,7 @@ int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s) {
     else
         k_alm_prep<float><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, (const float*)alm, p->d_sig,
                                                      p->d_sodd, p->d_rho, p->d_aeo);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 
@@ -999,7 +1029,7 @@ int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s) {
     leg_grid(p, LEG_R, P);
     if (p->n_items_syn == 0) return NUSHT_OK;
     k_legendre_synth<LEG_R><<<p->n_items_syn, SYN_THREADS, 0, s>>>(P, p->d_aeo, ft);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 
@@ -1009,7 +1039,7 @@ int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
     LegParams P = make_params(p, true);
     const dim3 grid = leg_grid(p, ADJ_R, P);
     k_legendre_adjoint<ADJ_R, ADJ_CHUNK><<<grid, 32, 0, s>>>(P, gt, p->d_aeo);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 
@@ -1021,7 +1051,7 @@ int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s) {
     else
         k_alm_post<float><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, p->d_aeo, p->d_sig, p->d_sodd,
                                                      p->d_rho, (float*)alm);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 

@@ -24,6 +24,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <type_traits>
 #include <vector>
 
@@ -704,7 +705,7 @@ int launch_interp(const NufftParams& P, const KernelHost& h, const void* grid, v
     constexpr int NU_WARPS = nu_warps<W, T>();
     const int blocks = (P.n_items + NU_WARPS - 1) / NU_WARPS;
     k_interp<W, T><<<blocks, NU_WARPS * 32, 0, s>>>(P, kp, (const T*)grid, (T*)map);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 template <int W, typename T>
@@ -713,7 +714,7 @@ int launch_spread(const NufftParams& P, const KernelHost& h, const void* map, vo
     constexpr int NU_WARPS = nu_warps<W, T>();
     const int blocks = (P.n_items + NU_WARPS - 1) / NU_WARPS;
     k_spread<W, T><<<blocks, NU_WARPS * 32, 0, s>>>(P, kp, (const T*)map, (T*)grid);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 
@@ -723,7 +724,7 @@ int launch_interp_gather(const NufftParams& P, const KernelHost& h, int64_t npts
     const KernelPoly<float> kp = make_device_poly<float>(h);
     const unsigned blocks = (unsigned)((npts + GATHER_THREADS - 1) / GATHER_THREADS);
     k_interp_gather<W><<<blocks, GATHER_THREADS, 0, s>>>(P, kp, npts, (const float*)grid, (float*)map);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 int dispatch_interp_gather(int w, const NufftParams& P, const KernelHost& h, int64_t npts, const void* grid, void* map,
@@ -1199,14 +1200,14 @@ int launch_interp_mma(const NufftParams& P, const KernelHost& h, const void* gri
     const KernelPoly<double> kp = make_device_poly<double>(h);
     constexpr int NW = mma_interp_warps(W);
     k_interp_mma<W><<<(P.n_items + NW - 1) / NW, 32 * NW, 0, s>>>(P, kp, (const double*)grid, (double*)map);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 template <int W>
 int launch_spread_mma(const NufftParams& P, const KernelHost& h, const void* map, void* grid, cudaStream_t s) {
     const KernelPoly<double> kp = make_device_poly<double>(h);
     k_spread_mma<W><<<(P.n_items + 3) / 4, 128, 0, s>>>(P, kp, (const double*)map, (double*)grid);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
 
@@ -1332,7 +1333,8 @@ int nufft_choose_kernel(nusht_plan_s* p) {
 double nufft_kernel_ft(const nusht_plan_s* p, double k, int n) {
     const KernelHost* h = g_kernel_of(p);
     static std::vector<long double> xg, wg;
-    if (xg.empty()) gauss_legendre(32, xg, wg);
+    static std::once_flag once;
+    std::call_once(once, [] { gauss_legendre(32, xg, wg); });
     const long double PI_L = 3.14159265358979323846264338327950288L;
     long double tot = 0;
     for (int i = 0; i < h->w; ++i) {
@@ -1377,10 +1379,14 @@ int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi) {
     sg.inv_hth = g.inv_hth; sg.inv_hph = g.inv_hph; sg.half_w = 0.5 * g.w;
 
     int *d_keys = nullptr, *d_hist = nullptr, *d_off = nullptr, *d_tot = nullptr, *d_bad = nullptr;
+    cudaEvent_t ev_sort[2] = {nullptr, nullptr};
     const int ntiles = (nbins + 1 + SCAN_TILE - 1) / SCAN_TILE;
     int status = NUSHT_OK;
     auto cleanup = [&]() {
         cudaFree(d_keys); cudaFree(d_hist); cudaFree(d_off); cudaFree(d_tot); cudaFree(d_bad);
+        if (ev_sort[0]) cudaEventDestroy(ev_sort[0]);
+        if (ev_sort[1]) cudaEventDestroy(ev_sort[1]);
+        ev_sort[0] = ev_sort[1] = nullptr;
     };
 #define SORT_TRY(expr)                                                              \
     do {                                                                            \
@@ -1398,11 +1404,14 @@ int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi) {
     SORT_TRY(cudaMalloc((void**)&d_bad, sizeof(int)));
     SORT_TRY(cudaMemset(d_hist, 0, sizeof(int) * ((size_t)nbins + 1)));
     SORT_TRY(cudaMemset(d_bad, 0, sizeof(int)));
+    SORT_TRY(cudaEventCreate(&ev_sort[0]));
+    SORT_TRY(cudaEventCreate(&ev_sort[1]));
+    SORT_TRY(cudaEventRecord(ev_sort[0], 0));
     if (n > 0) {
         const int threads = 256;
         const unsigned blocks = (unsigned)((n + threads - 1) / threads);
         k_point_keys<<<blocks, threads>>>(sg, n, theta, phi, d_keys, d_hist, d_bad);
-        SORT_TRY(cudaGetLastError());
+        SORT_TRY(nusht_launched());
         int bad = 0;
         SORT_TRY(cudaMemcpy(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost));
         if (bad != 0) {
@@ -1411,20 +1420,26 @@ int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi) {
         }
     }
     k_scan_tiles<<<ntiles, SCAN_BLOCK>>>(d_hist, d_off, d_tot, nbins + 1);
-    SORT_TRY(cudaGetLastError());
+    SORT_TRY(nusht_launched());
     k_scan_totals<<<1, 1024>>>(d_tot, ntiles);
-    SORT_TRY(cudaGetLastError());
+    SORT_TRY(nusht_launched());
     k_scan_add<<<ntiles, SCAN_BLOCK>>>(d_off, d_tot, nbins + 1);
-    SORT_TRY(cudaGetLastError());
+    SORT_TRY(nusht_launched());
     k_item_offsets<<<(p->n_items + 1 + 255) / 256, 256>>>(d_off, p->d_item_off, p->n_items, (int)n);
-    SORT_TRY(cudaGetLastError());
+    SORT_TRY(nusht_launched());
     if (n > 0) {
         const int threads = 256;
         const unsigned blocks = (unsigned)((n + threads - 1) / threads);
         k_point_scatter<<<blocks, threads>>>(sg, n, theta, phi, d_keys, d_off, p->d_px, p->d_py, p->d_perm);
-        SORT_TRY(cudaGetLastError());
+        SORT_TRY(nusht_launched());
     }
+    SORT_TRY(cudaEventRecord(ev_sort[1], 0));
     SORT_TRY(cudaDeviceSynchronize());
+    {
+        float ms = 0.f;
+        SORT_TRY(cudaEventElapsedTime(&ms, ev_sort[0], ev_sort[1]));
+        p->sort_ms = ms;      // includes the 4-byte device->host read of the bad-point counter between keys and scan
+    }
     cleanup();
     d_keys = d_hist = d_off = d_tot = d_bad = nullptr;
     // L2-blocked un-permutation tables (FP32 gather interpolation; see k_unpermute)
@@ -1451,15 +1466,15 @@ int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi) {
         SORT_TRY(cudaMalloc((void**)&d_tot, sizeof(int) * (size_t)nt));
         const int blocks = (nchunks + BUCKET_WARPS - 1) / BUCKET_WARPS;
         k_bucket_count<<<blocks, 32 * BUCKET_WARPS>>>(p->d_perm, n, bshift, nchunks, d_hist);
-        SORT_TRY(cudaGetLastError());
+        SORT_TRY(nusht_launched());
         k_scan_tiles<<<nt, SCAN_BLOCK>>>(d_hist, d_off, d_tot, ncnt);
-        SORT_TRY(cudaGetLastError());
+        SORT_TRY(nusht_launched());
         k_scan_totals<<<1, 1024>>>(d_tot, nt);
-        SORT_TRY(cudaGetLastError());
+        SORT_TRY(nusht_launched());
         k_scan_add<<<nt, SCAN_BLOCK>>>(d_off, d_tot, ncnt);
-        SORT_TRY(cudaGetLastError());
+        SORT_TRY(nusht_launched());
         k_bucket_place<<<blocks, 32 * BUCKET_WARPS>>>(p->d_perm, n, bshift, nchunks, d_off, p->d_slot, p->d_dest);
-        SORT_TRY(cudaGetLastError());
+        SORT_TRY(nusht_launched());
         SORT_TRY(cudaDeviceSynchronize());
         cleanup();
         p->n_buckets = nb;
@@ -1495,7 +1510,7 @@ int nufft_interp(nusht_plan_s* p, const void* grid, void* map, cudaStream_t s) {
         NUSHT_TRY(dispatch_interp_gather(p->ng.w, Q, *h, p->npts, grid, p->d_stage, s));
         k_unpermute<float><<<(unsigned)((p->npts + 255) / 256), 256, 0, s>>>((const float*)p->d_stage, p->d_dest,
                                                                            p->npts, (float*)map);
-        NUSHT_CUDA_TRY(cudaGetLastError());
+        NUSHT_CUDA_TRY(nusht_launched());
         return NUSHT_OK;
     }
     return dispatch_interp<float>(p->ng.w, P, *h, grid, map, s);

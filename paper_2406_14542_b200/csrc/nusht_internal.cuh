@@ -33,6 +33,8 @@
     } while (0)
 
 void nusht_note_cuda_error(cudaError_t e, const char* what, const char* file, int line);
+// called once after every launch of one of OUR kernels: counts it (nusht_launch_count) and returns cudaGetLastError()
+cudaError_t nusht_launched();
 void nusht_note_cufft_error(int r, const char* what, const char* file, int line);
 
 // ---- nuFFT geometry ------------------------------------------------------------------------
@@ -69,15 +71,17 @@ struct nusht_plan_s {
     NufftGeom ng{};
     int64_t workspace_bytes = 0;
     double plan_ms = 0;
+    double sort_ms = 0;             // a6 alone (keys + histogram, scan, scatter), CUDA events
+    int64_t leg_fma_syn = 0, leg_fma_adj = 0;   // FP64 FMAs one Legendre launch executes (after the plan-time fast-forward)
 
     // --- Legendre tables (device) ---
     int64_t* d_eoff = nullptr;      // [mmax+2] offsets of column m in the per-(m,n) tables
     int64_t n_e_total = 0;          // sum_m ne(m)
-    double2* d_ab = nullptr;        // (alpha_n, beta_n) of the x^2-stepping recurrence
+    double2* d_ab = nullptr;        // (-alpha_n, alpha_n + beta_n) of the x^2-stepping recurrence
     double* d_sig = nullptr;        // sigma_n: even-class scaling
     double* d_sodd = nullptr;       // sigma_n / c_{m+2n+1}: odd-class scaling
     double* d_rho = nullptr;        // c_{m+2n+2}/c_{m+2n+3}: odd-class fold ratio
-    double* d_x2 = nullptr;         // cos^2(theta_j) per ring pair
+    double* d_x2 = nullptr;         // sin^2(theta_j) per ring pair (t_n = ab.y + ab.x sin^2 theta)
     double* d_x = nullptr;          // cos(theta_j)
     double2* d_logsin = nullptr;    // log2 sin(theta_j) as (hi, lo)
     double2* d_logkap = nullptr;    // log2 |Pbar_mm| prefactor per m as (hi, lo)
@@ -106,6 +110,7 @@ struct nusht_plan_s {
     bool theta_fused = false;       // a3 + a4 + a5-theta (and their transposes) as one kernel per direction (fourier.cu)
     double2* d_tw2n = nullptr;      // tables of the fused theta chains (twiddles, position-ordered deconvolution factors)
     int n_sm = 0;                   // SM count of the plan's device (persistent grids)
+    bool chain_attr_set[2] = {false, false};   // MaxDynamicSharedMemorySize set for this plan's device (syn, adj)
     // --- points ---
     double* d_px = nullptr;         // sorted theta in fine-grid units
     double* d_py = nullptr;         // sorted phi in fine-grid units

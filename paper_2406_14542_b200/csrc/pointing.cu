@@ -61,6 +61,6 @@ extern "C" int nusht_pointing(int64_t npts, const double* theta, const double* p
     if (blocks > (int64_t)n_sm * 8) blocks = (int64_t)n_sm * 8;
     k_pointing<<<(unsigned)blocks, PT_THREADS, 0, (cudaStream_t)stream>>>(npts, theta, phi, alpha_theta, alpha_phi,
                                                                          theta_out, phi_out);
-    NUSHT_CUDA_TRY(cudaGetLastError());
+    NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }

@@ -22,7 +22,8 @@ EXPORTS = [
     "nusht_plan", "nusht_synthesis", "nusht_adjoint", "nusht_destroy", "nusht_synthesis_host",
     "nusht_adjoint_host", "nusht_host_sync", "nusht_stage_legendre_synthesis", "nusht_stage_legendre_adjoint",
     "nusht_stage_interp", "nusht_stage_spread", "nusht_set_stage_timing", "nusht_stage_times",
-    "nusht_plan_info", "nusht_strerror", "nusht_version", "nusht_pointing",
+    "nusht_plan_info", "nusht_strerror", "nusht_version", "nusht_pointing", "nusht_host_reserve",
+    "nusht_stage_fourier_synthesis", "nusht_stage_fourier_adjoint", "nusht_launch_count", "nusht_probe_fp64",
 ]
 
 
@@ -33,7 +34,8 @@ class NushtInfo(ctypes.Structure):
         ("n_rings", ctypes.c_int), ("n_theta", ctypes.c_int), ("n_theta_fine", ctypes.c_int),
         ("n_phi_fine", ctypes.c_int), ("kernel_width", ctypes.c_int), ("kernel_degree", ctypes.c_int),
         ("kernel_beta", ctypes.c_double), ("sigma", ctypes.c_double),
-        ("workspace_bytes", ctypes.c_int64), ("plan_ms", ctypes.c_double),
+        ("workspace_bytes", ctypes.c_int64), ("plan_ms", ctypes.c_double), ("sort_ms", ctypes.c_double),
+        ("legendre_fma_synthesis", ctypes.c_int64), ("legendre_fma_adjoint", ctypes.c_int64),
     ]
 
 
@@ -52,7 +54,7 @@ def _load():
     lib.nusht_plan.argtypes = [ctypes.POINTER(vp), ip, ip, ctypes.c_int64, vp, vp, ctypes.c_double, ip]
     for name in ("nusht_synthesis", "nusht_adjoint", "nusht_synthesis_host", "nusht_adjoint_host",
                  "nusht_stage_legendre_synthesis", "nusht_stage_legendre_adjoint", "nusht_stage_interp",
-                 "nusht_stage_spread"):
+                 "nusht_stage_spread", "nusht_stage_fourier_synthesis", "nusht_stage_fourier_adjoint"):
         getattr(lib, name).argtypes = [vp, vp, vp, vp]
         getattr(lib, name).restype = ip
     lib.nusht_plan.restype = ip
@@ -60,6 +62,12 @@ def _load():
     lib.nusht_destroy.restype = ip
     lib.nusht_host_sync.argtypes = [vp]
     lib.nusht_host_sync.restype = ip
+    lib.nusht_host_reserve.argtypes = [vp]
+    lib.nusht_host_reserve.restype = ip
+    lib.nusht_launch_count.argtypes = []
+    lib.nusht_launch_count.restype = ctypes.c_int64
+    lib.nusht_probe_fp64.argtypes = [ip, ctypes.POINTER(ctypes.c_double)]
+    lib.nusht_probe_fp64.restype = ip
     lib.nusht_set_stage_timing.argtypes = [vp, ip]
     lib.nusht_set_stage_timing.restype = ip
     lib.nusht_stage_times.argtypes = [vp, ip, ctypes.POINTER(ctypes.c_float), ip]
@@ -97,9 +105,16 @@ class Plan:
 
     def __init__(self, lmax, mmax, theta, phi, eps, dtype="f64"):
         self._h = ctypes.c_void_p()
-        self.dtype = NUSHT_F64 if dtype in ("f64", NUSHT_F64) else NUSHT_F32
+        if dtype in ("f64", NUSHT_F64):
+            self.dtype = NUSHT_F64
+        elif dtype in ("f32", NUSHT_F32):
+            self.dtype = NUSHT_F32
+        else:
+            raise ValueError("dtype must be 'f64' or 'f32'")
         npts = 0 if theta is None else int(theta.numel())
         if npts:
+            if phi is None or int(phi.numel()) != npts:
+                raise ValueError("theta and phi must have the same number of entries")
             if not (theta.is_cuda and phi.is_cuda and theta.dtype == torch.float64 and phi.dtype == torch.float64):
                 raise TypeError("theta/phi must be CUDA float64 tensors")
             theta, phi = theta.contiguous(), phi.contiguous()
@@ -160,6 +175,10 @@ class Plan:
                                       _stream_ptr(stream)))
         return out_host
 
+    def host_reserve(self):
+        """Allocate the staging buffers of the host-buffer calls now (nusht_host_reserve)."""
+        _check(lib.nusht_host_reserve(self._h))
+
     def host_sync(self):
         """Wait until every host-buffer transform issued so far has delivered its output."""
         _check(lib.nusht_host_sync(self._h))
@@ -180,6 +199,22 @@ class Plan:
 
     def grid_shape(self):
         return (self.info.n_theta_fine // 2 + 1, self.info.n_phi_fine)
+
+    def stage_fourier_synthesis(self, ft, stream=None):
+        if ft.dtype != torch.complex128 or tuple(ft.shape) != (self.mmax + 1, self.info.n_theta) or not ft.is_cuda:
+            raise TypeError("ftilde must be CUDA complex128 [(mmax+1), n_theta]")
+        out = torch.empty(self.grid_shape(), dtype=self.rdtype, device="cuda")
+        _check(lib.nusht_stage_fourier_synthesis(self._h, ft.contiguous().data_ptr(), out.data_ptr(),
+                                                 _stream_ptr(stream)))
+        return out
+
+    def stage_fourier_adjoint(self, grid, stream=None):
+        if grid.dtype != self.rdtype or tuple(grid.shape) != self.grid_shape() or not grid.is_cuda:
+            raise TypeError("grid must be CUDA %s %s" % (self.rdtype, self.grid_shape()))
+        out = torch.empty((self.mmax + 1, self.info.n_theta), dtype=torch.complex128, device="cuda")
+        _check(lib.nusht_stage_fourier_adjoint(self._h, grid.contiguous().data_ptr(), out.data_ptr(),
+                                               _stream_ptr(stream)))
+        return out
 
     def stage_interp(self, grid, stream=None):
         if grid.dtype != self.rdtype or tuple(grid.shape) != self.grid_shape() or not grid.is_cuda:
@@ -202,6 +237,18 @@ class Plan:
         _check(lib.nusht_stage_times(self._h, 0 if which in (0, "synthesis") else 1, buf, NUM_STAGES))
         names = SYN_STAGES if which in (0, "synthesis") else ADJ_STAGES
         return {n: float(buf[i]) for i, n in enumerate(names)}
+
+
+def launch_count() -> int:
+    """Kernels of this library launched so far in this process (nusht_launch_count)."""
+    return int(lib.nusht_launch_count())
+
+
+def probe_fp64(kind: str) -> float:
+    """Measured FP64 throughput of the current device in TFLOP/s: kind 'dfma' or 'dmma' (nusht_probe_fp64)."""
+    v = ctypes.c_double()
+    _check(lib.nusht_probe_fp64({"dfma": 0, "dmma": 1}[kind], ctypes.byref(v)))
+    return float(v.value)
 
 
 def nusht_plan(lmax, mmax, npts, theta, phi, eps, dtype="f64"):

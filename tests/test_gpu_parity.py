@@ -79,7 +79,8 @@ def test_legendre_synthesis_large_l_rescaling(nusht, oracle):
         if m == 0:
             am = am.real + 0j
         F = oracle.ring_sum(L, m, th, am, "ld")
-        tol = 2e-10 if m < 3 else 5e-12     # low m: cos(theta)^2 rounding next to the poles
+        tol = 2e-11 if m < 3 else 5e-12     # low m: the rings next to the poles carry most of the column's norm and
+                                            # the recurrence is worst conditioned there
         assert np.linalg.norm(ft[m, :nr] - F) <= tol * np.linalg.norm(F), m
         r = np.arange(nr, nth2)
         assert np.array_equal(ft[m, nr:], (-1) ** m * ft[m, nth2 - r]), m
@@ -273,7 +274,7 @@ def test_fp32_path(nusht, oracle, eps, L, M, npts):
     f = plan.synthesis(cu(alm.astype(np.complex64))).cpu().numpy()
     c = plan.adjoint(cu(x.astype(np.float32))).cpu().numpy()
     assert f.dtype == np.float32 and c.dtype == np.complex64
-    bar = max(1e-4, 10 * eps) if eps >= 1e-5 else 3e-4     # eps = 1e-6 asks for more than binary32 carries
+    bar = max(1e-4, 10 * eps) if eps >= 1e-5 else 2e-5     # eps = 1e-6: binary32 I/O and grid limit the result to ~1e-6
     assert rel(f.astype(np.float64), oracle.synthesis(L, M, theta, phi, alm, "ld")) <= bar
     assert rel(c.astype(np.complex128), oracle.adjoint(L, M, theta, phi, x, "ld")) <= bar
     assert np.all(c[: L + 1].imag == 0)
