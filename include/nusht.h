@@ -175,9 +175,46 @@ NUSHT_API int nusht_stage_times(nusht_plan_t* plan, int which, float* ms, int n)
  * DEVICE FP64 of length npts, caller-owned; the outputs may alias the inputs element for element (theta_out ==
  * theta is fine).  No plan is involved; the kernel is enqueued on `stream` and the call returns without
  * synchronising.  npts == 0 is a no-op; npts < 0 or a NULL array gives NUSHT_ERR_INVALID_ARG.  The deflection
- * field itself (Eq. C2, a spin-1 transform of the lensing potential) is an input, not computed here. */
+ * field itself (Eq. C2) is an input here; nusht_ring_gradient computes it from the lensing potential on a ring grid. */
 NUSHT_API int nusht_pointing(int64_t npts, const double* theta, const double* phi, const double* alpha_theta,
                              const double* alpha_phi, double* theta_out, double* phi_out, void* stream);
+
+/* ---- transforms on ring grids ("rSHT") and the deflection field of the
+ * lensing potential, Eq. C2 (8(f) rank 4) --------------------------------------------------------
+ * A ring grid is nrings iso-latitude rings; ring r has colatitude theta[r] in [0, pi], nphi[r] >= 1 equidistant
+ * pixels at phi0[r] + 2 pi j / nphi[r], j = 0 .. nphi[r]-1.  The map is the rings one after the other in the order
+ * given, npix = sum nphi reals of the plan's dtype (Gauss-Legendre, Clenshaw-Curtis, Fejer and HEALPix-style layouts
+ * all fit).  theta, nphi, phi0 (NULL: 0) and weight (NULL: 1) are HOST arrays of length nrings, copied by the call.
+ *   nusht_ring_synthesis  f(r, j) = sum_lm a_lm Y_lm(theta_r, phi_rj)                              (Eq. 3 on the grid)
+ *   nusht_ring_analysis   c_lm = sum_r weight[r] sum_j f(r, j) conj Y_lm(theta_r, phi_rj)          (Eq. 2; weight = 1
+ *                         is the plain adjoint; with quadrature weights, e.g. Gauss-Legendre w_r 2 pi / nphi, it inverts
+ *                         the synthesis up to lmax, the "special case" of PAPER.md:74).  alm is overwritten.
+ *   nusht_ring_gradient   alpha_theta + i alpha_phi = (d/dtheta + (i / sin theta) d/dphi) Phi, Phi = sum Phi_lm Y_lm
+ *                         (Eq. C2): two maps of npix reals, the input of nusht_pointing.  A grid with a ring exactly
+ *                         at a pole gives NUSHT_ERR_UNSUPPORTED (the components are undefined there).
+ * alm / philm: the layout of nusht_synthesis (lmax, mmax of the ring plan).  Rings that mirror each other through the
+ * equator (theta_a + theta_b = pi to 2 ulp) share one Legendre recurrence; any other ring costs a pair's work.
+ * Maps must start on a 16-byte boundary (any cudaMalloc / torch allocation does).
+ * All data pointers are DEVICE pointers; calls enqueue on `stream` and do not synchronise; a ring plan must not be used
+ * from two streams at once.  nusht_ring_pairing exposes the pairing rule (host only, no device needed): returns the
+ * number of pairs (>= 0) or a negative status; pair_s[j] = -1 marks a ring without mirror. */
+typedef struct nusht_ring_plan_s nusht_ring_plan_t;
+typedef struct {
+    int lmax, mmax, dtype, nrings;
+    int npairs;          /* ring pairs the Legendre stage works on (nrings/2 for a symmetric grid) */
+    int nruns;           /* runs of consecutive equal-length rings = batched FFT calls per transform */
+    int64_t npix, nlm, workspace_bytes;
+    double plan_ms;
+} nusht_ring_info_t;
+NUSHT_API int nusht_ring_plan(nusht_ring_plan_t** out, int lmax, int mmax, int nrings, const double* theta,
+                              const int64_t* nphi, const double* phi0, const double* weight, int dtype);
+NUSHT_API int nusht_ring_synthesis(nusht_ring_plan_t* plan, const void* alm, void* map, void* stream);
+NUSHT_API int nusht_ring_analysis(nusht_ring_plan_t* plan, const void* map, void* alm, void* stream);
+NUSHT_API int nusht_ring_gradient(nusht_ring_plan_t* plan, const void* philm, void* alpha_theta, void* alpha_phi,
+                                  void* stream);
+NUSHT_API int nusht_ring_info(const nusht_ring_plan_t* plan, nusht_ring_info_t* info);
+NUSHT_API int nusht_ring_destroy(nusht_ring_plan_t* plan);
+NUSHT_API int nusht_ring_pairing(int nrings, const double* theta, int* pair_n, int* pair_s);
 
 NUSHT_API int nusht_plan_info(const nusht_plan_t* plan, nusht_info_t* info);
 /* Number of kernels of THIS library launched by the process so far (cuFFT's kernels and memsets are not counted);

@@ -55,6 +55,10 @@ def _load():
             f = getattr(_lib, "oracle_adjoint_columns" + suf)
             f.argtypes = [ctypes.c_int, ctypes.c_int, ip, ctypes.c_long, dp, dp, dp, dp]
             f.restype = None
+        for suf in ("_d", "_ld"):
+            f = getattr(_lib, "oracle_gradient" + suf)
+            f.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_long, dp, dp, dp, dp, dp]
+            f.restype = None
         _lib.oracle_num_threads.restype = ctypes.c_int
         _lib.oracle_long_double_bits.restype = ctypes.c_int
     return _lib
@@ -150,6 +154,22 @@ def adjoint_columns(lmax: int, mlist, theta, phi, x, precision: str = "d"):
         lmax, ml.shape[0], ml.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), theta.shape[0],
         _dp(theta), _dp(phi), _dp(x), _dp(out.view(np.float64)))
     return out
+
+
+def gradient(lmax: int, mmax: int, theta, phi, philm, precision: str = "d"):
+    """Eq. C2: (alpha_theta, alpha_phi) = (d/dtheta, (1/sin theta) d/dphi) of
+    Phi = sum_lm Phi_lm Y_lm at the points, by the direct sum (see the C source).  Points at a pole give NaN / Inf."""
+    theta, phi = _f64(theta), _f64(phi)
+    a = np.ascontiguousarray(philm, dtype=np.complex128)
+    if a.shape != (nlm(lmax, mmax),):
+        raise ValueError("philm has wrong length")
+    if theta.shape != phi.shape or theta.ndim != 1:
+        raise ValueError("theta/phi must be 1-D and equal length")
+    a_t = np.empty(theta.shape[0], dtype=np.float64)
+    a_p = np.empty(theta.shape[0], dtype=np.float64)
+    getattr(_load(), "oracle_gradient" + _suf(precision))(
+        lmax, mmax, theta.shape[0], _dp(theta), _dp(phi), _dp(a.view(np.float64)), _dp(a_t), _dp(a_p))
+    return a_t, a_p
 
 
 def inner_alm(lmax: int, mmax: int, a, c) -> float:

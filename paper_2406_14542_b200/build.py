@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnusht.so")
-SOURCES = ["api.cu", "legendre.cu", "fourier.cu", "nufft.cu", "pointing.cu", "probe.cu"]
+SOURCES = ["api.cu", "legendre.cu", "fourier.cu", "nufft.cu", "pointing.cu", "probe.cu", "ring.cu"]
 HEADERS = [os.path.join(CSRC, "nusht_internal.cuh"), os.path.join(HERE, "..", "include", "nusht.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Wno-deprecated-gpu-targets",

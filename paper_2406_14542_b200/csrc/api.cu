@@ -100,6 +100,7 @@ extern "C" int nusht_plan(nusht_plan_t** out, int lmax, int mmax, int64_t npts, 
     nusht_plan_s* p = new (std::nothrow) nusht_plan_s();
     if (!p) return NUSHT_ERR_ALLOC;
     p->lmax = lmax;
+    p->lmax_io = lmax;
     p->mmax = mmax;
     p->npts = npts;
     p->eps = eps;
@@ -117,6 +118,7 @@ extern "C" int nusht_plan(nusht_plan_t** out, int lmax, int mmax, int64_t npts, 
         p->lg.nr = nth2 / 2 + 1;
         p->lg.npairs = (p->lg.nr + 1) / 2;
         p->lg.has_equator = p->lg.nr & 1;
+        p->lg.ring_mode = 0;
         // fine grid: up-sampling sigma = 2 of the 2 lmax + 2 (2 mmax + 2) Fourier modes (reading G7)
         const int w = p->ng.w;
         int nth = 2 * (2 * lmax + 2), nph = 2 * (2 * mmax + 2);

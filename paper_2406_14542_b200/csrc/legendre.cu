@@ -14,8 +14,12 @@
 //               evaluated as  t_n = (alpha_n + beta_n) - alpha_n sin^2(theta):  next to the poles x^2 = cos^2(theta)
 //               rounds with an absolute error of 1e-16, the SAME error for every n of a ring, i.e. a coherent
 //               shift of theta by 1e-16 / sin(2 theta) that grows to l * shift in the phase of Pbar_lm; sin^2 is
-//               small there and carries a relative error instead.  The tables hold
-//               (-alpha_n, alpha_n + beta_n) and sin^2(theta_j), the kernels do one FMA as before.
+//               small there and carries a relative error instead.  Next to the EQUATOR the roles
+//               swap (the x^2-stepping recurrence has double characteristic roots at theta = 0, pi/2 and pi): there
+//               sin^2 is the one that rounds coherently, so blocks of ring pairs with theta >= pi/4 use
+//               t_n = beta_n + alpha_n cos^2(theta).  Two tables, (-alpha_n, alpha_n + beta_n) and (alpha_n, beta_n);
+//               a warp fetches its tiles from the one its block uses, and the per-pair operand table holds sin^2 or
+//               cos^2 accordingly.  One FMA per step either way.
 //   odd class   Pbar_{m+2n+1} = (x q_n - c_{m+2n} Pbar_{m+2n-1})/c_{m+2n+1}  is folded into the
 //               coefficients once per transform (O(lmax^2)):  sum_n b_n Pbar_{m+2n+1} =
 //               x sum_j (r_j/c_{m+2j+1}) q_j,  r_j = b_j - rho_j r_{j+1},  rho_j = c_{m+2j+2}/c_{m+2j+3}.
@@ -58,7 +62,11 @@ constexpr double SCALE_UP_LIMIT = 1.6923032801030364e+125;   // 2^(512 - LIVE_BI
 constexpr double SCALE_DOWN = 7.458340731200207e-155;      // 2^-512
 
 struct LegParams {
-    int lmax, mmax, nr, nth2, npairs, has_equator;
+    // b_split: blocks bx >= b_split use the cos^2 form of t_n (header), and so do the remainder pairs iff
+    // nblk >= b_split.  (The struct must not grow: k_legendre_adjoint sits exactly at its 128-register budget and
+    // ptxas starts spilling inside its FMA loop when the parameter block gets larger; the cos^2 table is therefore
+    // reached as ab + eoff[mmax + 1], the second half of one allocation.)
+    int lmax, mmax, nr, nth2, npairs, b_split;
     int nblk, rem;   // main blocks of 32 R pairs per m; left-over pairs handled by the remainder blocks
     // fast-forward table (plan time): for warp (m, block) the first n-step (multiple of LEG_CHUNK) at which
     // one of its ring pairs is in range, and the scaled recurrence state of its pairs at that step
@@ -73,6 +81,10 @@ struct LegParams {
     const double* x;
     const double2* logsin;
     const double2* logkap;
+    // ring-list mode (rSHT on caller ring grids, ring.cu): pair j = (north ring pn[j], south ring ps[j] or -1);
+    // rows of F[m][.] then have nth2 = nrings entries and are NOT doubled
+    const int* pn;
+    const int* ps;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -111,7 +123,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 // plan-time tables, one thread per m (sequential in n: sigma is a two-step product)
 // ---------------------------------------------------------------------------------------------
 __global__ void k_legendre_tables(int L, int M, const int64_t* __restrict__ eoff, double2* __restrict__ ab,
-                                  double* __restrict__ sig, double* __restrict__ sodd, double* __restrict__ rho) {
+                                  double2* __restrict__ abx, double* __restrict__ sig, double* __restrict__ sodd, double* __restrict__ rho) {
     int m = blockIdx.x * blockDim.x + threadIdx.x;
     if (m > M) return;
     const int ne = (L - m) / 2 + 1;
@@ -133,6 +145,7 @@ __global__ void k_legendre_tables(int L, int M, const int64_t* __restrict__ eoff
         const double sg_next = (n == 0) ? 1.0 : -C * sg_prev;
         const double alpha = A * sg / sg_next;
         ab[o + n] = make_double2(-alpha, alpha * (1.0 - D));   // t_n = ab.y + ab.x sin^2(theta) = alpha (x^2 - D)
+        abx[o + n] = make_double2(alpha, -alpha * D);          // t_n = abx.y + abx.x cos^2(theta)
         sig[o + n] = sg;
         sodd[o + n] = sg / sqrt(c2l1);
         rho[o + n] = sqrt(c2l2 / c2l3);
@@ -150,9 +163,11 @@ __global__ void k_legendre_tables(int L, int M, const int64_t* __restrict__ eoff
 // ---------------------------------------------------------------------------------------------
 constexpr int PREP_THREADS = 128;
 
+// (Lio: band limit of the caller's alm layout; Lio < L only in ring plans built one degree higher, where the
+//  coefficients above Lio read as zero)
 template <typename T>
 __global__ void __launch_bounds__(PREP_THREADS)
-k_alm_prep(int L, int M, const int64_t* __restrict__ eoff, const T* __restrict__ alm,
+k_alm_prep(int L, int Lio, int M, const int64_t* __restrict__ eoff, const T* __restrict__ alm,
            const double* __restrict__ sig, const double* __restrict__ sodd,
            const double* __restrict__ rho, double4* __restrict__ aeo) {
     const int m = blockIdx.x * (PREP_THREADS / 32) + (threadIdx.x >> 5);
@@ -161,7 +176,7 @@ k_alm_prep(int L, int M, const int64_t* __restrict__ eoff, const T* __restrict__
     const int ne = (L - m) / 2 + 1;
     const int no = (L - m + 1) / 2;
     const int64_t o = eoff[m];
-    const T* col = alm + 2 * ((int64_t)m * (2 * L + 1 - m) / 2);   // col[2*l], col[2*l+1] for l >= m
+    const T* col = alm + 2 * ((int64_t)m * (2 * Lio + 1 - m) / 2);   // col[2*l], col[2*l+1] for l >= m
     double cre = 0.0, cim = 0.0;   // r_{j+1} entering the tile from above
     for (int base = ((ne - 1) / 32) * 32; base >= 0; base -= 32) {
         const int j = base + lane;
@@ -169,9 +184,11 @@ k_alm_prep(int L, int M, const int64_t* __restrict__ eoff, const T* __restrict__
         double are = 0.0, aim = 0.0, bre = 0.0, bim = 0.0, S = 0.0, sg = 0.0, so = 0.0;
         if (in) {
             const int le = m + 2 * j;
-            are = (double)col[2 * le];
-            aim = (double)col[2 * le + 1];
-            if (j < no) {
+            if (le <= Lio) {
+                are = (double)col[2 * le];
+                aim = (double)col[2 * le + 1];
+            }
+            if (j < no && le + 1 <= Lio) {
                 bre = (double)col[2 * le + 2];
                 bim = (double)col[2 * le + 3];
             }
@@ -211,7 +228,7 @@ k_alm_prep(int L, int M, const int64_t* __restrict__ eoff, const T* __restrict__
 // per m, prefix scan of the affine maps v -> u_n - rho_{n-1} v.
 template <typename T>
 __global__ void __launch_bounds__(PREP_THREADS)
-k_alm_post(int L, int M, const int64_t* __restrict__ eoff, const double4* __restrict__ eo,
+k_alm_post(int L, int Lio, int M, const int64_t* __restrict__ eoff, const double4* __restrict__ eo,
            const double* __restrict__ sig, const double* __restrict__ sodd,
            const double* __restrict__ rho, T* __restrict__ alm) {
     const int m = blockIdx.x * (PREP_THREADS / 32) + (threadIdx.x >> 5);
@@ -220,7 +237,7 @@ k_alm_post(int L, int M, const int64_t* __restrict__ eoff, const double4* __rest
     const int ne = (L - m) / 2 + 1;
     const int no = (L - m + 1) / 2;
     const int64_t o = eoff[m];
-    T* col = alm + 2 * ((int64_t)m * (2 * L + 1 - m) / 2);
+    T* col = alm + 2 * ((int64_t)m * (2 * Lio + 1 - m) / 2);
     double cre = 0.0, cim = 0.0;   // v_{n-1} entering the tile from below
     for (int base = 0; base < ne; base += 32) {
         const int n = base + lane;
@@ -249,9 +266,11 @@ k_alm_post(int L, int M, const int64_t* __restrict__ eoff, const double4* __rest
         const double vre = fma(S, cre, ure), vim = fma(S, cim, uim);
         if (in) {
             const int le = m + 2 * n;
-            col[2 * le] = (T)ere;
-            col[2 * le + 1] = (m == 0) ? (T)0 : (T)eim;
-            if (n < no) {
+            if (le <= Lio) {
+                col[2 * le] = (T)ere;
+                col[2 * le + 1] = (m == 0) ? (T)0 : (T)eim;
+            }
+            if (n < no && le + 1 <= Lio) {
                 col[2 * le + 2] = (T)vre;
                 col[2 * le + 3] = (m == 0) ? (T)0 : (T)vim;
             }
@@ -273,8 +292,8 @@ __device__ __forceinline__ void seed_pair(const LegParams& P, int m, int j, bool
         p = exp2(lk.x + lk.y);
         return;
     }
-    if (j == 0) return;   // poles: sin(theta) = 0, Pbar_lm = 0 for m > 0
     const double2 ls = P.logsin[j];
+    if (ls.x < -1e300) return;   // a pole ring (log2 sin theta = -inf in the table): Pbar_lm = 0 for m > 0
     const double dm = (double)m;
     // (mh + err) = m * ls.x exactly;  s = mh + lk.x with two-sum error err2
     const double mh = dm * ls.x;
@@ -295,11 +314,18 @@ __device__ __forceinline__ void seed_pair(const LegParams& P, int m, int j, bool
 
 // a2 for one ring pair: north = E + x O, south = E - x O; mirror rows carry (-1)^m (phi -> phi + pi)
 // (Fig. 1)
+template <bool RING>
 __device__ __forceinline__ void write_pair(const LegParams& P, double2* row, double sgn, int j, double ere,
                                            double eim, double ore_, double oim) {
     const double x = P.x[j];
     const double2 nv = make_double2(fma(x, ore_, ere), fma(x, oim, eim));
     const double2 sv = make_double2(fma(-x, ore_, ere), fma(-x, oim, eim));
+    if (RING) {                    // ring list: F[m][ring], no doubling
+        row[P.pn[j]] = nv;
+        const int rs = P.ps[j];
+        if (rs >= 0) row[rs] = sv;
+        return;
+    }
     const int ks = P.nr - 1 - j;   // south ring index
     row[j] = nv;
     if (j != 0) row[P.nth2 - j] = make_double2(sgn * nv.x, sgn * nv.y);
@@ -311,8 +337,20 @@ __device__ __forceinline__ void write_pair(const LegParams& P, double2* row, dou
 
 // a10 for one ring pair (D^T): G[k] = Gt[k] + (-1)^m Gt[Ntheta-k] away from the poles, then the even /
 // odd (in l - m) combinations of the north and south ring
+template <bool RING>
 __device__ __forceinline__ void fold_pair(const LegParams& P, const double2* __restrict__ row, double sgn, int j,
                                           double& ere, double& eim, double& ore_, double& oim) {
+    if (RING) {                    // ring list: G[m][ring] as it is (weights applied upstream)
+        const double2 gn = row[P.pn[j]];
+        const int rs = P.ps[j];
+        const double2 gs = rs >= 0 ? row[rs] : make_double2(0.0, 0.0);
+        const double x = P.x[j];
+        ere = gn.x + gs.x;
+        eim = gn.y + gs.y;
+        ore_ = x * (gn.x - gs.x);
+        oim = x * (gn.y - gs.y);
+        return;
+    }
     const int kn = j, ks = P.nr - 1 - j;
     double2 gn = row[kn];
     if (kn != 0) {
@@ -340,6 +378,7 @@ __device__ __forceinline__ void fold_pair(const LegParams& P, const double2* __r
 // number of 32 R blocks.  Rather than a 17th warp per m with a single busy lane, the last block
 // column of the grid takes the `rem` left-over pairs of 32/rem different m per warp, one (m, pair)
 // per lane, each lane streaming its own coefficient column from global memory.
+template <bool RING>
 __device__ void synth_remainder(const LegParams& P, const double4* __restrict__ aeo, double2* __restrict__ ft, int j0,
                                 int rem, int by) {
     const int gid = by * 32 + threadIdx.x;
@@ -353,7 +392,7 @@ __device__ void synth_remainder(const LegParams& P, const double4* __restrict__ 
     const double x2 = P.x2[j];
     double ere = 0.0, eim = 0.0, ore_ = 0.0, oim = 0.0;
     for (int n = 0; n < ne; ++n) {
-        const double2 ab = P.ab[o + n];
+        const double2 ab = P.ab[o + n + (P.nblk >= P.b_split ? P.eoff[P.mmax + 1] : 0)];
         const double t = fma(ab.x, x2, ab.y);
         if (ex == 0) {
             const double4 c = aeo[o + n];
@@ -371,9 +410,10 @@ __device__ void synth_remainder(const LegParams& P, const double4* __restrict__ 
             ex -= 1;
         }
     }
-    write_pair(P, ft + (int64_t)m * P.nth2, (m & 1) ? -1.0 : 1.0, j, ere, eim, ore_, oim);
+    write_pair<RING>(P, ft + (int64_t)m * P.nth2, (m & 1) ? -1.0 : 1.0, j, ere, eim, ore_, oim);
 }
 
+template <bool RING>
 __device__ void adjoint_remainder(const LegParams& P, const double2* __restrict__ gt, double4* __restrict__ eo, int j0,
                                   int rem, int by) {
     const int gid = by * 32 + threadIdx.x;
@@ -386,9 +426,9 @@ __device__ void adjoint_remainder(const LegParams& P, const double2* __restrict_
     seed_pair(P, m, j, true, p1, ex);
     const double x2 = P.x2[j];
     double ere, eim, ore_, oim;
-    fold_pair(P, gt + (int64_t)m * P.nth2, (m & 1) ? -1.0 : 1.0, j, ere, eim, ore_, oim);
+    fold_pair<RING>(P, gt + (int64_t)m * P.nth2, (m & 1) ? -1.0 : 1.0, j, ere, eim, ore_, oim);
     for (int n = 0; n < ne; ++n) {
-        const double2 ab = P.ab[o + n];
+        const double2 ab = P.ab[o + n];          // the launch hands over the table of this block's form
         const double t = fma(ab.x, x2, ab.y);
         if (ex == 0) {
             double* out = reinterpret_cast<double*>(eo + o + n);
@@ -423,6 +463,7 @@ k_legendre_fastforward(LegParams P, int* __restrict__ ff_n, double2* __restrict_
     const int ne = (P.lmax - m) / 2 + 1;
     const int64_t o = P.eoff[m];
     const int jb = blockIdx.x * (32 * R);
+    const bool xform = (int)blockIdx.x >= P.b_split;
     double x2[R], p0[R], p1[R];
     int ex[R];
     bool valid[R];
@@ -442,7 +483,7 @@ k_legendre_fastforward(LegParams P, int* __restrict__ ff_n, double2* __restrict_
         if (__any_sync(0xffffffffu, any_live)) break;
         const int ns = min(LEG_CHUNK, ne - n);
         for (int i = 0; i < ns; ++i) {
-            const double2 ab = P.ab[o + n + i];
+            const double2 ab = P.ab[o + n + i + (xform ? P.eoff[P.mmax + 1] : 0)];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const double t = fma(ab.x, x2[r], ab.y);
@@ -472,13 +513,13 @@ k_legendre_fastforward(LegParams P, int* __restrict__ ff_n, double2* __restrict_
 // ---------------------------------------------------------------------------------------------
 // a1 + a2: Legendre synthesis with fused DFS doubling.  grid = (pair blocks, m).
 // ---------------------------------------------------------------------------------------------
-template <int R>
+template <int R, bool RING>
 __global__ void __launch_bounds__(SYN_THREADS)
 k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restrict__ ft) {
     const int2 item = P.items[blockIdx.x];
     const int bx = item.x, by = item.y;
     if (P.rem > 0 && bx == P.nblk) {
-        synth_remainder(P, aeo, ft, P.nblk * (32 * R), P.rem, by);
+        synth_remainder<RING>(P, aeo, ft, P.nblk * (32 * R), P.rem, by);
         return;
     }
     __shared__ __align__(16) double2 s_ab[2][SYN_TN];
@@ -489,6 +530,7 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
     const int L = P.lmax;
     const int ne = (L - m) / 2 + 1;
     const int64_t o = P.eoff[m];
+    const bool xform = bx >= P.b_split;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int jb = (bx * SYN_WARPS + warp) * (32 * R);
     const int ntiles = (ne + SYN_TN - 1) / SYN_TN;
@@ -506,7 +548,8 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
         const int st = (tile - tile0) & 1;
         const int cnt = min(SYN_TN, ne - tile * SYN_TN);
         mbar_expect_tx(&s_bar[st], (uint32_t)cnt * 48u);
-        bulk_g2s(&s_ab[st][0], P.ab + o + (int64_t)tile * SYN_TN, (uint32_t)cnt * 16u, &s_bar[st]);
+        // blocks next to the equator take the cos^2 form of the table (header)
+        bulk_g2s(&s_ab[st][0], P.ab + (xform ? P.eoff[P.mmax + 1] : 0) + o + (int64_t)tile * SYN_TN, (uint32_t)cnt * 16u, &s_bar[st]);
         bulk_g2s(&s_aeo[st][0], aeo + o + (int64_t)tile * SYN_TN, (uint32_t)cnt * 32u, &s_bar[st]);
     };
     if (tid == 0 && n_start < ne) {
@@ -630,7 +673,7 @@ k_legendre_synth(LegParams P, const double4* __restrict__ aeo, double2* __restri
     double2* row = ft + (int64_t)m * P.nth2;
 #pragma unroll
     for (int r = 0; r < R; ++r)
-        if (valid[r]) write_pair(P, row, sgn, jb + r * 32 + lane, ere[r], eim[r], ore_[r], oim[r]);
+        if (valid[r]) write_pair<RING>(P, row, sgn, jb + r * 32 + lane, ere[r], eim[r], ore_[r], oim[r]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -649,14 +692,18 @@ __device__ __forceinline__ double shfl_xor_d(double v, int mask) {
 // No warp ever waits for another one, whatever its mix of live and dead ring pairs.  A dead pair
 // (scaled value below range) keeps G = 0 in registers, so the inner loop needs no masks; its folded
 // G values are loaded when the pair comes into range.
-template <int R, int C>
+template <int R, int C, bool RING>
 __global__ void __launch_bounds__(32, adj_min_ctas(R, C))
 k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restrict__ eo) {
     // plain 2-D grid (block of ring pairs, m): the blocks of one m run together and add into the same eo[m]
-    // column while it is L2-resident; a work list as in the synthesis was tried (see build_work_list)
-    const int bx = blockIdx.x, by = blockIdx.y;
+    // column while it is L2-resident; a work list as in the synthesis was tried (see build_work_list).
+    // The host launches this kernel once per form of t_n (header): blocks [0, b_split) with the sin^2 table, blocks
+    // from b_split on with P.ab pointing at the cos^2 table and P.b_split = the block offset.  (Choosing the table in
+    // here instead costs the registers that make ptxas spill inside the FMA loop: the kernel sits exactly at the
+    // 128 registers that four one-warp CTAs per scheduler leave.)
+    const int bx = blockIdx.x + P.b_split, by = blockIdx.y;
     if (P.rem > 0 && bx == P.nblk) {
-        adjoint_remainder(P, gt, eo, P.nblk * (32 * R), P.rem, by);
+        adjoint_remainder<RING>(P, gt, eo, P.nblk * (32 * R), P.rem, by);
         return;
     }
     __shared__ __align__(16) double2 s_ab[2][ADJ_TN];
@@ -702,7 +749,7 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
     int ex[R];
     bool valid[R];
     auto load_g = [&](int j, double& ere, double& eim, double& ore_, double& oim) {
-        fold_pair(P, row, sgn, j, ere, eim, ore_, oim);
+        fold_pair<RING>(P, row, sgn, j, ere, eim, ore_, oim);
     };
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -822,6 +869,10 @@ static dim3 leg_grid(const nusht_plan_s* p, int R, LegParams& P) {
     }
     P.nblk = nblk;
     P.rem = rem;
+    // form of t_n per block (header): pairs are ordered from the poles to the equator, so the blocks whose first pair
+    // lies at theta >= pi/4 (index >= j_quarter) are the last ones
+    P.b_split = (p->j_quarter + per - 1) / per;
+    P.x2 = (R == ADJ_R && ADJ_R != LEG_R) ? p->d_x2a : p->d_x2;
     const int need_y = rem ? ((p->mmax + 1) * rem + 31) / 32 : 0;   // remainder warps; they fit: rem <= 8
     (void)need_y;
     return dim3(nblk + (rem ? 1 : 0), p->mmax + 1);
@@ -836,13 +887,15 @@ static LegParams make_params(const nusht_plan_s* p, bool adjoint_tables = false)
     P.nr = p->lg.nr;
     P.nth2 = p->lg.nth2;
     P.npairs = p->lg.npairs;
-    P.has_equator = p->lg.has_equator;
+    P.b_split = 0;
     P.eoff = p->d_eoff;
     P.ab = p->d_ab;
     P.x2 = p->d_x2;
     P.x = p->d_x;
     P.logsin = p->d_logsin;
     P.logkap = p->d_logkap;
+    P.pn = p->d_pair_n;
+    P.ps = p->d_pair_s;
     const bool a = adjoint_tables && ADJ_R != LEG_R;
     P.ff_n = a ? p->d_ffa_n : p->d_ff_n;
     P.ff_p = a ? p->d_ffa_p : p->d_ff_p;
@@ -922,8 +975,53 @@ static int build_work_list(nusht_plan_s* p, int R, const int* d_ff_n, int2** d_i
     return NUSHT_OK;
 }
 
+int legendre_pair_rings(int nrings, const double* theta, int* pair_n, int* pair_s) {
+    const double PI_D = 3.14159265358979323846;
+    std::vector<int> order(nrings);
+    for (int i = 0; i < nrings; ++i) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return theta[a] < theta[b]; });
+    // two pointers from the poles inwards: the ring nearest to the north pole against the one nearest to the south
+    std::vector<std::pair<double, std::pair<int, int>>> pairs;     // (distance from the nearer pole, (north, south))
+    int lo = 0, hi = nrings - 1;
+    while (lo <= hi) {
+        const int a = order[lo], b = order[hi];
+        const double dn = theta[a], ds = PI_D - theta[b];          // distances from the north / south pole
+        if (lo < hi && fabs((theta[a] + theta[b]) - PI_D) <= 9.0e-16) {
+            pairs.push_back({dn, {a, b}});
+            ++lo;
+            --hi;
+        } else if (lo == hi || dn <= ds) {
+            pairs.push_back({fmin(theta[a], PI_D - theta[a]), {a, -1}});
+            ++lo;
+        } else {
+            pairs.push_back({fmin(theta[b], PI_D - theta[b]), {b, -1}});
+            --hi;
+        }
+    }
+    std::stable_sort(pairs.begin(), pairs.end(),
+                     [](const std::pair<double, std::pair<int, int>>& u, const std::pair<double, std::pair<int, int>>& v) {
+                         return u.first < v.first;
+                     });
+    for (size_t j = 0; j < pairs.size(); ++j) {
+        pair_n[j] = pairs[j].second.first;
+        pair_s[j] = pairs[j].second.second;
+    }
+    return (int)pairs.size();
+}
+
 int legendre_build_tables(nusht_plan_s* p) {
     const int L = p->lmax, M = p->mmax;
+    std::vector<int> h_pn, h_ps;
+    if (p->lg.ring_mode) {          // pairs of the caller's ring list (ring.cu set nr = nth2 = nrings)
+        h_pn.resize(p->lg.nr);
+        h_ps.resize(p->lg.nr);
+        p->lg.npairs = legendre_pair_rings(p->lg.nr, p->h_ring_theta, h_pn.data(), h_ps.data());
+        p->lg.has_equator = 0;
+        NUSHT_TRY(dev_alloc(&p->d_pair_n, (size_t)p->lg.npairs, p));
+        NUSHT_TRY(dev_alloc(&p->d_pair_s, (size_t)p->lg.npairs, p));
+        NUSHT_CUDA_TRY(cudaMemcpy(p->d_pair_n, h_pn.data(), sizeof(int) * p->lg.npairs, cudaMemcpyHostToDevice));
+        NUSHT_CUDA_TRY(cudaMemcpy(p->d_pair_s, h_ps.data(), sizeof(int) * p->lg.npairs, cudaMemcpyHostToDevice));
+    }
     const LegendreGeom& g = p->lg;
     // column offsets
     std::vector<int64_t> eoff(M + 2);
@@ -936,7 +1034,7 @@ int legendre_build_tables(nusht_plan_s* p) {
     p->n_e_total = acc;
     NUSHT_TRY(dev_alloc(&p->d_eoff, (size_t)M + 2, p));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_eoff, eoff.data(), sizeof(int64_t) * (M + 2), cudaMemcpyHostToDevice));
-    NUSHT_TRY(dev_alloc(&p->d_ab, (size_t)acc, p));
+    NUSHT_TRY(dev_alloc(&p->d_ab, 2 * (size_t)acc, p));     // sin^2 form, then the cos^2 form (header)
     NUSHT_TRY(dev_alloc(&p->d_sig, (size_t)acc, p));
     NUSHT_TRY(dev_alloc(&p->d_sodd, (size_t)acc, p));
     NUSHT_TRY(dev_alloc(&p->d_rho, (size_t)acc, p));
@@ -944,23 +1042,34 @@ int legendre_build_tables(nusht_plan_s* p) {
     NUSHT_TRY(dev_alloc(&p->d_ft, (size_t)(M + 1) * (size_t)g.nth2, p));
     {
         const int threads = 32;
-        k_legendre_tables<<<(M + 1 + threads - 1) / threads, threads>>>(L, M, p->d_eoff, p->d_ab, p->d_sig,
+        k_legendre_tables<<<(M + 1 + threads - 1) / threads, threads>>>(L, M, p->d_eoff, p->d_ab, p->d_ab + acc, p->d_sig,
                                                                          p->d_sodd, p->d_rho);
         NUSHT_CUDA_TRY(nusht_launched());
     }
     // ring tables in extended precision on the host: theta_j = pi j/(nr-1)
     const long double PI_L = 3.14159265358979323846264338327950288L;
-    std::vector<double> x2(g.npairs), x(g.npairs);
+    std::vector<double> x2(g.npairs), x2c(g.npairs), x(g.npairs);    // sin^2, cos^2, cos of the pair's colatitude
     std::vector<double2> ls(g.npairs);
+    p->j_quarter = g.npairs;
     for (int j = 0; j < g.npairs; ++j) {
         long double th = PI_L * (long double)j / (long double)(g.nr - 1);
+        if (g.ring_mode) {
+            // the pair's colatitude: the north ring's, averaged with the mirror of its partner (they agree to 2 ulp)
+            th = (long double)p->h_ring_theta[h_pn[j]];
+            if (h_ps[j] >= 0) th = 0.5L * (th + (PI_L - (long double)p->h_ring_theta[h_ps[j]]));
+        }
         long double c = cosl(th), s = sinl(th);
         if (g.has_equator && j == g.npairs - 1) c = 0.0L;
         x[j] = (double)c;
-        x2[j] = (double)(s * s);          // the kernels' "x2" operand is sin^2(theta): see the header
-        if (g.has_equator && j == g.npairs - 1) x2[j] = 1.0;
-        if (j == 0) {
-            ls[j] = make_double2(0.0, 0.0);   // unused: poles are special-cased
+        x2[j] = (double)(s * s);          // the kernels' "x2" operand is sin^2(theta) or cos^2(theta): see the header
+        x2c[j] = (double)(c * c);
+        if (g.has_equator && j == g.npairs - 1) { x2[j] = 1.0; x2c[j] = 0.0; }
+        if (fminl(th, PI_L - th) >= 0.25L * PI_L && j < p->j_quarter) p->j_quarter = j;   // pairs run pole -> equator
+        if (!(s > 0.0L)) {
+            ls[j] = make_double2(-INFINITY, 0.0);   // a pole ring: seed_pair returns Pbar_lm = 0 for m > 0
+            x2[j] = 0.0;
+            x2c[j] = 1.0;
+            x[j] = (c < 0.0L) ? -1.0 : 1.0;
         } else {
             long double v = log2l(s);
             double hi = (double)v;
@@ -977,10 +1086,24 @@ int legendre_build_tables(nusht_plan_s* p) {
         }
     }
     NUSHT_TRY(dev_alloc(&p->d_x2, (size_t)g.npairs, p));
+    NUSHT_TRY(dev_alloc(&p->d_x2a, (size_t)g.npairs, p));
+    for (int which = 0; which < 2; ++which) {
+        // operand table of each decomposition: sin^2 for the blocks that use t = (alpha + beta) - alpha sin^2, cos^2
+        // for the blocks (and remainder pairs) that use t = beta + alpha cos^2
+        LegParams P = make_params(p);
+        const int R = which ? ADJ_R : LEG_R, per = 32 * R;
+        leg_grid(p, R, P);
+        std::vector<double> u(g.npairs);
+        for (int j = 0; j < g.npairs; ++j) {
+            const bool in_rem = P.rem > 0 && j >= P.nblk * per;
+            const bool xf = in_rem ? (P.nblk >= P.b_split) : (j / per >= P.b_split);
+            u[j] = xf ? x2c[j] : x2[j];
+        }
+        NUSHT_CUDA_TRY(cudaMemcpy(which ? p->d_x2a : p->d_x2, u.data(), sizeof(double) * g.npairs, cudaMemcpyHostToDevice));
+    }
     NUSHT_TRY(dev_alloc(&p->d_x, (size_t)g.npairs, p));
     NUSHT_TRY(dev_alloc(&p->d_logsin, (size_t)g.npairs, p));
     NUSHT_TRY(dev_alloc(&p->d_logkap, (size_t)M + 1, p));
-    NUSHT_CUDA_TRY(cudaMemcpy(p->d_x2, x2.data(), sizeof(double) * g.npairs, cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_x, x.data(), sizeof(double) * g.npairs, cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_logsin, ls.data(), sizeof(double2) * g.npairs, cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_logkap, lk.data(), sizeof(double2) * (M + 1), cudaMemcpyHostToDevice));
@@ -1015,10 +1138,10 @@ int legendre_build_tables(nusht_plan_s* p) {
 int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s) {
     const int threads = PREP_THREADS, blocks = (p->mmax + 1 + threads / 32 - 1) / (threads / 32);
     if (p->dtype == NUSHT_F64)
-        k_alm_prep<double><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, (const double*)alm, p->d_sig,
+        k_alm_prep<double><<<blocks, threads, 0, s>>>(p->lmax, p->lmax_io, p->mmax, p->d_eoff, (const double*)alm, p->d_sig,
                                                       p->d_sodd, p->d_rho, p->d_aeo);
     else
-        k_alm_prep<float><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, (const float*)alm, p->d_sig,
+        k_alm_prep<float><<<blocks, threads, 0, s>>>(p->lmax, p->lmax_io, p->mmax, p->d_eoff, (const float*)alm, p->d_sig,
                                                      p->d_sodd, p->d_rho, p->d_aeo);
     NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
@@ -1028,7 +1151,10 @@ int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s) {
     LegParams P = make_params(p);
     leg_grid(p, LEG_R, P);
     if (p->n_items_syn == 0) return NUSHT_OK;
-    k_legendre_synth<LEG_R><<<p->n_items_syn, SYN_THREADS, 0, s>>>(P, p->d_aeo, ft);
+    if (p->lg.ring_mode)
+        k_legendre_synth<LEG_R, true><<<p->n_items_syn, SYN_THREADS, 0, s>>>(P, p->d_aeo, ft);
+    else
+        k_legendre_synth<LEG_R, false><<<p->n_items_syn, SYN_THREADS, 0, s>>>(P, p->d_aeo, ft);
     NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
@@ -1038,18 +1164,31 @@ int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
     NUSHT_CUDA_TRY(cudaMemsetAsync(p->d_aeo, 0, sizeof(double4) * (size_t)p->n_e_total, s));
     LegParams P = make_params(p, true);
     const dim3 grid = leg_grid(p, ADJ_R, P);
-    k_legendre_adjoint<ADJ_R, ADJ_CHUNK><<<grid, 32, 0, s>>>(P, gt, p->d_aeo);
-    NUSHT_CUDA_TRY(nusht_launched());
+    // one launch per form of t_n (see the kernel): blocks next to the equator first (they are the longer ones)
+    const int nbx = (int)grid.x, split = std::min(P.b_split, nbx);
+    for (int part = 1; part >= 0; --part) {
+        LegParams Q = P;
+        const int first = part ? split : 0, count = part ? nbx - split : split;
+        if (count <= 0) continue;
+        Q.b_split = first;                                   // block offset of this launch
+        if (part) Q.ab = P.ab + p->n_e_total;                // cos^2 form of the table
+        const dim3 g2(count, grid.y);
+        if (p->lg.ring_mode)
+            k_legendre_adjoint<ADJ_R, ADJ_CHUNK, true><<<g2, 32, 0, s>>>(Q, gt, p->d_aeo);
+        else
+            k_legendre_adjoint<ADJ_R, ADJ_CHUNK, false><<<g2, 32, 0, s>>>(Q, gt, p->d_aeo);
+        NUSHT_CUDA_TRY(nusht_launched());
+    }
     return NUSHT_OK;
 }
 
 int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s) {
     const int threads = PREP_THREADS, blocks = (p->mmax + 1 + threads / 32 - 1) / (threads / 32);
     if (p->dtype == NUSHT_F64)
-        k_alm_post<double><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, p->d_aeo, p->d_sig, p->d_sodd,
+        k_alm_post<double><<<blocks, threads, 0, s>>>(p->lmax, p->lmax_io, p->mmax, p->d_eoff, p->d_aeo, p->d_sig, p->d_sodd,
                                                       p->d_rho, (double*)alm);
     else
-        k_alm_post<float><<<blocks, threads, 0, s>>>(p->lmax, p->mmax, p->d_eoff, p->d_aeo, p->d_sig, p->d_sodd,
+        k_alm_post<float><<<blocks, threads, 0, s>>>(p->lmax, p->lmax_io, p->mmax, p->d_eoff, p->d_aeo, p->d_sig, p->d_sodd,
                                                      p->d_rho, (float*)alm);
     NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
@@ -1058,8 +1197,11 @@ int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s) {
 void legendre_free(nusht_plan_s* p) {
     cudaFree(p->d_items_syn);
     p->d_items_syn = nullptr;
+    cudaFree(p->d_pair_n); cudaFree(p->d_pair_s);
+    p->d_pair_n = p->d_pair_s = nullptr;
     cudaFree(p->d_eoff); cudaFree(p->d_ab); cudaFree(p->d_sig); cudaFree(p->d_sodd); cudaFree(p->d_rho);
-    cudaFree(p->d_aeo); cudaFree(p->d_ft); cudaFree(p->d_x2); cudaFree(p->d_x); cudaFree(p->d_logsin);
+    cudaFree(p->d_aeo); cudaFree(p->d_ft); cudaFree(p->d_x2); cudaFree(p->d_x2a); cudaFree(p->d_x); cudaFree(p->d_logsin);
+    p->d_x2a = nullptr;
     cudaFree(p->d_logkap);
     cudaFree(p->d_ff_n); cudaFree(p->d_ff_p); cudaFree(p->d_ff_e);
     cudaFree(p->d_ffa_n); cudaFree(p->d_ffa_p); cudaFree(p->d_ffa_e);

@@ -60,6 +60,7 @@ struct LegendreGeom {
     int nth2;            // doubled length 2 (nr - 1)
     int npairs;          // ring pairs (north j, south nr-1-j): ceil(nr/2)
     int has_equator;     // nr odd: last pair is the equator ring alone
+    int ring_mode;       // 1: caller ring list (ring.cu): nr = nth2 = number of rings, pairs from d_pair_n / d_pair_s
 };
 
 struct nusht_plan_s {
@@ -77,11 +78,15 @@ struct nusht_plan_s {
     // --- Legendre tables (device) ---
     int64_t* d_eoff = nullptr;      // [mmax+2] offsets of column m in the per-(m,n) tables
     int64_t n_e_total = 0;          // sum_m ne(m)
-    double2* d_ab = nullptr;        // (-alpha_n, alpha_n + beta_n) of the x^2-stepping recurrence
+    double2* d_ab = nullptr;        // (-alpha_n, alpha_n + beta_n) of the x^2-stepping recurrence (sin^2 form), followed at
+                                    // + n_e_total by (alpha_n, beta_n), the cos^2 form used by the blocks next to the equator
     double* d_sig = nullptr;        // sigma_n: even-class scaling
     double* d_sodd = nullptr;       // sigma_n / c_{m+2n+1}: odd-class scaling
     double* d_rho = nullptr;        // c_{m+2n+2}/c_{m+2n+3}: odd-class fold ratio
-    double* d_x2 = nullptr;         // sin^2(theta_j) per ring pair (t_n = ab.y + ab.x sin^2 theta)
+    double* d_x2 = nullptr;         // operand of t_n per ring pair, synthesis decomposition: sin^2(theta_j) for blocks
+                                    // before j_quarter, cos^2(theta_j) after (legendre.cu header)
+    double* d_x2a = nullptr;        // the same for the adjoint's decomposition (more pairs per block)
+    int j_quarter = 0;              // first ring pair with theta >= pi/4 (pairs run from the poles to the equator)
     double* d_x = nullptr;          // cos(theta_j)
     double2* d_logsin = nullptr;    // log2 sin(theta_j) as (hi, lo)
     double2* d_logkap = nullptr;    // log2 |Pbar_mm| prefactor per m as (hi, lo)
@@ -91,6 +96,10 @@ struct nusht_plan_s {
     int* d_ffa_n = nullptr;         // the same for the adjoint's decomposition (more ring pairs per thread)
     double2* d_ffa_p = nullptr;
     int* d_ffa_e = nullptr;
+    int* d_pair_n = nullptr;        // ring-list mode: ring index of the north member of pair j
+    int* d_pair_s = nullptr;        //   and of its mirror ring (theta_s = pi - theta_n), -1 if the grid has none
+    const double* h_ring_theta = nullptr;   // ring-list mode: HOST colatitudes, valid during legendre_build_tables only
+    int lmax_io = 0;                // band limit of the caller's alm layout (= lmax except in ring plans built one degree higher)
     int2* d_items_syn = nullptr;    // work list of the Legendre synthesis: (block of ring pairs, m) per CTA, longest first
     int n_items_syn = 0;
     // --- Legendre work buffers ---
@@ -136,6 +145,10 @@ struct nusht_plan_s {
 
 // ---- legendre.cu ----
 int legendre_build_tables(nusht_plan_s* p);
+// pairs rings theta_a + theta_b = pi (to 2 ulp of pi); pair_n / pair_s (size >= nrings) receive the ring indices of
+// each pair (pair_s = -1 for a ring without mirror), pairs ordered by increasing distance from the nearer pole.
+// Returns the number of pairs.  Host only.
+int legendre_pair_rings(int nrings, const double* theta, int* pair_n, int* pair_s);
 int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s);
 int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s);
 int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s);

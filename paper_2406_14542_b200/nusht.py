@@ -24,6 +24,8 @@ EXPORTS = [
     "nusht_stage_interp", "nusht_stage_spread", "nusht_set_stage_timing", "nusht_stage_times",
     "nusht_plan_info", "nusht_strerror", "nusht_version", "nusht_pointing", "nusht_host_reserve",
     "nusht_stage_fourier_synthesis", "nusht_stage_fourier_adjoint", "nusht_launch_count", "nusht_probe_fp64",
+    "nusht_ring_plan", "nusht_ring_synthesis", "nusht_ring_analysis", "nusht_ring_gradient", "nusht_ring_info",
+    "nusht_ring_destroy", "nusht_ring_pairing",
 ]
 
 
@@ -36,6 +38,15 @@ class NushtInfo(ctypes.Structure):
         ("kernel_beta", ctypes.c_double), ("sigma", ctypes.c_double),
         ("workspace_bytes", ctypes.c_int64), ("plan_ms", ctypes.c_double), ("sort_ms", ctypes.c_double),
         ("legendre_fma_synthesis", ctypes.c_int64), ("legendre_fma_adjoint", ctypes.c_int64),
+    ]
+
+
+class NushtRingInfo(ctypes.Structure):
+    _fields_ = [
+        ("lmax", ctypes.c_int), ("mmax", ctypes.c_int), ("dtype", ctypes.c_int), ("nrings", ctypes.c_int),
+        ("npairs", ctypes.c_int), ("nruns", ctypes.c_int),
+        ("npix", ctypes.c_int64), ("nlm", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64),
+        ("plan_ms", ctypes.c_double),
     ]
 
 
@@ -76,6 +87,20 @@ def _load():
     lib.nusht_plan_info.restype = ip
     lib.nusht_pointing.argtypes = [ctypes.c_int64, vp, vp, vp, vp, vp, vp, vp]
     lib.nusht_pointing.restype = ip
+    dp, lp = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64)
+    lib.nusht_ring_plan.argtypes = [ctypes.POINTER(vp), ip, ip, ip, dp, lp, dp, dp, ip]
+    lib.nusht_ring_plan.restype = ip
+    for name in ("nusht_ring_synthesis", "nusht_ring_analysis"):
+        getattr(lib, name).argtypes = [vp, vp, vp, vp]
+        getattr(lib, name).restype = ip
+    lib.nusht_ring_gradient.argtypes = [vp, vp, vp, vp, vp]
+    lib.nusht_ring_gradient.restype = ip
+    lib.nusht_ring_info.argtypes = [vp, ctypes.POINTER(NushtRingInfo)]
+    lib.nusht_ring_info.restype = ip
+    lib.nusht_ring_destroy.argtypes = [vp]
+    lib.nusht_ring_destroy.restype = ip
+    lib.nusht_ring_pairing.argtypes = [ip, dp, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int)]
+    lib.nusht_ring_pairing.restype = ip
     lib.nusht_strerror.argtypes = [ip]
     lib.nusht_strerror.restype = ctypes.c_char_p
     lib.nusht_version.restype = ctypes.c_char_p
@@ -237,6 +262,97 @@ class Plan:
         _check(lib.nusht_stage_times(self._h, 0 if which in (0, "synthesis") else 1, buf, NUM_STAGES))
         names = SYN_STAGES if which in (0, "synthesis") else ADJ_STAGES
         return {n: float(buf[i]) for i, n in enumerate(names)}
+
+
+class RingPlan:
+    """nusht_ring_plan(lmax, mmax, nrings, theta, nphi, phi0, weight, dtype): transforms on a ring grid.  theta, nphi,
+    phi0, weight are HOST sequences (numpy arrays / lists) of one entry per ring; maps are CUDA tensors of npix reals."""
+
+    def __init__(self, lmax, mmax, theta, nphi, phi0=None, weight=None, dtype="f64"):
+        import numpy as np
+        self._h = ctypes.c_void_p()
+        if dtype in ("f64", NUSHT_F64):
+            self.dtype = NUSHT_F64
+        elif dtype in ("f32", NUSHT_F32):
+            self.dtype = NUSHT_F32
+        else:
+            raise ValueError("dtype must be 'f64' or 'f32'")
+        th = np.ascontiguousarray(theta, dtype=np.float64)
+        n = np.ascontiguousarray(nphi, dtype=np.int64)
+        if th.ndim != 1 or n.shape != th.shape:
+            raise ValueError("theta and nphi must be 1-D with one entry per ring")
+        dp, lp = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64)
+
+        def opt(a):
+            if a is None:
+                return None, None
+            a = np.ascontiguousarray(a, dtype=np.float64)
+            if a.shape != th.shape:
+                raise ValueError("phi0 / weight must have one entry per ring")
+            return a, a.ctypes.data_as(dp)
+        p0, p0p = opt(phi0)
+        w, wp = opt(weight)
+        _check(lib.nusht_ring_plan(ctypes.byref(self._h), int(lmax), int(mmax), int(th.shape[0]), th.ctypes.data_as(dp),
+                                   n.ctypes.data_as(lp), p0p, wp, self.dtype))
+        self.info = NushtRingInfo()
+        _check(lib.nusht_ring_info(self._h, ctypes.byref(self.info)))
+        self.lmax, self.mmax, self.npix, self.nlm = int(lmax), int(mmax), int(self.info.npix), int(self.info.nlm)
+        self.rdtype = torch.float64 if self.dtype == NUSHT_F64 else torch.float32
+        self.cdtype = torch.complex128 if self.dtype == NUSHT_F64 else torch.complex64
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib.nusht_ring_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def _alm_arg(self, alm):
+        if alm.dtype != self.cdtype or alm.numel() != self.nlm or not alm.is_cuda or not alm.is_contiguous():
+            raise TypeError("alm must be a contiguous CUDA %s tensor of %d entries" % (self.cdtype, self.nlm))
+        return alm.data_ptr()
+
+    def _map_arg(self, m):
+        if m.dtype != self.rdtype or m.numel() != self.npix or not m.is_cuda or not m.is_contiguous():
+            raise TypeError("map must be a contiguous CUDA %s tensor of %d entries" % (self.rdtype, self.npix))
+        return m.data_ptr()
+
+    def synthesis(self, alm, out=None, stream=None):
+        if out is None:
+            out = torch.empty(self.npix, dtype=self.rdtype, device="cuda")
+        _check(lib.nusht_ring_synthesis(self._h, self._alm_arg(alm), self._map_arg(out), _stream_ptr(stream)))
+        return out
+
+    def analysis(self, m, out=None, stream=None):
+        if out is None:
+            out = torch.empty(self.nlm, dtype=self.cdtype, device="cuda")
+        _check(lib.nusht_ring_analysis(self._h, self._map_arg(m), self._alm_arg(out), _stream_ptr(stream)))
+        return out
+
+    def gradient(self, philm, stream=None):
+        a_t = torch.empty(self.npix, dtype=self.rdtype, device="cuda")
+        a_p = torch.empty(self.npix, dtype=self.rdtype, device="cuda")
+        _check(lib.nusht_ring_gradient(self._h, self._alm_arg(philm), a_t.data_ptr(), a_p.data_ptr(),
+                                       _stream_ptr(stream)))
+        return a_t, a_p
+
+
+def ring_pairing(theta):
+    """Pairs of mirror rings as the ring plan forms them (nusht_ring_pairing; host only): list of (north, south | -1)."""
+    import numpy as np
+    th = np.ascontiguousarray(theta, dtype=np.float64)
+    pn = np.empty(len(th), dtype=np.int32)
+    ps = np.empty(len(th), dtype=np.int32)
+    ip = ctypes.POINTER(ctypes.c_int)
+    n = lib.nusht_ring_pairing(len(th), th.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), pn.ctypes.data_as(ip),
+                               ps.ctypes.data_as(ip))
+    if n < 0:
+        _check(n)
+    return [(int(pn[j]), int(ps[j])) for j in range(n)]
 
 
 def launch_count() -> int:

@@ -36,8 +36,10 @@ def test_hot_kernels_keep_their_occupancy_step():
     assert len(res) > 50
     # (mangled-name fragments, max registers, threads per CTA, CTAs per SM that must still fit)
     cases = [
-        (("k_legendre_synth", "ILi4E"), 32, 16),
-        (("k_legendre_adjoint", "ILi5ELi8E"), 32, 16),
+        (("k_legendre_synth", "ILi4ELb0E"), 32, 16),
+        (("k_legendre_adjoint", "ILi5ELi8ELb0E"), 32, 16),
+        (("k_legendre_synth", "ILi4ELb1E"), 32, 16),          # ring-list variants (rSHT front end)
+        (("k_legendre_adjoint", "ILi5ELi8ELb1E"), 32, 16),
         (("k_interp_mma", "ILi11E"), 128, 6),
         (("k_spread_mma", "ILi11E"), 128, 5),
         (("k_interp_mma", "ILi9E"), 128, 6),

@@ -394,3 +394,85 @@ def test_ring_sum_single_coefficient_vs_mpmath_golden(oracle):
             assert abs(F - ref) <= tol * abs(ref), (l, m, th, prec, F, ref)
         n += 1
     assert n >= 8
+
+
+# ---- gradient of the lensing potential (Eq. C2) --------------------------------------------------
+def _grad_closed_form(l, m, a, th, ph):
+    """(d/dtheta, (1/sin theta) d/dphi) of w_m Re(a Y_lm), from the textbook table of Y_lm for l <= 2."""
+    s, c = np.sin(th), np.cos(th)
+    e = np.exp(1j * m * ph)
+    dtab = {     # (P(theta), dP/dtheta) with Y_lm = P e^{i m phi}
+        (1, 0): (np.sqrt(3 / (4 * np.pi)) * c, -np.sqrt(3 / (4 * np.pi)) * s),
+        (1, 1): (-np.sqrt(3 / (8 * np.pi)) * s, -np.sqrt(3 / (8 * np.pi)) * c),
+        (2, 0): (np.sqrt(5 / (16 * np.pi)) * (3 * c * c - 1), -np.sqrt(5 / (16 * np.pi)) * 6 * c * s),
+        (2, 1): (-np.sqrt(15 / (8 * np.pi)) * s * c, -np.sqrt(15 / (8 * np.pi)) * (c * c - s * s)),
+        (2, 2): (np.sqrt(15 / (32 * np.pi)) * s * s, np.sqrt(15 / (32 * np.pi)) * 2 * s * c),
+    }
+    P, dP = dtab[(l, m)]
+    wm = 1.0 if m == 0 else 2.0
+    return wm * np.real(a * dP * e), wm * np.real(a * 1j * m * P * e) / s
+
+
+@pytest.mark.parametrize("l,m", [(1, 0), (1, 1), (2, 0), (2, 1), (2, 2)])
+@pytest.mark.parametrize("prec", ["d", "ld"])
+def test_gradient_closed_forms(oracle, l, m, prec):
+    rng = np.random.default_rng(40 + l * 3 + m)
+    th = np.arccos(rng.uniform(-0.999, 0.999, 300))
+    ph = rng.uniform(0, 2 * np.pi, 300)
+    a = 0.7 - 1.3j if m > 0 else 0.7 + 0j
+    gt, gp = oracle.gradient(5, 4, th, ph, single_alm(5, 4, l, m, a), prec)
+    rt, rp = _grad_closed_form(l, m, a, th, ph)
+    assert np.max(np.abs(gt - rt)) < 5e-15 and np.max(np.abs((gp - rp) * np.sin(th))) < 5e-15
+
+
+def test_gradient_vs_finite_differences_of_synthesis(oracle):
+    """alpha_theta = dPhi/dtheta and alpha_phi = (1/sin theta) dPhi/dphi against 5-point central differences (h = 1e-4:
+    truncation ~ h^4 l^5 / 30, round-off ~ 1e-16 / h) of the oracle's synthesis, itself pinned above."""
+    lmax, mmax = 40, 33
+    a = inputs.random_alm(lmax, mmax, 44)
+    rng = np.random.default_rng(45)
+    th = np.arccos(rng.uniform(-0.98, 0.98, 400))
+    ph = rng.uniform(0.1, 6.1, 400)
+    h = 1e-4
+
+    def d5(f):
+        return (f(-2 * h) - 8 * f(-h) + 8 * f(h) - f(2 * h)) / (12 * h)
+    dt = d5(lambda e: oracle.synthesis(lmax, mmax, th + e, ph, a, "ld"))
+    dph = d5(lambda e: oracle.synthesis(lmax, mmax, th, ph + e, a, "ld")) / np.sin(th)
+    gt, gp = oracle.gradient(lmax, mmax, th, ph, a, "ld")
+    scale = np.sqrt(np.mean(gt ** 2))
+    assert np.max(np.abs(gt - dt)) < 2e-8 * scale
+    assert np.max(np.abs((gp - dph) * np.sin(th))) < 2e-8 * scale
+
+
+@pytest.mark.parametrize("prec", ["d", "ld"])
+def test_gradient_rescaling_regime_vs_coefficient_identity(oracle, prec):
+    """lmax = 1500 with near-pole points: sin^m theta underflows and the gradient's copy of the l loop goes through
+    its own exponent refresh.  Pin: the ladder identity sin(theta) dPbar_lm/dtheta = l c_{l+1} Pbar_{l+1,m} -
+    (l+1) c_l Pbar_{l-1,m}, c_l^2 = (l^2 - m^2)/(4 l^2 - 1) (a DIFFERENT relation from the one the oracle sums), turns
+    sin(theta) dPhi/dtheta into a plain synthesis at band limit lmax + 1, evaluated by oracle.synthesis (pinned to
+    mpmath in this regime above); likewise dPhi/dphi is the synthesis of i m Phi_lm."""
+    L = M = 1500
+    th, ph = _near_pole_points(60, 46)
+    phl = inputs.random_alm(L, M, 46, "inv_l2")
+    gt, gp = oracle.gradient(L, M, th, ph, phl, prec)
+    L1 = L + 1
+    a1 = np.zeros(inputs.nlm(L1, M), dtype=np.complex128)
+    b1 = np.zeros(inputs.nlm(L1, M), dtype=np.complex128)
+    for m in range(M + 1):
+        l = np.arange(m, L + 1, dtype=np.float64)
+        p = phl[inputs.lm_index(L, m, m): inputs.lm_index(L, m, m) + L - m + 1]
+        c = lambda ll: np.sqrt((ll * ll - m * m) / (4 * ll * ll - 1))        # noqa: E731
+        o1 = inputs.lm_index(L1, m, m)
+        # Phi_lm contributes l c_{l+1} to l' = l + 1 and -(l + 1) c_l to l' = l - 1
+        a1[o1 + 1: o1 + 1 + len(l)] += l * c(l + 1) * p
+        a1[o1: o1 + len(l) - 1] += (-(l + 1) * c(l) * p)[1:]
+        b1[o1: o1 + len(l)] = 1j * m * p
+    if True:
+        a1[: L1 + 1] = a1[: L1 + 1].real
+    st = oracle.synthesis(L1, M, th, ph, a1, prec)
+    sp = oracle.synthesis(L1, M, th, ph, b1, prec)
+    scale = np.sqrt(np.mean(st ** 2))
+    tol = 2e-11 if prec == "d" else 2e-13
+    assert np.max(np.abs(gt * np.sin(th) - st)) <= tol * scale
+    assert np.max(np.abs(gp * np.sin(th) - sp)) <= tol * scale
