@@ -128,6 +128,16 @@ def oracle_sample(cfg, theta, phi, alm, x, seconds):
                      "steps_per_s": 2 * nlm * n / (t_syn + t_adj)}
 
 
+def oracle_points(cfg, theta, phi, sl=slice(None)):
+    """The checker's point set: Eq. C1 by oracle.pointing for the lensing-like config, the points themselves else."""
+    if cfg.get("deflection") is None:
+        return theta[sl], phi[sl]
+    from oracle import oracle as o
+    a_t, a_p = cfg["deflection"]
+    t2, p2 = o.pointing(theta[sl], phi[sl], a_t[sl], a_p[sl])
+    return np.asarray(t2, dtype=np.float64), np.asarray(p2, dtype=np.float64)
+
+
 def run_reference(args, rank):
     if rank != 0:
         return
@@ -136,6 +146,7 @@ def run_reference(args, rank):
     # the oracle only ever sees a sample: generate just a prefix-sized workload with the config's recipe
     nsample = min(npts_full, 1 << 16)
     cfg2, theta, phi, alm, x = inputs.make_config(args.config, npts=nsample)
+    theta, phi = oracle_points(cfg2, theta, phi)
     vals, last = [], None
     per_step = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
     for i in range(args.warmup + args.steps):
@@ -283,6 +294,8 @@ def run_b200(args, rank, world):
     npts = len(theta)
     L, M, eps = cfg["lmax"], cfg["mmax"], cfg["eps"]
     d_theta, d_phi = torch.from_numpy(theta).cuda(), torch.from_numpy(phi).cuda()
+    if cfg["deflection"] is not None:      # lensing-like config: the points are the deflected pixels, Eq. C1 on the GPU
+        d_theta, d_phi = nusht.nusht_pointing(d_theta, d_phi, *(torch.from_numpy(a).cuda() for a in cfg["deflection"]))
     plan = nusht.Plan(L, M, d_theta, d_phi, eps, cfg["dtype"])
     del d_theta, d_phi
     d_alm, d_x = torch.from_numpy(alm).cuda(), torch.from_numpy(x).cuda()
@@ -410,7 +423,8 @@ def run_b200(args, rank, world):
     }
     if not args.no_cpu_baseline and world == 1:
         ns = min(npts, 1 << 16)
-        _, desc = oracle_sample(cfg, theta[:ns], phi[:ns], alm, x[:ns], args.cpu_seconds)
+        o_theta, o_phi = oracle_points(cfg, theta, phi, slice(0, ns))
+        _, desc = oracle_sample(cfg, o_theta, o_phi, alm, x[:ns], args.cpu_seconds)
         desc["value"] *= npts / ns
         desc["sample"] += "; then x%.0f from the %d-point prefix to %d points" % (npts / ns, ns, npts)
         out["cpu_baseline"] = desc
@@ -430,11 +444,14 @@ def run_eps_sweep(args):
     L, M, npts = cfg["lmax"], cfg["mmax"], len(theta)
     rng = np.random.default_rng(12345)
     sub = np.sort(rng.choice(npts, min(args.sweep_subset, npts), replace=False))
-    f_ref = o.synthesis(L, M, theta[sub], phi[sub], alm, "ld")
+    o_theta, o_phi = oracle_points(cfg, theta, phi, sub)
+    f_ref = o.synthesis(L, M, o_theta, o_phi, alm, "ld")
     xs = np.zeros(npts)
     xs[sub] = x[sub]
-    c_ref = o.adjoint(L, M, theta[sub], phi[sub], x[sub], "ld")
+    c_ref = o.adjoint(L, M, o_theta, o_phi, x[sub], "ld")
     d_theta, d_phi = torch.from_numpy(theta).cuda(), torch.from_numpy(phi).cuda()
+    if cfg["deflection"] is not None:
+        d_theta, d_phi = nusht.nusht_pointing(d_theta, d_phi, *(torch.from_numpy(a).cuda() for a in cfg["deflection"]))
     for dtype, eps in (("f32", 1e-4), ("f32", 1e-6), ("f64", 1e-8), ("f64", 1e-10), ("f64", 1e-12)):
         plan = nusht.Plan(L, M, d_theta, d_phi, eps, dtype)
         rd, cd = (np.float32, np.complex64) if dtype == "f32" else (np.float64, np.complex128)

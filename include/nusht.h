@@ -115,6 +115,18 @@ typedef struct {
 NUSHT_API int nusht_plan(nusht_plan_t** out, int lmax, int mmax, int64_t npts, const double* theta,
                const double* phi, double eps, int dtype);
 
+/* Plan options.  sigma: up-sampling factor of the nuFFT grid, 2 (default; 0 means default) or 1.25, the paper's own
+ * choice "to reduce the memory usage at a small price of increased computation time": the fine grid
+ * shrinks by (1.25/2)^2 while the kernel widens (w = 17 instead of 11 at eps = 1e-10).  At sigma = 1.25 eps is limited
+ * to [1e-10, 1e-1] in FP64 (the floor the paper states, fn. 6 at PAPER.md:164) and [1e-5, 1e-1] in FP32.
+ * Other values of sigma: NUSHT_ERR_INVALID_ARG.  nusht_plan(...) == nusht_plan_ex(..., NULL). */
+typedef struct {
+    double sigma;
+    int reserved[6];    /* must be zero */
+} nusht_opts_t;
+NUSHT_API int nusht_plan_ex(nusht_plan_t** out, int lmax, int mmax, int64_t npts, const double* theta,
+                            const double* phi, double eps, int dtype, const nusht_opts_t* opts);
+
 /* Synthesis, Eq. 3 / Eq. 5: alm (DEVICE, nlm complex) -> map (DEVICE, npts real).  npts == 0: no-op. */
 NUSHT_API int nusht_synthesis(nusht_plan_t* plan, const void* alm, void* map, void* stream);
 

@@ -83,13 +83,22 @@ extern "C" int nusht_destroy(nusht_plan_t* plan) {
 
 extern "C" int nusht_plan(nusht_plan_t** out, int lmax, int mmax, int64_t npts, const double* theta,
                           const double* phi, double eps, int dtype) {
+    return nusht_plan_ex(out, lmax, mmax, npts, theta, phi, eps, dtype, nullptr);
+}
+
+extern "C" int nusht_plan_ex(nusht_plan_t** out, int lmax, int mmax, int64_t npts, const double* theta,
+                             const double* phi, double eps, int dtype, const nusht_opts_t* opts) {
     if (!out) return NUSHT_ERR_INVALID_ARG;
     *out = nullptr;
     if (lmax < 0 || mmax < 0 || mmax > lmax || npts < 0 || npts >= ((int64_t)1 << 31)) return NUSHT_ERR_INVALID_ARG;
     if (dtype != NUSHT_F64 && dtype != NUSHT_F32) return NUSHT_ERR_INVALID_ARG;
+    double sigma = 2.0;
+    if (opts && opts->sigma != 0.0) sigma = opts->sigma;
+    if (sigma != 2.0 && sigma != 1.25) return NUSHT_ERR_INVALID_ARG;
     if (!(eps <= 1e-1)) return NUSHT_ERR_INVALID_ARG;
-    if (dtype == NUSHT_F64 && !(eps >= 1e-13)) return NUSHT_ERR_INVALID_ARG;
-    if (dtype == NUSHT_F32 && !(eps >= 1e-6)) return NUSHT_ERR_INVALID_ARG;
+    // accuracy floors: FP64 1e-13 at sigma = 2, 1e-10 at sigma = 1.25 (the paper's fn. 6); FP32 1e-6 / 1e-5
+    if (dtype == NUSHT_F64 && !(eps >= (sigma == 2.0 ? 1e-13 : 1e-10))) return NUSHT_ERR_INVALID_ARG;
+    if (dtype == NUSHT_F32 && !(eps >= (sigma == 2.0 ? 1e-6 : 1e-5))) return NUSHT_ERR_INVALID_ARG;
     if (npts > 0 && (!theta || !phi)) return NUSHT_ERR_INVALID_ARG;
     if (lmax > 32000) return NUSHT_ERR_UNSUPPORTED;
 
@@ -105,6 +114,7 @@ extern "C" int nusht_plan(nusht_plan_t** out, int lmax, int mmax, int64_t npts, 
     p->npts = npts;
     p->eps = eps;
     p->dtype = dtype;
+    p->sigma = sigma;
     p->device = dev;
     p->nlm = (int64_t)(mmax + 1) * (lmax + 1) - (int64_t)mmax * (mmax + 1) / 2;
 
@@ -119,9 +129,11 @@ extern "C" int nusht_plan(nusht_plan_t** out, int lmax, int mmax, int64_t npts, 
         p->lg.npairs = (p->lg.nr + 1) / 2;
         p->lg.has_equator = p->lg.nr & 1;
         p->lg.ring_mode = 0;
-        // fine grid: up-sampling sigma = 2 of the 2 lmax + 2 (2 mmax + 2) Fourier modes (reading G7)
+        // fine grid: up-sampling sigma (2, or the paper's 1.25: PAPER.md:152) of the 2 lmax + 2 (2 mmax + 2) Fourier
+        // modes (reading G7)
         const int w = p->ng.w;
-        int nth = 2 * (2 * lmax + 2), nph = 2 * (2 * mmax + 2);
+        int nth = (int)ceil(sigma * (2 * lmax + 2)), nph = (int)ceil(sigma * (2 * mmax + 2));
+        p->fourier_general = sigma != 2.0;
         if (nth < 2 * w + 2) nth = 2 * w + 2;
         if (nph < 2 * w + 2) nph = 2 * w + 2;
         p->ng.nth = good_even_size(nth);

@@ -95,6 +95,111 @@ __global__ void k_deconv_trunc(int L, int M, int nth2, int nh, const typename Cp
     ft[(int64_t)m * nth2 + r] = out;
 }
 
+// ---------------------------------------------------------------------------------------------
+// General chain (up-sampling sigma != 2, the paper's 1.25: PAPER.md:152).  The two-half-length trick above needs
+// n_theta/2 >= 2 lmax + 1 and the half-length real-FFT trick below needs mmax < n_phi/4; neither holds at
+// sigma = 1.25, so here the fine theta transform is ONE full-length complex FFT per column and the phi transform a
+// real (C2R / R2C) cuFFT out of place between a half-spectrum buffer Z[a][m], m = 0 .. n_phi/2, and the grid rows:
+//   synthesis  c[m,k] --(p_theta p_phi, zero-pad)--> H[m][k mod n_theta] --iFFT--> H[m][a] --transpose-->
+//              Z[a][m] (a <= n_theta/2; zero for m > mmax) --C2R--> g[a][b]   (the Hermitian extension of the C2R
+//              supplies the weights w_m of the real field)
+//   adjoint    g --R2C--> Z[a][m] --transpose, zero-extend a > n_theta/2--> H[m][a] --FFT--> truncate, deconvolve.
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void k_deconv_pad_gen(int L, int M, int nth2, int nth, const double2* __restrict__ ft,
+                                 const double* __restrict__ pth, const double* __restrict__ pph,
+                                 typename Cplx<T>::type* __restrict__ h) {
+    const int kp = blockIdx.x * blockDim.x + threadIdx.x;
+    const int m = blockIdx.y;
+    if (kp >= nth) return;
+    int k;
+    bool in = true;
+    if (kp <= L) k = kp;
+    else if (kp >= nth - L) k = kp - nth;
+    else { k = 0; in = false; }
+    typename Cplx<T>::type v;
+    v.x = v.y = 0;
+    if (in) {
+        const double2 c = ft[(int64_t)m * nth2 + (k >= 0 ? k : k + nth2)];
+        const double f = pth[k + L] * pph[m];
+        v.x = (T)(c.x * f);
+        v.y = (T)(c.y * f);
+    }
+    h[(int64_t)m * nth + kp] = v;
+}
+
+template <typename T>
+__global__ void k_deconv_trunc_gen(int L, int M, int nth2, int nth, const typename Cplx<T>::type* __restrict__ h,
+                                   const double* __restrict__ pth, const double* __restrict__ pph,
+                                   double2* __restrict__ ft) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const int m = blockIdx.y;
+    if (r >= nth2) return;
+    int k;
+    bool in = true;
+    if (r <= L) k = r;
+    else if (r >= nth2 - L) k = r - nth2;
+    else { k = 0; in = false; }
+    double2 out = make_double2(0.0, 0.0);
+    if (in) {
+        const typename Cplx<T>::type v = h[(int64_t)m * nth + (k >= 0 ? k : k + nth)];
+        const double f = pth[k + L] * pph[m];
+        out.x = (double)v.x * f;
+        out.y = (double)v.y * f;
+    }
+    ft[(int64_t)m * nth2 + r] = out;
+}
+
+// H[m][a] -> Z[a][m], rows a < nrow_half; columns mmax < m <= n_phi/2 are zeroed, Im Z[a][0] := 0 (a real row)
+template <typename C>
+__global__ void __launch_bounds__(256)
+k_h_to_zc(int M, int nth, int nrow_half, int nzc, const C* __restrict__ h, C* __restrict__ z) {
+    __shared__ C tile[32][33];
+    const int a0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int m = m0 + r, a = a0 + tx;
+        if (m <= M && a < nrow_half) tile[r][tx] = h[(int64_t)m * nth + a];
+    }
+    __syncthreads();
+    C zero;
+    zero.x = 0;
+    zero.y = 0;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int a = a0 + r, m = m0 + tx;
+        if (a >= nrow_half || m >= nzc) continue;
+        C v = (m <= M) ? tile[tx][r] : zero;
+        if (m == 0) v.y = 0;
+        z[(int64_t)a * nzc + m] = v;
+    }
+}
+
+// Z[a][m] -> H[m][a] for a < nrow_half, H[m][a] = 0 for the rest of the theta period (transpose of "keep rows 0 .. n_theta/2")
+template <typename C>
+__global__ void __launch_bounds__(256)
+k_zc_to_h(int M, int nth, int nrow_half, int nzc, const C* __restrict__ z, C* __restrict__ h) {
+    __shared__ C tile[32][33];
+    const int a0 = blockIdx.x * 32, m0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int a = a0 + r, m = m0 + tx;
+        if (a < nrow_half && m <= M) tile[r][tx] = z[(int64_t)a * nzc + m];
+    }
+    __syncthreads();
+    C zero;
+    zero.x = 0;
+    zero.y = 0;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int m = m0 + r, a = a0 + tx;
+        if (m > M || a >= nth) continue;
+        h[(int64_t)m * nth + a] = (a < nrow_half) ? tile[tx][r] : zero;
+    }
+}
+
 // a5 / a9, phi pass.  The real transform of length N = n_phi on row a is done as ONE complex transform of
 // length N/2 on the row itself (the real row viewed as N/2 complex numbers x[2j] + i x[2j+1]), with the
 // usual pre-/post-processing of a real FFT fused into the transposes between the theta-pass layout
@@ -772,6 +877,34 @@ int fourier_build(nusht_plan_s* p) {
     NUSHT_CUDA_TRY(cudaMemset(p->d_h, 0, hbytes));
     NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
 
+    if (p->fourier_general) {
+        // sigma != 2: plain cuFFT chain (see k_deconv_pad_gen)
+        p->theta_chain = 0;
+        p->theta_fused = false;
+        const size_t zbytes = (size_t)g.nrow_half * (size_t)(g.nph / 2 + 1) * csz;
+        NUSHT_TRY(f_alloc(&p->d_z, zbytes, p));
+        size_t ws = 0, wtot = 0;
+        int n1[1] = {nth2}, n2[1] = {g.nth}, n3[1] = {g.nph};
+        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_theta_coarse));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_coarse, 1, n1, nullptr, 1, nth2, nullptr, 1, nth2, CUFFT_Z2Z, M + 1, &ws));
+        wtot += ws;
+        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_theta_fine));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_fine, 1, n2, nullptr, 1, g.nth, nullptr, 1, g.nth,
+                                          f64 ? CUFFT_Z2Z : CUFFT_C2C, M + 1, &ws));
+        wtot += ws;
+        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi, 1, n3, nullptr, 1, 0, nullptr, 1, 0, f64 ? CUFFT_Z2D : CUFFT_C2R,
+                                          g.nrow_half, &ws));
+        wtot += ws;
+        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi_r2c));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_r2c, 1, n3, nullptr, 1, 0, nullptr, 1, 0, f64 ? CUFFT_D2Z : CUFFT_R2C,
+                                          g.nrow_half, &ws));
+        wtot += ws;
+        p->workspace_bytes += (int64_t)wtot;
+        p->have_fft = true;
+        return NUSHT_OK;
+    }
+
     // fused theta chains: coarse length == half fine length, a power of two.  theta_chain = 1: one CTA per
     // column (128 <= N <= 8192, the default there: 0.73 / 0.84 ms against 0.76 / 0.87 ms at N = 8192);
     // 2: a cluster pair per column (2048 <= N <= 16384; the default at 16384, where one SM cannot hold a column)
@@ -870,7 +1003,74 @@ int fourier_build(nusht_plan_s* p) {
 
 // synthesis: d_ft (Ftilde) -> d_grid.  ev (optional) = events at the boundaries of stages 2..5:
 // ev[0] before a3, ev[1] after a3, ev[2] after a4, ev[3] after a5-theta, ev[4] after a5-phi.
+static int fourier_synthesis_general(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
+    const int L = p->lmax, M = p->mmax;
+    const NufftGeom& g = p->ng;
+    const int nth2 = p->lg.nth2, nzc = g.nph / 2 + 1;
+    const bool f64 = p->dtype == NUSHT_F64;
+    REC(0);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_coarse, s));
+    NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_coarse, (cufftDoubleComplex*)p->d_ft, (cufftDoubleComplex*)p->d_ft, CUFFT_FORWARD));
+    REC(1);
+    {
+        dim3 grid((g.nth + 255) / 256, M + 1);
+        if (f64) k_deconv_pad_gen<double><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, p->d_ft, p->d_pth, p->d_pph, (double2*)p->d_h);
+        else k_deconv_pad_gen<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, p->d_ft, p->d_pth, p->d_pph, (float2*)p->d_h);
+        NUSHT_CUDA_TRY(nusht_launched());
+    }
+    REC(2);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_fine, s));
+    if (f64) NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_fine, (cufftDoubleComplex*)p->d_h, (cufftDoubleComplex*)p->d_h, CUFFT_INVERSE));
+    else NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_theta_fine, (cufftComplex*)p->d_h, (cufftComplex*)p->d_h, CUFFT_INVERSE));
+    REC(3);
+    {
+        dim3 grid((g.nrow_half + 31) / 32, (nzc + 31) / 32);
+        if (f64) k_h_to_zc<double2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, nzc, (const double2*)p->d_h, (double2*)p->d_z);
+        else k_h_to_zc<float2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, nzc, (const float2*)p->d_h, (float2*)p->d_z);
+        NUSHT_CUDA_TRY(nusht_launched());
+    }
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi, s));
+    if (f64) NUSHT_CUFFT_TRY(cufftExecZ2D(p->fft_phi, (cufftDoubleComplex*)p->d_z, (double*)p->d_grid));
+    else NUSHT_CUFFT_TRY(cufftExecC2R(p->fft_phi, (cufftComplex*)p->d_z, (float*)p->d_grid));
+    REC(4);
+    return NUSHT_OK;
+}
+
+static int fourier_adjoint_general(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
+    const int L = p->lmax, M = p->mmax;
+    const NufftGeom& g = p->ng;
+    const int nth2 = p->lg.nth2, nzc = g.nph / 2 + 1;
+    const bool f64 = p->dtype == NUSHT_F64;
+    REC(0);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi_r2c, s));
+    if (f64) NUSHT_CUFFT_TRY(cufftExecD2Z(p->fft_phi_r2c, (double*)p->d_grid, (cufftDoubleComplex*)p->d_z));
+    else NUSHT_CUFFT_TRY(cufftExecR2C(p->fft_phi_r2c, (float*)p->d_grid, (cufftComplex*)p->d_z));
+    {
+        dim3 grid((g.nth + 31) / 32, (M + 32) / 32);
+        if (f64) k_zc_to_h<double2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, nzc, (const double2*)p->d_z, (double2*)p->d_h);
+        else k_zc_to_h<float2><<<grid, 256, 0, s>>>(M, g.nth, g.nrow_half, nzc, (const float2*)p->d_z, (float2*)p->d_h);
+        NUSHT_CUDA_TRY(nusht_launched());
+    }
+    REC(1);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_fine, s));
+    if (f64) NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_fine, (cufftDoubleComplex*)p->d_h, (cufftDoubleComplex*)p->d_h, CUFFT_FORWARD));
+    else NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_theta_fine, (cufftComplex*)p->d_h, (cufftComplex*)p->d_h, CUFFT_FORWARD));
+    REC(2);
+    {
+        dim3 grid((nth2 + 255) / 256, M + 1);
+        if (f64) k_deconv_trunc_gen<double><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, (const double2*)p->d_h, p->d_pth, p->d_pph, p->d_ft);
+        else k_deconv_trunc_gen<float><<<grid, 256, 0, s>>>(L, M, nth2, g.nth, (const float2*)p->d_h, p->d_pth, p->d_pph, p->d_ft);
+        NUSHT_CUDA_TRY(nusht_launched());
+    }
+    REC(3);
+    NUSHT_CUFFT_TRY(cufftSetStream(p->fft_theta_coarse, s));
+    NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_theta_coarse, (cufftDoubleComplex*)p->d_ft, (cufftDoubleComplex*)p->d_ft, CUFFT_INVERSE));
+    REC(4);
+    return NUSHT_OK;
+}
+
 int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
+    if (p->fourier_general) return fourier_synthesis_general(p, s, ev);
     const int L = p->lmax, M = p->mmax;
     const NufftGeom& g = p->ng;
     const int nth2 = p->lg.nth2;
@@ -930,6 +1130,7 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
 // adjoint: d_grid -> d_ft (Gtilde).  ev[0] before R2C, ev[1] after R2C, ev[2] after fine theta FFT,
 // ev[3] after truncate/deconvolve, ev[4] after the coarse inverse FFT.
 int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
+    if (p->fourier_general) return fourier_adjoint_general(p, s, ev);
     const int L = p->lmax, M = p->mmax;
     const NufftGeom& g = p->ng;
     const int nth2 = p->lg.nth2;
@@ -994,7 +1195,10 @@ void fourier_free(nusht_plan_s* p) {
     if (p->fft_theta_coarse) cufftDestroy(p->fft_theta_coarse);
     if (p->fft_theta_fine) cufftDestroy(p->fft_theta_fine);
     if (p->fft_phi) cufftDestroy(p->fft_phi);
-    p->fft_theta_coarse = p->fft_theta_fine = p->fft_phi = 0;
+    if (p->fft_phi_r2c) cufftDestroy(p->fft_phi_r2c);
+    p->fft_theta_coarse = p->fft_theta_fine = p->fft_phi = p->fft_phi_r2c = 0;
+    cudaFree(p->d_z);
+    p->d_z = nullptr;
     cudaFree(p->d_pth); cudaFree(p->d_pph); cudaFree(p->d_h); cudaFree(p->d_twz); cudaFree(p->d_grid); cudaFree(p->d_tw2n);
     p->d_tw2n = nullptr;
     p->d_pth = p->d_pph = nullptr;

@@ -743,7 +743,7 @@ int dispatch_interp(int w, const NufftParams& P, const KernelHost& h, const void
 #define NUSHT_CASE(WW) case WW: return launch_interp<WW, T>(P, h, grid, map, s);
         NUSHT_CASE(2) NUSHT_CASE(3) NUSHT_CASE(4) NUSHT_CASE(5) NUSHT_CASE(6) NUSHT_CASE(7) NUSHT_CASE(8)
         NUSHT_CASE(9) NUSHT_CASE(10) NUSHT_CASE(11) NUSHT_CASE(12) NUSHT_CASE(13) NUSHT_CASE(14)
-        NUSHT_CASE(15) NUSHT_CASE(16)
+        NUSHT_CASE(15) NUSHT_CASE(16) NUSHT_CASE(17) NUSHT_CASE(18)
 #undef NUSHT_CASE
     }
     return NUSHT_ERR_UNSUPPORTED;
@@ -754,7 +754,7 @@ int dispatch_spread(int w, const NufftParams& P, const KernelHost& h, const void
 #define NUSHT_CASE(WW) case WW: return launch_spread<WW, T>(P, h, map, grid, s);
         NUSHT_CASE(2) NUSHT_CASE(3) NUSHT_CASE(4) NUSHT_CASE(5) NUSHT_CASE(6) NUSHT_CASE(7) NUSHT_CASE(8)
         NUSHT_CASE(9) NUSHT_CASE(10) NUSHT_CASE(11) NUSHT_CASE(12) NUSHT_CASE(13) NUSHT_CASE(14)
-        NUSHT_CASE(15) NUSHT_CASE(16)
+        NUSHT_CASE(15) NUSHT_CASE(16) NUSHT_CASE(17) NUSHT_CASE(18)
 #undef NUSHT_CASE
     }
     return NUSHT_ERR_UNSUPPORTED;
@@ -791,11 +791,12 @@ __device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, do
                  : "d"(a), "d"(b));
 }
 
-__host__ __device__ constexpr int mma_nt(int w) { return w <= 8 ? 2 : 3; }                 // n-tiles per strip
+__host__ __device__ constexpr int mma_nt(int w) { return w <= 8 ? 2 : (w <= 14 ? 3 : 4); }   // n-tiles per strip
 __host__ __device__ constexpr int mma_ks(int w) { return w <= 6 ? 2 : (w <= 11 ? 3 : (w <= 14 ? 4 : 5)); }
 __host__ __device__ constexpr int mma_mt(int w) { return w <= 6 ? 1 : (w <= 14 ? 2 : 3); }
-// warps (work items) per CTA of the interpolation kernel: static shared memory stays below 48 KB
+// warps (work items) per CTA of the interpolation / spreading kernel: static shared memory stays below 48 KB
 __host__ __device__ constexpr int mma_interp_warps(int w) { return w <= 11 ? 4 : 2; }
+__host__ __device__ constexpr int mma_spread_warps(int w) { return w <= 14 ? 4 : 2; }
 __host__ __device__ constexpr int mma_th_stride(int s) { return s <= 12 ? 12 : (s <= 16 ? 20 : 36); }  // = 4 or 12 mod 16
 
 template <int W, int S>
@@ -1036,14 +1037,14 @@ k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
 // a8: type-1 spreading, FP64 / DMMA (grid must be zero on entry)
 // ---------------------------------------------------------------------------------------------
 template <int W>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(32 * mma_spread_warps(W))
 k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<double> kp,
              const double* __restrict__ map, double* __restrict__ grid) {
-    constexpr int NT = mma_nt(W), MT = mma_mt(W), S = 8 * MT, SPAN = S - W, OFF = 2 * S;
+    constexpr int NT = mma_nt(W), MT = mma_mt(W), S = 8 * MT, SPAN = S - W, OFF = 2 * S, NW = mma_spread_warps(W);
     using WS = MmaScratch<W, S>;
-    __shared__ __align__(16) WS s_ws[4];
+    __shared__ __align__(16) WS s_ws[NW];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int item = blockIdx.x * 4 + warp;
+    const int item = blockIdx.x * NW + warp;
     if (item >= P.n_items) return;
     const int start = P.item_off[item], end = P.item_off[item + 1];
     if (start >= end) return;
@@ -1206,7 +1207,8 @@ int launch_interp_mma(const NufftParams& P, const KernelHost& h, const void* gri
 template <int W>
 int launch_spread_mma(const NufftParams& P, const KernelHost& h, const void* map, void* grid, cudaStream_t s) {
     const KernelPoly<double> kp = make_device_poly<double>(h);
-    k_spread_mma<W><<<(P.n_items + 3) / 4, 128, 0, s>>>(P, kp, (const double*)map, (double*)grid);
+    constexpr int NW = mma_spread_warps(W);
+    k_spread_mma<W><<<(P.n_items + NW - 1) / NW, 32 * NW, 0, s>>>(P, kp, (const double*)map, (double*)grid);
     NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;
 }
@@ -1215,7 +1217,8 @@ int dispatch_interp_mma(int w, const NufftParams& P, const KernelHost& h, const 
     switch (w) {
 #define NUSHT_CASE(WW) case WW: return launch_interp_mma<WW>(P, h, grid, map, s);
         NUSHT_CASE(2) NUSHT_CASE(3) NUSHT_CASE(4) NUSHT_CASE(5) NUSHT_CASE(6) NUSHT_CASE(7) NUSHT_CASE(8)
-        NUSHT_CASE(9) NUSHT_CASE(10) NUSHT_CASE(11) NUSHT_CASE(12) NUSHT_CASE(13) NUSHT_CASE(14)   // eps >= 1e-13 -> w <= 14
+        NUSHT_CASE(9) NUSHT_CASE(10) NUSHT_CASE(11) NUSHT_CASE(12) NUSHT_CASE(13) NUSHT_CASE(14)   // sigma = 2: eps >= 1e-13 -> w <= 14
+        NUSHT_CASE(15) NUSHT_CASE(16) NUSHT_CASE(17) NUSHT_CASE(18)                                // sigma = 1.25: eps >= 1e-10 -> w <= 17
 #undef NUSHT_CASE
     }
     return NUSHT_ERR_UNSUPPORTED;
@@ -1224,7 +1227,8 @@ int dispatch_spread_mma(int w, const NufftParams& P, const KernelHost& h, const 
     switch (w) {
 #define NUSHT_CASE(WW) case WW: return launch_spread_mma<WW>(P, h, map, grid, s);
         NUSHT_CASE(2) NUSHT_CASE(3) NUSHT_CASE(4) NUSHT_CASE(5) NUSHT_CASE(6) NUSHT_CASE(7) NUSHT_CASE(8)
-        NUSHT_CASE(9) NUSHT_CASE(10) NUSHT_CASE(11) NUSHT_CASE(12) NUSHT_CASE(13) NUSHT_CASE(14)   // eps >= 1e-13 -> w <= 14
+        NUSHT_CASE(9) NUSHT_CASE(10) NUSHT_CASE(11) NUSHT_CASE(12) NUSHT_CASE(13) NUSHT_CASE(14)   // sigma = 2: eps >= 1e-13 -> w <= 14
+        NUSHT_CASE(15) NUSHT_CASE(16) NUSHT_CASE(17) NUSHT_CASE(18)                                // sigma = 1.25: eps >= 1e-10 -> w <= 17
 #undef NUSHT_CASE
     }
     return NUSHT_ERR_UNSUPPORTED;
@@ -1261,14 +1265,25 @@ void gauss_legendre(int n, std::vector<long double>& x, std::vector<long double>
 static KernelHost* g_kernel_of(const nusht_plan_s* p) { return static_cast<KernelHost*>(p->kernel_host); }
 
 int nufft_choose_kernel(nusht_plan_s* p) {
-    // width / shape rule of the ES kernel at up-sampling 2 (reading G8)
-    int w = (int)ceil(log10(1.0 / p->eps)) + 1;
-    if (w < 2) w = 2;
+    // width / shape rule of the ES kernel (reading G8, the published rule of the paper's ref. [38]):
+    // up-sampling 2:      w = ceil(log10(1/eps)) + 1,               beta = 2.30 w
+    // other up-sampling:  w = ceil(-ln eps / (pi sqrt(1 - 1/sigma))), beta = 0.97 pi w (1 - 1/(2 sigma))
+    int w;
+    double bw;
+    if (p->sigma == 2.0) {
+        w = (int)ceil(log10(1.0 / p->eps)) + 1;
+        if (w < 2) w = 2;
+        bw = 2.30;
+        if (w == 2) bw = 2.20;
+        if (w == 3) bw = 2.26;
+        if (w == 4) bw = 2.38;
+    } else {
+        const double PI_D = 3.14159265358979323846;
+        w = (int)ceil(-log(p->eps) / (PI_D * sqrt(1.0 - 1.0 / p->sigma)));
+        if (w < 2) w = 2;
+        bw = 0.97 * PI_D * (1.0 - 0.5 / p->sigma);
+    }
     if (w > NUSHT_MAX_W) return NUSHT_ERR_INVALID_ARG;
-    double bw = 2.30;
-    if (w == 2) bw = 2.20;
-    if (w == 3) bw = 2.26;
-    if (w == 4) bw = 2.38;
     KernelHost* h = new KernelHost();
     h->w = w;
     h->deg = poly_degree(w);

@@ -38,8 +38,8 @@ cudaError_t nusht_launched();
 void nusht_note_cufft_error(int r, const char* what, const char* file, int line);
 
 // ---- nuFFT geometry ------------------------------------------------------------------------
-constexpr int NUSHT_MAX_W = 16;          // kernel width limit (eps = 1e-13 -> w = 14)
-constexpr int NUSHT_MAX_DEG = 17;        // polynomial degree limit (degree = w)
+constexpr int NUSHT_MAX_W = 18;          // kernel width limit (sigma = 2: eps = 1e-13 -> w = 14; sigma = 1.25: eps = 1e-10 -> w = 17)
+constexpr int NUSHT_MAX_DEG = 19;        // polynomial degree limit (degree = w)
 constexpr int NUSHT_SEG_ROWS = 128;      // theta rows of patch origins per work item (strip segment)
 
 struct NufftGeom {
@@ -117,6 +117,9 @@ struct nusht_plan_s {
     bool have_fft = false;
     int theta_chain = 0;            // 0: cuFFT chain, 1: fused chain, one CTA per column, 2: fused chain, cluster pair per column
     bool theta_fused = false;       // a3 + a4 + a5-theta (and their transposes) as one kernel per direction (fourier.cu)
+    bool fourier_general = false;   // sigma != 2: full-length fine theta FFT and an out-of-place real phi FFT (fourier.cu)
+    void* d_z = nullptr;            //   half spectra of the grid rows, [nth/2+1][nph/2+1] complex (dtype)
+    cufftHandle fft_phi_r2c = 0;    //   R2C (dtype), length nph, batch nth/2+1 (fft_phi is then the C2R plan)
     double2* d_tw2n = nullptr;      // tables of the fused theta chains (twiddles, position-ordered deconvolution factors)
     int n_sm = 0;                   // SM count of the plan's device (persistent grids)
     bool chain_attr_set[2] = {false, false};   // MaxDynamicSharedMemorySize set for this plan's device (syn, adj)

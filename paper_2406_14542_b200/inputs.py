@@ -5,9 +5,10 @@ random draws and the geometry of the workloads.  Recipes follow BASELINE.json `c
 SURVEY.md 8(d); see DESIGN.md "Input recipe".
 
 * points uniform on the sphere: theta = arccos(U[-1,1]), phi ~ U[0, 2 pi)
-* CMB-lensing-like points (config 2): an equi-angular ring grid displaced per pixel by
-  arXiv 2406.14542 Eq. C1 with iid Gaussian deflection components
-  (sigma = 2.5 arcmin => |alpha| ~ Rayleigh(sigma)); the paper's real deflection fields
+* CMB-lensing-like points (config 2): an equi-angular ring grid and, per pixel, an iid Gaussian
+  deflection (sigma = 2.5 arcmin per component => |alpha| ~ Rayleigh(sigma)); the displaced
+  positions (arXiv 2406.14542 Eq. C1) are NOT computed here but by
+  nusht_pointing / oracle.pointing from these draws.  The paper's real deflection fields
    are not available offline, this stands in for them.
 * a_lm: complex, m >= 0, real-field convention, m-major triangular layout
   idx(l, m) = m (2 lmax + 1 - m)/2 + l; white (C_l = 1) or C_l = 1/(l+1)^2.
@@ -66,11 +67,12 @@ def random_map(npts: int, seed: int):
     return rng.standard_normal(npts)
 
 
-def lensing_like_points(nrings: int, npix: int, seed: int, sigma: float = 2.5 * ARCMIN):
-    """nrings x npix equi-angular grid theta_i = pi (i + 1/2)/nrings, phi_j = 2 pi j/npix (ring-major
-    order), each pixel displaced along a random direction by Eq. C1:
-        n' = cos(a) n + sin(a)/a (a_theta e_theta + a_phi e_phi),  a = |(a_theta, a_phi)|.
-    Returns theta', phi' in [0, pi] x [0, 2 pi)."""
+def lensing_grid_and_deflection(nrings: int, npix: int, seed: int, sigma: float = 2.5 * ARCMIN):
+    """The undeflected nrings x npix equi-angular grid theta_i = pi (i + 1/2)/nrings, phi_j = 2 pi j/npix (ring-major
+    order) and an iid Gaussian deflection (alpha_theta, alpha_phi) per pixel, each component N(0, sigma^2), so that
+    |alpha| ~ Rayleigh(sigma) along a uniformly random direction (BASELINE.json configs[1]).  Random draws only: the
+    deflected positions of Eq. C1 are computed by nusht_pointing on the CUDA side and by
+    oracle.pointing on the checker's side, each from these same arrays."""
     rng = np.random.default_rng(seed)
     th = np.pi * (np.arange(nrings) + 0.5) / nrings
     ph = 2.0 * np.pi * np.arange(npix) / npix
@@ -78,18 +80,7 @@ def lensing_like_points(nrings: int, npix: int, seed: int, sigma: float = 2.5 * 
     phi = np.tile(ph, nrings)
     a_t = rng.normal(0.0, sigma, size=theta.shape[0])
     a_p = rng.normal(0.0, sigma, size=theta.shape[0])
-    a = np.hypot(a_t, a_p)
-    st, ct, sp, cp = np.sin(theta), np.cos(theta), np.sin(phi), np.cos(phi)
-    n = np.stack([st * cp, st * sp, ct])
-    e_t = np.stack([ct * cp, ct * sp, -st])
-    e_p = np.stack([-sp, cp, np.zeros_like(sp)])
-    with np.errstate(invalid="ignore", divide="ignore"):
-        sinc = np.where(a > 0, np.sin(a) / a, 1.0)
-    npr = np.cos(a) * n + sinc * (a_t * e_t + a_p * e_p)
-    theta2 = np.arccos(np.clip(npr[2], -1.0, 1.0))
-    phi2 = np.mod(np.arctan2(npr[1], npr[0]), 2.0 * np.pi)
-    phi2[phi2 >= 2.0 * np.pi] = 0.0
-    return theta2, phi2
+    return theta, phi, a_t, a_p
 
 
 # BASELINE.json `configs`, in order.  npts / spectrum / eps / dtype per config.
@@ -102,15 +93,20 @@ CONFIGS = {
 
 
 def make_config(i: int, npts: int | None = None):
-    """(cfg, theta, phi, alm, x) for BASELINE config i; `npts` overrides the point count (tests)."""
+    """(cfg, theta, phi, alm, x) for BASELINE config i; `npts` overrides the point count (tests).
+    For the lensing-like config the returned (theta, phi) is the UNDEFLECTED pixel grid and cfg["deflection"] holds
+    (alpha_theta, alpha_phi): the caller turns them into the point set with Eq. C1, through nusht_pointing (CUDA
+    path) or oracle.pointing (checker).  cfg["deflection"] is None for the other configs."""
     cfg = dict(CONFIGS[i])
+    cfg["deflection"] = None
     if npts is not None:
         cfg["npts"] = int(npts)
     if cfg["points"] == "uniform":
         theta, phi = uniform_sphere_points(cfg["npts"], cfg["seed"])
     else:
         side = int(round(np.sqrt(cfg["npts"])))
-        theta, phi = lensing_like_points(side, side, cfg["seed"])
+        theta, phi, a_t, a_p = lensing_grid_and_deflection(side, side, cfg["seed"])
+        cfg["deflection"] = (a_t, a_p)
         cfg["npts"] = side * side
     alm = random_alm(cfg["lmax"], cfg["mmax"], cfg["seed"], cfg["spectrum"])
     x = random_map(cfg["npts"], cfg["seed"])

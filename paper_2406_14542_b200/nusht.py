@@ -25,7 +25,7 @@ EXPORTS = [
     "nusht_plan_info", "nusht_strerror", "nusht_version", "nusht_pointing", "nusht_host_reserve",
     "nusht_stage_fourier_synthesis", "nusht_stage_fourier_adjoint", "nusht_launch_count", "nusht_probe_fp64",
     "nusht_ring_plan", "nusht_ring_synthesis", "nusht_ring_analysis", "nusht_ring_gradient", "nusht_ring_info",
-    "nusht_ring_destroy", "nusht_ring_pairing",
+    "nusht_ring_destroy", "nusht_ring_pairing", "nusht_plan_ex",
 ]
 
 
@@ -50,6 +50,10 @@ class NushtRingInfo(ctypes.Structure):
     ]
 
 
+class NushtOpts(ctypes.Structure):
+    _fields_ = [("sigma", ctypes.c_double), ("reserved", ctypes.c_int * 6)]
+
+
 class NushtError(RuntimeError):
     def __init__(self, code, msg):
         super().__init__("nusht error %d: %s" % (code, msg))
@@ -69,6 +73,9 @@ def _load():
         getattr(lib, name).argtypes = [vp, vp, vp, vp]
         getattr(lib, name).restype = ip
     lib.nusht_plan.restype = ip
+    lib.nusht_plan_ex.argtypes = [ctypes.POINTER(vp), ip, ip, ctypes.c_int64, vp, vp, ctypes.c_double, ip,
+                                  ctypes.POINTER(NushtOpts)]
+    lib.nusht_plan_ex.restype = ip
     lib.nusht_destroy.argtypes = [vp]
     lib.nusht_destroy.restype = ip
     lib.nusht_host_sync.argtypes = [vp]
@@ -126,9 +133,10 @@ def _stream_ptr(stream):
 
 
 class Plan:
-    """nusht_plan(lmax, mmax, npts, theta, phi, eps, dtype): theta/phi are CUDA float64 tensors."""
+    """nusht_plan(lmax, mmax, npts, theta, phi, eps, dtype): theta/phi are CUDA float64 tensors.
+    sigma (nusht_plan_ex): up-sampling factor of the nuFFT grid, 2 (default) or 1.25."""
 
-    def __init__(self, lmax, mmax, theta, phi, eps, dtype="f64"):
+    def __init__(self, lmax, mmax, theta, phi, eps, dtype="f64", sigma=None):
         self._h = ctypes.c_void_p()
         if dtype in ("f64", NUSHT_F64):
             self.dtype = NUSHT_F64
@@ -146,7 +154,13 @@ class Plan:
             tp, pp = theta.data_ptr(), phi.data_ptr()
         else:
             tp = pp = None
-        _check(lib.nusht_plan(ctypes.byref(self._h), int(lmax), int(mmax), npts, tp, pp, float(eps), self.dtype))
+        if sigma is None:
+            _check(lib.nusht_plan(ctypes.byref(self._h), int(lmax), int(mmax), npts, tp, pp, float(eps), self.dtype))
+        else:
+            opts = NushtOpts()
+            opts.sigma = float(sigma)
+            _check(lib.nusht_plan_ex(ctypes.byref(self._h), int(lmax), int(mmax), npts, tp, pp, float(eps), self.dtype,
+                                     ctypes.byref(opts)))
         self.info = NushtInfo()
         _check(lib.nusht_plan_info(self._h, ctypes.byref(self.info)))
         self.lmax, self.mmax, self.npts, self.nlm = int(lmax), int(mmax), npts, int(self.info.nlm)

@@ -36,13 +36,24 @@ def test_fullsize_sampled(oracle, config, nsample, eps_over):
     L, M, eps, npts = cfg["lmax"], cfg["mmax"], cfg["eps"], cfg["npts"]
     if eps_over is not None:
         eps = eps_over
-    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps)
+    d_theta, d_phi = cu(theta), cu(phi)
+    if cfg["deflection"] is not None:
+        # lensing-like config: the point set is the deflected pixel grid.  The CUDA path gets it from nusht_pointing,
+        # the oracle from oracle.pointing on the sampled pixels (Eq. C1); the two agree to 4e-15 rad
+        # (tests/test_gpu_pointing.py), i.e. to lmax x 4e-15 in the map values
+        d_theta, d_phi = nusht.nusht_pointing(d_theta, d_phi, *(cu(a) for a in cfg["deflection"]))
+    plan = nusht.Plan(L, M, d_theta, d_phi, eps)
+    del d_theta, d_phi
     d_alm = cu(alm)
     f = plan.synthesis(d_alm).cpu().numpy()
     rng = np.random.default_rng(99)
     idx = np.sort(rng.choice(npts, nsample, replace=False))
     # a few deliberately awkward samples: closest to the poles and to phi = 0 / 2 pi
     idx = np.unique(np.concatenate([idx, [np.argmin(theta), np.argmax(theta), np.argmin(phi), np.argmax(phi)]]))
+    if cfg["deflection"] is not None:
+        t2, p2 = oracle.pointing(theta[idx], phi[idx], cfg["deflection"][0][idx], cfg["deflection"][1][idx])
+        theta, phi = theta.copy(), phi.copy()
+        theta[idx], phi[idx] = np.asarray(t2, dtype=np.float64), np.asarray(p2, dtype=np.float64)
     f_ref = oracle.synthesis(L, M, theta[idx], phi[idx], alm, "ld")
     assert rel(f[idx], f_ref) <= 10 * eps
     assert rel_max(f[idx], f_ref) <= 100 * eps
