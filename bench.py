@@ -44,6 +44,8 @@ def parse():
     ap.add_argument("--npts", type=int, default=None, help="override the point count (debugging)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--sigma", type=float, default=None,
+                    help="up-sampling factor of the nuFFT grid: 2 (default) or 1.25, the paper's own (PAPER.md:152)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--eps-sweep", action="store_true",
@@ -252,7 +254,7 @@ def stage_rooflines(cfg, info, npts, syn_ms, adj_ms, sm_mhz, probe):
     # HBM: report that fraction too.  Executed FMA per point: 4 KS NT 256/8 (interp) or
     # 2 MT NT 256/4 (spread) tensor-core FMA + 2 (w/2)(deg+1) evaluation FMA.
     w = info.kernel_width
-    nt = 2 if w <= 8 else 3
+    nt = 2 if w <= 8 else (3 if w <= 14 else 4)
     ks = 2 if w <= 6 else (3 if w <= 11 else (4 if w <= 14 else 5))
     mt = 1 if w <= 6 else (2 if w <= 14 else 3)
     ev = 2 * ((w + 1) // 2) * (max(w, 5) + 1)
@@ -296,7 +298,7 @@ def run_b200(args, rank, world):
     d_theta, d_phi = torch.from_numpy(theta).cuda(), torch.from_numpy(phi).cuda()
     if cfg["deflection"] is not None:      # lensing-like config: the points are the deflected pixels, Eq. C1 on the GPU
         d_theta, d_phi = nusht.nusht_pointing(d_theta, d_phi, *(torch.from_numpy(a).cuda() for a in cfg["deflection"]))
-    plan = nusht.Plan(L, M, d_theta, d_phi, eps, cfg["dtype"])
+    plan = nusht.Plan(L, M, d_theta, d_phi, eps, cfg["dtype"], sigma=args.sigma)
     del d_theta, d_phi
     d_alm, d_x = torch.from_numpy(alm).cuda(), torch.from_numpy(x).cuda()
     d_map = torch.empty(npts, dtype=torch.float64, device="cuda")
@@ -419,7 +421,8 @@ def run_b200(args, rank, world):
                  "sort_frac_of_hbm": (60 * npts / (plan.info.sort_ms * 1e-3) / 1e9 / measured_peaks()[0])
                  if plan.info.sort_ms > 0 else None,
                  "n_rings": plan.info.n_rings, "n_theta": plan.info.n_theta, "n_theta_fine": plan.info.n_theta_fine,
-                 "n_phi_fine": plan.info.n_phi_fine, "kernel_width": plan.info.kernel_width},
+                 "n_phi_fine": plan.info.n_phi_fine, "kernel_width": plan.info.kernel_width,
+                 "sigma": plan.info.sigma},
     }
     if not args.no_cpu_baseline and world == 1:
         ns = min(npts, 1 << 16)

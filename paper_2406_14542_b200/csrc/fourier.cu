@@ -872,10 +872,18 @@ int fourier_build(nusht_plan_s* p) {
 
     const size_t hbytes = (size_t)(M + 1) * (size_t)g.nth * csz;
     const size_t gbytes = (size_t)g.nrow_half * (size_t)g.nph * rsz;
-    NUSHT_TRY(f_alloc(&p->d_h, hbytes, p));
-    NUSHT_TRY(f_alloc(&p->d_grid, gbytes, p));
-    NUSHT_CUDA_TRY(cudaMemset(p->d_h, 0, hbytes));
-    NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
+    if (p->fourier_general) {
+        // sigma != 2 exists to save memory: H[m][a] and the fine grid are never live together (synthesis: H -> Z, then
+        // Z -> grid; adjoint: grid -> Z, then Z -> H), so they share one allocation
+        NUSHT_TRY(f_alloc(&p->d_h, std::max(hbytes, gbytes), p));
+        p->d_grid = p->d_h;
+        NUSHT_CUDA_TRY(cudaMemset(p->d_h, 0, std::max(hbytes, gbytes)));
+    } else {
+        NUSHT_TRY(f_alloc(&p->d_h, hbytes, p));
+        NUSHT_TRY(f_alloc(&p->d_grid, gbytes, p));
+        NUSHT_CUDA_TRY(cudaMemset(p->d_h, 0, hbytes));
+        NUSHT_CUDA_TRY(cudaMemset(p->d_grid, 0, gbytes));
+    }
 
     if (p->fourier_general) {
         // sigma != 2: plain cuFFT chain (see k_deconv_pad_gen)
@@ -883,24 +891,28 @@ int fourier_build(nusht_plan_s* p) {
         p->theta_fused = false;
         const size_t zbytes = (size_t)g.nrow_half * (size_t)(g.nph / 2 + 1) * csz;
         NUSHT_TRY(f_alloc(&p->d_z, zbytes, p));
-        size_t ws = 0, wtot = 0;
+        // the four plans run one after the other on the transform's stream: ONE work area, sized for the largest
+        // (this variant exists to save memory; non-power-of-two lengths need a work area of the size of their data)
+        size_t ws = 0, wmax = 0;
         int n1[1] = {nth2}, n2[1] = {g.nth}, n3[1] = {g.nph};
-        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_theta_coarse));
+        cufftHandle* hs[4] = {&p->fft_theta_coarse, &p->fft_theta_fine, &p->fft_phi, &p->fft_phi_r2c};
+        for (int i = 0; i < 4; ++i) {
+            NUSHT_CUFFT_TRY(cufftCreate(hs[i]));
+            NUSHT_CUFFT_TRY(cufftSetAutoAllocation(*hs[i], 0));
+        }
         NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_coarse, 1, n1, nullptr, 1, nth2, nullptr, 1, nth2, CUFFT_Z2Z, M + 1, &ws));
-        wtot += ws;
-        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_theta_fine));
+        wmax = std::max(wmax, ws);
         NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_theta_fine, 1, n2, nullptr, 1, g.nth, nullptr, 1, g.nth,
                                           f64 ? CUFFT_Z2Z : CUFFT_C2C, M + 1, &ws));
-        wtot += ws;
-        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi));
+        wmax = std::max(wmax, ws);
         NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi, 1, n3, nullptr, 1, 0, nullptr, 1, 0, f64 ? CUFFT_Z2D : CUFFT_C2R,
                                           g.nrow_half, &ws));
-        wtot += ws;
-        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi_r2c));
+        wmax = std::max(wmax, ws);
         NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi_r2c, 1, n3, nullptr, 1, 0, nullptr, 1, 0, f64 ? CUFFT_D2Z : CUFFT_R2C,
                                           g.nrow_half, &ws));
-        wtot += ws;
-        p->workspace_bytes += (int64_t)wtot;
+        wmax = std::max(wmax, ws);
+        NUSHT_TRY(f_alloc(&p->d_fftwork, wmax, p));
+        for (int i = 0; i < 4; ++i) NUSHT_CUFFT_TRY(cufftSetWorkArea(*hs[i], p->d_fftwork));
         p->have_fft = true;
         return NUSHT_OK;
     }
@@ -1198,7 +1210,10 @@ void fourier_free(nusht_plan_s* p) {
     if (p->fft_phi_r2c) cufftDestroy(p->fft_phi_r2c);
     p->fft_theta_coarse = p->fft_theta_fine = p->fft_phi = p->fft_phi_r2c = 0;
     cudaFree(p->d_z);
+    cudaFree(p->d_fftwork);
     p->d_z = nullptr;
+    p->d_fftwork = nullptr;
+    if (p->d_grid == p->d_h) p->d_grid = nullptr;      // sigma != 2: one allocation
     cudaFree(p->d_pth); cudaFree(p->d_pph); cudaFree(p->d_h); cudaFree(p->d_twz); cudaFree(p->d_grid); cudaFree(p->d_tw2n);
     p->d_tw2n = nullptr;
     p->d_pth = p->d_pph = nullptr;

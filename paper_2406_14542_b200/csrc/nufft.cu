@@ -857,7 +857,9 @@ __global__ void __launch_bounds__(32 * mma_interp_warps(W), mma_interp_warps(W) 
 k_interp_mma(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPoly<double> kp,
              const double* __restrict__ grid, double* __restrict__ map) {
     constexpr int NT = mma_nt(W), KS = mma_ks(W), S = 4 * KS, SPAN = S - W, OFF = 2 * S, NC = 8 * NT;
-    constexpr int RB = S <= 12 ? 12 : NU_RING_ROWS, CH = S <= 12 ? 4 : NU_RING_CHUNK;   // ring rows >= window slots
+    // ring rows >= window slots S (a jump of the window loads S rows at once); 48 is a multiple of every RB
+    constexpr int RB = S <= 12 ? 12 : (S <= 16 ? NU_RING_ROWS : 24), CH = S == 16 ? NU_RING_CHUNK : 4;
+    static_assert(RB >= S && 48 % RB == 0, "staging ring too small for the register window");
     using WS = MmaScratch<W, S>;
     constexpr int NW = mma_interp_warps(W);
     __shared__ __align__(16) WS s_ws[NW];

@@ -120,6 +120,7 @@ struct nusht_plan_s {
     bool fourier_general = false;   // sigma != 2: full-length fine theta FFT and an out-of-place real phi FFT (fourier.cu)
     void* d_z = nullptr;            //   half spectra of the grid rows, [nth/2+1][nph/2+1] complex (dtype)
     cufftHandle fft_phi_r2c = 0;    //   R2C (dtype), length nph, batch nth/2+1 (fft_phi is then the C2R plan)
+    void* d_fftwork = nullptr;      //   one cuFFT work area shared by the four plans of that chain
     double2* d_tw2n = nullptr;      // tables of the fused theta chains (twiddles, position-ordered deconvolution factors)
     int n_sm = 0;                   // SM count of the plan's device (persistent grids)
     bool chain_attr_set[2] = {false, false};   // MaxDynamicSharedMemorySize set for this plan's device (syn, adj)

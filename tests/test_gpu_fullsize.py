@@ -26,9 +26,11 @@ def rel_max(a, b):
 
 # (config, sample size, eps): the configs' own eps, then BASELINE.json configs[4]'s FP64 rows (lmax = 4095 on 67 M
 # points at eps = 1e-8 and 1e-12: w = 9 and w = 13, other template paths of the nuFFT kernels than w = 11)
-@pytest.mark.parametrize("config,nsample,eps_over", [(2, 1500, None), (3, 300, None), (4, 100, None),
-                                                     (3, 300, 1e-8), (3, 300, 1e-12)])
-def test_fullsize_sampled(oracle, config, nsample, eps_over):
+# ... and lmax = 4095 / 67 M points at the paper's own up-sampling sigma = 1.25 (w = 17 at eps = 1e-10)
+@pytest.mark.parametrize("config,nsample,eps_over,sigma", [(2, 1500, None, None), (3, 300, None, None),
+                                                           (4, 100, None, None), (3, 300, 1e-8, None),
+                                                           (3, 300, 1e-12, None), (3, 300, None, 1.25)])
+def test_fullsize_sampled(oracle, config, nsample, eps_over, sigma):
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     from paper_2406_14542_b200 import nusht
@@ -42,7 +44,7 @@ def test_fullsize_sampled(oracle, config, nsample, eps_over):
         # the oracle from oracle.pointing on the sampled pixels (Eq. C1); the two agree to 4e-15 rad
         # (tests/test_gpu_pointing.py), i.e. to lmax x 4e-15 in the map values
         d_theta, d_phi = nusht.nusht_pointing(d_theta, d_phi, *(cu(a) for a in cfg["deflection"]))
-    plan = nusht.Plan(L, M, d_theta, d_phi, eps)
+    plan = nusht.Plan(L, M, d_theta, d_phi, eps, sigma=sigma)
     del d_theta, d_phi
     d_alm = cu(alm)
     f = plan.synthesis(d_alm).cpu().numpy()

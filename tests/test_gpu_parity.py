@@ -451,3 +451,52 @@ def test_fused_theta_chain_few_columns(nusht, oracle, monkeypatch, mode, L, M):
     lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
     assert abs(lhs - oracle.inner_alm(L, M, alm, c)) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
     plan.destroy()
+
+
+# ---- sigma = 1.25, the paper's own up-sampling factor --------------------------
+@pytest.mark.parametrize("eps", [1e-1, 1e-2, 1e-3, 1e-4, 1e-5, 1e-6, 1e-7, 1e-8, 1e-9, 1e-10])
+@pytest.mark.parametrize("L,M,npts", [(63, 63, 4000), (89, 70, 5000)])
+def test_sigma_125_all_widths(nusht, oracle, eps, L, M, npts):
+    """nusht_plan_ex with sigma = 1.25: kernel width w = ceil(-ln eps / (pi sqrt(1 - 1/sigma))) (w = 17 at 1e-10), fine
+    grid 1.25 x the modes, the general cuFFT chain.  Same bars as sigma = 2 down to the 1e-10 floor the paper states
+    (fn. 6): <= 10 eps against the oracle in both directions, adjointness 1e-12."""
+    theta, phi = inputs.uniform_sphere_points(npts, 171)
+    theta[:4] = [0.0, np.pi, 1e-9, np.pi - 1e-9]
+    phi[:4] = [0.0, 2 * np.pi - 1e-12, 6.28, 1e-15]
+    alm = inputs.random_alm(L, M, 171)
+    x = inputs.random_map(npts, 171)
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps, sigma=1.25)
+    assert plan.info.sigma == 1.25
+    assert plan.info.kernel_width == max(2, int(np.ceil(-np.log(eps) / (np.pi * np.sqrt(1 - 1 / 1.25)))))
+    assert plan.info.n_theta_fine < 2 * plan.info.n_theta            # the grid is smaller than at sigma = 2
+    f = plan.synthesis(cu(alm)).cpu().numpy()
+    c = plan.adjoint(cu(x)).cpu().numpy()
+    assert rel(f, oracle.synthesis(L, M, theta, phi, alm, "ld")) <= 10 * eps
+    assert rel(c, oracle.adjoint(L, M, theta, phi, x, "ld")) <= 10 * eps
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+    rhs = oracle.inner_alm(L, M, alm, c)
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    assert strong_adjointness(plan, oracle, L, M, alm, f) <= 1e-12
+    plan.destroy()
+
+
+def test_sigma_125_fp32_and_argument_checks(nusht, oracle):
+    L, npts = 63, 4000
+    theta, phi = inputs.uniform_sphere_points(npts, 172)
+    alm = inputs.random_alm(L, L, 172)
+    plan = nusht.Plan(L, L, cu(theta), cu(phi), 1e-4, dtype="f32", sigma=1.25)
+    f = plan.synthesis(cu(alm.astype(np.complex64))).cpu().numpy().astype(np.float64)
+    assert rel(f, oracle.synthesis(L, L, theta, phi, alm, "ld")) <= 1e-3
+    c = plan.adjoint(cu(inputs.random_map(npts, 172).astype(np.float32))).cpu().numpy().astype(np.complex128)
+    assert rel(c, oracle.adjoint(L, L, theta, phi, inputs.random_map(npts, 172), "ld")) <= 1e-3
+    plan.destroy()
+    for bad in (dict(eps=1e-11, sigma=1.25), dict(eps=1e-6, sigma=1.5), dict(eps=1e-6, sigma=1.25, dtype="f32")):
+        with pytest.raises(nusht.NushtError) as e:
+            nusht.Plan(L, L, cu(theta), cu(phi), bad["eps"], dtype=bad.get("dtype", "f64"), sigma=bad["sigma"])
+        assert e.value.code == -1
+    # sigma = 2 through the extended call is the default plan
+    p2 = nusht.Plan(L, L, cu(theta), cu(phi), 1e-8, sigma=2.0)
+    p0 = nusht.Plan(L, L, cu(theta), cu(phi), 1e-8)
+    assert torch.equal(p2.synthesis(cu(alm)), p0.synthesis(cu(alm)))
+    p2.destroy()
+    p0.destroy()
