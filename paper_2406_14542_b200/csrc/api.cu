@@ -9,9 +9,18 @@
 #include <chrono>
 #include <new>
 
+#include <nvtx3/nvToolsExt.h>   // header-only; a no-op unless a profiler injects the NVTX library
+
 #include "nusht_internal.cuh"
 
 static thread_local char g_last_error[512] = "";
+
+// NVTX range over the host-side enqueue of one stage (tracing); Nsight tools project it onto
+// the kernels launched inside
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 void nusht_note_cuda_error(cudaError_t e, const char* what, const char* file, int line) {
     snprintf(g_last_error, sizeof(g_last_error), "CUDA error %d (%s) at %s:%d: %s", (int)e, cudaGetErrorString(e),
@@ -201,14 +210,27 @@ extern "C" int nusht_synthesis(nusht_plan_t* p, const void* alm, void* map, void
     if (p->npts == 0) return NUSHT_OK;
     cudaStream_t s = (cudaStream_t)stream;
     cudaEvent_t fev[5];
+    NvtxRange r_all("nusht_synthesis");
     STAGE_MARK(0, 0);
-    NUSHT_TRY(legendre_alm_prep(p, alm, s));
+    {
+        NvtxRange r("nusht:a1 alm_prep");
+        NUSHT_TRY(legendre_alm_prep(p, alm, s));
+    }
     STAGE_MARK(0, 1);
-    NUSHT_TRY(legendre_synthesis(p, p->d_ft, s));
+    {
+        NvtxRange r("nusht:a1+a2 legendre_synthesis");
+        NUSHT_TRY(legendre_synthesis(p, p->d_ft, s));
+    }
     // stages 2..5 are bracketed inside fourier_synthesis: ev[2] .. ev[6]
     for (int i = 0; i < 5; ++i) fev[i] = p->ev[0][2 + i];
-    NUSHT_TRY(fourier_synthesis(p, s, p->timing ? fev : nullptr));
-    NUSHT_TRY(nufft_interp(p, p->d_grid, map, s));
+    {
+        NvtxRange r("nusht:a3-a5 fourier_synthesis");
+        NUSHT_TRY(fourier_synthesis(p, s, p->timing ? fev : nullptr));
+    }
+    {
+        NvtxRange r("nusht:a7 interp");
+        NUSHT_TRY(nufft_interp(p, p->d_grid, map, s));
+    }
     STAGE_MARK(0, 7);
     if (p->timing) p->ev_valid[0] = true;
     return NUSHT_OK;
@@ -222,14 +244,27 @@ extern "C" int nusht_adjoint(nusht_plan_t* p, const void* map, void* alm, void* 
         return NUSHT_OK;
     }
     cudaEvent_t fev[5];
+    NvtxRange r_all("nusht_adjoint");
     STAGE_MARK(1, 0);
-    NUSHT_TRY(nufft_spread(p, map, p->d_grid, s));
+    {
+        NvtxRange r("nusht:a8 spread");
+        NUSHT_TRY(nufft_spread(p, map, p->d_grid, s));
+    }
     // stages 1..4 are bracketed inside fourier_adjoint: ev[1] .. ev[5]
     for (int i = 0; i < 5; ++i) fev[i] = p->ev[1][1 + i];
-    NUSHT_TRY(fourier_adjoint(p, s, p->timing ? fev : nullptr));
-    NUSHT_TRY(legendre_adjoint(p, p->d_ft, s));
+    {
+        NvtxRange r("nusht:a9 fourier_adjoint");
+        NUSHT_TRY(fourier_adjoint(p, s, p->timing ? fev : nullptr));
+    }
+    {
+        NvtxRange r("nusht:a10+a11 legendre_adjoint");
+        NUSHT_TRY(legendre_adjoint(p, p->d_ft, s));
+    }
     STAGE_MARK(1, 6);
-    NUSHT_TRY(legendre_alm_post(p, alm, s));
+    {
+        NvtxRange r("nusht:a11 alm_post");
+        NUSHT_TRY(legendre_alm_post(p, alm, s));
+    }
     STAGE_MARK(1, 7);
     if (p->timing) p->ev_valid[1] = true;
     return NUSHT_OK;
