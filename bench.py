@@ -52,6 +52,11 @@ def parse():
                     help="BASELINE.json configs[4]: lmax=4095 on 67M points, eps in {1e-4, 1e-6} FP32 and "
                          "{1e-8, 1e-10, 1e-12} FP64; one JSON line per eps (accuracy on an oracle subset + timing)")
     ap.add_argument("--sweep-subset", type=int, default=1500, help="points of the oracle subset of the sweep")
+    ap.add_argument("--ring", default=None, choices=["gl", "equi"],
+                    help="ring-grid transforms (SURVEY 8(f) rank 3/4) instead of the nuSHT step: 'gl' = Gauss-Legendre grid "
+                         "(lmax+1 rings x 2 lmax+2 pixels, the paper's output grid, PAPER.md:154): step = synthesis + "
+                         "analysis; 'equi' = the 2(lmax+1)^2 equi-angular grid of config 2: step = gradient (Eq. C2) + pointing")
+    ap.add_argument("--lmax", type=int, default=4095, help="band limit of the --ring modes")
     return ap.parse_args()
 
 
@@ -489,8 +494,68 @@ def run_eps_sweep(args):
         del d_alm, d_x, d_xs, f, c, d_map, d_out
 
 
+def run_ring(args):
+    """Ring-grid modes: not the headline metric; one JSON line with CUDA-event times and the Legendre share."""
+    import torch
+    from paper_2406_14542_b200 import nusht
+    torch.cuda.set_device(0)
+    L = args.lmax
+    stream = torch.cuda.current_stream()
+    if args.ring == "gl":
+        xg, wg = np.polynomial.legendre.leggauss(L + 1)
+        theta = np.arccos(xg[::-1])
+        half = (L + 1) // 2
+        theta[L + 1 - half:] = np.pi - theta[:half][::-1]
+        nphi = np.full(L + 1, 2 * L + 2)
+        weight = wg[::-1] * (2 * np.pi / (2 * L + 2))
+    else:
+        nr = 2 * (L + 1)
+        theta = np.pi * (np.arange(nr) + 0.5) / nr
+        nphi = np.full(nr, nr)
+        weight = None
+    plan = nusht.RingPlan(L, L, theta, nphi, None, weight)
+    alm = torch.from_numpy(inputs.random_alm(L, L, 7, "inv_l2")).cuda()
+    f = torch.empty(plan.npix, dtype=torch.float64, device="cuda")
+    out = torch.empty(plan.nlm, dtype=torch.complex128, device="cuda")
+    if args.ring == "gl":
+        def step():
+            plan.synthesis(alm, f, stream)
+            plan.analysis(f, out, stream)
+        what = "ring synthesis + analysis on a Gauss-Legendre grid"
+    else:
+        th = torch.from_numpy(np.repeat(theta, nphi)).cuda()
+        ph = torch.from_numpy(np.tile(2 * np.pi * np.arange(nphi[0]) / nphi[0], len(theta))).cuda()
+        philm = alm * 2e-5
+
+        def step():
+            a_t, a_p = plan.gradient(philm, stream)
+            nusht.nusht_pointing(th, ph, a_t, a_p, stream)
+        what = "deflection field (Eq. C2) + pointing (Eq. C1) on the 2(lmax+1)^2 equi-angular grid"
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    n0 = nusht.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    print(json.dumps({"metric": "ring_%s_ms" % args.ring, "value": ms, "unit": "ms", "n_gpus": 1, "steps": args.steps,
+                      "warmup": max(args.warmup, 3), "higher_is_better": False, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": what, "lmax": L, "nrings": int(len(theta)), "npix": int(plan.npix)},
+                      "pixels_per_s": plan.npix / (ms * 1e-3), "gpu_launches": int(nusht.launch_count() - n0),
+                      "plan": {"ms": plan.info.plan_ms, "workspace_gb": plan.info.workspace_bytes / 1e9,
+                               "npairs": plan.info.npairs, "nruns": plan.info.nruns}}))
+    plan.destroy()
+
+
 def main():
     args = parse()
+    if args.ring:
+        run_ring(args)
+        return
     if args.eps_sweep:
         run_eps_sweep(args)
         return

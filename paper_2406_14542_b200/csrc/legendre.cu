@@ -1132,6 +1132,9 @@ int legendre_build_tables(nusht_plan_s* p) {
     }
     NUSHT_CUDA_TRY(cudaDeviceSynchronize());
     NUSHT_TRY(build_work_list(p, LEG_R, p->d_ff_n, &p->d_items_syn, &p->n_items_syn));
+    NUSHT_CUDA_TRY(cudaStreamCreateWithFlags(&p->s_leg_aux, cudaStreamNonBlocking));
+    NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_leg_fork, cudaEventDisableTiming));
+    NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_leg_join, cudaEventDisableTiming));
     return NUSHT_OK;
 }
 
@@ -1164,8 +1167,15 @@ int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
     NUSHT_CUDA_TRY(cudaMemsetAsync(p->d_aeo, 0, sizeof(double4) * (size_t)p->n_e_total, s));
     LegParams P = make_params(p, true);
     const dim3 grid = leg_grid(p, ADJ_R, P);
-    // one launch per form of t_n (see the kernel): blocks next to the equator first (they are the longer ones)
+    // one launch per form of t_n (see the kernel).  The two grids are independent (both add into eo with global
+    // reductions), so the second one runs on a plan-owned side stream, forked from and joined to `s` with events:
+    // they share the SMs instead of draining one after the other.
     const int nbx = (int)grid.x, split = std::min(P.b_split, nbx);
+    const bool both = split > 0 && split < nbx;
+    if (both) {
+        NUSHT_CUDA_TRY(cudaEventRecord(p->ev_leg_fork, s));
+        NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_leg_aux, p->ev_leg_fork, 0));
+    }
     for (int part = 1; part >= 0; --part) {
         LegParams Q = P;
         const int first = part ? split : 0, count = part ? nbx - split : split;
@@ -1173,11 +1183,16 @@ int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s) {
         Q.b_split = first;                                   // block offset of this launch
         if (part) Q.ab = P.ab + p->n_e_total;                // cos^2 form of the table
         const dim3 g2(count, grid.y);
+        cudaStream_t sl = (both && part == 0) ? p->s_leg_aux : s;
         if (p->lg.ring_mode)
-            k_legendre_adjoint<ADJ_R, ADJ_CHUNK, true><<<g2, 32, 0, s>>>(Q, gt, p->d_aeo);
+            k_legendre_adjoint<ADJ_R, ADJ_CHUNK, true><<<g2, 32, 0, sl>>>(Q, gt, p->d_aeo);
         else
-            k_legendre_adjoint<ADJ_R, ADJ_CHUNK, false><<<g2, 32, 0, s>>>(Q, gt, p->d_aeo);
+            k_legendre_adjoint<ADJ_R, ADJ_CHUNK, false><<<g2, 32, 0, sl>>>(Q, gt, p->d_aeo);
         NUSHT_CUDA_TRY(nusht_launched());
+    }
+    if (both) {
+        NUSHT_CUDA_TRY(cudaEventRecord(p->ev_leg_join, p->s_leg_aux));
+        NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_leg_join, 0));
     }
     return NUSHT_OK;
 }
@@ -1195,6 +1210,11 @@ int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s) {
 }
 
 void legendre_free(nusht_plan_s* p) {
+    if (p->s_leg_aux) cudaStreamDestroy(p->s_leg_aux);
+    if (p->ev_leg_fork) cudaEventDestroy(p->ev_leg_fork);
+    if (p->ev_leg_join) cudaEventDestroy(p->ev_leg_join);
+    p->s_leg_aux = nullptr;
+    p->ev_leg_fork = p->ev_leg_join = nullptr;
     cudaFree(p->d_items_syn);
     p->d_items_syn = nullptr;
     cudaFree(p->d_pair_n); cudaFree(p->d_pair_s);

@@ -100,6 +100,8 @@ struct nusht_plan_s {
     int* d_pair_s = nullptr;        //   and of its mirror ring (theta_s = pi - theta_n), -1 if the grid has none
     const double* h_ring_theta = nullptr;   // ring-list mode: HOST colatitudes, valid during legendre_build_tables only
     int lmax_io = 0;                // band limit of the caller's alm layout (= lmax except in ring plans built one degree higher)
+    cudaStream_t s_leg_aux = nullptr;       // side stream of the adjoint Legendre stage (second of its two launches)
+    cudaEvent_t ev_leg_fork = nullptr, ev_leg_join = nullptr;
     int2* d_items_syn = nullptr;    // work list of the Legendre synthesis: (block of ring pairs, m) per CTA, longest first
     int n_items_syn = 0;
     // --- Legendre work buffers ---

@@ -9,8 +9,16 @@
 // One thread per point, FP64 throughout ("double precision accuracy on the pointing").  The x and y
 // components are formed in the frame rotated by -phi about z (u = n'.(cos p, sin p, 0), v = n'.e_phi), so that
 // phi' = phi + atan2(v, u): two sincos instead of three and no cancellation in phi' for small deflections.
-// HBM-bound: 4 loads + 2 stores of 8 bytes per point, all coalesced.  The CPU oracle (oracle/oracle.py) writes
-// out the Cartesian form of Eq. C1 in long double and shares nothing with this file.
+// HBM floor: 4 loads + 2 stores of 8 bytes per point, all coalesced; what binds is the issue rate of the FP64
+// elementary functions (the first version: two sincos, two atan2, two sqrt, a division, about 500 instructions per
+// point).  Lensing deflections are arcminutes, so the common case is served by short series and the
+// general functions stay for the rest, per lane:
+//   * sin(a)/a and cos(a) as even polynomials in a^2 for a < 1/4 (no sqrt, no sincos, no division);
+//   * theta' = theta + atan2(rho cos t - z sin t, z cos t + rho sin t), rho = |n'_xy| (the rotation angle in the
+//     meridian plane of n'), and phi' = phi + atan2(v, u): both arguments are small unless the point sits next to a
+//     pole, and atan(x) is a 6-term odd series for |x| < 0.03 (truncation 4e-20).
+// The CPU oracle (oracle/oracle.py) writes out the Cartesian form of Eq. C1 in long double and shares nothing with
+// this file.
 #include <math.h>
 
 #include "nusht_internal.cuh"
@@ -18,7 +26,19 @@
 namespace {
 
 constexpr double PT_TWO_PI = 6.283185307179586476925286766559;
+constexpr double PT_PI = 3.14159265358979323846;
 constexpr int PT_THREADS = 256;
+
+// atan(x) for |x| < 0.03: x (1 - x^2/3 + x^4/5 - x^6/7 + x^8/9 - x^10/11), next term 0.03^12 / 13 = 4e-20
+__device__ __forceinline__ double atan_small(double x) {
+    const double y = x * x;
+    double p = -1.0 / 11.0;
+    p = fma(p, y, 1.0 / 9.0);
+    p = fma(p, y, -1.0 / 7.0);
+    p = fma(p, y, 1.0 / 5.0);
+    p = fma(p, y, -1.0 / 3.0);
+    return fma(x * y, p, x);
+}
 
 __global__ void __launch_bounds__(PT_THREADS)
 k_pointing(int64_t npts, const double* __restrict__ theta, const double* __restrict__ phi,
@@ -27,17 +47,47 @@ k_pointing(int64_t npts, const double* __restrict__ theta, const double* __restr
     const int64_t stride = (int64_t)gridDim.x * PT_THREADS;
     for (int64_t i = (int64_t)blockIdx.x * PT_THREADS + threadIdx.x; i < npts; i += stride) {
         const double t = theta[i], p = phi[i], at = a_theta[i], ap = a_phi[i];
-        const double a = sqrt(fma(at, at, ap * ap));      // angles: no overflow to guard against
-        double st, ct, sa, ca;
+        const double a2 = fma(at, at, ap * ap);           // angles: no overflow to guard against
+        double st, ct, sinc, ca;
         sincos(t, &st, &ct);
-        sincos(a, &sa, &ca);
-        const double sinc = (a > 0.0) ? sa / a : 1.0;
+        if (a2 < 0.0625) {
+            // sin(a)/a = sum (-a^2)^k / (2k+1)!,  cos(a) = sum (-a^2)^k / (2k)!;  a^2 <= 1/16: 7 and 8 terms reach 1e-17
+            double q = 1.0 / 6227020800.0;                     // 1/13!
+            q = fma(q, -a2, 1.0 / 39916800.0);                 // 1/11!
+            q = fma(q, -a2, 1.0 / 362880.0);                   // 1/9!
+            q = fma(q, -a2, 1.0 / 5040.0);
+            q = fma(q, -a2, 1.0 / 120.0);
+            q = fma(q, -a2, 1.0 / 6.0);
+            sinc = fma(q, -a2, 1.0);
+            double c = 1.0 / 87178291200.0;                    // 1/14!
+            c = fma(c, -a2, 1.0 / 479001600.0);                // 1/12!
+            c = fma(c, -a2, 1.0 / 3628800.0);                  // 1/10!
+            c = fma(c, -a2, 1.0 / 40320.0);
+            c = fma(c, -a2, 1.0 / 720.0);
+            c = fma(c, -a2, 1.0 / 24.0);
+            c = fma(c, -a2, 0.5);
+            ca = fma(c, -a2, 1.0);
+        } else {
+            const double a = sqrt(a2);
+            double sa;
+            sincos(a, &sa, &ca);
+            sinc = sa / a;
+        }
         // components of n' along (cos p, sin p, 0), e_phi and z
-        const double u = fma(ca, st, sinc * at * ct);
+        const double bt = sinc * at;
+        const double u = fma(ca, st, bt * ct);
         const double v = sinc * ap;
-        const double z = fma(ca, ct, -sinc * at * st);
-        const double t2 = atan2(sqrt(fma(u, u, v * v)), z);
-        double p2 = p + atan2(v, u);
+        const double z = fma(ca, ct, -bt * st);
+        const double rho = sqrt(fma(u, u, v * v));
+        // theta' = atan2(rho, z) = theta + (angle from n to n' in the meridian plane of n')
+        // (two rounded products, not an FMA: with zero deflection rho = sin t and z = cos t exactly, and the
+        //  difference must then be exactly zero so that theta' == theta)
+        const double sd = __dsub_rn(__dmul_rn(rho, ct), __dmul_rn(z, st)), cd = fma(z, ct, rho * st);
+        double t2;
+        if (fabs(sd) < 0.03 * cd) t2 = t + atan_small(sd / cd);
+        else t2 = atan2(rho, z);
+        t2 = fmin(fmax(t2, 0.0), PT_PI);
+        double p2 = p + ((fabs(v) < 0.03 * u) ? atan_small(v / u) : atan2(v, u));
         p2 -= PT_TWO_PI * floor(p2 * (1.0 / PT_TWO_PI));
         if (p2 < 0.0) p2 = 0.0;
         if (p2 >= PT_TWO_PI) p2 -= PT_TWO_PI;
