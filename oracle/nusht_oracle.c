@@ -10,8 +10,10 @@
  *
  * Parity pins (tests/test_oracle_pins.py): closed forms Y_00, Y_10, Y_11, Y_20..Y_22; mpmath
  * and scipy library values of Y_lm; the addition theorem; orthonormality under Gauss-Legendre
- * quadrature; the adjoint identity <S a, x> = <a, S^T x>; special cases.  No function here is
- * "parity unpinned".
+ * quadrature; the adjoint identity <S a, x> = <a, S^T x>; special cases; every copy of the l loop also in the
+ * exponent-rescaling regime (lmax 1500 .. 8191, near-pole points: mpmath values, the adjoint identity, ring_sum
+ * against synthesis); oracle_gradient (Eq. C2) by closed forms, finite differences of the synthesis and the ladder
+ * identity at lmax = 1500.  No function here is "parity unpinned".
  *
  * Build (done by __graft_entry__.build() and by oracle/oracle.py on first use):
  *   gcc -O2 -fopenmp -fPIC -shared -o liboracle.so nusht_oracle.c -lm
