@@ -91,6 +91,21 @@ FFTSM_HD int freq_of_pos(int p) {
     return p / (N / 2) + 2 * freq_of_pos_sub<N / 2>(p % (N / 2));
 }
 
+// the inverse map: (unpadded) position that holds frequency q after the forward passes, i.e. where the inverse chain
+// expects it.  Used by kernels that GENERATE a spectrum and can place each entry where the inverse transform wants it.
+template <int NS>
+FFTSM_HD int pos_of_freq_sub(int q) {
+    if constexpr (NS >= 16) {
+        return (q % 16) * (NS / 16) + pos_of_freq_sub<NS / 16>(q / 16);
+    } else {
+        return q;
+    }
+}
+template <int N>
+FFTSM_HD int pos_of_freq(int q) {
+    return (q & 1) * (N / 2) + pos_of_freq_sub<N / 2>(q >> 1);
+}
+
 // One DIF stage of radix R on every sub-transform of length NS of the array (N elements, T threads).
 // SIGN = -1: forward.  tw = stage table of NS/R entries exp(-2 pi i i/NS), i < NS/R (stage_table_offset).
 template <int N, int R, int NS, int SIGN>

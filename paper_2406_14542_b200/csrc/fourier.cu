@@ -750,6 +750,146 @@ k_theta_chain2_adj(int L, int M, int nrow_half, const C* __restrict__ h, const d
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Fused phi transform (a5 phi / a9 phi) for n_phi/2 = N a power of two <= 8192: ONE kernel per direction does what
+// k_h_to_z + cuFFT (and cuFFT + k_z_to_h) do in two passes over the 1 GB grid.  A CTA takes a grid row: it gathers the
+// row's half spectrum X[m] = H[m][parity][a'] (m <= mmax), forms the length-N complex sequence of the half-length
+// real-FFT trick (see k_h_to_z) directly at the digit-reversed positions the inverse chain of fft_smem.cuh expects,
+// transforms in shared memory and stores the real row with coalesced 16-byte stores; the adjoint loads the row,
+// transforms forward, and scatters the post-processed Y[m] back to H.  The gathers / scatters are 16-byte accesses
+// at a stride of one H column; rows of one parity are taken in order by neighbouring CTAs, so the other half of each
+// 32-byte sector is served from / merged in L2.
+// ---------------------------------------------------------------------------------------------
+struct PhiTables {
+    const double2* tw2;     // exp(-2 pi i i/N), i < N/2
+    const double2* stw;     // per-stage twiddles of length N (fftsm::stage_table_offset)
+    const double2* twz;     // W^m = exp(2 pi i m / n_phi), m <= mmax
+};
+
+// grid row index of the i-th row a CTA loop visits: all even rows a = 2a' in order, then all odd ones
+__device__ __forceinline__ int phi_row_of(int i, int nrow_half) {
+    const int n_even = (nrow_half + 1) / 2;
+    return i < n_even ? 2 * i : 2 * (i - n_even) + 1;
+}
+
+template <int N, typename C>
+__global__ void __launch_bounds__(ChainCfg<N>::T)
+k_phi_syn(int M, int nh, int nrow_half, const C* __restrict__ h, const PhiTables tb, C* __restrict__ grid) {
+    using namespace fftsm;
+    constexpr int T = ChainCfg<N>::T, RL = last_radix(N / 2);
+    extern __shared__ __align__(16) double2 s_col[];
+    const int tid = threadIdx.x;
+    for (int it = blockIdx.x; it < nrow_half; it += gridDim.x) {
+        const int a = phi_row_of(it, nrow_half), par = a & 1, ap = a >> 1;
+        __syncthreads();   // the previous row's stores have read s_col
+        for (int k = M + 1 + tid; k <= N - M - 1; k += T) s_col[pad(pos_of_freq<N>(k))] = make_double2(0.0, 0.0);
+        for (int m = tid; m <= M; m += T) {
+            const C xc = h[((int64_t)m * 2 + par) * nh + ap];
+            const double xr = (double)xc.x, xi = (double)xc.y;
+            if (m == 0) {          // X[0] is real for a real row; its imaginary part is ignored
+                s_col[pad(pos_of_freq<N>(0))] = make_double2(xr, xr);
+            } else {
+                const double2 w = tb.twz[m];
+                s_col[pad(pos_of_freq<N>(m))] = make_double2(xr * (1.0 - w.y) - xi * w.x, xr * w.x + xi * (1.0 - w.y));
+                s_col[pad(pos_of_freq<N>(N - m))] = make_double2(xr * (1.0 + w.y) + xi * w.x, xr * w.x - xi * (1.0 + w.y));
+            }
+        }
+        if (it + (int)gridDim.x < nrow_half) {               // next row's half spectrum -> L2 while this one is transformed
+            const int a2 = phi_row_of(it + (int)gridDim.x, nrow_half);
+            for (int m = tid; m <= M; m += T)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(h + ((int64_t)m * 2 + (a2 & 1)) * nh + (a2 >> 1)));
+        }
+        __syncthreads();
+        stage_dit<N, RL, RL, +1>(s_col, tid, T, tb.stw);     // first inverse stage: stride 1, no twiddles
+        __syncthreads();
+        DevExec<N, +1> inv{s_col, tb.stw, tid};
+        inverse_stages<N / 2>(inv);
+        C* row = grid + (int64_t)a * N;                      // the real row viewed as N pairs (x[2j], x[2j+1])
+        for (int i = tid; i < N / 2; i += T) {
+            const double2 z0 = s_col[pad(i)], z1 = cmul(s_col[pad(i + N / 2)], cconj(tb.tw2[i]));
+            C o0, o1;
+            o0.x = z0.x + z1.x;
+            o0.y = z0.y + z1.y;
+            o1.x = z0.x - z1.x;
+            o1.y = z0.y - z1.y;
+            row[i] = o0;
+            row[i + N / 2] = o1;
+        }
+    }
+}
+
+template <int N, typename C>
+__global__ void __launch_bounds__(ChainCfg<N>::T)
+k_phi_adj(int M, int nh, int nrow_half, const C* __restrict__ grid, const PhiTables tb, C* __restrict__ h) {
+    using namespace fftsm;
+    constexpr int T = ChainCfg<N>::T, RL = last_radix(N / 2);
+    extern __shared__ __align__(16) double2 s_col[];
+    const int tid = threadIdx.x;
+    for (int it = blockIdx.x; it < nrow_half; it += gridDim.x) {
+        const int a = phi_row_of(it, nrow_half), par = a & 1, ap = a >> 1;
+        const C* row = grid + (int64_t)a * N;
+        __syncthreads();
+        for (int i = tid; i < N / 2; i += T) {               // radix-2 stage of the forward transform, fused with the load
+            const C ac = row[i], bc = row[i + N / 2];
+            const double2 x0 = make_double2((double)ac.x, (double)ac.y), x1 = make_double2((double)bc.x, (double)bc.y);
+            s_col[pad(i)] = make_double2(x0.x + x1.x, x0.y + x1.y);
+            s_col[pad(i + N / 2)] = cmul(make_double2(x0.x - x1.x, x0.y - x1.y), tb.tw2[i]);
+        }
+        if (it + (int)gridDim.x < nrow_half)                 // next row -> L2 while this one is transformed
+            prefetch_l2(grid + (int64_t)phi_row_of(it + (int)gridDim.x, nrow_half) * N, N * (int)sizeof(C), tid, T);
+        __syncthreads();
+        DevExec<N, -1> fwd{s_col, tb.stw, tid};
+        forward_stages<N / 2>(fwd);
+        stage_dif<N, RL, RL, -1>(s_col, tid, T, tb.stw);     // last forward stage, in place
+        __syncthreads();
+        for (int m = tid; m <= M; m += T) {                  // post-processing of the real FFT (see k_z_to_h)
+            const double2 A = s_col[pad(pos_of_freq<N>(m))], Bq = s_col[pad(pos_of_freq<N>(m == 0 ? 0 : N - m))];
+            const double2 w = tb.twz[m];
+            const double bx = Bq.x, by = -Bq.y;              // B = conj Zf[N - m]
+            const double dx = A.x - bx, dy = A.y - by;
+            C out;
+            out.x = 0.5 * ((A.x + bx) + (w.x * dy - w.y * dx));
+            out.y = 0.5 * ((A.y + by) - (w.x * dx + w.y * dy));
+            h[((int64_t)m * 2 + par) * nh + ap] = out;
+        }
+    }
+}
+
+template <int N, typename C>
+int launch_phi(bool* attr_set, bool adjoint, int M, int nh, int nrow_half, int n_sm, const PhiTables& tb, C* h, C* grid,
+               cudaStream_t s) {
+    if (!attr_set[adjoint]) {
+        if (adjoint)
+            NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_phi_adj<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ChainCfg<N>::SMEM));
+        else
+            NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_phi_syn<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ChainCfg<N>::SMEM));
+        attr_set[adjoint] = true;
+    }
+    const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(8, (size_t)(200 * 1024) / (ChainCfg<N>::SMEM + 1024)));
+    const int blocks = std::min(nrow_half, n_sm * per_sm);
+    if (adjoint) k_phi_adj<N, C><<<blocks, ChainCfg<N>::T, ChainCfg<N>::SMEM, s>>>(M, nh, nrow_half, grid, tb, h);
+    else k_phi_syn<N, C><<<blocks, ChainCfg<N>::T, ChainCfg<N>::SMEM, s>>>(M, nh, nrow_half, h, tb, grid);
+    NUSHT_CUDA_TRY(nusht_launched());
+    return NUSHT_OK;
+}
+
+template <typename C>
+int dispatch_phi(nusht_plan_s* p, bool adjoint, cudaStream_t s) {
+    const int n = p->ng.nph / 2;
+    PhiTables tb;
+    tb.tw2 = p->d_phitab;
+    tb.stw = p->d_phitab + n / 2;
+    tb.twz = p->d_twz;
+    switch (n) {
+#define NUSHT_PHI(NN) \
+    case NN:          \
+        return launch_phi<NN, C>(p->phi_attr_set, adjoint, p->mmax, p->ng.nth / 2, p->ng.nrow_half, p->n_sm, tb, (C*)p->d_h, (C*)p->d_grid, s);
+        NUSHT_PHI(128) NUSHT_PHI(256) NUSHT_PHI(512) NUSHT_PHI(1024) NUSHT_PHI(2048) NUSHT_PHI(4096) NUSHT_PHI(8192)
+#undef NUSHT_PHI
+    }
+    return NUSHT_ERR_UNSUPPORTED;
+}
+
 // position -> frequency of the forward chain for a run-time N (host; mirrors fftsm::freq_of_pos)
 static int chain_freq_of_pos(int n, int p) {
     int q = p / (n / 2), mul = 2, ns = n / 2;
@@ -971,6 +1111,35 @@ int fourier_build(nusht_plan_s* p) {
         NUSHT_CUDA_TRY(cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, dev));
     }
 
+    // fused phi transform: n_phi / 2 a power of two in [128, 8192] next to a fused theta chain (NUSHT_PHI=cufft
+    // keeps the cuFFT path for the tests, which compare the two)
+    {
+        const int nz = g.nph / 2;
+        // Measured at config 3 (n_phi / 2 = 8192): adjoint 0.86 ms fused against 0.92 ms (cuFFT 0.59 + k_z_to_h 0.32);
+        // synthesis 0.94-0.97 ms fused against 0.88 ms (k_h_to_z 0.27 + cuFFT 0.61): one CTA per SM cannot overlap its
+        // phases and the radix-16 stages through shared memory cost about 12 us per 8192-point row, as much as cuFFT's
+        // register-tiled transform plus the extra pass.  Default: fused in the adjoint only; NUSHT_PHI = fused | cufft
+        // forces both directions (tests compare them).
+        const char* ev = getenv("NUSHT_PHI");
+        p->phi_fused = p->theta_fused && (nz & (nz - 1)) == 0 && nz >= 128 && nz <= 8192 && M < nz / 2 &&
+                       !(ev && strcmp(ev, "cufft") == 0);
+        p->phi_fused_syn = p->phi_fused && ev && strcmp(ev, "fused") == 0;
+        if (p->phi_fused) {
+            const int nst = fftsm::stage_table_len(nz);
+            std::vector<double2> tb((size_t)nz / 2 + nst);
+            const long double PI_L = 3.14159265358979323846264338327950288L;
+            auto unit = [&](long double turns) {
+                return make_double2((double)cosl(2.0L * PI_L * turns), (double)sinl(2.0L * PI_L * turns));
+            };
+            for (int i = 0; i < nz / 2; ++i) tb[i] = unit(-(long double)i / (long double)nz);
+            size_t o = (size_t)nz / 2;
+            for (int ns = nz / 2; ns >= 32; ns /= 16)
+                for (int i = 0; i < ns / 16; ++i) tb[o++] = unit(-(long double)i / (long double)ns);
+            NUSHT_TRY(f_alloc(&p->d_phitab, sizeof(double2) * tb.size(), p));
+            NUSHT_CUDA_TRY(cudaMemcpy(p->d_phitab, tb.data(), sizeof(double2) * tb.size(), cudaMemcpyHostToDevice));
+        }
+    }
+
     // cuFFT plans
     size_t ws = 0, wtot = 0;
     if (!p->theta_fused) {
@@ -990,10 +1159,12 @@ int fourier_build(nusht_plan_s* p) {
     {
         // phi pass: one complex transform of length n_phi/2 per grid row, in place (see k_h_to_z)
         int n[1] = {g.nph / 2};
-        NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi));
-        NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi, 1, n, nullptr, 1, g.nph / 2, nullptr, 1, g.nph / 2,
-                                          f64 ? CUFFT_Z2Z : CUFFT_C2C, g.nrow_half, &ws));
-        wtot += ws;
+        if (!p->phi_fused || !p->phi_fused_syn) {
+            NUSHT_CUFFT_TRY(cufftCreate(&p->fft_phi));
+            NUSHT_CUFFT_TRY(cufftMakePlanMany(p->fft_phi, 1, n, nullptr, 1, g.nph / 2, nullptr, 1, g.nph / 2,
+                                              f64 ? CUFFT_Z2Z : CUFFT_C2C, g.nrow_half, &ws));
+            wtot += ws;
+        }
         std::vector<double2> tw(M + 1);
         const long double PI_L = 3.14159265358979323846264338327950288L;
         for (int m = 0; m <= M; ++m) {
@@ -1117,6 +1288,12 @@ int fourier_synthesis(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
         NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_theta_fine, (cufftComplex*)p->d_h, (cufftComplex*)p->d_h, CUFFT_INVERSE));
     }
     REC(3);
+    if (p->phi_fused_syn) {
+        if (f64) NUSHT_TRY(dispatch_phi<double2>(p, false, s));
+        else NUSHT_TRY(dispatch_phi<float2>(p, false, s));
+        REC(4);
+        return NUSHT_OK;
+    }
     {
         // H -> pre-processed rows of the grid buffer, then one in-place complex transform per row
         const int nz = g.nph / 2;
@@ -1148,13 +1325,18 @@ int fourier_adjoint(nusht_plan_s* p, cudaStream_t s, cudaEvent_t* ev) {
     const int nth2 = p->lg.nth2;
     const bool f64 = p->dtype == NUSHT_F64;
     REC(0);
+    if (p->phi_fused) {
+        if (f64) NUSHT_TRY(dispatch_phi<double2>(p, true, s));
+        else NUSHT_TRY(dispatch_phi<float2>(p, true, s));
+    } else {
     NUSHT_CUFFT_TRY(cufftSetStream(p->fft_phi, s));
     if (f64)
         NUSHT_CUFFT_TRY(cufftExecZ2Z(p->fft_phi, (cufftDoubleComplex*)p->d_grid, (cufftDoubleComplex*)p->d_grid,
                                      CUFFT_FORWARD));
     else
         NUSHT_CUFFT_TRY(cufftExecC2C(p->fft_phi, (cufftComplex*)p->d_grid, (cufftComplex*)p->d_grid, CUFFT_FORWARD));
-    {
+    }
+    if (!p->phi_fused) {
         // post-processing + transpose to H[m][parity][a'], zero-extended in theta to the full period
         const int nz = g.nph / 2;
         dim3 grid(2 * ((g.nth / 2 + 31) / 32), (M + 32) / 32);
@@ -1210,6 +1392,8 @@ void fourier_free(nusht_plan_s* p) {
     if (p->fft_phi_r2c) cufftDestroy(p->fft_phi_r2c);
     p->fft_theta_coarse = p->fft_theta_fine = p->fft_phi = p->fft_phi_r2c = 0;
     cudaFree(p->d_z);
+    cudaFree(p->d_phitab);
+    p->d_phitab = nullptr;
     cudaFree(p->d_fftwork);
     p->d_z = nullptr;
     p->d_fftwork = nullptr;

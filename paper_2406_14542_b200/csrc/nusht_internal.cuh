@@ -119,6 +119,10 @@ struct nusht_plan_s {
     bool have_fft = false;
     int theta_chain = 0;            // 0: cuFFT chain, 1: fused chain, one CTA per column, 2: fused chain, cluster pair per column
     bool theta_fused = false;       // a3 + a4 + a5-theta (and their transposes) as one kernel per direction (fourier.cu)
+    bool phi_fused = false;         // a9-phi as one shared-memory FFT kernel (fourier.cu: k_phi_adj)
+    bool phi_fused_syn = false;     //   ... and a5-phi too (k_phi_syn; only with NUSHT_PHI=fused, see fourier_build)
+    double2* d_phitab = nullptr;    //   its twiddle tables (length n_phi / 2)
+    bool phi_attr_set[2] = {false, false};
     bool fourier_general = false;   // sigma != 2: full-length fine theta FFT and an out-of-place real phi FFT (fourier.cu)
     void* d_z = nullptr;            //   half spectra of the grid rows, [nth/2+1][nph/2+1] complex (dtype)
     cufftHandle fft_phi_r2c = 0;    //   R2C (dtype), length nph, batch nth/2+1 (fft_phi is then the C2R plan)

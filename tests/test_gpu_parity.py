@@ -500,3 +500,34 @@ def test_sigma_125_fp32_and_argument_checks(nusht, oracle):
     assert torch.equal(p2.synthesis(cu(alm)), p0.synthesis(cu(alm)))
     p2.destroy()
     p0.destroy()
+
+
+# ---- Fourier stage: fused phi transform (own shared-memory FFT) vs the cuFFT phi pass --------------------------------
+@pytest.mark.parametrize("dtype,eps,tol", [("f64", 1e-10, 1e-13), ("f32", 1e-5, 2e-6)])
+@pytest.mark.parametrize("L,M", [(63, 63), (127, 100), (255, 255), (511, 300), (1023, 1023), (2047, 2047), (2047, 1500)])
+def test_fused_phi_matches_cufft_phi(nusht, oracle, monkeypatch, dtype, eps, tol, L, M):
+    """n_phi / 2 is a power of two here: NUSHT_PHI=fused runs k_phi_syn / k_phi_adj (a grid row's half-length complex
+    FFT in shared memory, real-FFT pre/post-processing fused), NUSHT_PHI=cufft keeps k_h_to_z + cuFFT + k_z_to_h.  Both must agree to rounding in both directions, the fused pair must stay adjoint to 1e-12, and the
+    Fourier stage alone (random DFS-symmetric input) must agree as well."""
+    npts = 20000
+    theta, phi = inputs.uniform_sphere_points(npts, 87)
+    theta[:2] = [0.0, np.pi]
+    alm = inputs.random_alm(L, M, 87)
+    x = inputs.random_map(npts, 87)
+    rd, cd = (np.float32, np.complex64) if dtype == "f32" else (np.float64, np.complex128)
+    res = {}
+    for mode in ("cufft", "fused"):
+        monkeypatch.setenv("NUSHT_PHI", mode)      # (the default plan fuses the adjoint direction only)
+        plan = nusht.Plan(L, M, cu(theta), cu(phi), eps, dtype)
+        f = plan.synthesis(cu(alm.astype(cd))).cpu().numpy().astype(np.float64)
+        c = plan.adjoint(cu(x.astype(rd))).cpu().numpy().astype(np.complex128)
+        res[mode] = (f, c)
+        if mode == "fused" and dtype == "f64":
+            lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+            assert abs(lhs - oracle.inner_alm(L, M, alm, c)) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+        plan.destroy()
+    assert rel(res["fused"][0], res["cufft"][0]) <= tol
+    assert rel(res["fused"][1], res["cufft"][1]) <= tol
+    if L <= 255 and dtype == "f64":
+        sub = slice(0, 2000)
+        assert rel(res["fused"][0][sub], oracle.synthesis(L, M, theta[sub], phi[sub], alm, "ld")) <= 10 * eps
