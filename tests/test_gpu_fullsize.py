@@ -173,3 +173,55 @@ def test_fullsize_all_points_sparse_alm(oracle):
     assert rel(got, ref) <= 10 * eps
     assert np.max(np.abs(got - ref)) <= 100 * eps * np.sqrt(np.mean(np.abs(ref) ** 2))
     plan.destroy()
+
+
+def test_fullsize_ring_grid_gauss_legendre_4095(oracle):
+    """Ring-grid transforms at the band limit of the headline workload: a Gauss-Legendre grid with lmax = 4095 (4096
+    rings x 8192 pixels = 33.6 M pixels, the kind of grid the paper computes its maps on), in the
+    configuration `bench.py --ring gl` times.  Sampled pixels against Eq. 3 (long-double oracle; Pbar_mm underflows on
+    most rings at this lmax), the quadrature round trip analysis(synthesis(a)) = a (the special case of PAPER.md:74),
+    and the deflection field of Eq. C2 on the same grid against the oracle's direct sum."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2406_14542_b200 import nusht
+    L = 4095
+    x = np.polynomial.legendre.leggauss(L + 1)[0].astype(np.longdouble)
+    for _ in range(3):                      # polish numpy's nodes in long double (they lose digits at n ~ 1000)
+        p0, p1 = np.ones_like(x), x.copy()
+        for k in range(2, L + 2):
+            p0, p1 = p1, ((2 * k - 1) * x * p1 - (k - 1) * p0) / k
+        dp = (L + 1) * (x * p1 - p0) / (x * x - 1)
+        x = x - p1 / dp
+    p0, p1 = np.ones_like(x), x.copy()
+    for k in range(2, L + 2):
+        p0, p1 = p1, ((2 * k - 1) * x * p1 - (k - 1) * p0) / k
+    dp = (L + 1) * (x * p1 - p0) / (x * x - 1)
+    wq = np.asarray(2 / ((1 - x * x) * dp * dp), dtype=np.float64)
+    theta = np.asarray(np.arccos(x[::-1]), dtype=np.float64)
+    half = (L + 1) // 2
+    theta[L + 1 - half:] = np.pi - theta[:half][::-1]
+    nphi = np.full(L + 1, 2 * L + 2)
+    plan = nusht.RingPlan(L, L, theta, nphi, None, wq[::-1] * (2 * np.pi / (2 * L + 2)))
+    assert plan.info.npairs == (L + 1) // 2 and plan.info.nruns == 1
+    alm = inputs.random_alm(L, L, 601)
+    f = plan.synthesis(cu(alm))
+    back = plan.analysis(f).cpu().numpy()
+    assert rel(back, alm) <= 5e-12
+    assert np.max(np.abs(back - alm)) <= 2e-10 * np.max(np.abs(alm))
+    th = np.repeat(theta, nphi)
+    ph = np.tile(2 * np.pi * np.arange(2 * L + 2) / (2 * L + 2), L + 1)
+    rng = np.random.default_rng(602)
+    idx = np.sort(rng.choice(len(th), 300, replace=False))
+    idx = np.unique(np.concatenate([idx, [0, 5, len(th) - 1, (L // 2) * (2 * L + 2) + 7, (L // 2 + 1) * (2 * L + 2) + 7]]))
+    f_ref = oracle.synthesis(L, L, th[idx], ph[idx], alm, "ld")
+    fh = f.cpu().numpy()
+    assert rel(fh[idx], f_ref) <= 5e-11
+    assert rel_max(fh[idx], f_ref) <= 5e-10
+    philm = inputs.random_alm(L, L, 603, "inv_l2")
+    a_t, a_p = (t.cpu().numpy() for t in plan.gradient(cu(philm)))
+    r_t, r_p = oracle.gradient(L, L, th[idx], ph[idx], philm, "ld")
+    s = np.sin(th[idx])
+    scale = np.sqrt(np.mean(r_t ** 2 + r_p ** 2))
+    assert np.max(np.abs(a_t[idx] - r_t) * s) <= 1e-10 * scale
+    assert np.max(np.abs(a_p[idx] - r_p) * s) <= 1e-10 * scale
+    plan.destroy()
