@@ -531,3 +531,29 @@ def test_fused_phi_matches_cufft_phi(nusht, oracle, monkeypatch, dtype, eps, tol
     if L <= 255 and dtype == "f64":
         sub = slice(0, 2000)
         assert rel(res["fused"][0][sub], oracle.synthesis(L, M, theta[sub], phi[sub], alm, "ld")) <= 10 * eps
+
+
+@pytest.mark.parametrize("L,M,npts", [(0, 0, 50), (1, 1, 200), (5, 3, 500), (200, 10, 3000), (33, 33, 0)])
+def test_sigma_125_small_and_ragged_sizes(nusht, oracle, L, M, npts):
+    """sigma = 1.25 where the fine grid is set by the kernel footprint rather than by the band limit (tiny lmax), with
+    mmax << lmax (the shared H / grid allocation is then sized by the grid), and with no points at all."""
+    eps = 1e-8
+    if npts == 0:
+        plan = nusht.Plan(L, M, None, None, eps, sigma=1.25)
+        out = torch.full((plan.nlm,), 3.0 + 1j, dtype=torch.complex128, device="cuda")
+        plan.adjoint(torch.empty(0, dtype=torch.float64, device="cuda"), out)
+        assert torch.all(out == 0)
+        plan.destroy()
+        return
+    theta, phi = inputs.uniform_sphere_points(npts, 173)
+    theta[:2] = [0.0, np.pi]
+    alm = inputs.random_alm(L, M, 173)
+    x = inputs.random_map(npts, 173)
+    plan = nusht.Plan(L, M, cu(theta), cu(phi), eps, sigma=1.25)
+    f = plan.synthesis(cu(alm)).cpu().numpy()
+    c = plan.adjoint(cu(x)).cpu().numpy()
+    assert rel(f, oracle.synthesis(L, M, theta, phi, alm, "ld")) <= 10 * eps
+    assert rel(c, oracle.adjoint(L, M, theta, phi, x, "ld")) <= 10 * eps
+    lhs = float(np.sum(np.longdouble(f) * np.longdouble(x)))
+    assert abs(lhs - oracle.inner_alm(L, M, alm, c)) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    plan.destroy()
