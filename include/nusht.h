@@ -195,7 +195,7 @@ NUSHT_API int nusht_pointing(int64_t npts, const double* theta, const double* ph
  * lensing potential, Eq. C2 (8(f) rank 4) --------------------------------------------------------
  * A ring grid is nrings iso-latitude rings; ring r has colatitude theta[r] in [0, pi], nphi[r] >= 1 equidistant
  * pixels at phi0[r] + 2 pi j / nphi[r], j = 0 .. nphi[r]-1.  The map is the rings one after the other in the order
- * given, npix = sum nphi reals of the plan's dtype (Gauss-Legendre, Clenshaw-Curtis, Fejer and HEALPix-style layouts
+ * given (1 <= nphi[r] <= 2^21), npix = sum nphi reals of the plan's dtype (Gauss-Legendre, Clenshaw-Curtis, Fejer and HEALPix-style layouts
  * all fit).  theta, nphi, phi0 (NULL: 0) and weight (NULL: 1) are HOST arrays of length nrings, copied by the call.
  *   nusht_ring_synthesis  f(r, j) = sum_lm a_lm Y_lm(theta_r, phi_rj)                              (Eq. 3 on the grid)
  *   nusht_ring_analysis   c_lm = sum_r weight[r] sum_j f(r, j) conj Y_lm(theta_r, phi_rj)          (Eq. 2; weight = 1

@@ -103,6 +103,9 @@ extern "C" int nusht_plan_ex(nusht_plan_t** out, int lmax, int mmax, int64_t npt
     if (dtype != NUSHT_F64 && dtype != NUSHT_F32) return NUSHT_ERR_INVALID_ARG;
     double sigma = 2.0;
     if (opts && opts->sigma != 0.0) sigma = opts->sigma;
+    if (opts)
+        for (int i = 0; i < 6; ++i)
+            if (opts->reserved[i] != 0) return NUSHT_ERR_INVALID_ARG;
     if (sigma != 2.0 && sigma != 1.25) return NUSHT_ERR_INVALID_ARG;
     if (!(eps <= 1e-1)) return NUSHT_ERR_INVALID_ARG;
     // accuracy floors: FP64 1e-13 at sigma = 2, 1e-10 at sigma = 1.25 (the paper's fn. 6); FP32 1e-6 / 1e-5

@@ -348,7 +348,7 @@ extern "C" int nusht_ring_plan(nusht_ring_plan_t** out, int lmax, int mmax, int 
         if (!(theta[r] >= 0.0) || !(theta[r] <= 3.14159265358979323846)) return NUSHT_ERR_BAD_POINTS;
         if (phi0 && !isfinite(phi0[r])) return NUSHT_ERR_BAD_POINTS;
         if (weight && !isfinite(weight[r])) return NUSHT_ERR_INVALID_ARG;
-        if (nphi[r] < 1 || nphi[r] > (1 << 27)) return NUSHT_ERR_INVALID_ARG;
+        if (nphi[r] < 1 || nphi[r] > (1 << 21)) return NUSHT_ERR_INVALID_ARG;   // (grid.y of k_ring_spec_syn: n/64 blocks)
         npix += nphi[r];
     }
     const auto t0 = std::chrono::steady_clock::now();

@@ -69,3 +69,37 @@ def test_no_device_is_a_loud_error(lib):
     h = ctypes.c_void_p()
     assert lib.nusht_plan(ctypes.byref(h), 4, 4, 0, None, None, 1e-6, 0) == -3      # NUSHT_ERR_CUDA, no fallback
     assert lib.nusht_destroy(None) == 0
+
+
+def test_plan_ex_rejects_bad_options_without_device(lib):
+    class Opts(ctypes.Structure):
+        _fields_ = [("sigma", ctypes.c_double), ("reserved", ctypes.c_int * 6)]
+    lib.nusht_plan_ex.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_int, ctypes.c_int64,
+                                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.POINTER(Opts)]
+    h = ctypes.c_void_p()
+    o = Opts()
+    o.sigma = 1.5
+    assert lib.nusht_plan_ex(ctypes.byref(h), 4, 4, 0, None, None, 1e-6, 0, ctypes.byref(o)) == -1     # unsupported sigma
+    o.sigma = 1.25
+    assert lib.nusht_plan_ex(ctypes.byref(h), 4, 4, 0, None, None, 1e-11, 0, ctypes.byref(o)) == -1    # below the 1e-10 floor
+    o.reserved[2] = 7
+    assert lib.nusht_plan_ex(ctypes.byref(h), 4, 4, 0, None, None, 1e-6, 0, ctypes.byref(o)) == -1     # reserved must be zero
+    assert h.value is None
+
+
+def test_ring_plan_rejects_bad_arguments_without_device(lib):
+    dp, lp = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int64)
+    lib.nusht_ring_plan.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, lp, dp,
+                                    dp, ctypes.c_int]
+    h = ctypes.c_void_p()
+    th = (ctypes.c_double * 2)(0.5, 4.0)
+    n = (ctypes.c_int64 * 2)(8, 8)
+    assert lib.nusht_ring_plan(ctypes.byref(h), 4, 4, 2, th, n, None, None, 0) == -6       # theta outside [0, pi]
+    th[1] = 2.0
+    n[1] = 0
+    assert lib.nusht_ring_plan(ctypes.byref(h), 4, 4, 2, th, n, None, None, 0) == -1       # empty ring
+    n[1] = 8
+    assert lib.nusht_ring_plan(ctypes.byref(h), 4, 5, 2, th, n, None, None, 0) == -1       # mmax > lmax
+    assert lib.nusht_ring_plan(ctypes.byref(h), 4, 4, 0, th, n, None, None, 0) == -1       # no rings
+    assert h.value is None
+    assert lib.nusht_ring_destroy(None) == 0
