@@ -1121,9 +1121,12 @@ int fourier_build(nusht_plan_s* p) {
         // register-tiled transform plus the extra pass.  Default: fused in the adjoint only; NUSHT_PHI = fused | cufft
         // forces both directions (tests compare them).
         const char* ev = getenv("NUSHT_PHI");
+        // (FP32 plans keep cuFFT unless forced: its binary32 transform takes 0.37 ms where the fused kernel, which
+        //  computes in binary64 whatever the storage type, takes 0.83 ms)
+        const bool forced = ev && strcmp(ev, "fused") == 0;
         p->phi_fused = p->theta_fused && (nz & (nz - 1)) == 0 && nz >= 128 && nz <= 8192 && M < nz / 2 &&
-                       !(ev && strcmp(ev, "cufft") == 0);
-        p->phi_fused_syn = p->phi_fused && ev && strcmp(ev, "fused") == 0;
+                       !(ev && strcmp(ev, "cufft") == 0) && (f64 || forced);
+        p->phi_fused_syn = p->phi_fused && forced;
         if (p->phi_fused) {
             const int nst = fftsm::stage_table_len(nz);
             std::vector<double2> tb((size_t)nz / 2 + nst);
