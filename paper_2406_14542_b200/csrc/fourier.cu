@@ -22,6 +22,7 @@
 
 #include <cooperative_groups.h>
 
+#include "fft_reg.cuh"
 #include "fft_smem.cuh"
 #include "nusht_internal.cuh"
 
@@ -855,6 +856,125 @@ k_phi_adj(int M, int nh, int nrow_half, const C* __restrict__ grid, const PhiTab
     }
 }
 
+// The same two kernels at N = 8192 on the register-tiled transform of fft_reg.cuh.  The radix-2 split of the length-N
+// transform gives two INDEPENDENT 4096-point transforms (even / odd outputs of the inverse, even / odd frequencies of
+// the forward one; Zf[m] and its partner Zf[N - m] of the real-FFT post-processing have the same parity), so a work
+// item is (grid row, half): one CTA of 256 threads, 16 points per thread in registers, two exchanges through 70 KB of
+// shared memory.  Two such CTAs fit an SM (registers), so the loads / stores of one overlap the transform of the
+// other, which the one-CTA-per-SM kernels above cannot do.
+template <typename C>
+__global__ void __launch_bounds__(256, 2)
+k_phi_syn_r(int M, int nh, int nrow_half, const C* __restrict__ h, const PhiTables tb, C* __restrict__ grid) {
+    using namespace fftsm;
+    constexpr int N = 8192, H = N / 2;
+    extern __shared__ __align__(16) double2 s_half[];
+    const int th = threadIdx.x;
+    const double2* tw4096 = tb.stw + stage_table_offset(N, 4096);
+    const double2* tw256 = tb.stw + stage_table_offset(N, 256);
+    for (int item = blockIdx.x; item < 2 * nrow_half; item += gridDim.x) {
+        const int hf = item & 1, a = phi_row_of(item >> 1, nrow_half), par = a & 1, ap = a >> 1;
+        const C* hrow = h + (int64_t)par * nh + ap;          // X[m] = hrow[m * 2 nh]
+        double2 x[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            // Z[q] and Z[q + N/2] of the half-length real-FFT sequence (see k_h_to_z), q = th + 256 j
+            const int q = th + 256 * j, mq = H - q;
+            double2 zlo = make_double2(0.0, 0.0), zhi = make_double2(0.0, 0.0);
+            if (q <= M) {
+                const C xc = hrow[(int64_t)q * 2 * nh];
+                const double xr = (double)xc.x, xi = (double)xc.y;
+                if (q == 0) {
+                    zlo = make_double2(xr, xr);              // X[0] is real for a real row
+                } else {
+                    const double2 w = tb.twz[q];
+                    zlo = make_double2(xr * (1.0 - w.y) - xi * w.x, xr * w.x + xi * (1.0 - w.y));
+                }
+            }
+            if (q > 0 && mq <= M) {                          // Z[N - m], m = N/2 - q
+                const C xc = hrow[(int64_t)mq * 2 * nh];
+                const double xr = (double)xc.x, xi = (double)xc.y;
+                const double2 w = tb.twz[mq];
+                zhi = make_double2(xr * (1.0 + w.y) + xi * w.x, xr * w.x - xi * (1.0 + w.y));
+            }
+            // radix-2 split of the inverse transform: even outputs from Z[q] + Z[q + N/2], odd ones from the twiddled difference
+            x[j] = hf ? cmul(make_double2(zlo.x - zhi.x, zlo.y - zhi.y), cconj(tb.tw2[q]))
+                      : make_double2(zlo.x + zhi.x, zlo.y + zhi.y);
+        }
+        __syncthreads();                                     // the previous item's last exchange has been read
+        fftreg::fft4096<+1>(x, s_half, th, tw4096, tw256);
+        C* row = grid + (int64_t)a * N;                      // the real row viewed as N pairs (x[2j], x[2j+1])
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+            const double2 v = x[bitrev(c, 16)];
+            C o;
+            o.x = v.x;
+            o.y = v.y;
+            row[2 * (th + 256 * c) + hf] = o;
+        }
+    }
+}
+
+template <typename C>
+__global__ void __launch_bounds__(256, 2)
+k_phi_adj_r(int M, int nh, int nrow_half, const C* __restrict__ grid, const PhiTables tb, C* __restrict__ h) {
+    using namespace fftsm;
+    constexpr int N = 8192, H = N / 2;
+    extern __shared__ __align__(16) double2 s_half[];
+    const int th = threadIdx.x;
+    const double2* tw4096 = tb.stw + stage_table_offset(N, 4096);
+    const double2* tw256 = tb.stw + stage_table_offset(N, 256);
+    for (int item = blockIdx.x; item < 2 * nrow_half; item += gridDim.x) {
+        const int hf = item & 1, a = phi_row_of(item >> 1, nrow_half), par = a & 1, ap = a >> 1;
+        const C* row = grid + (int64_t)a * N;
+        double2 x[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {                       // radix-2 split of the forward transform, fused with the load
+            const int i = th + 256 * j;
+            const C ac = row[i], bc = row[i + H];
+            const double2 x0 = make_double2((double)ac.x, (double)ac.y), x1 = make_double2((double)bc.x, (double)bc.y);
+            x[j] = hf ? cmul(make_double2(x0.x - x1.x, x0.y - x1.y), tb.tw2[i]) : make_double2(x0.x + x1.x, x0.y + x1.y);
+        }
+        __syncthreads();                                     // the previous item's post-processing has read s_half
+        fftreg::fft4096<-1>(x, s_half, th, tw4096, tw256);
+        __syncthreads();                                     // every thread is past its last read of the exchange buffer
+#pragma unroll
+        for (int c = 0; c < 16; ++c) s_half[pad(th + 256 * c)] = x[bitrev(c, 16)];   // Zf[2 q + hf] at q
+        __syncthreads();
+        // post-processing of the real FFT (see k_z_to_h) for the m of this half's parity: m = 2 q + hf, and its partner
+        // N - m = 2 (N/2 - q - hf) + hf lives in the same half
+#pragma unroll 4
+        for (int j = 0; j < 16; ++j) {
+            const int q = th + 256 * j, m = 2 * q + hf;
+            if (m > M) break;
+            const int qp = (m == 0) ? 0 : H - q - hf;
+            const double2 A = s_half[pad(q)], Bq = s_half[pad(qp)];
+            const double2 w = tb.twz[m];
+            const double bx = Bq.x, by = -Bq.y;              // B = conj Zf[N - m]
+            const double dx = A.x - bx, dy = A.y - by;
+            C out;
+            out.x = 0.5 * ((A.x + bx) + (w.x * dy - w.y * dx));
+            out.y = 0.5 * ((A.y + by) - (w.x * dx + w.y * dy));
+            h[((int64_t)m * 2 + par) * nh + ap] = out;
+        }
+    }
+}
+
+template <typename C>
+int launch_phi_r(bool* attr_set, bool adjoint, int M, int nh, int nrow_half, int n_sm, const PhiTables& tb, C* h, C* grid,
+                 cudaStream_t s) {
+    constexpr int SMEM = fftreg::HSMEM * (int)sizeof(double2);
+    if (!attr_set[adjoint]) {
+        if (adjoint) NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_phi_adj_r<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
+        else NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_phi_syn_r<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
+        attr_set[adjoint] = true;
+    }
+    const int blocks = std::min(2 * nrow_half, 2 * n_sm);
+    if (adjoint) k_phi_adj_r<C><<<blocks, 256, SMEM, s>>>(M, nh, nrow_half, grid, tb, h);
+    else k_phi_syn_r<C><<<blocks, 256, SMEM, s>>>(M, nh, nrow_half, h, tb, grid);
+    NUSHT_CUDA_TRY(nusht_launched());
+    return NUSHT_OK;
+}
+
 template <int N, typename C>
 int launch_phi(bool* attr_set, bool adjoint, int M, int nh, int nrow_half, int n_sm, const PhiTables& tb, C* h, C* grid,
                cudaStream_t s) {
@@ -880,6 +1000,9 @@ int dispatch_phi(nusht_plan_s* p, bool adjoint, cudaStream_t s) {
     tb.tw2 = p->d_phitab;
     tb.stw = p->d_phitab + n / 2;
     tb.twz = p->d_twz;
+    if (n == 8192 && !getenv("NUSHT_PHI_SMEM"))       // register-tiled transform (NUSHT_PHI_SMEM keeps the stage-by-stage one: tests)
+        return launch_phi_r<C>(p->phi_attr_set, adjoint, p->mmax, p->ng.nth / 2, p->ng.nrow_half, p->n_sm, tb, (C*)p->d_h,
+                               (C*)p->d_grid, s);
     switch (n) {
 #define NUSHT_PHI(NN) \
     case NN:          \

@@ -21,3 +21,16 @@ def test_fft_smem_against_direct_dft(tmp_path):
     out = subprocess.run([exe], capture_output=True, text=True)
     assert out.returncode == 0, out.stdout + out.stderr
     assert "OK" in out.stdout
+
+
+def test_fft_reg_against_direct_dft(tmp_path):
+    """The register-tiled 4096-point transform of the fused phi kernels (csrc/fft_reg.cuh), phase by phase on the host."""
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not available")
+    exe = str(tmp_path / "fft_reg_check")
+    src = os.path.join(ROOT, "tests", "fft_reg_host_check.cu")
+    subprocess.check_call([nvcc, "-std=c++17", "-O1", "-Wno-deprecated-gpu-targets", "-o", exe, src])
+    out = subprocess.run([exe], capture_output=True, text=True)
+    assert out.returncode == 0, out.stdout + out.stderr
+    assert "OK" in out.stdout

@@ -504,7 +504,8 @@ def test_sigma_125_fp32_and_argument_checks(nusht, oracle):
 
 # ---- Fourier stage: fused phi transform (own shared-memory FFT) vs the cuFFT phi pass --------------------------------
 @pytest.mark.parametrize("dtype,eps,tol", [("f64", 1e-10, 1e-13), ("f32", 1e-5, 2e-6)])
-@pytest.mark.parametrize("L,M", [(63, 63), (127, 100), (255, 255), (511, 300), (1023, 1023), (2047, 2047), (2047, 1500)])
+@pytest.mark.parametrize("L,M", [(63, 63), (127, 100), (255, 255), (511, 300), (1023, 1023), (2047, 2047), (2047, 1500),
+                                 (4095, 4095), (4095, 3000)])
 def test_fused_phi_matches_cufft_phi(nusht, oracle, monkeypatch, dtype, eps, tol, L, M):
     """n_phi / 2 is a power of two here: NUSHT_PHI=fused runs k_phi_syn / k_phi_adj (a grid row's half-length complex
     FFT in shared memory, real-FFT pre/post-processing fused), NUSHT_PHI=cufft keeps k_h_to_z + cuFFT + k_z_to_h.  Both must agree to rounding in both directions, the fused pair must stay adjoint to 1e-12, and the
