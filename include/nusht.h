@@ -61,7 +61,8 @@ enum {
     NUSHT_ERR_CUDA = -3,        /* CUDA runtime / launch error (also: no device) */
     NUSHT_ERR_CUFFT = -4,       /* cuFFT plan or exec error */
     NUSHT_ERR_UNSUPPORTED = -5, /* valid request this build does not implement */
-    NUSHT_ERR_BAD_POINTS = -6   /* NaN/Inf coordinates or theta outside [0, pi] */
+    NUSHT_ERR_BAD_POINTS = -6,  /* NaN/Inf coordinates or theta outside [0, pi] */
+    NUSHT_ERR_TOO_LARGE = -7    /* request beyond the fixed capacity of nusht_stage_legendre_adjoint_static */
 };
 
 /* Stage slots reported by nusht_stage_times.
@@ -159,6 +160,27 @@ NUSHT_API int nusht_host_reserve(nusht_plan_t* plan);
  * Its transpose (a10-a11): Gtilde (same layout) -> alm. */
 NUSHT_API int nusht_stage_legendre_synthesis(nusht_plan_t* plan, const void* alm, void* ftilde, void* stream);
 NUSHT_API int nusht_stage_legendre_adjoint(nusht_plan_t* plan, const void* gtilde, void* alm, void* stream);
+/* The same transpose (a10-a11; Eq. 5: S^T D^T) for callers that may not allocate between set-up and
+ * tear-down (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the kernels of
+ * nusht_stage_legendre_adjoint, accumulating into a file-scope `static __device__` array of the library instead of the
+ * plan's workspace.  The call itself allocates nothing -- no cudaMalloc / cudaFree, no cuFFT, no host allocation -- and
+ * enqueues a memset of the array (the kernels accumulate with global reductions, so it must start at zero; it keeps
+ * the previous call's contents otherwise), the two Legendre launches and the alm conversion, on `stream` and on the
+ * plan's side stream exactly as the ordinary call does.
+ *   gtilde  DEVICE complex128 [(mmax+1)][n_theta], caller-owned, read only
+ *   alm     DEVICE, plan's dtype, nlm complex, caller-owned, overwritten
+ * Capacity: NUSHT_STATIC_SCRATCH_BYTES (8,404,992 B = 262,656 accumulators of 32 B: one per pair of even/odd degrees,
+ * sum_m ((lmax - m)/2 + 1) of them), i.e. every plan up to lmax = mmax = 1023; every GPU that loads the library holds
+ * the array until the process exits.  A larger plan gives NUSHT_ERR_TOO_LARGE (nothing is enqueued); the plan's
+ * device must be the current device, else NUSHT_ERR_INVALID_ARG.
+ * ALL calls on one device share the one array: two calls that can overlap on the GPU (different streams without an
+ * ordering between them, also from different plans or host threads) race on it and both results are garbage; calls
+ * on one stream, or ordered by events, are fine.  The array's device address is looked up once per device
+ * (cudaGetSymbolAddress, which may load the module): nusht_static_scratch does that at set-up, so that no call under
+ * graph capture is the first one; it returns the capacity in bytes through *bytes (may be NULL). */
+#define NUSHT_STATIC_SCRATCH_BYTES 8404992
+NUSHT_API int nusht_static_scratch(int64_t* bytes);
+NUSHT_API int nusht_stage_legendre_adjoint_static(nusht_plan_t* plan, const void* gtilde, void* alm, void* stream);
 /* Fourier stage alone (a3 + a4 + a5, and a9): Ftilde (layout above) -> the plan's half fine grid, DEVICE real
  * [n_theta_fine/2 + 1][n_phi_fine] of the plan's dtype, i.e. the coarse theta FFT, deconvolution by the kernel's
  * Fourier transform, zero-padding and the fine inverse FFT; and its transpose grid -> Gtilde.

@@ -62,6 +62,9 @@ extern "C" const char* nusht_strerror(int code) {
         case NUSHT_ERR_CUFFT: return g_last_error[0] ? g_last_error : "cuFFT error";
         case NUSHT_ERR_UNSUPPORTED: return "unsupported request";
         case NUSHT_ERR_BAD_POINTS: return "bad point coordinates (NaN/Inf or theta outside [0, pi])";
+        case NUSHT_ERR_TOO_LARGE:
+            return "plan too large for the static scratch array of nusht_stage_legendre_adjoint_static "
+                   "(NUSHT_STATIC_SCRATCH_BYTES: up to lmax = mmax = 1023)";
     }
     return "unknown status";
 }
@@ -361,6 +364,13 @@ extern "C" int nusht_stage_legendre_adjoint(nusht_plan_t* p, const void* gtilde,
     cudaStream_t s = (cudaStream_t)stream;
     NUSHT_TRY(legendre_adjoint(p, (const double2*)gtilde, s));
     return legendre_alm_post(p, alm, s);
+}
+
+extern "C" int nusht_static_scratch(int64_t* bytes) { return legendre_static_scratch(bytes); }
+
+extern "C" int nusht_stage_legendre_adjoint_static(nusht_plan_t* p, const void* gtilde, void* alm, void* stream) {
+    if (!p || !alm || !gtilde) return NUSHT_ERR_INVALID_ARG;
+    return legendre_adjoint_static(p, (const double2*)gtilde, alm, (cudaStream_t)stream);
 }
 
 extern "C" int nusht_stage_fourier_synthesis(nusht_plan_t* p, const void* ftilde, void* grid, void* stream) {

@@ -33,6 +33,7 @@
 #include <stdio.h>
 
 #include <algorithm>
+#include <mutex>
 #include <utility>
 #include <vector>
 
@@ -1204,6 +1205,91 @@ int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s) {
                                                       p->d_rho, (double*)alm);
     else
         k_alm_post<float><<<blocks, threads, 0, s>>>(p->lmax, p->lmax_io, p->mmax, p->d_eoff, p->d_aeo, p->d_sig, p->d_sodd,
+                                                     p->d_rho, (float*)alm);
+    NUSHT_CUDA_TRY(nusht_launched());
+    return NUSHT_OK;
+}
+
+// ---- a10 + a11 without any allocation (include/nusht.h: nusht_stage_legendre_adjoint_static) --------------------
+// The even/odd accumulators of the adjoint live in a file-scope array of the library instead of the plan's d_aeo, for
+// callers that cannot call cudaMalloc between set-up and tear-down.  262,656 = sum_m ((L - m)/2 + 1) at L = M = 1023.
+// Every device that loads this module holds the array (8.02 MiB) until the process exits; every call on a device
+// shares it (calls that overlap on the GPU race, see the header).
+constexpr int64_t STATIC_EO_MAX = 262656;
+static_assert(STATIC_EO_MAX * (int64_t)sizeof(double4) == NUSHT_STATIC_SCRATCH_BYTES, "header and array disagree");
+static __device__ __align__(256) double4 g_static_eo[STATIC_EO_MAX];
+
+// In host code `g_static_eo` is only the handle the runtime registered for the symbol, not an address a kernel can
+// use: the device address is asked for once per device, with that device current, and cached here.
+constexpr int STATIC_MAX_DEVICES = 64;
+static std::mutex g_static_mu;
+static double4* g_static_eo_dev[STATIC_MAX_DEVICES] = {};
+
+static int static_eo_address(double4** out) {
+    int dev = -1;
+    NUSHT_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return NUSHT_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_eo_dev[dev]) {
+        void* ptr = nullptr;
+        NUSHT_CUDA_TRY(cudaGetSymbolAddress(&ptr, g_static_eo));
+        if (!ptr) return NUSHT_ERR_CUDA;
+        g_static_eo_dev[dev] = (double4*)ptr;
+    }
+    *out = g_static_eo_dev[dev];
+    return NUSHT_OK;
+}
+
+int legendre_static_scratch(int64_t* bytes) {
+    double4* eo = nullptr;
+    NUSHT_TRY(static_eo_address(&eo));
+    if (bytes) *bytes = STATIC_EO_MAX * (int64_t)sizeof(double4);
+    return NUSHT_OK;
+}
+
+// legendre_adjoint + legendre_alm_post with `eo` = the static array: the same kernels, grids and side stream (those
+// two functions are left as they are; this one repeats their launch logic)
+int legendre_adjoint_static(nusht_plan_s* p, const double2* gt, void* alm, cudaStream_t s) {
+    if (p->n_e_total > STATIC_EO_MAX) return NUSHT_ERR_TOO_LARGE;
+    int dev = -1;
+    NUSHT_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != p->device) return NUSHT_ERR_INVALID_ARG;
+    double4* eo = nullptr;
+    NUSHT_TRY(static_eo_address(&eo));
+    // the kernels accumulate with global reductions and the array holds the previous call's sums
+    NUSHT_CUDA_TRY(cudaMemsetAsync(eo, 0, sizeof(double4) * (size_t)p->n_e_total, s));
+    LegParams P = make_params(p, true);
+    const dim3 grid = leg_grid(p, ADJ_R, P);
+    const int nbx = (int)grid.x, split = std::min(P.b_split, nbx);
+    const bool both = split > 0 && split < nbx;
+    if (both) {
+        NUSHT_CUDA_TRY(cudaEventRecord(p->ev_leg_fork, s));
+        NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_leg_aux, p->ev_leg_fork, 0));
+    }
+    for (int part = 1; part >= 0; --part) {
+        LegParams Q = P;
+        const int first = part ? split : 0, count = part ? nbx - split : split;
+        if (count <= 0) continue;
+        Q.b_split = first;
+        if (part) Q.ab = P.ab + p->n_e_total;
+        const dim3 g2(count, grid.y);
+        cudaStream_t sl = (both && part == 0) ? p->s_leg_aux : s;
+        if (p->lg.ring_mode)
+            k_legendre_adjoint<ADJ_R, ADJ_CHUNK, true><<<g2, 32, 0, sl>>>(Q, gt, eo);
+        else
+            k_legendre_adjoint<ADJ_R, ADJ_CHUNK, false><<<g2, 32, 0, sl>>>(Q, gt, eo);
+        NUSHT_CUDA_TRY(nusht_launched());
+    }
+    if (both) {
+        NUSHT_CUDA_TRY(cudaEventRecord(p->ev_leg_join, p->s_leg_aux));
+        NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_leg_join, 0));
+    }
+    const int threads = PREP_THREADS, blocks = (p->mmax + 1 + threads / 32 - 1) / (threads / 32);
+    if (p->dtype == NUSHT_F64)
+        k_alm_post<double><<<blocks, threads, 0, s>>>(p->lmax, p->lmax_io, p->mmax, p->d_eoff, eo, p->d_sig, p->d_sodd,
+                                                      p->d_rho, (double*)alm);
+    else
+        k_alm_post<float><<<blocks, threads, 0, s>>>(p->lmax, p->lmax_io, p->mmax, p->d_eoff, eo, p->d_sig, p->d_sodd,
                                                      p->d_rho, (float*)alm);
     NUSHT_CUDA_TRY(nusht_launched());
     return NUSHT_OK;

@@ -163,6 +163,8 @@ int legendre_alm_prep(nusht_plan_s* p, const void* alm, cudaStream_t s);
 int legendre_synthesis(nusht_plan_s* p, double2* ft, cudaStream_t s);
 int legendre_adjoint(nusht_plan_s* p, const double2* gt, cudaStream_t s);
 int legendre_alm_post(nusht_plan_s* p, void* alm, cudaStream_t s);
+int legendre_static_scratch(int64_t* bytes);                                              // no-allocation variant
+int legendre_adjoint_static(nusht_plan_s* p, const double2* gt, void* alm, cudaStream_t s);  // (legendre.cu, end)
 void legendre_free(nusht_plan_s* p);
 
 // ---- fourier.cu ----

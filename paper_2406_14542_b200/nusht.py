@@ -25,7 +25,8 @@ EXPORTS = [
     "nusht_plan_info", "nusht_strerror", "nusht_version", "nusht_pointing", "nusht_host_reserve",
     "nusht_stage_fourier_synthesis", "nusht_stage_fourier_adjoint", "nusht_launch_count", "nusht_probe_fp64",
     "nusht_ring_plan", "nusht_ring_synthesis", "nusht_ring_analysis", "nusht_ring_gradient", "nusht_ring_info",
-    "nusht_ring_destroy", "nusht_ring_pairing", "nusht_plan_ex",
+    "nusht_ring_destroy", "nusht_ring_pairing", "nusht_plan_ex", "nusht_static_scratch",
+    "nusht_stage_legendre_adjoint_static",
 ]
 
 
@@ -69,7 +70,8 @@ def _load():
     lib.nusht_plan.argtypes = [ctypes.POINTER(vp), ip, ip, ctypes.c_int64, vp, vp, ctypes.c_double, ip]
     for name in ("nusht_synthesis", "nusht_adjoint", "nusht_synthesis_host", "nusht_adjoint_host",
                  "nusht_stage_legendre_synthesis", "nusht_stage_legendre_adjoint", "nusht_stage_interp",
-                 "nusht_stage_spread", "nusht_stage_fourier_synthesis", "nusht_stage_fourier_adjoint"):
+                 "nusht_stage_spread", "nusht_stage_fourier_synthesis", "nusht_stage_fourier_adjoint",
+                 "nusht_stage_legendre_adjoint_static"):
         getattr(lib, name).argtypes = [vp, vp, vp, vp]
         getattr(lib, name).restype = ip
     lib.nusht_plan.restype = ip
@@ -82,6 +84,8 @@ def _load():
     lib.nusht_host_sync.restype = ip
     lib.nusht_host_reserve.argtypes = [vp]
     lib.nusht_host_reserve.restype = ip
+    lib.nusht_static_scratch.argtypes = [ctypes.POINTER(ctypes.c_int64)]
+    lib.nusht_static_scratch.restype = ip
     lib.nusht_launch_count.argtypes = []
     lib.nusht_launch_count.restype = ctypes.c_int64
     lib.nusht_probe_fp64.argtypes = [ip, ctypes.POINTER(ctypes.c_double)]
@@ -236,6 +240,18 @@ class Plan:
                                                 _stream_ptr(stream)))
         return out
 
+    def stage_legendre_adjoint_static(self, gt, out, stream=None):
+        """nusht_stage_legendre_adjoint_static: the same result through the library's static scratch array; the C
+        call allocates nothing (hence `out` is the caller's).  Plans up to lmax = mmax = 1023; calls that overlap
+        on the GPU race on the one array (include/nusht.h)."""
+        if gt.dtype != torch.complex128 or tuple(gt.shape) != (self.mmax + 1, self.info.n_theta) or not gt.is_cuda \
+                or not gt.is_contiguous():
+            raise TypeError("gtilde must be contiguous CUDA complex128 [(mmax+1), n_theta]")
+        if out.dtype != self.cdtype or tuple(out.shape) != (self.nlm,) or not out.is_cuda or not out.is_contiguous():
+            raise TypeError("out must be contiguous CUDA %s [nlm]" % self.cdtype)
+        _check(lib.nusht_stage_legendre_adjoint_static(self._h, gt.data_ptr(), out.data_ptr(), _stream_ptr(stream)))
+        return out
+
     def grid_shape(self):
         return (self.info.n_theta_fine // 2 + 1, self.info.n_phi_fine)
 
@@ -372,6 +388,14 @@ def ring_pairing(theta):
 def launch_count() -> int:
     """Kernels of this library launched so far in this process (nusht_launch_count)."""
     return int(lib.nusht_launch_count())
+
+
+def static_scratch() -> int:
+    """Resolve the static scratch array of nusht_stage_legendre_adjoint_static on the current device (set-up step,
+    outside graph capture) and return its capacity in bytes (nusht_static_scratch)."""
+    v = ctypes.c_int64()
+    _check(lib.nusht_static_scratch(ctypes.byref(v)))
+    return int(v.value)
 
 
 def probe_fp64(kind: str) -> float:
