@@ -52,10 +52,11 @@ def parse():
                     help="BASELINE.json configs[4]: lmax=4095 on 67M points, eps in {1e-4, 1e-6} FP32 and "
                          "{1e-8, 1e-10, 1e-12} FP64; one JSON line per eps (accuracy on an oracle subset + timing)")
     ap.add_argument("--sweep-subset", type=int, default=1500, help="points of the oracle subset of the sweep")
-    ap.add_argument("--ring", default=None, choices=["gl", "equi"],
+    ap.add_argument("--ring", default=None, choices=["gl", "equi", "healpix"],
                     help="ring-grid transforms (SURVEY 8(f) rank 3/4) instead of the nuSHT step: 'gl' = Gauss-Legendre grid "
                          "(lmax+1 rings x 2 lmax+2 pixels, the paper's output grid, PAPER.md:154): step = synthesis + "
-                         "analysis; 'equi' = the 2(lmax+1)^2 equi-angular grid of config 2: step = gradient (Eq. C2) + pointing")
+                         "analysis; 'healpix' = the same on a HEALPix-style ring layout (PAPER.md:218), nside = (lmax+1)/2; "
+                         "'equi' = the 2(lmax+1)^2 equi-angular grid of config 2: step = gradient (Eq. C2) + pointing")
     ap.add_argument("--lmax", type=int, default=4095, help="band limit of the --ring modes")
     return ap.parse_args()
 
@@ -501,6 +502,7 @@ def run_ring(args):
     torch.cuda.set_device(0)
     L = args.lmax
     stream = torch.cuda.current_stream()
+    phi0 = None
     if args.ring == "gl":
         xg, wg = np.polynomial.legendre.leggauss(L + 1)
         theta = np.arccos(xg[::-1])
@@ -508,20 +510,23 @@ def run_ring(args):
         theta[L + 1 - half:] = np.pi - theta[:half][::-1]
         nphi = np.full(L + 1, 2 * L + 2)
         weight = wg[::-1] * (2 * np.pi / (2 * L + 2))
+    elif args.ring == "healpix":            # nside = (lmax + 1) / 2: the caps are 2 (nside - 1) rings of distinct lengths
+        theta, nphi, phi0, weight = inputs.healpix_ring_layout((L + 1) // 2)
     else:
         nr = 2 * (L + 1)
         theta = np.pi * (np.arange(nr) + 0.5) / nr
         nphi = np.full(nr, nr)
         weight = None
-    plan = nusht.RingPlan(L, L, theta, nphi, None, weight)
+    plan = nusht.RingPlan(L, L, theta, nphi, phi0, weight)
     alm = torch.from_numpy(inputs.random_alm(L, L, 7, "inv_l2")).cuda()
     f = torch.empty(plan.npix, dtype=torch.float64, device="cuda")
     out = torch.empty(plan.nlm, dtype=torch.complex128, device="cuda")
-    if args.ring == "gl":
+    if args.ring in ("gl", "healpix"):
         def step():
             plan.synthesis(alm, f, stream)
             plan.analysis(f, out, stream)
-        what = "ring synthesis + analysis on a Gauss-Legendre grid"
+        what = "ring synthesis + analysis on " + ("a Gauss-Legendre grid" if args.ring == "gl" else
+                                                 "a HEALPix-style ring layout, nside = (lmax + 1) / 2")
     else:
         th = torch.from_numpy(np.repeat(theta, nphi)).cuda()
         ph = torch.from_numpy(np.tile(2 * np.pi * np.arange(nphi[0]) / nphi[0], len(theta))).cuda()

@@ -236,7 +236,8 @@ typedef struct nusht_ring_plan_s nusht_ring_plan_t;
 typedef struct {
     int lmax, mmax, dtype, nrings;
     int npairs;          /* ring pairs the Legendre stage works on (nrings/2 for a symmetric grid) */
-    int nruns;           /* runs of consecutive equal-length rings = batched FFT calls per transform */
+    int nruns;           /* batched FFT plans per transform: runs of >= 16 consecutive equal-length rings (one real
+                          * cuFFT plan each) + one chirp-z group per padded power-of-two length for all other rings */
     int64_t npix, nlm, workspace_bytes;
     double plan_ms;
 } nusht_ring_info_t;

@@ -12,8 +12,17 @@
 // Pipeline: the Legendre kernels of legendre.cu in ring-list mode (rings paired north/south where the grid is
 // symmetric, any colatitudes otherwise) between alm and F[m][ring], then per ring the phi transform: the m of a ring
 // are folded onto its n_r Fourier bins (aliasing: rings near the poles have fewer pixels than 2 mmax + 1), followed
-// by one real FFT per ring.  cuFFT does the uniform FFTs (runs of consecutive rings of one length are one batched
-// plan); everything else is our own kernels.
+// by one real FFT per ring.  cuFFT does the uniform FFTs; everything else is our own kernels.  Long runs of
+// consecutive rings of one length (a Gauss-Legendre grid, the equatorial belt of a HEALPix-style layout) are one
+// batched real cuFFT plan each.  Rings in short runs (the polar caps of a HEALPix-style layout: 4 i pixels on ring i,
+// every ring its own length, 2 x 2047 lengths at nside = 2048) go to a POOL instead, transformed by Bluestein's
+// chirp-z algorithm so that a handful of batched power-of-two cuFFT plans serve all of them: with
+// c_j = exp(i pi j^2 / n),  exp(2 pi i j k / n) = c_j c_k conj(c_{j-k}),  hence
+//   f_j = sum_k Z_k exp(2 pi i j k / n) = c_j * [ (Z c) (*) conj(c) ]_j,
+// a linear convolution done as a circular one of length P = 2^p >= 2 n - 1: FFT_P, product with the plan-time
+// spectrum of the chirp, inverse FFT_P.  Pool rings are grouped by P; per direction the pool costs two batched Z2Z
+// per group plus three elementwise kernels, instead of one cuFFT call of an awkward length per ring (measured at
+// nside = 2048: 90 ms per transform with 4095 per-ring calls and 28 s of plan time).
 //
 // Eq. C2 needs no spin-1 recurrence: with c_l^2 = (l^2 - m^2)/(4 l^2 - 1),
 //   sin(theta) dPbar_lm/dtheta = l c_{l+1} Pbar_{l+1,m} - (l + 1) c_l Pbar_{l-1,m},
@@ -21,8 +30,10 @@
 //   a'_{l'm} = (l' - 1) c_{l'} Phi_{l'-1,m} - (l' + 2) c_{l'+1} Phi_{l'+1,m},
 // dPhi/dphi is the scalar synthesis of i m Phi_lm, and both are divided by sin(theta_r) ring by ring.  The ring plan
 // therefore builds its Legendre tables one degree higher than the caller's lmax.
+#include <limits.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -182,6 +193,123 @@ k_grad_coeffs(int L, int M, const T* __restrict__ philm, T* __restrict__ ga, T* 
     gb[2 * (out + lp) + 1] = (T)bim;
 }
 
+// ---- Bluestein pool -------------------------------------------------------------------------------------------
+struct BlueMeta {
+    const int* ring;          // pool slot q -> ring index
+    const int* P;             // padded length of the slot's work row
+    const int64_t* woff;      // offset of the work row (double2 elements)
+    const int64_t* boff;      // offset of the chirp spectrum FFT_P(conj c) of the ring's length
+    const int64_t* coff;      // offset of the chirp table c_j, j = 0 .. n-1
+    const int64_t* pixoff;    // offset of the ring's pixels in the map
+    const int* nphi;          // per ring (not per slot)
+    const int64_t* zoff;      // per ring
+};
+
+__device__ __forceinline__ double2 zmul(double2 a, double2 b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+
+// c_j = exp(i pi j^2 / n), the argument reduced exactly: j^2 mod 2 n in integers
+__global__ void __launch_bounds__(256)
+k_blue_chirp(int n, double2* __restrict__ c) {
+    const int j = blockIdx.x * 256 + threadIdx.x;
+    if (j >= n) return;
+    const long long q = ((long long)j * j) % (2LL * n);
+    double sn, cs;
+    sincospi((double)q / (double)n, &sn, &cs);
+    c[j] = make_double2(cs, sn);
+}
+
+// b~_p = conj(c_p) for p < n, conj(c_{P-p}) for P - p < n, else 0  (the chirp, wrapped for the circular convolution)
+__global__ void __launch_bounds__(256)
+k_blue_kernel_row(int n, int P, const double2* __restrict__ c, double2* __restrict__ row) {
+    const int p = blockIdx.x * 256 + threadIdx.x;
+    if (p >= P) return;
+    double2 v = make_double2(0.0, 0.0);
+    if (p < n) v = c[p];
+    else if (P - p < n) v = c[P - p];
+    v.y = -v.y;
+    row[p] = v;
+}
+
+// synthesis, before the forward FFT: a_k = Z_k c_k (Z: the ring's Hermitian spectrum from its stored half), zero-padded
+template <typename C>
+__global__ void __launch_bounds__(256)
+k_blue_pre_syn(BlueMeta B, const C* __restrict__ z, const double2* __restrict__ chirp, double2* __restrict__ work) {
+    const int q = blockIdx.x, k = blockIdx.y * 256 + threadIdx.x;
+    const int P = B.P[q];
+    if (k >= P) return;
+    const int r = B.ring[q], n = B.nphi[r];
+    double2 a = make_double2(0.0, 0.0);
+    if (k < n) {
+        const bool upper = k > n / 2;
+        const C zz = z[B.zoff[r] + (upper ? n - k : k)];
+        a = zmul(make_double2((double)zz.x, upper ? -(double)zz.y : (double)zz.y), chirp[B.coff[q] + k]);
+    }
+    work[B.woff[q] + k] = a;
+}
+
+// between the two FFTs: times the chirp spectrum (analysis: its conjugate, the spectrum of the conjugate chirp)
+template <bool CONJ>
+__global__ void __launch_bounds__(256)
+k_blue_mul(BlueMeta B, const double2* __restrict__ spec, double2* __restrict__ work) {
+    const int q = blockIdx.x, p = blockIdx.y * 256 + threadIdx.x;
+    if (p >= B.P[q]) return;
+    double2 b = spec[B.boff[q] + p];
+    if (CONJ) b.y = -b.y;
+    const int64_t i = B.woff[q] + p;
+    work[i] = zmul(work[i], b);
+}
+
+// synthesis, after the inverse FFT: f_j = Re(c_j conv_j) / P
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_blue_post_syn(BlueMeta B, const double2* __restrict__ work, const double2* __restrict__ chirp, T* __restrict__ map) {
+    const int q = blockIdx.x, j = blockIdx.y * 256 + threadIdx.x;
+    const int r = B.ring[q], n = B.nphi[r];
+    if (j >= n) return;
+    const double2 w = work[B.woff[q] + j], c = chirp[B.coff[q] + j];
+    map[B.pixoff[q] + j] = (T)((w.x * c.x - w.y * c.y) / (double)B.P[q]);
+}
+
+// analysis, before the forward FFT: a_j = f_j conj(c_j), zero-padded
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_blue_pre_ana(BlueMeta B, const T* __restrict__ map, const double2* __restrict__ chirp, double2* __restrict__ work) {
+    const int q = blockIdx.x, j = blockIdx.y * 256 + threadIdx.x;
+    const int P = B.P[q];
+    if (j >= P) return;
+    const int r = B.ring[q], n = B.nphi[r];
+    double2 a = make_double2(0.0, 0.0);
+    if (j < n) {
+        const double f = (double)map[B.pixoff[q] + j];
+        const double2 c = chirp[B.coff[q] + j];
+        a = make_double2(f * c.x, -f * c.y);
+    }
+    work[B.woff[q] + j] = a;
+}
+
+// analysis, after the inverse FFT: Y_k = conj(c_k) conv_k / P, k = 0 .. n/2
+template <typename C>
+__global__ void __launch_bounds__(256)
+k_blue_post_ana(BlueMeta B, const double2* __restrict__ work, const double2* __restrict__ chirp, C* __restrict__ z) {
+    const int q = blockIdx.x, k = blockIdx.y * 256 + threadIdx.x;
+    const int r = B.ring[q], n = B.nphi[r];
+    if (k > n / 2) return;
+    const double2 w = work[B.woff[q] + k], c = chirp[B.coff[q] + k];
+    const double inv = 1.0 / (double)B.P[q];
+    C out;
+    out.x = (typename RealOf<C>::type)((w.x * c.x + w.y * c.y) * inv);
+    out.y = (typename RealOf<C>::type)((w.y * c.x - w.x * c.y) * inv);
+    z[B.zoff[r] + k] = out;
+}
+
+struct BlueGroup {
+    int P, count, first;      // padded length, rings, first pool slot
+    int64_t woff;             // offset of the group's [count][P] block in the work array
+    cufftHandle z2z;
+};
+
 }  // namespace
 
 struct nusht_ring_plan_s {
@@ -196,8 +324,14 @@ struct nusht_ring_plan_s {
     void* d_fftwork = nullptr;         // one cuFFT work area shared by all plans (executions are stream-ordered)
     void* d_stage = nullptr;           // aligned staging for runs whose pixels start off cuFFT's alignment (odd ring lengths)
     void *d_ga = nullptr, *d_gb = nullptr;   // Eq. C2 coefficients
-    std::vector<RingRun> runs;
+    std::vector<RingRun> runs;         // long runs: batched real cuFFT
     std::map<std::pair<int, int>, std::pair<cufftHandle, cufftHandle>> fft;   // (nphi, batch) -> (C2R, R2C)
+    // Bluestein pool (rings of short runs), slots ordered by group
+    std::vector<BlueGroup> groups;
+    int npool = 0, pool_maxP = 0;
+    int *d_bring = nullptr, *d_bP = nullptr;
+    int64_t *d_bwoff = nullptr, *d_bboff = nullptr, *d_bcoff = nullptr, *d_bpix = nullptr;
+    double2 *d_bwork = nullptr, *d_bspec = nullptr, *d_bchirp = nullptr;
     int64_t workspace_bytes = 0;
     double plan_ms = 0;
 };
@@ -211,6 +345,10 @@ static void ring_release(nusht_ring_plan_s* rp) {
     }
     cudaFree(rp->d_nphi); cudaFree(rp->d_zoff); cudaFree(rp->d_phi0); cudaFree(rp->d_weight); cudaFree(rp->d_isin);
     cudaFree(rp->d_z); cudaFree(rp->d_fftwork); cudaFree(rp->d_ga); cudaFree(rp->d_gb); cudaFree(rp->d_stage);
+    for (auto& g : rp->groups)
+        if (g.z2z) cufftDestroy(g.z2z);
+    cudaFree(rp->d_bring); cudaFree(rp->d_bP); cudaFree(rp->d_bwoff); cudaFree(rp->d_bboff); cudaFree(rp->d_bcoff);
+    cudaFree(rp->d_bpix); cudaFree(rp->d_bwork); cudaFree(rp->d_bspec); cudaFree(rp->d_bchirp);
     delete rp;
 }
 
@@ -255,6 +393,7 @@ static int ring_build(nusht_ring_plan_s* rp, const double* theta, const int64_t*
     std::vector<int> h_n(nr);
     std::vector<int64_t> h_zoff(nr);
     std::vector<double> h_phi0(nr), h_w(nr), h_isin(nr);
+    std::vector<RingRun> all_runs;
     int64_t pix = 0, zo = 0;
     const long double PI_L = 3.14159265358979323846264338327950288L;
     for (int r = 0; r < nr; ++r) {
@@ -266,13 +405,13 @@ static int ring_build(nusht_ring_plan_s* rp, const double* theta, const int64_t*
         const bool pole = !(theta[r] > 0.0) || !((long double)theta[r] < PI_L) || !(s > 0.0L);
         if (pole) rp->has_pole_ring = true;
         h_isin[r] = pole ? 0.0 : (double)(1.0L / s);
-        if (!rp->runs.empty() && rp->runs.back().nphi == h_n[r]) {
-            rp->runs.back().count += 1;
+        if (!all_runs.empty() && all_runs.back().nphi == h_n[r]) {
+            all_runs.back().count += 1;
         } else {
             RingRun run;
             run.first = r; run.count = 1; run.nphi = h_n[r]; run.pixoff = pix; run.zoff = zo; run.c2r = run.r2c = 0;
             run.staged = (pix % 2) != 0;      // cuFFT wants real data aligned like complex data (map base: 16 bytes)
-            rp->runs.push_back(run);
+            all_runs.push_back(run);
         }
         pix += h_n[r];
         zo += h_n[r] / 2 + 1;
@@ -280,6 +419,35 @@ static int ring_build(nusht_ring_plan_s* rp, const double* theta, const int64_t*
     }
     rp->npix = pix;
     rp->nz = zo;
+    // long runs keep a batched real cuFFT plan each; the rings of short runs go to the Bluestein pool (header).
+    // NUSHT_RING_POOL=0 pools nothing, =all pools every ring (tests compare the two routes).
+    struct PoolSlot { int ring, n, P; int64_t pixoff; };
+    std::vector<PoolSlot> slots;
+    {
+        int min_run = 16;
+        if (const char* ev = getenv("NUSHT_RING_POOL")) {
+            if (strcmp(ev, "0") == 0) min_run = 0;
+            else if (strcmp(ev, "all") == 0) min_run = INT_MAX;
+        }
+        for (const auto& run : all_runs) {
+            if (run.count >= min_run) {
+                rp->runs.push_back(run);
+                continue;
+            }
+            for (int i = 0; i < run.count; ++i) {
+                PoolSlot sl;
+                sl.ring = run.first + i;
+                sl.n = run.nphi;
+                sl.pixoff = run.pixoff + (int64_t)i * run.nphi;
+                sl.P = 4;
+                while (sl.P < 2 * sl.n - 1) sl.P *= 2;
+                slots.push_back(sl);
+            }
+        }
+        std::stable_sort(slots.begin(), slots.end(), [](const PoolSlot& a, const PoolSlot& b) {
+            return a.P != b.P ? a.P < b.P : a.n < b.n;
+        });
+    }
     NUSHT_TRY(r_alloc(&rp->d_nphi, sizeof(int) * (size_t)nr, rp));
     NUSHT_TRY(r_alloc(&rp->d_zoff, sizeof(int64_t) * (size_t)nr, rp));
     NUSHT_TRY(r_alloc(&rp->d_phi0, sizeof(double) * (size_t)nr, rp));
@@ -321,7 +489,84 @@ static int ring_build(nusht_ring_plan_s* rp, const double* theta, const int64_t*
         run.c2r = it->second.first;
         run.r2c = it->second.second;
     }
+    // Bluestein pool: slots in group order, one batched Z2Z plan per padded length
+    rp->npool = (int)slots.size();
+    std::vector<int> h_bring, h_bP;
+    std::vector<int64_t> h_bwoff, h_bboff, h_bcoff, h_bpix;
+    struct Distinct { int n, P; int64_t coff, boff; };
+    std::vector<Distinct> distinct;           // distinct ring lengths in slot order (grouped by P)
+    int64_t wtot = 0, ctot = 0, btot = 0;
+    for (int q = 0; q < rp->npool; ++q) {
+        const PoolSlot& sl = slots[q];
+        if (rp->groups.empty() || rp->groups.back().P != sl.P) {
+            BlueGroup g;
+            g.P = sl.P; g.count = 0; g.first = q; g.woff = wtot; g.z2z = 0;
+            rp->groups.push_back(g);
+        }
+        rp->groups.back().count += 1;
+        if (distinct.empty() || distinct.back().n != sl.n) {
+            distinct.push_back({sl.n, sl.P, ctot, btot});
+            ctot += sl.n;
+            btot += sl.P;
+        }
+        h_bring.push_back(sl.ring);
+        h_bP.push_back(sl.P);
+        h_bwoff.push_back(wtot);
+        h_bboff.push_back(distinct.back().boff);
+        h_bcoff.push_back(distinct.back().coff);
+        h_bpix.push_back(sl.pixoff);
+        wtot += sl.P;
+        if (sl.P > rp->pool_maxP) rp->pool_maxP = sl.P;
+    }
+    for (auto& g : rp->groups) {
+        size_t ws = 0;
+        int n[1] = {g.P};
+        NUSHT_CUFFT_TRY(cufftCreate(&g.z2z));
+        NUSHT_CUFFT_TRY(cufftSetAutoAllocation(g.z2z, 0));
+        NUSHT_CUFFT_TRY(cufftMakePlanMany(g.z2z, 1, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_Z2Z, g.count, &ws));
+        if (ws > wmax) wmax = ws;
+    }
     NUSHT_TRY(r_alloc(&rp->d_fftwork, wmax, rp));
+    if (rp->npool) {
+        const size_t nq = (size_t)rp->npool;
+        NUSHT_TRY(r_alloc(&rp->d_bring, sizeof(int) * nq, rp));
+        NUSHT_TRY(r_alloc(&rp->d_bP, sizeof(int) * nq, rp));
+        NUSHT_TRY(r_alloc(&rp->d_bwoff, sizeof(int64_t) * nq, rp));
+        NUSHT_TRY(r_alloc(&rp->d_bboff, sizeof(int64_t) * nq, rp));
+        NUSHT_TRY(r_alloc(&rp->d_bcoff, sizeof(int64_t) * nq, rp));
+        NUSHT_TRY(r_alloc(&rp->d_bpix, sizeof(int64_t) * nq, rp));
+        NUSHT_CUDA_TRY(cudaMemcpy(rp->d_bring, h_bring.data(), sizeof(int) * nq, cudaMemcpyHostToDevice));
+        NUSHT_CUDA_TRY(cudaMemcpy(rp->d_bP, h_bP.data(), sizeof(int) * nq, cudaMemcpyHostToDevice));
+        NUSHT_CUDA_TRY(cudaMemcpy(rp->d_bwoff, h_bwoff.data(), sizeof(int64_t) * nq, cudaMemcpyHostToDevice));
+        NUSHT_CUDA_TRY(cudaMemcpy(rp->d_bboff, h_bboff.data(), sizeof(int64_t) * nq, cudaMemcpyHostToDevice));
+        NUSHT_CUDA_TRY(cudaMemcpy(rp->d_bcoff, h_bcoff.data(), sizeof(int64_t) * nq, cudaMemcpyHostToDevice));
+        NUSHT_CUDA_TRY(cudaMemcpy(rp->d_bpix, h_bpix.data(), sizeof(int64_t) * nq, cudaMemcpyHostToDevice));
+        NUSHT_TRY(r_alloc(&rp->d_bwork, sizeof(double2) * (size_t)wtot, rp));
+        NUSHT_TRY(r_alloc(&rp->d_bspec, sizeof(double2) * (size_t)btot, rp));
+        NUSHT_TRY(r_alloc(&rp->d_bchirp, sizeof(double2) * (size_t)ctot, rp));
+        // chirp tables, then their spectra: the distinct lengths of a group fill the first rows of the group's work
+        // block, the group's own plan transforms the block, the rows are kept
+        for (const auto& d : distinct) {
+            k_blue_chirp<<<(d.n + 255) / 256, 256>>>(d.n, rp->d_bchirp + d.coff);
+            NUSHT_CUDA_TRY(nusht_launched());
+        }
+        size_t di = 0;
+        for (auto& g : rp->groups) {
+            NUSHT_CUFFT_TRY(cufftSetWorkArea(g.z2z, rp->d_fftwork));
+            double2* block = rp->d_bwork + g.woff;
+            NUSHT_CUDA_TRY(cudaMemset(block, 0, sizeof(double2) * (size_t)g.count * (size_t)g.P));
+            const size_t d0 = di;
+            for (; di < distinct.size() && distinct[di].P == g.P; ++di) {
+                k_blue_kernel_row<<<(g.P + 255) / 256, 256>>>(distinct[di].n, g.P, rp->d_bchirp + distinct[di].coff,
+                                                               block + (di - d0) * (size_t)g.P);
+                NUSHT_CUDA_TRY(nusht_launched());
+            }
+            NUSHT_CUFFT_TRY(cufftSetStream(g.z2z, 0));
+            NUSHT_CUFFT_TRY(cufftExecZ2Z(g.z2z, (cufftDoubleComplex*)block, (cufftDoubleComplex*)block, CUFFT_FORWARD));
+            NUSHT_CUDA_TRY(cudaMemcpy(rp->d_bspec + distinct[d0].boff, block, sizeof(double2) * (di - d0) * (size_t)g.P,
+                                      cudaMemcpyDeviceToDevice));
+        }
+    }
     {
         size_t smax = 0;
         for (const auto& run : rp->runs)
@@ -381,11 +626,37 @@ extern "C" int nusht_ring_info(const nusht_ring_plan_t* rp, nusht_ring_info_t* i
     info->dtype = rp->dtype;
     info->nrings = rp->nrings;
     info->npairs = rp->core.lg.npairs;
-    info->nruns = (int)rp->runs.size();
+    info->nruns = (int)(rp->runs.size() + rp->groups.size());     // batched FFT plans: long runs + pool groups
     info->npix = rp->npix;
     info->nlm = rp->core.nlm;
     info->workspace_bytes = rp->workspace_bytes;
     info->plan_ms = rp->plan_ms;
+    return NUSHT_OK;
+}
+
+static BlueMeta blue_meta(const nusht_ring_plan_s* rp) {
+    BlueMeta B;
+    B.ring = rp->d_bring; B.P = rp->d_bP; B.woff = rp->d_bwoff; B.boff = rp->d_bboff; B.coff = rp->d_bcoff;
+    B.pixoff = rp->d_bpix; B.nphi = rp->d_nphi; B.zoff = rp->d_zoff;
+    return B;
+}
+
+// the two batched FFTs of the pool with the chirp-spectrum product between them (work array in place)
+static int blue_convolve(nusht_ring_plan_s* rp, bool analysis, cudaStream_t s) {
+    const BlueMeta B = blue_meta(rp);
+    const dim3 grid(rp->npool, (rp->pool_maxP + 255) / 256);
+    for (auto& g : rp->groups) {
+        cufftDoubleComplex* block = (cufftDoubleComplex*)(rp->d_bwork + g.woff);
+        NUSHT_CUFFT_TRY(cufftSetStream(g.z2z, s));
+        NUSHT_CUFFT_TRY(cufftExecZ2Z(g.z2z, block, block, CUFFT_FORWARD));
+    }
+    if (analysis) k_blue_mul<true><<<grid, 256, 0, s>>>(B, rp->d_bspec, rp->d_bwork);
+    else k_blue_mul<false><<<grid, 256, 0, s>>>(B, rp->d_bspec, rp->d_bwork);
+    NUSHT_CUDA_TRY(nusht_launched());
+    for (auto& g : rp->groups) {
+        cufftDoubleComplex* block = (cufftDoubleComplex*)(rp->d_bwork + g.woff);
+        NUSHT_CUFFT_TRY(cufftExecZ2Z(g.z2z, block, block, CUFFT_INVERSE));
+    }
     return NUSHT_OK;
 }
 
@@ -421,6 +692,17 @@ static int ring_phi_synthesis(nusht_ring_plan_s* rp, const double* scale, void* 
             NUSHT_CUDA_TRY(cudaMemcpyAsync((char*)map + (size_t)run.pixoff * esz, rp->d_stage,
                                            (size_t)run.count * run.nphi * esz, cudaMemcpyDeviceToDevice, s));
     }
+    if (rp->npool) {
+        const BlueMeta B = blue_meta(rp);
+        const dim3 bgrid(rp->npool, (rp->pool_maxP + 255) / 256);
+        if (f64) k_blue_pre_syn<double2><<<bgrid, 256, 0, s>>>(B, (const double2*)rp->d_z, rp->d_bchirp, rp->d_bwork);
+        else k_blue_pre_syn<float2><<<bgrid, 256, 0, s>>>(B, (const float2*)rp->d_z, rp->d_bchirp, rp->d_bwork);
+        NUSHT_CUDA_TRY(nusht_launched());
+        NUSHT_TRY(blue_convolve(rp, false, s));
+        if (f64) k_blue_post_syn<double><<<bgrid, 256, 0, s>>>(B, rp->d_bwork, rp->d_bchirp, (double*)map);
+        else k_blue_post_syn<float><<<bgrid, 256, 0, s>>>(B, rp->d_bwork, rp->d_bchirp, (float*)map);
+        NUSHT_CUDA_TRY(nusht_launched());
+    }
     return NUSHT_OK;
 }
 
@@ -439,6 +721,17 @@ static int ring_phi_analysis(nusht_ring_plan_s* rp, const double* scale, const v
             NUSHT_CUFFT_TRY(cufftExecD2Z(run.r2c, (double*)src, (cufftDoubleComplex*)rp->d_z + run.zoff));
         else
             NUSHT_CUFFT_TRY(cufftExecR2C(run.r2c, (float*)src, (cufftComplex*)rp->d_z + run.zoff));
+    }
+    if (rp->npool) {
+        const BlueMeta B = blue_meta(rp);
+        const dim3 bgrid(rp->npool, (rp->pool_maxP + 255) / 256);
+        if (f64) k_blue_pre_ana<double><<<bgrid, 256, 0, s>>>(B, (const double*)map, rp->d_bchirp, rp->d_bwork);
+        else k_blue_pre_ana<float><<<bgrid, 256, 0, s>>>(B, (const float*)map, rp->d_bchirp, rp->d_bwork);
+        NUSHT_CUDA_TRY(nusht_launched());
+        NUSHT_TRY(blue_convolve(rp, true, s));
+        if (f64) k_blue_post_ana<double2><<<bgrid, 256, 0, s>>>(B, rp->d_bwork, rp->d_bchirp, (double2*)rp->d_z);
+        else k_blue_post_ana<float2><<<bgrid, 256, 0, s>>>(B, rp->d_bwork, rp->d_bchirp, (float2*)rp->d_z);
+        NUSHT_CUDA_TRY(nusht_launched());
     }
     const RingMeta R = ring_meta(rp, scale);
     const dim3 grid((rp->nrings + 31) / 32, (rp->mmax + 32) / 32);

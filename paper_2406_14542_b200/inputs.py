@@ -111,3 +111,30 @@ def make_config(i: int, npts: int | None = None):
     alm = random_alm(cfg["lmax"], cfg["mmax"], cfg["seed"], cfg["spectrum"])
     x = random_map(cfg["npts"], cfg["seed"])
     return cfg, theta, phi, alm, x
+
+
+def healpix_ring_layout(nside: int):
+    """Ring layout of the HEALPix pixelisation (Gorski et al. 2005; "standard pixelization schemes such as
+    HEALPix"), restated from its definition: 4 nside - 1 rings; polar caps with 4 i pixels on ring i at
+    cos(theta) = 1 - i^2 / (3 nside^2), first pixel at pi / (4 i); equatorial belt with 4 nside pixels at
+    cos(theta) = 4/3 - 2 i / (3 nside), shifted by half a pixel on every other ring.  Returns (theta, nphi, phi0,
+    weight) with the equal-area weight 4 pi / npix.  Geometry only: no transform arithmetic."""
+    theta, nphi, phi0 = [], [], []
+    for i in range(1, 4 * nside):
+        if i < nside:
+            z, n, p0 = 1 - i * i / (3.0 * nside * nside), 4 * i, np.pi / (4 * i)
+        elif i <= 3 * nside:
+            z, n = 4.0 / 3 - 2.0 * i / (3 * nside), 4 * nside
+            p0 = ((i - nside + 1) % 2) * np.pi / (4 * nside)
+        else:
+            k = 4 * nside - i
+            z, n, p0 = -(1 - k * k / (3.0 * nside * nside)), 4 * k, np.pi / (4 * k)
+        theta.append(np.arccos(z))
+        nphi.append(n)
+        phi0.append(p0)
+    theta = np.array(theta)
+    half = len(theta) // 2                      # exact mirror symmetry of the colatitudes
+    theta[len(theta) - half:] = np.pi - theta[:half][::-1]
+    nphi = np.array(nphi, dtype=np.int64)
+    return theta, nphi, np.array(phi0), np.full(len(theta), 4 * np.pi / float(nphi.sum()))
+

@@ -135,6 +135,63 @@ def test_gauss_legendre_roundtrip_lmax_1023(nusht, oracle):
     plan.destroy()
 
 
+# ---- the Bluestein pool (rings of short runs) against the per-run cuFFT route and against the oracle --------------
+@pytest.mark.parametrize("grid", ["healpix", "irregular", "gl"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_ring_pool_matches_per_run_fft(nusht, monkeypatch, grid, dtype):
+    """NUSHT_RING_POOL=0: every run of equal-length rings is a real cuFFT plan; =all: every ring goes through the
+    chirp-z pool; default: short runs only.  Same transform three ways."""
+    L = 95
+    theta, nphi, phi0, weight = {"gl": lambda: gauss_legendre_grid(L), "healpix": lambda: healpix_like_grid(32),
+                                 "irregular": lambda: irregular_grid(510)}[grid]()
+    cd = np.complex128 if dtype == "f64" else np.complex64
+    rd = np.float64 if dtype == "f64" else np.float32
+    alm = inputs.random_alm(L, L, 511).astype(cd)
+    x = inputs.random_map(int(np.sum(nphi)), 512).astype(rd)
+    res = {}
+    for mode in ["0", "all", None]:
+        if mode is None:
+            monkeypatch.delenv("NUSHT_RING_POOL", raising=False)
+        else:
+            monkeypatch.setenv("NUSHT_RING_POOL", mode)
+        plan = nusht.RingPlan(L, L, theta, nphi, phi0, weight, dtype=dtype)
+        res[mode] = (plan.synthesis(cu(alm)).cpu().numpy().astype(np.float64),
+                     plan.analysis(cu(x)).cpu().numpy().astype(np.complex128), plan.info.nruns)
+        plan.destroy()
+    bar = 2e-13 if dtype == "f64" else 2e-6
+    for mode in ["all", None]:
+        assert rel(res[mode][0], res["0"][0]) <= bar, mode
+        assert rel(res[mode][1], res["0"][1]) <= bar, mode
+    if grid == "healpix":
+        assert res["0"][2] == 2 * 31 + 1            # one plan per cap ring + the belt
+        assert res[None][2] <= 8                    # the belt + one pool group per padded length 8 .. 256
+
+
+def test_healpix_nside_256_sampled(nusht, oracle):
+    """2 x 255 cap rings of distinct lengths (4 .. 1020, most of them awkward FFT sizes) through the pool, at
+    lmax = 2 nside - 1: sampled pixels against Eq. 3, and <S a, x> = <a, S^T x> over the whole map."""
+    nside, L = 256, 511
+    theta, nphi, phi0, weight = healpix_like_grid(nside)
+    plan = nusht.RingPlan(L, L, theta, nphi, phi0, None)
+    assert plan.info.nruns <= 12
+    alm = inputs.random_alm(L, L, 513)
+    f = plan.synthesis(cu(alm)).cpu().numpy()
+    th, ph = pixel_centres(theta, nphi, phi0)
+    rng = np.random.default_rng(514)
+    idx = np.unique(np.concatenate([rng.choice(len(th), 1500, replace=False), np.arange(0, 40),
+                                    len(th) - 1 - np.arange(0, 40), rng.choice(4 * nside * nside // 2, 300)]))
+    f_ref = oracle.synthesis(L, L, th[idx], ph[idx], alm, "ld")
+    assert rel(f[idx], f_ref) <= 5e-12
+    assert np.max(np.abs(f[idx] - f_ref)) <= 5e-11 * np.sqrt(np.mean(f_ref ** 2))
+    x = inputs.random_map(len(th), 515)
+    c = plan.analysis(cu(x)).cpu().numpy()
+    w = np.where(np.arange(plan.nlm) <= L, 1.0, 2.0)                     # m = 0 block first: weights of the G3 product
+    lhs = np.sum(np.asarray(f, dtype=np.longdouble) * x)
+    rhs = np.sum(np.asarray(w * (alm.real * c.real + alm.imag * c.imag), dtype=np.longdouble))
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(f) * np.linalg.norm(x)
+    plan.destroy()
+
+
 def test_ring_fp32_and_edge_cases(nusht, oracle):
     L = 63
     theta, nphi, phi0, weight = gauss_legendre_grid(L)
