@@ -141,16 +141,19 @@ NUSHT_API int nusht_destroy(nusht_plan_t* plan);
 /* Same transforms with HOST buffers (pinned for overlap; pageable works but serialises): the call
  * uploads the input on a plan-owned copy stream, runs the transform on `stream`, downloads the result on
  * a second plan-owned copy stream, and returns without synchronising.  Uploads, kernels and downloads of
- * consecutive calls overlap (each direction has its own device staging buffers, allocated on first use).
- * The outputs are valid after nusht_host_sync(plan) (or a device-wide synchronisation); synchronising
- * `stream` alone is NOT enough.  The host buffers must stay untouched until then. */
+ * consecutive calls overlap: each direction has its own device staging buffers (allocated on first use), two sets
+ * used in turn, so a call never waits for the copies of the call before it and a loop of host-buffer calls keeps the
+ * kernels back to back (PCIe permitting).  The outputs are valid after nusht_host_sync(plan) (or a device-wide
+ * synchronisation); synchronising `stream` alone is NOT enough.  The host buffers of a call must stay untouched
+ * until then: calls in flight together need host buffers of their own. */
 NUSHT_API int nusht_synthesis_host(nusht_plan_t* plan, const void* alm_host, void* map_host, void* stream);
 NUSHT_API int nusht_adjoint_host(nusht_plan_t* plan, const void* map_host, void* alm_host, void* stream);
 /* Block the calling thread until every host-buffer transform issued so far on this plan has delivered
  * its output. */
 NUSHT_API int nusht_host_sync(nusht_plan_t* plan);
-/* Allocate the device staging buffers and copy streams of the host-buffer calls now (2 x alm + 2 x map of device
- * memory), so that the first nusht_*_host call allocates nothing either.  Idempotent. */
+/* Allocate the device staging buffers and copy streams of the host-buffer calls now (4 x alm + 4 x map of device
+ * memory: input and output of each direction, twice), so that the first nusht_*_host call allocates nothing either.
+ * Idempotent. */
 NUSHT_API int nusht_host_reserve(nusht_plan_t* plan);
 
 /* Stage entry points (tests and per-stage measurement).

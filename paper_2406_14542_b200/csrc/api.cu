@@ -74,13 +74,17 @@ static void plan_release(nusht_plan_s* p) {
     legendre_free(p);
     fourier_free(p);
     nufft_free(p);
-    cudaFree(p->d_in_alm); cudaFree(p->d_out_alm); cudaFree(p->d_in_map); cudaFree(p->d_out_map);
+    for (int b = 0; b < 2; ++b) {
+        cudaFree(p->d_in_alm[b]); cudaFree(p->d_out_alm[b]); cudaFree(p->d_in_map[b]); cudaFree(p->d_out_map[b]);
+    }
     if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
     if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
     for (int k = 0; k < 2; ++k) {
-        if (p->ev_in[k]) cudaEventDestroy(p->ev_in[k]);
-        if (p->ev_cdone[k]) cudaEventDestroy(p->ev_cdone[k]);
-        if (p->ev_out[k]) cudaEventDestroy(p->ev_out[k]);
+        for (int b = 0; b < 2; ++b) {
+            if (p->ev_in[k][b]) cudaEventDestroy(p->ev_in[k][b]);
+            if (p->ev_cdone[k][b]) cudaEventDestroy(p->ev_cdone[k][b]);
+            if (p->ev_out[k][b]) cudaEventDestroy(p->ev_out[k][b]);
+        }
     }
     for (int k = 0; k < 2; ++k)
         for (int i = 0; i <= NUSHT_NUM_STAGES; ++i)
@@ -279,22 +283,27 @@ extern "C" int nusht_adjoint(nusht_plan_t* p, const void* map, void* alm, void* 
 // Host-buffer transforms.  Copies run on two plan-owned streams (host->device, device->host) and are
 // ordered against the compute on `stream` with events, so that with pinned host memory the upload of
 // the next input and the download of the previous result overlap the kernels of the current call
-// (PCIe is full duplex).  Each direction has its own input and output staging buffer.
+// (PCIe is full duplex).  Each direction has its own input and output staging buffers, two sets of them used in
+// turn: a call waits for the call before the previous one of its direction to have released its set, never for the
+// previous one, so a loop of host-buffer calls without a nusht_host_sync in between runs the kernels back to back.
 static int host_setup(nusht_plan_s* p) {
     if (p->s_h2d) return NUSHT_OK;
     const size_t abytes = (size_t)p->nlm * 2 * real_size(p), mbytes = (size_t)p->npts * real_size(p);
     NUSHT_CUDA_TRY(cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
     NUSHT_CUDA_TRY(cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
-    for (int k = 0; k < 2; ++k) {
-        NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_in[k], cudaEventDisableTiming));
-        NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_cdone[k], cudaEventDisableTiming));
-        NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_out[k], cudaEventDisableTiming));
+    for (int k = 0; k < 2; ++k)
+        for (int b = 0; b < 2; ++b) {
+            NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_in[k][b], cudaEventDisableTiming));
+            NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_cdone[k][b], cudaEventDisableTiming));
+            NUSHT_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_out[k][b], cudaEventDisableTiming));
+        }
+    for (int b = 0; b < 2; ++b) {
+        NUSHT_CUDA_TRY(cudaMalloc(&p->d_in_alm[b], abytes ? abytes : 16));
+        NUSHT_CUDA_TRY(cudaMalloc(&p->d_out_alm[b], abytes ? abytes : 16));
+        NUSHT_CUDA_TRY(cudaMalloc(&p->d_in_map[b], mbytes ? mbytes : 16));
+        NUSHT_CUDA_TRY(cudaMalloc(&p->d_out_map[b], mbytes ? mbytes : 16));
     }
-    NUSHT_CUDA_TRY(cudaMalloc(&p->d_in_alm, abytes ? abytes : 16));
-    NUSHT_CUDA_TRY(cudaMalloc(&p->d_out_alm, abytes ? abytes : 16));
-    NUSHT_CUDA_TRY(cudaMalloc(&p->d_in_map, mbytes ? mbytes : 16));
-    NUSHT_CUDA_TRY(cudaMalloc(&p->d_out_map, mbytes ? mbytes : 16));
-    p->workspace_bytes += (int64_t)(2 * abytes + 2 * mbytes);
+    p->workspace_bytes += (int64_t)(4 * abytes + 4 * mbytes);
     return NUSHT_OK;
 }
 
@@ -308,19 +317,20 @@ extern "C" int nusht_synthesis_host(nusht_plan_t* p, const void* alm_host, void*
     cudaStream_t s = (cudaStream_t)stream;
     const size_t abytes = (size_t)p->nlm * 2 * real_size(p), mbytes = (size_t)p->npts * real_size(p);
     NUSHT_TRY(host_setup(p));
-    // upload: the input staging buffer is free once the previous synthesis has consumed it
-    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_h2d, p->ev_cdone[0], 0));
-    NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_in_alm, alm_host, abytes, cudaMemcpyHostToDevice, p->s_h2d));
-    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_in[0], p->s_h2d));
-    // compute: needs the input, and the output staging buffer back from the previous download
-    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_in[0], 0));
-    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_out[0], 0));
-    NUSHT_TRY(nusht_synthesis(p, p->d_in_alm, p->d_out_map, stream));
-    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_cdone[0], s));
+    const int b = (int)(p->host_seq[0]++ & 1u);
+    // upload: this set's input buffer is free once the synthesis that last used it (two calls ago) has consumed it
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_h2d, p->ev_cdone[0][b], 0));
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_in_alm[b], alm_host, abytes, cudaMemcpyHostToDevice, p->s_h2d));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_in[0][b], p->s_h2d));
+    // compute: needs the input, and this set's output buffer back from its previous download
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_in[0][b], 0));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_out[0][b], 0));
+    NUSHT_TRY(nusht_synthesis(p, p->d_in_alm[b], p->d_out_map[b], stream));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_cdone[0][b], s));
     // download
-    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_d2h, p->ev_cdone[0], 0));
-    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(map_host, p->d_out_map, mbytes, cudaMemcpyDeviceToHost, p->s_d2h));
-    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_out[0], p->s_d2h));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_d2h, p->ev_cdone[0][b], 0));
+    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(map_host, p->d_out_map[b], mbytes, cudaMemcpyDeviceToHost, p->s_d2h));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_out[0][b], p->s_d2h));
     return NUSHT_OK;
 }
 
@@ -329,16 +339,17 @@ extern "C" int nusht_adjoint_host(nusht_plan_t* p, const void* map_host, void* a
     cudaStream_t s = (cudaStream_t)stream;
     const size_t abytes = (size_t)p->nlm * 2 * real_size(p), mbytes = (size_t)p->npts * real_size(p);
     NUSHT_TRY(host_setup(p));
-    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_h2d, p->ev_cdone[1], 0));
-    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_in_map, map_host, mbytes, cudaMemcpyHostToDevice, p->s_h2d));
-    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_in[1], p->s_h2d));
-    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_in[1], 0));
-    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_out[1], 0));
-    NUSHT_TRY(nusht_adjoint(p, p->d_in_map, p->d_out_alm, stream));
-    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_cdone[1], s));
-    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_d2h, p->ev_cdone[1], 0));
-    NUSHT_CUDA_TRY(cudaMemcpyAsync(alm_host, p->d_out_alm, abytes, cudaMemcpyDeviceToHost, p->s_d2h));
-    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_out[1], p->s_d2h));
+    const int b = (int)(p->host_seq[1]++ & 1u);
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_h2d, p->ev_cdone[1][b], 0));
+    if (mbytes) NUSHT_CUDA_TRY(cudaMemcpyAsync(p->d_in_map[b], map_host, mbytes, cudaMemcpyHostToDevice, p->s_h2d));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_in[1][b], p->s_h2d));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_in[1][b], 0));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(s, p->ev_out[1][b], 0));
+    NUSHT_TRY(nusht_adjoint(p, p->d_in_map[b], p->d_out_alm[b], stream));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_cdone[1][b], s));
+    NUSHT_CUDA_TRY(cudaStreamWaitEvent(p->s_d2h, p->ev_cdone[1][b], 0));
+    NUSHT_CUDA_TRY(cudaMemcpyAsync(alm_host, p->d_out_alm[b], abytes, cudaMemcpyDeviceToHost, p->s_d2h));
+    NUSHT_CUDA_TRY(cudaEventRecord(p->ev_out[1][b], p->s_d2h));
     return NUSHT_OK;
 }
 

@@ -144,9 +144,12 @@ struct nusht_plan_s {
     void* d_stage = nullptr;        // [npts] results in slot order (dtype)
     void* kernel_host = nullptr;    // nufft.cu: host model of the kernel polynomial
     // --- host-buffer staging (allocated on first use of *_host) ---
-    void *d_in_alm = nullptr, *d_out_alm = nullptr, *d_in_map = nullptr, *d_out_map = nullptr;
+    // every staging buffer twice: call k of a direction uses set k & 1, so that the upload of the next call and the
+    // download of the previous one overlap the kernels of the current one without waiting for each other's buffers
+    void *d_in_alm[2] = {}, *d_out_alm[2] = {}, *d_in_map[2] = {}, *d_out_map[2] = {};
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
-    cudaEvent_t ev_in[2] = {}, ev_cdone[2] = {}, ev_out[2] = {};   // [0] synthesis, [1] adjoint
+    cudaEvent_t ev_in[2][2] = {}, ev_cdone[2][2] = {}, ev_out[2][2] = {};   // [0] synthesis, [1] adjoint; [set]
+    unsigned host_seq[2] = {0, 0};                                          // host-buffer calls so far, per direction
     // --- stage timing ---
     int timing = 0;
     cudaEvent_t ev[2][NUSHT_NUM_STAGES + 1] = {};

@@ -268,6 +268,30 @@ def test_host_buffer_calls_match_device_calls(nusht):
     plan.destroy()
 
 
+def test_host_buffer_pipeline_with_distinct_inputs(nusht):
+    """Six host-buffer steps in flight without a synchronisation, every step with inputs and host buffers of its own:
+    the two sets of staging buffers are reused three times each, and every result must be that of its own input."""
+    L, npts, nstep = 127, 30000, 6
+    theta, phi = inputs.uniform_sphere_points(npts, 71)
+    plan = nusht.Plan(L, L, cu(theta), cu(phi), 1e-9)
+    alms = [inputs.random_alm(L, L, 720 + k) for k in range(nstep)]
+    xs = [inputs.random_map(npts, 740 + k) for k in range(nstep)]
+    f_ref = [plan.synthesis(cu(a)).cpu() for a in alms]
+    c_ref = [plan.adjoint(cu(x)).cpu() for x in xs]
+    h_a = [torch.from_numpy(a).pin_memory() for a in alms]
+    h_x = [torch.from_numpy(x).pin_memory() for x in xs]
+    h_f = [torch.full((npts,), float("nan"), dtype=torch.float64).pin_memory() for _ in range(nstep)]
+    h_c = [torch.full((plan.nlm,), float("nan"), dtype=torch.complex128).pin_memory() for _ in range(nstep)]
+    for k in range(nstep):
+        plan.synthesis_host(h_a[k], h_f[k])
+        plan.adjoint_host(h_x[k], h_c[k])
+    plan.host_sync()
+    for k in range(nstep):
+        assert torch.equal(h_f[k], f_ref[k]), k
+        assert torch.allclose(h_c[k], c_ref[k], rtol=0, atol=1e-12 * float(c_ref[k].abs().max())), k
+    plan.destroy()
+
+
 # ---- FP32 path (BASELINE.json configs[4]: eps in {1e-4, 1e-6} on the FP32 path) -----------------
 @pytest.mark.parametrize("eps", [1e-2, 1e-4, 1e-5, 1e-6])
 @pytest.mark.parametrize("L,M,npts", [(63, 63, 4000), (200, 150, 6000)])
