@@ -106,6 +106,7 @@ typedef struct {
     int64_t legendre_fma_synthesis; /* FP64 FMAs ONE launch of the Legendre synthesis kernel executes: the (l, m, ring */
     int64_t legendre_fma_adjoint;   /* pair) steps left after the plan-time fast-forward x 3 (measurement: the roofline's
                                        executed fraction); the adjoint's cross-lane adds are not counted */
+    double set_points_ms; /* wall time of the last nusht_set_points (0: never called) */
 } nusht_info_t;
 
 /* Build a plan: choose grid sizes / kernel width from (lmax, mmax, eps), build recurrence and
@@ -127,6 +128,18 @@ typedef struct {
 } nusht_opts_t;
 NUSHT_API int nusht_plan_ex(nusht_plan_t** out, int lmax, int mmax, int64_t npts, const double* theta,
                             const double* phi, double eps, int dtype, const nusht_opts_t* opts);
+
+/* Replace the plan's point set, keeping everything that depends on (lmax, mmax, eps, dtype, sigma) only: recurrence
+ * and deconvolution tables, FFT plans, the fine grid.  Only the plan-time point sort (a6) runs again; the paper makes
+ * the same split ("The plans allow for repeated and fast transforms, without reinitialization") and its
+ * lensing use case needs it, one point set per deflection field (Appendix C).  theta, phi as in nusht_plan: DEVICE
+ * FP64 arrays of the NEW length npts (0 <= npts < 2^31), read during the call only.  The call synchronises the device
+ * (no transform of this plan may be in flight on the old points); with an unchanged npts the point tables are
+ * overwritten in place, otherwise the old tables and the host-buffer staging maps are freed (the latter re-created on
+ * the next nusht_*_host call or nusht_host_reserve) and new ones allocated; the sort's scratch (40 B per point) is
+ * allocated and freed inside the call either way.  The plan's device must be current.  NaN/Inf coordinates or theta outside [0, pi]: NUSHT_ERR_BAD_POINTS, and the plan is
+ * left valid WITHOUT points (npts = 0).  nusht_plan_info reports the new npts, workspace and set_points_ms. */
+NUSHT_API int nusht_set_points(nusht_plan_t* plan, int64_t npts, const double* theta, const double* phi);
 
 /* Synthesis, Eq. 3 / Eq. 5: alm (DEVICE, nlm complex) -> map (DEVICE, npts real).  npts == 0: no-op. */
 NUSHT_API int nusht_synthesis(nusht_plan_t* plan, const void* alm, void* map, void* stream);

@@ -69,23 +69,35 @@ extern "C" const char* nusht_strerror(int code) {
     return "unknown status";
 }
 
+// the staging buffers, streams and events of the host-buffer calls (sized by npts: nusht_set_points drops them too)
+static void host_release(nusht_plan_s* p) {
+    if (p->s_h2d) {
+        const int64_t esz = p->dtype == NUSHT_F64 ? 8 : 4;
+        p->workspace_bytes -= 4 * (p->nlm * 2 * esz) + 4 * (p->host_npts * esz);
+    }
+    for (int b = 0; b < 2; ++b) {
+        cudaFree(p->d_in_alm[b]); cudaFree(p->d_out_alm[b]); cudaFree(p->d_in_map[b]); cudaFree(p->d_out_map[b]);
+        p->d_in_alm[b] = p->d_out_alm[b] = p->d_in_map[b] = p->d_out_map[b] = nullptr;
+    }
+    if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
+    if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
+    p->s_h2d = p->s_d2h = nullptr;
+    for (int k = 0; k < 2; ++k)
+        for (int b = 0; b < 2; ++b) {
+            if (p->ev_in[k][b]) cudaEventDestroy(p->ev_in[k][b]);
+            if (p->ev_cdone[k][b]) cudaEventDestroy(p->ev_cdone[k][b]);
+            if (p->ev_out[k][b]) cudaEventDestroy(p->ev_out[k][b]);
+            p->ev_in[k][b] = p->ev_cdone[k][b] = p->ev_out[k][b] = nullptr;
+        }
+    p->host_seq[0] = p->host_seq[1] = 0;
+}
+
 static void plan_release(nusht_plan_s* p) {
     if (!p) return;
     legendre_free(p);
     fourier_free(p);
     nufft_free(p);
-    for (int b = 0; b < 2; ++b) {
-        cudaFree(p->d_in_alm[b]); cudaFree(p->d_out_alm[b]); cudaFree(p->d_in_map[b]); cudaFree(p->d_out_map[b]);
-    }
-    if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
-    if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
-    for (int k = 0; k < 2; ++k) {
-        for (int b = 0; b < 2; ++b) {
-            if (p->ev_in[k][b]) cudaEventDestroy(p->ev_in[k][b]);
-            if (p->ev_cdone[k][b]) cudaEventDestroy(p->ev_cdone[k][b]);
-            if (p->ev_out[k][b]) cudaEventDestroy(p->ev_out[k][b]);
-        }
-    }
+    host_release(p);
     for (int k = 0; k < 2; ++k)
         for (int i = 0; i <= NUSHT_NUM_STAGES; ++i)
             if (p->ev[k][i]) cudaEventDestroy(p->ev[k][i]);
@@ -180,6 +192,29 @@ extern "C" int nusht_plan_ex(nusht_plan_t** out, int lmax, int mmax, int64_t npt
     return NUSHT_OK;
 }
 
+extern "C" int nusht_set_points(nusht_plan_t* p, int64_t npts, const double* theta, const double* phi) {
+    if (!p || npts < 0 || npts >= ((int64_t)1 << 31) || (npts > 0 && (!theta || !phi))) return NUSHT_ERR_INVALID_ARG;
+    int dev = -1;
+    NUSHT_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != p->device) return NUSHT_ERR_INVALID_ARG;
+    const auto t0 = std::chrono::steady_clock::now();
+    NUSHT_CUDA_TRY(cudaDeviceSynchronize());      // no transform of this plan may still read the old tables
+    if (npts != p->npts) {                        // same count: the tables and staging maps are kept and overwritten
+        nufft_free_points(p);
+        host_release(p);                          // the staging maps are sized by npts
+    }
+    p->npts = npts;
+    const int st = nufft_sort_points(p, theta, phi);
+    if (st != NUSHT_OK || cudaDeviceSynchronize() != cudaSuccess) {
+        nufft_free_points(p);                     // leave a valid plan without points
+        p->npts = 0;
+        p->set_points_ms = 0;
+        return st != NUSHT_OK ? st : NUSHT_ERR_CUDA;
+    }
+    p->set_points_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    return NUSHT_OK;
+}
+
 extern "C" int nusht_plan_info(const nusht_plan_t* p, nusht_info_t* info) {
     if (!p || !info) return NUSHT_ERR_INVALID_ARG;
     memset(info, 0, sizeof(*info));
@@ -202,6 +237,7 @@ extern "C" int nusht_plan_info(const nusht_plan_t* p, nusht_info_t* info) {
     info->sort_ms = p->sort_ms;
     info->legendre_fma_synthesis = p->leg_fma_syn;
     info->legendre_fma_adjoint = p->leg_fma_adj;
+    info->set_points_ms = p->set_points_ms;
     return NUSHT_OK;
 }
 
@@ -304,6 +340,7 @@ static int host_setup(nusht_plan_s* p) {
         NUSHT_CUDA_TRY(cudaMalloc(&p->d_out_map[b], mbytes ? mbytes : 16));
     }
     p->workspace_bytes += (int64_t)(4 * abytes + 4 * mbytes);
+    p->host_npts = p->npts;
     return NUSHT_OK;
 }
 

@@ -1397,7 +1397,16 @@ static int nu_alloc(T** ptr, size_t count, nusht_plan_s* p) {
     return NUSHT_OK;
 }
 
+// the point tables are accounted for separately, so that nusht_set_points can replace them
+static int sort_points_impl(nusht_plan_s* p, const double* theta, const double* phi);
 int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi) {
+    const int64_t before = p->workspace_bytes;
+    const int st = sort_points_impl(p, theta, phi);
+    p->points_bytes += p->workspace_bytes - before;
+    return st;
+}
+
+static int sort_points_impl(nusht_plan_s* p, const double* theta, const double* phi) {
     NufftGeom& g = p->ng;
     g.nstrip = (g.nph + 1 + g.mb - 1) / g.mb;   // origins cb = 0..nph inclusive
     g.nseg = (g.nth / 2 + 2 + NUSHT_SEG_ROWS - 1) / NUSHT_SEG_ROWS;
@@ -1408,10 +1417,12 @@ int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi) {
     if (nbins64 + 1 >= (int64_t)1 << 31) return NUSHT_ERR_UNSUPPORTED;
     const int nbins = (int)nbins64;
     const int64_t n = p->npts;
-    NUSHT_TRY(nu_alloc(&p->d_px, (size_t)n, p));
-    NUSHT_TRY(nu_alloc(&p->d_py, (size_t)n, p));
-    NUSHT_TRY(nu_alloc(&p->d_perm, (size_t)n, p));
-    NUSHT_TRY(nu_alloc(&p->d_item_off, (size_t)p->n_items + 1, p));
+    if (!p->d_px) {     // (nusht_set_points with an unchanged point count keeps the tables and overwrites them)
+        NUSHT_TRY(nu_alloc(&p->d_px, (size_t)n, p));
+        NUSHT_TRY(nu_alloc(&p->d_py, (size_t)n, p));
+        NUSHT_TRY(nu_alloc(&p->d_perm, (size_t)n, p));
+        NUSHT_TRY(nu_alloc(&p->d_item_off, (size_t)p->n_items + 1, p));
+    }
 
     SortGeom sg;
     sg.nth = g.nth; sg.nph = g.nph; sg.w = g.w; sg.fl = g.fl; sg.mb = g.mb; sg.nstrip = g.nstrip; sg.nseg = g.nseg;
@@ -1505,11 +1516,13 @@ int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi) {
         const int nchunks = (int)((n + BUCKET_CHUNK - 1) / BUCKET_CHUNK);
         const int ncnt = BUCKET_MAX * nchunks;
         const int nt = (ncnt + SCAN_TILE - 1) / SCAN_TILE;
-        NUSHT_TRY(nu_alloc(&p->d_slot, (size_t)n, p));
-        NUSHT_TRY(nu_alloc(&p->d_dest, (size_t)n, p));
-        float* stage = nullptr;
-        NUSHT_TRY(nu_alloc(&stage, (size_t)n, p));
-        p->d_stage = stage;
+        if (!p->d_slot) {
+            NUSHT_TRY(nu_alloc(&p->d_slot, (size_t)n, p));
+            NUSHT_TRY(nu_alloc(&p->d_dest, (size_t)n, p));
+            float* stage = nullptr;
+            NUSHT_TRY(nu_alloc(&stage, (size_t)n, p));
+            p->d_stage = stage;
+        }
         SORT_TRY(cudaMalloc((void**)&d_hist, sizeof(int) * (size_t)ncnt));
         SORT_TRY(cudaMalloc((void**)&d_off, sizeof(int) * (size_t)ncnt));
         SORT_TRY(cudaMalloc((void**)&d_tot, sizeof(int) * (size_t)nt));
@@ -1575,11 +1588,18 @@ int nufft_spread(nusht_plan_s* p, const void* map, void* grid, cudaStream_t s) {
     return dispatch_spread<float>(p->ng.w, P, *h, map, grid, s);
 }
 
-void nufft_free(nusht_plan_s* p) {
+void nufft_free_points(nusht_plan_s* p) {
     cudaFree(p->d_px); cudaFree(p->d_py); cudaFree(p->d_perm); cudaFree(p->d_item_off);
     p->d_px = p->d_py = nullptr; p->d_perm = nullptr; p->d_item_off = nullptr;
     cudaFree(p->d_slot); cudaFree(p->d_dest); cudaFree(p->d_stage);
     p->d_slot = p->d_dest = nullptr; p->d_stage = nullptr;
+    p->n_buckets = 1;
+    p->workspace_bytes -= p->points_bytes;
+    p->points_bytes = 0;
+}
+
+void nufft_free(nusht_plan_s* p) {
+    nufft_free_points(p);
     delete static_cast<KernelHost*>(p->kernel_host);
     p->kernel_host = nullptr;
 }

@@ -142,6 +142,7 @@ struct nusht_plan_s {
     int* d_slot = nullptr;          // sorted position -> slot (bucket-major, stable inside a bucket)
     int* d_dest = nullptr;          // slot -> caller index
     void* d_stage = nullptr;        // [npts] results in slot order (dtype)
+    int64_t points_bytes = 0;       // device memory of the point tables (the part of workspace_bytes nusht_set_points replaces)
     void* kernel_host = nullptr;    // nufft.cu: host model of the kernel polynomial
     // --- host-buffer staging (allocated on first use of *_host) ---
     // every staging buffer twice: call k of a direction uses set k & 1, so that the upload of the next call and the
@@ -150,6 +151,8 @@ struct nusht_plan_s {
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
     cudaEvent_t ev_in[2][2] = {}, ev_cdone[2][2] = {}, ev_out[2][2] = {};   // [0] synthesis, [1] adjoint; [set]
     unsigned host_seq[2] = {0, 0};                                          // host-buffer calls so far, per direction
+    int64_t host_npts = 0;                                                  // npts the staging maps were sized for
+    double set_points_ms = 0;                                               // wall time of the last nusht_set_points
     // --- stage timing ---
     int timing = 0;
     cudaEvent_t ev[2][NUSHT_NUM_STAGES + 1] = {};
@@ -181,6 +184,7 @@ int nufft_choose_kernel(nusht_plan_s* p);   // w, beta, degree, polynomial + dec
 int nufft_sort_points(nusht_plan_s* p, const double* theta, const double* phi);
 int nufft_interp(nusht_plan_s* p, const void* grid, void* map, cudaStream_t s);
 int nufft_spread(nusht_plan_s* p, const void* map, void* grid, cudaStream_t s);
+void nufft_free_points(nusht_plan_s* p);     // the point tables only (nusht_set_points)
 void nufft_free(nusht_plan_s* p);
 // host-side kernel model used by fourier_build: Fourier transform of the piecewise-polynomial kernel
 double nufft_kernel_ft(const nusht_plan_s* p, double k, int n);

@@ -26,7 +26,7 @@ EXPORTS = [
     "nusht_stage_fourier_synthesis", "nusht_stage_fourier_adjoint", "nusht_launch_count", "nusht_probe_fp64",
     "nusht_ring_plan", "nusht_ring_synthesis", "nusht_ring_analysis", "nusht_ring_gradient", "nusht_ring_info",
     "nusht_ring_destroy", "nusht_ring_pairing", "nusht_plan_ex", "nusht_static_scratch",
-    "nusht_stage_legendre_adjoint_static",
+    "nusht_stage_legendre_adjoint_static", "nusht_set_points",
 ]
 
 
@@ -39,6 +39,7 @@ class NushtInfo(ctypes.Structure):
         ("kernel_beta", ctypes.c_double), ("sigma", ctypes.c_double),
         ("workspace_bytes", ctypes.c_int64), ("plan_ms", ctypes.c_double), ("sort_ms", ctypes.c_double),
         ("legendre_fma_synthesis", ctypes.c_int64), ("legendre_fma_adjoint", ctypes.c_int64),
+        ("set_points_ms", ctypes.c_double),
     ]
 
 
@@ -84,6 +85,8 @@ def _load():
     lib.nusht_host_sync.restype = ip
     lib.nusht_host_reserve.argtypes = [vp]
     lib.nusht_host_reserve.restype = ip
+    lib.nusht_set_points.argtypes = [vp, ctypes.c_int64, vp, vp]
+    lib.nusht_set_points.restype = ip
     lib.nusht_static_scratch.argtypes = [ctypes.POINTER(ctypes.c_int64)]
     lib.nusht_static_scratch.restype = ip
     lib.nusht_launch_count.argtypes = []
@@ -170,6 +173,23 @@ class Plan:
         self.lmax, self.mmax, self.npts, self.nlm = int(lmax), int(mmax), npts, int(self.info.nlm)
         self.rdtype = torch.float64 if self.dtype == NUSHT_F64 else torch.float32
         self.cdtype = torch.complex128 if self.dtype == NUSHT_F64 else torch.complex64
+
+    def set_points(self, theta, phi):
+        """nusht_set_points: a new point set for the same (lmax, mmax, eps, dtype, sigma); only the point sort runs."""
+        npts = 0 if theta is None else int(theta.numel())
+        if npts:
+            if phi is None or int(phi.numel()) != npts:
+                raise ValueError("theta and phi must have the same number of entries")
+            if not (theta.is_cuda and phi.is_cuda and theta.dtype == torch.float64 and phi.dtype == torch.float64):
+                raise TypeError("theta/phi must be CUDA float64 tensors")
+            theta, phi = theta.contiguous(), phi.contiguous()
+            tp, pp = theta.data_ptr(), phi.data_ptr()
+        else:
+            tp = pp = None
+        code = lib.nusht_set_points(self._h, npts, tp, pp)
+        _check(lib.nusht_plan_info(self._h, ctypes.byref(self.info)))
+        self.npts = int(self.info.npts)
+        _check(code)
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -268,6 +268,55 @@ def test_host_buffer_calls_match_device_calls(nusht):
     plan.destroy()
 
 
+@pytest.mark.parametrize("dtype,eps", [("f64", 1e-10), ("f32", 1e-5)])
+def test_set_points_equals_a_fresh_plan(nusht, dtype, eps, monkeypatch):
+    """nusht_set_points (plan once, transform often; Appendix C: one point set per deflection field):
+    after it the plan must behave exactly like a plan built on the new points -- more points, fewer points, none,
+    bad ones -- and the host-buffer calls must follow the new size."""
+    if dtype == "f32":
+        monkeypatch.setenv("NUSHT_UNPERMUTE_SHIFT", "12")        # several un-permutation buckets at these sizes
+    L, M = 95, 80
+    cd = np.complex128 if dtype == "f64" else np.complex64
+    rd = np.float64 if dtype == "f64" else np.float32
+    alm = inputs.random_alm(L, M, 750).astype(cd)
+    th0, ph0 = inputs.uniform_sphere_points(9000, 751)
+    plan = nusht.Plan(L, M, cu(th0), cu(ph0), eps, dtype=dtype)
+    ws0 = plan.info.workspace_bytes
+    for k, npts in enumerate([20000, 3000, 9000]):
+        theta, phi = inputs.uniform_sphere_points(npts, 752 + k)
+        theta[:2] = [0.0, np.pi]
+        x = inputs.random_map(npts, 760 + k).astype(rd)
+        plan.set_points(cu(theta), cu(phi))
+        assert plan.npts == npts and plan.info.npts == npts and plan.info.set_points_ms > 0
+        fresh = nusht.Plan(L, M, cu(theta), cu(phi), eps, dtype=dtype)
+        assert plan.info.workspace_bytes == fresh.info.workspace_bytes
+        assert torch.equal(plan.synthesis(cu(alm)), fresh.synthesis(cu(alm)))
+        a, b = plan.adjoint(cu(x)), fresh.adjoint(cu(x))
+        assert float((a - b).abs().max()) <= (1e-12 if dtype == "f64" else 1e-5) * float(b.abs().max())
+        hf = torch.empty(npts, dtype=plan.rdtype).pin_memory()
+        plan.synthesis_host(torch.from_numpy(alm).pin_memory(), hf)
+        plan.host_sync()
+        assert torch.equal(hf, fresh.synthesis(cu(alm)).cpu())
+        fresh.destroy()
+    plan.set_points(cu(th0), cu(ph0))            # same count as the last set: tables and staging maps are kept
+    esz = 8 if dtype == "f64" else 4
+    assert plan.info.workspace_bytes == ws0 + 4 * plan.nlm * 2 * esz + 4 * 9000 * esz
+    # bad points: the error is reported and the plan is left valid, without points
+    bad = th0.copy()
+    bad[17] = np.nan
+    with pytest.raises(nusht.NushtError) as e:
+        plan.set_points(cu(bad), cu(ph0))
+    assert e.value.code == -6 and plan.npts == 0
+    assert plan.synthesis(cu(alm)).numel() == 0
+    plan.set_points(None, None)
+    assert plan.npts == 0
+    plan.set_points(cu(th0), cu(ph0))
+    ref = nusht.Plan(L, M, cu(th0), cu(ph0), eps, dtype=dtype)
+    assert torch.equal(plan.synthesis(cu(alm)), ref.synthesis(cu(alm)))
+    ref.destroy()
+    plan.destroy()
+
+
 def test_host_buffer_pipeline_with_distinct_inputs(nusht):
     """Six host-buffer steps in flight without a synchronisation, every step with inputs and host buffers of its own:
     the two sets of staging buffers are reused three times each, and every result must be that of its own input."""
