@@ -7,7 +7,7 @@ the metric "nuSHT synth+adjoint ms at lmax=4095" is quoted on): lmax = mmax = 40
 eps = 1e-10, 67,108,864 uniform random points, white a_lm.  Planning (point sort, tables, cuFFT
 plans) is excluded from the timed region, as in the paper.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1|2|3|4|6] [--impl reference]
 
 Prints ONE JSON line (rank 0).  Multi-GPU: the method is single-GPU: N ranks run N
 independent replicas ("replicas only"), no collective on the data path.
@@ -178,8 +178,9 @@ def run_reference(args, rank):
 
 
 def workload_config(cfg, npts):
-    return {"workload": "BASELINE.json config lmax=%d eps=%g: %d %s points, %s a_lm; step = synthesis + adjoint"
-                        % (cfg["lmax"], cfg["eps"], npts, cfg["points"], cfg["spectrum"]),
+    origin = "BASELINE.json config" if cfg["lmax"] <= 8191 else "beyond BASELINE.json (inputs.CONFIGS[6]):"
+    return {"workload": "%s lmax=%d eps=%g: %d %s points, %s a_lm; step = synthesis + adjoint"
+                        % (origin, cfg["lmax"], cfg["eps"], npts, cfg["points"], cfg["spectrum"]),
             "lmax": cfg["lmax"], "mmax": cfg["mmax"], "npts": int(npts), "eps": cfg["eps"],
             "l2": "inputs larger than L2 (alm %.0f MB, map %.0f MB, fine grid > 126 MB at lmax >= 1023)"
                   % (inputs.nlm(cfg["lmax"], cfg["mmax"]) * 16 / 1e6, npts * 8 / 1e6),

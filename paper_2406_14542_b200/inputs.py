@@ -89,6 +89,9 @@ CONFIGS = {
     2: dict(lmax=1023, mmax=1023, eps=1e-10, dtype="f64", npts=2048 * 2048, points="lensing", spectrum="inv_l2", seed=2),
     3: dict(lmax=4095, mmax=4095, eps=1e-10, dtype="f64", npts=4 * 4096 * 4096, points="uniform", spectrum="white", seed=3),
     4: dict(lmax=8191, mmax=8191, eps=1e-8, dtype="f64", npts=2 * 8192 * 8192, points="uniform", spectrum="inv_l2", seed=4),
+    # not a BASELINE.json config: twice the band limit of the largest one (the paper's A100 limit is lmax ~ 9000,
+    # PAPER.md:156), 2 (lmax + 1)^2 points as in config 4; 108 GB of plan workspace at sigma = 2
+    6: dict(lmax=16383, mmax=16383, eps=1e-10, dtype="f64", npts=2 * 16384 * 16384, points="uniform", spectrum="inv_l2", seed=6),
 }
 
 
