@@ -17,7 +17,7 @@ SOURCES = ["api.cu", "legendre.cu", "fourier.cu", "nufft.cu", "pointing.cu", "pr
 HEADERS = [os.path.join(CSRC, "nusht_internal.cuh"), os.path.join(HERE, "..", "include", "nusht.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Wno-deprecated-gpu-targets",
-         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+         "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-Xcompiler", "-pthread"]
 
 
 def _stale(target, deps):
@@ -44,7 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError("nvcc failed on " + src)
     if force or procs or _stale(LIB, objs):
         tmp = LIB + ".tmp.%d" % os.getpid()
-        cmd = [NVCC, "-Wno-deprecated-gpu-targets", "-shared", "-o", tmp] + objs + ["-lcufft", "-Xlinker", "-rpath,/usr/local/cuda/lib64"]
+        cmd = [NVCC, "-Wno-deprecated-gpu-targets", "-shared", "-o", tmp] + objs + ["-lcufft", "-lpthread", "-Xlinker", "-rpath,/usr/local/cuda/lib64"]
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
     return LIB

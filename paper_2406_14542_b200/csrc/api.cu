@@ -149,7 +149,17 @@ extern "C" int nusht_plan_ex(nusht_plan_t** out, int lmax, int mmax, int64_t npt
     p->device = dev;
     p->nlm = (int64_t)(mmax + 1) * (lmax + 1) - (int64_t)mmax * (mmax + 1) / 2;
 
+    // NUSHT_VERBOSE: wall time of each planning phase on stderr
+    const bool verbose = getenv("NUSHT_VERBOSE") != nullptr;
+    auto lap = [&, last = t0](const char* what) mutable {
+        if (!verbose) return;
+        cudaDeviceSynchronize();
+        const auto now = std::chrono::steady_clock::now();
+        fprintf(stderr, "[nusht] plan: %-28s %8.2f ms\n", what, std::chrono::duration<double, std::milli>(now - last).count());
+        last = now;
+    };
     int st = nufft_choose_kernel(p);
+    lap("kernel width + polynomial fit");
     if (st == NUSHT_OK) {
         // Clenshaw-Curtis rings: N_r >= lmax + 2 with the doubled length 2 (N_r - 1) a good FFT size (reading G4/G5)
         const int nth2 = good_even_size(2 * (lmax + 1));
@@ -171,9 +181,12 @@ extern "C" int nusht_plan_ex(nusht_plan_t** out, int lmax, int mmax, int64_t npt
         p->ng.nph = good_even_size(nph);
         p->ng.nrow_half = p->ng.nth / 2 + 1;
         st = legendre_build_tables(p);
+        lap("Legendre tables");
     }
     if (st == NUSHT_OK) st = fourier_build(p);
+    lap("Fourier tables + FFT plans");
     if (st == NUSHT_OK) st = nufft_sort_points(p, theta, phi);
+    lap("point sort");
     if (st == NUSHT_OK) {
         for (int k = 0; k < 2 && st == NUSHT_OK; ++k)
             for (int i = 0; i <= NUSHT_NUM_STAGES; ++i)

@@ -1122,12 +1122,17 @@ int fourier_build(nusht_plan_s* p) {
 
     // deconvolution tables (host, extended precision inside nufft_kernel_ft); 1/Ntheta folded into p_theta
     std::vector<double> pth(2 * L + 1), pph(M + 1);
-    for (int k = 0; k <= L; ++k) {
-        const double v = 1.0 / (nufft_kernel_ft(p, (double)k, g.nth) * (double)nth2);
-        pth[L + k] = v;
-        pth[L - k] = v;
-    }
-    for (int m = 0; m <= M; ++m) pph[m] = 1.0 / nufft_kernel_ft(p, (double)m, g.nph);
+    nufft_kernel_ft(p, 0.0, g.nth);     // (builds its quadrature nodes once, before the threads start)
+    nusht_parallel_for(L + 1, [&](int lo, int hi) {
+        for (int k = lo; k < hi; ++k) {
+            const double v = 1.0 / (nufft_kernel_ft(p, (double)k, g.nth) * (double)nth2);
+            pth[L + k] = v;
+            pth[L - k] = v;
+        }
+    });
+    nusht_parallel_for(M + 1, [&](int lo, int hi) {
+        for (int m = lo; m < hi; ++m) pph[m] = 1.0 / nufft_kernel_ft(p, (double)m, g.nph);
+    });
     NUSHT_TRY(f_alloc(&p->d_pth, sizeof(double) * (2 * L + 1), p));
     NUSHT_TRY(f_alloc(&p->d_pph, sizeof(double) * (M + 1), p));
     NUSHT_CUDA_TRY(cudaMemcpy(p->d_pth, pth.data(), sizeof(double) * (2 * L + 1), cudaMemcpyHostToDevice));

@@ -2,6 +2,8 @@
 // libnusht.so.  Nothing here is visible across the C ABI (include/nusht.h).
 #pragma once
 
+#include <thread>
+#include <vector>
 #include <cuda_runtime.h>
 #include <cufft.h>
 #include <stdint.h>
@@ -188,3 +190,20 @@ void nufft_free_points(nusht_plan_s* p);     // the point tables only (nusht_set
 void nufft_free(nusht_plan_s* p);
 // host-side kernel model used by fourier_build: Fourier transform of the piecewise-polynomial kernel
 double nufft_kernel_ft(const nusht_plan_s* p, double k, int n);
+
+// plan-time host loops over independent entries (deconvolution tables): the index range cut into one slice per
+// hardware thread; body(lo, hi) must not touch shared state
+template <typename F>
+inline void nusht_parallel_for(int n, F body) {
+    unsigned nt = std::thread::hardware_concurrency();
+    if (nt > 32) nt = 32;
+    if (nt < 2 || n < 64) {
+        body(0, n);
+        return;
+    }
+    const int chunk = (n + (int)nt - 1) / (int)nt;
+    std::vector<std::thread> pool;
+    for (int lo = chunk; lo < n; lo += chunk) pool.emplace_back(body, lo, lo + chunk < n ? lo + chunk : n);
+    body(0, chunk < n ? chunk : n);
+    for (auto& t : pool) t.join();
+}
