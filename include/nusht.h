@@ -141,7 +141,11 @@ NUSHT_API int nusht_plan_ex(nusht_plan_t** out, int lmax, int mmax, int64_t npts
  * left valid WITHOUT points (npts = 0).  nusht_plan_info reports the new npts, workspace and set_points_ms. */
 NUSHT_API int nusht_set_points(nusht_plan_t* plan, int64_t npts, const double* theta, const double* phi);
 
-/* Synthesis, Eq. 3 / Eq. 5: alm (DEVICE, nlm complex) -> map (DEVICE, npts real).  npts == 0: no-op. */
+/* Synthesis, Eq. 3 / Eq. 5: alm (DEVICE, nlm complex) -> map (DEVICE, npts real).  npts == 0: no-op.
+ * nusht_synthesis and nusht_adjoint allocate nothing and synchronise nothing: they enqueue kernels, cuFFT launches and
+ * memsets on `stream` (the adjoint also forks to and joins from a plan-owned side stream with events).  After one eager
+ * call of each (which sets kernel attributes) they can be recorded by a stream capture and replayed as a CUDA graph
+ * (tests/test_gpu_parity.py::test_transforms_under_cuda_graph_capture). */
 NUSHT_API int nusht_synthesis(nusht_plan_t* plan, const void* alm, void* map, void* stream);
 
 /* Adjoint, Eq. 2 / Eq. 6: map (DEVICE, npts real) -> alm (DEVICE, nlm complex, overwritten).

@@ -317,6 +317,43 @@ def test_set_points_equals_a_fresh_plan(nusht, dtype, eps, monkeypatch):
     plan.destroy()
 
 
+@pytest.mark.parametrize("L,sigma,dtype,eps", [(255, None, "f64", 1e-10), (89, None, "f64", 1e-8),
+                                               (127, 1.25, "f64", 1e-8), (127, None, "f32", 1e-5)])
+def test_transforms_under_cuda_graph_capture(nusht, L, sigma, dtype, eps):
+    """A serving loop replays one captured graph: nusht_synthesis + nusht_adjoint allocate nothing and synchronise
+    nothing, so a stream capture records them (kernels, cuFFT launches, memsets, and the event fork / join of the
+    adjoint Legendre stage's side stream).  The replayed graph must give the bits of the eager calls on new inputs."""
+    npts = 20000
+    theta, phi = inputs.uniform_sphere_points(npts, 81)
+    plan = nusht.Plan(L, L, cu(theta), cu(phi), eps, dtype=dtype, sigma=sigma)
+    cd = np.complex128 if dtype == "f64" else np.complex64
+    rd = np.float64 if dtype == "f64" else np.float32
+    alm = cu(inputs.random_alm(L, L, 810).astype(cd))
+    x = cu(inputs.random_map(npts, 811).astype(rd))
+    f = torch.empty(npts, dtype=plan.rdtype, device="cuda")
+    c = torch.empty(plan.nlm, dtype=plan.cdtype, device="cuda")
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):                      # warm-up on the capture stream (function attributes, modules)
+        plan.synthesis(alm, f, side)
+        plan.adjoint(x, c, side)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        plan.synthesis(alm, f, torch.cuda.current_stream())
+        plan.adjoint(x, c, torch.cuda.current_stream())
+    for k in range(3):
+        alm.copy_(cu(inputs.random_alm(L, L, 820 + k).astype(cd)))
+        x.copy_(cu(inputs.random_map(npts, 830 + k).astype(rd)))
+        f.fill_(float("nan"))
+        c.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        f_ref, c_ref = plan.synthesis(alm), plan.adjoint(x)
+        assert torch.equal(f, f_ref), k
+        assert float((c - c_ref).abs().max()) <= (1e-12 if dtype == "f64" else 1e-5) * float(c_ref.abs().max()), k
+    plan.destroy()
+
+
 def test_host_buffer_pipeline_with_distinct_inputs(nusht):
     """Six host-buffer steps in flight without a synchronisation, every step with inputs and host buffers of its own:
     the two sets of staging buffers are reused three times each, and every result must be that of its own input."""
