@@ -103,3 +103,18 @@ def test_ring_plan_rejects_bad_arguments_without_device(lib):
     assert lib.nusht_ring_plan(ctypes.byref(h), 4, 4, 0, th, n, None, None, 0) == -1       # no rings
     assert h.value is None
     assert lib.nusht_ring_destroy(None) == 0
+
+
+def test_round2_entry_points_reject_null_plans_without_device(lib):
+    vp = ctypes.c_void_p
+    lib.nusht_set_points.argtypes = [vp, ctypes.c_int64, vp, vp]
+    lib.nusht_stage_legendre_adjoint_static.argtypes = [vp, vp, vp, vp]
+    lib.nusht_static_scratch.argtypes = [ctypes.POINTER(ctypes.c_int64)]
+    lib.nusht_strerror.restype = ctypes.c_char_p
+    assert lib.nusht_set_points(None, 0, None, None) == -1
+    assert lib.nusht_stage_legendre_adjoint_static(None, None, None, None) == -1
+    assert b"static scratch" in lib.nusht_strerror(-7)          # NUSHT_ERR_TOO_LARGE names the entry point and the limit
+    import torch
+    if not torch.cuda.is_available():
+        n = ctypes.c_int64(-1)
+        assert lib.nusht_static_scratch(ctypes.byref(n)) == -3   # NUSHT_ERR_CUDA: the array lives on a device
