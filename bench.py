@@ -52,11 +52,14 @@ def parse():
                     help="BASELINE.json configs[4]: lmax=4095 on 67M points, eps in {1e-4, 1e-6} FP32 and "
                          "{1e-8, 1e-10, 1e-12} FP64; one JSON line per eps (accuracy on an oracle subset + timing)")
     ap.add_argument("--sweep-subset", type=int, default=1500, help="points of the oracle subset of the sweep")
-    ap.add_argument("--ring", default=None, choices=["gl", "equi", "healpix"],
+    ap.add_argument("--ring", default=None, choices=["gl", "equi", "healpix", "healpix-lens"],
                     help="ring-grid transforms (SURVEY 8(f) rank 3/4) instead of the nuSHT step: 'gl' = Gauss-Legendre grid "
                          "(lmax+1 rings x 2 lmax+2 pixels, the paper's output grid, PAPER.md:154): step = synthesis + "
                          "analysis; 'healpix' = the same on a HEALPix-style ring layout (PAPER.md:218), nside = (lmax+1)/2; "
-                         "'equi' = the 2(lmax+1)^2 equi-angular grid of config 2: step = gradient (Eq. C2) + pointing")
+                         "'equi' = the 2(lmax+1)^2 equi-angular grid of config 2: step = gradient (Eq. C2) + pointing; "
+                         "'healpix-lens' = the paper's use case (Eq. 8, Appendix C) on the HEALPix-style layout: step = "
+                         "deflection field of a lensing potential (Eq. C2) + pointing (Eq. C1) + nusht_set_points + "
+                         "synthesis of the unlensed field at the deflected pixel centres")
     ap.add_argument("--lmax", type=int, default=4095, help="band limit of the --ring modes")
     return ap.parse_args()
 
@@ -539,7 +542,7 @@ def run_ring(args):
         theta[L + 1 - half:] = np.pi - theta[:half][::-1]
         nphi = np.full(L + 1, 2 * L + 2)
         weight = wg[::-1] * (2 * np.pi / (2 * L + 2))
-    elif args.ring == "healpix":            # nside = (lmax + 1) / 2: the caps are 2 (nside - 1) rings of distinct lengths
+    elif args.ring in ("healpix", "healpix-lens"):   # nside = (lmax + 1) / 2: 2 (nside - 1) cap rings of distinct lengths
         theta, nphi, phi0, weight = inputs.healpix_ring_layout((L + 1) // 2)
     else:
         nr = 2 * (L + 1)
@@ -556,6 +559,20 @@ def run_ring(args):
             plan.analysis(f, out, stream)
         what = "ring synthesis + analysis on " + ("a Gauss-Legendre grid" if args.ring == "gl" else
                                                  "a HEALPix-style ring layout, nside = (lmax + 1) / 2")
+    elif args.ring == "healpix-lens":
+        th = torch.from_numpy(np.repeat(theta, nphi)).cuda()
+        ph = torch.from_numpy(np.concatenate([p0 + 2 * np.pi * np.arange(n) / n for n, p0 in zip(nphi, phi0)])).cuda()
+        philm = torch.from_numpy(inputs.random_alm(L, L, 8, "inv_l2")).cuda() * 2e-5      # a few arcminutes rms
+        eps = 1e-10
+        lens = nusht.Plan(L, L, th, ph, eps)          # planned once; every step re-points it (nusht_set_points)
+
+        def step():
+            a_t, a_p = plan.gradient(philm, stream)
+            t2, p2 = nusht.nusht_pointing(th, ph, a_t, a_p, stream)
+            lens.set_points(t2, p2)
+            lens.synthesis(alm, f, stream)
+        what = ("lensed map on a HEALPix-style layout, nside = (lmax + 1) / 2: Eq. C2 (two ring syntheses) + Eq. C1 + "
+                "nusht_set_points + nuSHT synthesis at eps = %g" % eps)
     else:
         th = torch.from_numpy(np.repeat(theta, nphi)).cuda()
         ph = torch.from_numpy(np.tile(2 * np.pi * np.arange(nphi[0]) / nphi[0], len(theta))).cuda()
@@ -576,7 +593,7 @@ def run_ring(args):
     e1.record(stream)
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / args.steps
-    print(json.dumps({"metric": "ring_%s_ms" % args.ring, "value": ms, "unit": "ms", "n_gpus": 1, "steps": args.steps,
+    print(json.dumps({"metric": "ring_%s_ms" % args.ring.replace("-", "_"), "value": ms, "unit": "ms", "n_gpus": 1, "steps": args.steps,
                       "warmup": max(args.warmup, 3), "higher_is_better": False, "dtype": "f64", "data": "synthetic",
                       "config": {"workload": what, "lmax": L, "nrings": int(len(theta)), "npix": int(plan.npix)},
                       "pixels_per_s": plan.npix / (ms * 1e-3), "gpu_launches": int(nusht.launch_count() - n0),
