@@ -277,3 +277,33 @@ def test_lensing_chain_gradient_pointing_synthesis(nusht, oracle):
     assert rel(f[idx], f_ref) <= 1e-9
     plan.destroy()
     rplan.destroy()
+
+
+def test_lensing_chain_on_a_healpix_layout_with_set_points(nusht, oracle):
+    """The same chain as bench.py --ring healpix-lens runs it: the nuSHT plan is built once on the undeflected pixel
+    centres and re-pointed with nusht_set_points for every potential (two realisations here), on a HEALPix-style
+    layout whose cap rings go through the chirp-z pool."""
+    nside, L = 64, 127
+    theta, nphi, phi0, _ = healpix_like_grid(nside)
+    rplan = nusht.RingPlan(L, L, theta, nphi, phi0)
+    th, ph = pixel_centres(theta, nphi, phi0)
+    d_th, d_ph = cu(th), cu(ph)
+    plan = nusht.Plan(L, L, d_th, d_ph, 1e-10)
+    alm = inputs.random_alm(L, L, 520, "inv_l2")
+    idx = np.sort(np.random.default_rng(521).choice(len(th), 1500, replace=False))
+    idx = np.unique(np.concatenate([idx, np.arange(12), len(th) - 1 - np.arange(12)]))      # cap pixels too
+    for k in range(2):
+        philm = inputs.random_alm(L, L, 522 + k, "inv_l2") * 4.0e-5
+        philm[:2] = 0
+        a_t, a_p = rplan.gradient(cu(philm))
+        t2, p2 = nusht.nusht_pointing(d_th, d_ph, a_t, a_p)
+        plan.set_points(t2, p2)
+        f = plan.synthesis(cu(alm)).cpu().numpy()
+        g_t, g_p = oracle.gradient(L, L, th[idx], ph[idx], philm, "ld")
+        o_t, o_p = oracle.pointing(th[idx], ph[idx], g_t, g_p)
+        o_t, o_p = np.asarray(o_t, dtype=np.float64), np.asarray(o_p, dtype=np.float64)
+        assert np.max(np.abs(t2.cpu().numpy()[idx] - o_t)) <= 1e-12, k
+        f_ref = oracle.synthesis(L, L, o_t, o_p, alm, "ld")
+        assert rel(f[idx], f_ref) <= 1e-9, k
+    plan.destroy()
+    rplan.destroy()
