@@ -61,6 +61,8 @@ struct RingMeta {
     const double* scale;      // per-ring factor (analysis: quadrature weight; gradient: 1 / sin theta) or nullptr
     int nrings, M;
     int64_t stride;           // row stride of F[m][ring]
+    int small_below;          // synthesis: rings shorter than this are left to k_ring_spec_syn_small (0: none)
+    const int* small;         // their indices
 };
 
 template <typename C> struct RealOf;
@@ -87,7 +89,8 @@ k_ring_spec_syn(RingMeta R, const double2* __restrict__ F, C* __restrict__ z) {
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     {
         const int r = r0 + tx;
-        const int n = r < R.nrings ? R.nphi[r] : 0;
+        int n = r < R.nrings ? R.nphi[r] : 0;
+        if (n < R.small_below) n = 0;                 // short rings: k_ring_spec_syn_small
         const double phi0 = r < R.nrings ? R.phi0[r] : 0.0;
         const double sc = (r < R.nrings && R.scale) ? R.scale[r] : 1.0;
 #pragma unroll 1
@@ -95,18 +98,32 @@ k_ring_spec_syn(RingMeta R, const double2* __restrict__ F, C* __restrict__ z) {
             const int k = k0 + kk;
             double2 acc = make_double2(0.0, 0.0);
             if (n > 0 && k <= n / 2) {
-                for (int m = k; m <= R.M; m += n) {
-                    const double2 g = F[(int64_t)m * R.stride + r], e = phase(m, phi0);
-                    const double w = m == 0 ? 0.5 : 1.0;
-                    acc.x += w * (g.x * e.x - g.y * e.y);
-                    acc.y += w * (g.x * e.y + g.y * e.x);
-                }
-                for (int m = (n - k) % n; m <= R.M; m += n) {
-                    const double2 g = F[(int64_t)m * R.stride + r], e = phase(m, phi0);
-                    const double w = m == 0 ? 0.5 : 1.0;
-                    acc.x += w * (g.x * e.x - g.y * e.y);
-                    acc.y -= w * (g.x * e.y + g.y * e.x);
-                }
+                // a ring of n pixels folds (M + 1) / n modes onto each bin: rings next to the poles loop long, so the
+                // loads of four terms are issued together (one dependent L2 round trip per term otherwise: the
+                // 4-pixel ring of a HEALPix-style grid at lmax = 4095 alone took 0.7 ms)
+                auto fold = [&](int m0, double sgn) {
+                    int m = m0;
+                    for (; m + 3 * n <= R.M; m += 4 * n) {
+                        double2 g[4];
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) g[u] = F[(int64_t)(m + u * n) * R.stride + r];
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const double2 e = phase(m + u * n, phi0);
+                            const double w = (m + u * n) == 0 ? 0.5 : 1.0;
+                            acc.x += w * (g[u].x * e.x - g[u].y * e.y);
+                            acc.y += sgn * w * (g[u].x * e.y + g[u].y * e.x);
+                        }
+                    }
+                    for (; m <= R.M; m += n) {
+                        const double2 g = F[(int64_t)m * R.stride + r], e = phase(m, phi0);
+                        const double w = m == 0 ? 0.5 : 1.0;
+                        acc.x += w * (g.x * e.x - g.y * e.y);
+                        acc.y += sgn * w * (g.x * e.y + g.y * e.x);
+                    }
+                };
+                fold(k, 1.0);
+                fold((n - k) % n, -1.0);
                 acc.x *= sc;
                 acc.y *= sc;
             }
@@ -119,12 +136,58 @@ k_ring_spec_syn(RingMeta R, const double2* __restrict__ F, C* __restrict__ z) {
         const int r = r0 + rr, k = k0 + tx;
         if (r >= R.nrings) continue;
         const int n = R.nphi[r];
-        if (k > n / 2) continue;
+        if (k > n / 2 || n < R.small_below) continue;
         const double2 v = tile[tx][rr];
         C out;
         out.x = (typename RealOf<C>::type)v.x;
         out.y = (typename RealOf<C>::type)v.y;
         z[R.zoff[r] + k] = out;
+    }
+}
+
+// synthesis, rings of fewer than RING_SMALL pixels (the first rings of a polar cap): such a ring folds (M + 1) / n modes
+// onto each of its few bins, a loop of thousands of dependent global loads for a handful of threads in the kernel above
+// (0.7 ms for the 4-pixel ring of a HEALPix-style grid at lmax = 4095).  Here one CTA takes one ring: all threads bring
+// A_m = w_m F_m e^{i m phi0} for a block of 4096 modes into shared memory, then thread k sums the entries of bin k.
+// Same terms in the same order as the kernel above.
+constexpr int RING_SMALL = 64;
+constexpr int RING_SMALL_MODES = 4096;
+template <typename C>
+__global__ void __launch_bounds__(256)
+k_ring_spec_syn_small(RingMeta R, const double2* __restrict__ F, C* __restrict__ z) {
+    extern __shared__ double2 s_a[];
+    const int r = R.small[blockIdx.x], t = threadIdx.x;
+    const int n = R.nphi[r];
+    const double phi0 = R.phi0[r], sc = R.scale ? R.scale[r] : 1.0;
+    double2 acc = make_double2(0.0, 0.0), accm = make_double2(0.0, 0.0);   // terms m = k, and m = -k (mod n)
+    for (int m0 = 0; m0 <= R.M; m0 += RING_SMALL_MODES) {
+        const int cnt = min(RING_SMALL_MODES, R.M + 1 - m0);
+        for (int i = t; i < cnt; i += 256) {
+            const int m = m0 + i;
+            const double2 g = F[(int64_t)m * R.stride + r], e = phase(m, phi0);
+            const double w = m == 0 ? 0.5 : 1.0;
+            s_a[i] = make_double2(w * (g.x * e.x - g.y * e.y), w * (g.x * e.y + g.y * e.x));
+        }
+        __syncthreads();
+        if (t <= n / 2) {
+            int i = ((t - m0) % n + n) % n;                 // first mode of this block with m = t (mod n)
+            for (; i < cnt; i += n) {
+                acc.x += s_a[i].x;
+                acc.y += s_a[i].y;
+            }
+            i = (((n - t) % n - m0) % n + n) % n;           // ... with m = -t (mod n)
+            for (; i < cnt; i += n) {
+                accm.x += s_a[i].x;
+                accm.y -= s_a[i].y;
+            }
+        }
+        __syncthreads();
+    }
+    if (t <= n / 2) {
+        C out;
+        out.x = (typename RealOf<C>::type)((acc.x + accm.x) * sc);
+        out.y = (typename RealOf<C>::type)((acc.y + accm.y) * sc);
+        z[R.zoff[r] + t] = out;
     }
 }
 
@@ -328,6 +391,8 @@ struct nusht_ring_plan_s {
     std::map<std::pair<int, int>, std::pair<cufftHandle, cufftHandle>> fft;   // (nphi, batch) -> (C2R, R2C)
     // Bluestein pool (rings of short runs), slots ordered by group
     std::vector<BlueGroup> groups;
+    int nsmall = 0;                    // rings of fewer than RING_SMALL pixels (k_ring_spec_syn_small)
+    int* d_small = nullptr;
     int npool = 0, pool_maxP = 0;
     int *d_bring = nullptr, *d_bP = nullptr;
     int64_t *d_bwoff = nullptr, *d_bboff = nullptr, *d_bcoff = nullptr, *d_bpix = nullptr;
@@ -347,6 +412,7 @@ static void ring_release(nusht_ring_plan_s* rp) {
     cudaFree(rp->d_z); cudaFree(rp->d_fftwork); cudaFree(rp->d_ga); cudaFree(rp->d_gb); cudaFree(rp->d_stage);
     for (auto& g : rp->groups)
         if (g.z2z) cufftDestroy(g.z2z);
+    cudaFree(rp->d_small);
     cudaFree(rp->d_bring); cudaFree(rp->d_bP); cudaFree(rp->d_bwoff); cudaFree(rp->d_bboff); cudaFree(rp->d_bcoff);
     cudaFree(rp->d_bpix); cudaFree(rp->d_bwork); cudaFree(rp->d_bspec); cudaFree(rp->d_bchirp);
     delete rp;
@@ -459,6 +525,20 @@ static int ring_build(nusht_ring_plan_s* rp, const double* theta, const int64_t*
     NUSHT_CUDA_TRY(cudaMemcpy(rp->d_weight, h_w.data(), sizeof(double) * (size_t)nr, cudaMemcpyHostToDevice));
     NUSHT_CUDA_TRY(cudaMemcpy(rp->d_isin, h_isin.data(), sizeof(double) * (size_t)nr, cudaMemcpyHostToDevice));
     NUSHT_TRY(r_alloc(&rp->d_z, (size_t)zo * (f64 ? 16 : 8), rp));
+    {
+        std::vector<int> h_small;
+        for (int r = 0; r < nr; ++r)
+            if (h_n[r] < RING_SMALL) h_small.push_back(r);
+        rp->nsmall = (int)h_small.size();
+        if (rp->nsmall) {
+            NUSHT_TRY(r_alloc(&rp->d_small, sizeof(int) * h_small.size(), rp));
+            NUSHT_CUDA_TRY(cudaMemcpy(rp->d_small, h_small.data(), sizeof(int) * h_small.size(), cudaMemcpyHostToDevice));
+            NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_ring_spec_syn_small<double2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                RING_SMALL_MODES * (int)sizeof(double2)));
+            NUSHT_CUDA_TRY(cudaFuncSetAttribute(k_ring_spec_syn_small<float2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                RING_SMALL_MODES * (int)sizeof(double2)));
+        }
+    }
     {   // Eq. C2 coefficient buffers (band limit lmax + 1)
         const int64_t nlm1 = (int64_t)(M + 1) * (rp->lmax + 2) - (int64_t)M * (M + 1) / 2;
         NUSHT_TRY(r_alloc(&rp->d_ga, (size_t)nlm1 * (f64 ? 16 : 8), rp));
@@ -669,17 +749,26 @@ static RingMeta ring_meta(const nusht_ring_plan_s* rp, const double* scale) {
     R.nrings = rp->nrings;
     R.M = rp->mmax;
     R.stride = rp->nrings;
+    R.small_below = 0;
+    R.small = rp->d_small;
     return R;
 }
 
 // F[m][ring] -> pixels
 static int ring_phi_synthesis(nusht_ring_plan_s* rp, const double* scale, void* map, cudaStream_t s) {
     const bool f64 = rp->dtype == NUSHT_F64;
-    const RingMeta R = ring_meta(rp, scale);
+    RingMeta R = ring_meta(rp, scale);
+    if (rp->nsmall) R.small_below = RING_SMALL;
     const dim3 grid((rp->nrings + 31) / 32, (rp->max_nphi / 2 + 1 + 31) / 32);
     if (f64) k_ring_spec_syn<double2><<<grid, 256, 0, s>>>(R, rp->core.d_ft, (double2*)rp->d_z);
     else k_ring_spec_syn<float2><<<grid, 256, 0, s>>>(R, rp->core.d_ft, (float2*)rp->d_z);
     NUSHT_CUDA_TRY(nusht_launched());
+    if (rp->nsmall) {
+        const size_t smem = RING_SMALL_MODES * sizeof(double2);
+        if (f64) k_ring_spec_syn_small<double2><<<rp->nsmall, 256, smem, s>>>(R, rp->core.d_ft, (double2*)rp->d_z);
+        else k_ring_spec_syn_small<float2><<<rp->nsmall, 256, smem, s>>>(R, rp->core.d_ft, (float2*)rp->d_z);
+        NUSHT_CUDA_TRY(nusht_launched());
+    }
     const size_t esz = f64 ? 8 : 4;
     for (const auto& run : rp->runs) {
         NUSHT_CUFFT_TRY(cufftSetStream(run.c2r, s));
