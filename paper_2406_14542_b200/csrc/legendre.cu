@@ -807,25 +807,52 @@ k_legendre_adjoint(LegParams P, const double2* __restrict__ gt, double4* __restr
                 }
                 // cross-lane sums: transpose through shared memory (value q of lane l at s_tr[q][l]); the
                 // 32 / NV lanes of row q = lane % NV add NV entries each and are combined by shuffles
+                double tot;
+                int qout;
+                if (NV == 32) {
+                    // values (2 qp, 2 qp + 1) of a lane travel as one 128-bit store; lane = (qp, half) then adds the pair
+                    // over 16 lanes and the two halves meet in one shuffle
+                    double2* tr2 = reinterpret_cast<double2*>(&s_tr[0][0]);        // [16][33] double2
 #pragma unroll
-                for (int q = 0; q < NV; ++q) s_tr[q][lane] = v[q];
-                __syncwarp();
-                const double2* src = reinterpret_cast<const double2*>(&s_tr[lane % NV][NV * (lane / NV)]);
-                double ta = 0.0, tb2 = 0.0, tc = 0.0, td = 0.0;      // four short add chains
+                    for (int qp = 0; qp < NV / 2; ++qp) tr2[qp * 33 + lane] = make_double2(v[2 * qp], v[2 * qp + 1]);
+                    __syncwarp();
+                    const double2* src = tr2 + (lane & 15) * 33 + 16 * (lane >> 4);
+                    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
 #pragma unroll
-                for (int k = 0; k < NV / 2; k += 2) {
-                    const double2 u = src[k], w = src[k + 1];
-                    ta += u.x;
-                    tb2 += u.y;
-                    tc += w.x;
-                    td += w.y;
+                    for (int k = 0; k < 16; k += 2) {
+                        const double2 u = src[k], w = src[k + 1];
+                        a0 += u.x;
+                        b0 += u.y;
+                        a1 += w.x;
+                        b1 += w.y;
+                    }
+                    double s0 = a0 + a1, s1 = b0 + b1;
+                    s0 += shfl_xor_d(s0, 16);
+                    s1 += shfl_xor_d(s1, 16);
+                    tot = (lane < 16) ? s0 : s1;
+                    qout = 2 * (lane & 15) + (lane >> 4);
+                } else {
+#pragma unroll
+                    for (int q = 0; q < NV; ++q) s_tr[q][lane] = v[q];
+                    __syncwarp();
+                    const double2* src = reinterpret_cast<const double2*>(&s_tr[lane % NV][NV * (lane / NV)]);
+                    double ta = 0.0, tb2 = 0.0, tc = 0.0, td = 0.0;      // four short add chains
+#pragma unroll
+                    for (int k = 0; k < NV / 2; k += 2) {
+                        const double2 u = src[k], w = src[k + 1];
+                        ta += u.x;
+                        tb2 += u.y;
+                        tc += w.x;
+                        td += w.y;
+                    }
+                    tot = (ta + tb2) + (tc + td);
+#pragma unroll
+                    for (int sh = NV; sh < 32; sh *= 2) tot += shfl_xor_d(tot, sh);
+                    qout = lane;
                 }
-                double tot = (ta + tb2) + (tc + td);
-#pragma unroll
-                for (int sh = NV; sh < 32; sh *= 2) tot += shfl_xor_d(tot, sh);
                 __syncwarp();
-                if (lane < NV && (lane >> 2) < ns)      // lane = 4 * step + component
-                    atomicAdd(reinterpret_cast<double*>(eo + o + (int64_t)tile * ADJ_TN + i0) + lane, tot);
+                if (qout < NV && (qout >> 2) < ns)      // q = 4 * step + component
+                    atomicAdd(reinterpret_cast<double*>(eo + o + (int64_t)tile * ADJ_TN + i0) + qout, tot);
             } else {
                 for (int i = 0; i < ns; ++i) {
                     const double2 ab = s_ab[st][i0 + i];
