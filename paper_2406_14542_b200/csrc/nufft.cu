@@ -637,13 +637,15 @@ k_spread(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
     for (int i = 0; i < W; ++i) acc[i] = 0;
     int a_base = INT_MIN;
 
-    double Xn = 0.0, Yn = 0.0;
+    double Xn = 0.0, Yn = 0.0;     // one batch ahead; the index of the value two batches ahead (see k_spread_mma)
     T vn = 0;
+    int pn = 0;
     if (start + lane < end) {
         Xn = P.px[start + lane];
         Yn = P.py[start + lane];
         vn = map[P.perm[start + lane]];
     }
+    if (start + 32 + lane < end) pn = P.perm[start + 32 + lane];
     for (int batch = start; batch < end; batch += 32) {
         const int idx = batch + lane;
         const bool has = idx < end;
@@ -652,8 +654,9 @@ k_spread(const __grid_constant__ NufftParams P, const __grid_constant__ KernelPo
         if (idx + 32 < end) {
             Xn = P.px[idx + 32];
             Yn = P.py[idx + 32];
-            vn = map[P.perm[idx + 32]];
+            vn = map[pn];
         }
+        if (idx + 64 < end) pn = P.perm[idx + 64];
         int a0;
         // the point's value rides on the theta weights
         const unsigned starts = publish_weights<W, T>(ws, kp, lane, has, X, Y, val, c0, a0);
@@ -1145,12 +1148,16 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
         else if (MT == 2 || mtu == 1) body(std::integral_constant<int, MT >= 2 ? 1 : 0>{});
         else body(std::integral_constant<int, MT >= 3 ? 2 : 0>{});
     };
+    // coordinates and value one batch ahead, the caller index of the value two batches ahead: map[perm[.]] is a
+    // dependent load, issued with the index still in flight it stalls the warp for a DRAM round trip
     double Xn = 0.0, Yn = 0.0, vn = 0.0;
+    int pn = 0;
     if (start + lane < end) {
         Xn = P.px[start + lane];
         Yn = P.py[start + lane];
         vn = map[P.perm[start + lane]];
     }
+    if (start + 32 + lane < end) pn = P.perm[start + 32 + lane];
     for (int batch = start; batch < end; batch += 32) {
         const int idx = batch + lane;
         const bool has = idx < end;
@@ -1158,8 +1165,9 @@ k_spread_mma(const __grid_constant__ NufftParams P, const __grid_constant__ Kern
         if (idx + 32 < end) {
             Xn = P.px[idx + 32];
             Yn = P.py[idx + 32];
-            vn = map[P.perm[idx + 32]];
+            vn = map[pn];
         }
+        if (idx + 64 < end) pn = P.perm[idx + 64];
         // the point's value rides on the theta weights
         const int a0 = mma_publish<W, S, true>(ws, kp, lane, X, Y, val, c0);
         __syncwarp();
